@@ -1,0 +1,243 @@
+// ORACLE — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, single-threaded C++ loops for the SPGD/NNLS hot path of
+// Ma & Qian (arXiv 1901.09266), written from the paper under the
+// readings of SURVEY.md §8(c) / DESIGN.md.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may load this file.  It
+// shares no code, header, table or helper with the CUDA path
+// (paper_1901_09266_b200/csrc) and neither side includes the other.
+//
+// What is computed (per day d of cluster c, all sums in double, storage fp32):
+//   O2a  r[t][l] = sum_{h=0..min(H,t)} sum_n R[c][t-h][h][l][n] q[t-h][n] - x[t][l]
+//        -- "B_o x - y", PAPER.md:406 (Alg. 1 line 9); Eq. 40/42;
+//           entry layout of Table 2: q entry (h1-1)|K|+k,
+//           x entry (h2-1)|A|+a, rho entry [(h2-1)|A|+a, (h1-1)Pi+k];
+//           block (h2,h1) with lag h = h2-h1 >= 0 (FIFO);
+//           cross-midnight flow dropped: no s+h >= T term.
+//   O2b  g[s][n] = sum_{h=0..min(H,T-1-s)} sum_l R[c][s][h][l][n] r[s+h][l]
+//        -- "g = B_o^T (B_o x - y)".  No factor 2 (reading A1).
+//   O2c  q[s][n] = max(0, q[s][n] - eta g[s][n])
+//        -- "x = max(x,0)"; plain step instead of Adagrad (reading A3,
+//           BASELINE.json north_star).  r is complete before any q changes.
+//   O3   f = sum_t sum_l r[t][l]^2, no 1/2, no mean -- Eq. 42.
+//   O4   L_c = lambda_max(rho_c^T rho_c) by power iteration from the all-ones
+//        vector (reading A10; PAPER.md:416 only says the rate depends on scale).
+//
+// Pins (tests/test_oracle_pins.py): P1 active-set NNLS on the T=12 instance,
+// P2 KKT, P3 finite differences, P4 planted recovery, P5 closed-form linear
+// iteration, P6 Example 1, P8 adjoint, P9 descent,
+// P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR.
+// No function here is "parity unpinned".
+#include <cmath>
+#include <cstddef>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Dims { int N, L, T, H; };
+
+inline size_t blk(const Dims& d, int s, int h) {            // offset of R_c[s][h] (L x N, n fastest)
+    return ((size_t)s * (d.H + 1) + h) * (size_t)d.L * d.N;
+}
+
+// O2a in double (no rounding of r); x may be null (then r = rho q).
+void forward_d(const Dims& d, const float* Rc, const float* q, const float* x, double* r) {
+    for (int t = 0; t < d.T; ++t)
+        for (int l = 0; l < d.L; ++l) {
+            double acc = 0.0;
+            const int hmax = d.H < t ? d.H : t;
+            for (int h = 0; h <= hmax; ++h) {
+                const float* row = Rc + blk(d, t - h, h) + (size_t)l * d.N;
+                const float* qs = q + (size_t)(t - h) * d.N;
+                for (int n = 0; n < d.N; ++n) acc += (double)row[n] * (double)qs[n];
+            }
+            r[(size_t)t * d.L + l] = acc - (x ? (double)x[(size_t)t * d.L + l] : 0.0);
+        }
+}
+
+// O2b: g = rho^T r, r given in fp32 storage.
+void gradient_f(const Dims& d, const float* Rc, const float* r, double* g) {
+    for (int s = 0; s < d.T; ++s)
+        for (int n = 0; n < d.N; ++n) {
+            double acc = 0.0;
+            const int hmax = d.H < d.T - 1 - s ? d.H : d.T - 1 - s;
+            for (int h = 0; h <= hmax; ++h) {
+                const float* B = Rc + blk(d, s, h);
+                const float* rt = r + (size_t)(s + h) * d.L;
+                for (int l = 0; l < d.L; ++l) acc += (double)B[(size_t)l * d.N + n] * (double)rt[l];
+            }
+            g[(size_t)s * d.N + n] = acc;
+        }
+}
+
+void visit(const Dims& d, const float* Rc, float* q, const float* x, float eta,
+           std::vector<double>& rd, std::vector<float>& rf, std::vector<double>& g) {
+    const size_t TL = (size_t)d.T * d.L, TN = (size_t)d.T * d.N;
+    rd.resize(TL); rf.resize(TL); g.resize(TN);
+    forward_d(d, Rc, q, x, rd.data());
+    for (size_t i = 0; i < TL; ++i) rf[i] = (float)rd[i];                 // r stored fp32 (O2a)
+    gradient_f(d, Rc, rf.data(), g.data());
+    for (size_t i = 0; i < TN; ++i) {                                     // O2c
+        const double v = (double)q[i] - (double)eta * g[i];
+        q[i] = (float)(v > 0.0 ? v : 0.0);
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+// r[t][l] (fp32) for one day; Rc = R[c] as [T][H+1][L][N].
+void oracle_forward_residual(int N, int L, int T, int H, const float* Rc, const float* q,
+                             const float* x, float* r) {
+    Dims d{N, L, T, H};
+    std::vector<double> rd((size_t)T * L);
+    forward_d(d, Rc, q, x, rd.data());
+    for (size_t i = 0; i < rd.size(); ++i) r[i] = (float)rd[i];
+}
+
+// g[s][n] (double) = rho_c^T r.
+void oracle_gradient(int N, int L, int T, int H, const float* Rc, const float* r, double* g) {
+    Dims d{N, L, T, H};
+    gradient_f(d, Rc, r, g);
+}
+
+// One SPGD visit of one day, in place on q (O2a-O2c).
+void oracle_visit(int N, int L, int T, int H, const float* Rc, float* q, const float* x, float eta) {
+    Dims d{N, L, T, H};
+    std::vector<double> rd, g; std::vector<float> rf;
+    visit(d, Rc, q, x, eta, rd, rf, g);
+}
+
+// O3: f = sum r^2 with r in double from the current q.
+double oracle_objective_day(int N, int L, int T, int H, const float* Rc, const float* q, const float* x) {
+    Dims d{N, L, T, H};
+    std::vector<double> rd((size_t)T * L);
+    forward_d(d, Rc, q, x, rd.data());
+    double f = 0.0;
+    for (double v : rd) f += v * v;
+    return f;
+}
+
+// Replays a schedule: iteration k visits days sched_days[sched_ptr[k] .. sched_ptr[k+1])
+// with step eta[k].  R is [C][T][H+1][L][N]; labels[D]; x [D][T][L]; q [D][T][N] in place.
+// day_mask (nullable, [D]): days with mask 0 are skipped -- valid because days
+// are independent units (pin P10).
+void oracle_run_schedule(int N, int L, int T, int H, int C, int D, const float* R,
+                         const int32_t* labels, const float* x, float* q,
+                         const int32_t* sched_days, const int64_t* sched_ptr, const float* sched_eta,
+                         int K, const uint8_t* day_mask) {
+    (void)C;
+    Dims d{N, L, T, H};
+    const size_t Rc_sz = (size_t)T * (H + 1) * L * N, TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<double> rd, g; std::vector<float> rf;
+    for (int k = 0; k < K; ++k)
+        for (int64_t i = sched_ptr[k]; i < sched_ptr[k + 1]; ++i) {
+            const int day = sched_days[i];
+            if (day < 0 || day >= D) continue;
+            if (day_mask && !day_mask[day]) continue;
+            visit(d, R + Rc_sz * labels[day], q + TN * day, x + TL * day, sched_eta[k], rd, rf, g);
+        }
+}
+
+// O4: Rayleigh quotient of rho_c^T rho_c after `iters` power iterations from all-ones, in double.
+double oracle_power_iteration(int N, int L, int T, int H, const float* Rc, int iters) {
+    Dims d{N, L, T, H};
+    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<double> u(TN, 1.0), v(TL), w(TN);
+    double lam = 0.0;
+    for (int it = 0; it < iters; ++it) {
+        double nu = 0.0;
+        for (double a : u) nu += a * a;
+        nu = std::sqrt(nu);
+        for (double& a : u) a /= nu;
+        // v = rho u
+        for (int t = 0; t < T; ++t)
+            for (int l = 0; l < L; ++l) {
+                double acc = 0.0;
+                const int hmax = H < t ? H : t;
+                for (int h = 0; h <= hmax; ++h) {
+                    const float* row = Rc + blk(d, t - h, h) + (size_t)l * N;
+                    const double* us = u.data() + (size_t)(t - h) * N;
+                    for (int n = 0; n < N; ++n) acc += (double)row[n] * us[n];
+                }
+                v[(size_t)t * L + l] = acc;
+            }
+        lam = 0.0;
+        for (double a : v) lam += a * a;          // u^T rho^T rho u with |u| = 1
+        // w = rho^T v
+        for (int s = 0; s < T; ++s)
+            for (int n = 0; n < N; ++n) {
+                double acc = 0.0;
+                const int hmax = H < T - 1 - s ? H : T - 1 - s;
+                for (int h = 0; h <= hmax; ++h) {
+                    const float* B = Rc + blk(d, s, h);
+                    const double* vt = v.data() + (size_t)(s + h) * L;
+                    for (int l = 0; l < L; ++l) acc += (double)B[(size_t)l * N + n] * vt[l];
+                }
+                w[(size_t)s * N + n] = acc;
+            }
+        u = w;
+    }
+    return lam;
+}
+
+// ---- a6: the same O2a-O2c with R_c given as CSR per (s,h) block ("coordinate format
+// sparse representation"; Table 2 "Sparse").
+// blk_off[(s*(H+1)+h)] = first nnz of block (s,h) (int64, T*(H+1)+1 entries, for this cluster);
+// row_ptr[(s*(H+1)+h)*(L+1) + l] = offset of row l relative to the block start; col = OD index n.
+void oracle_visit_csr(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
+                      const int32_t* col_idx, const float* val, float* q, const float* x, float eta) {
+    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<float> rf(TL);
+    std::vector<double> g(TN, 0.0);
+    for (int t = 0; t < T; ++t)
+        for (int l = 0; l < L; ++l) {
+            double acc = 0.0;
+            const int hmax = H < t ? H : t;
+            for (int h = 0; h <= hmax; ++h) {
+                const size_t b = (size_t)(t - h) * (H + 1) + h;
+                const int32_t* rp = row_ptr + b * (L + 1);
+                for (int64_t k = blk_off[b] + rp[l]; k < blk_off[b] + rp[l + 1]; ++k)
+                    acc += (double)val[k] * (double)q[(size_t)(t - h) * N + col_idx[k]];
+            }
+            rf[(size_t)t * L + l] = (float)(acc - (double)x[(size_t)t * L + l]);
+        }
+    for (int s = 0; s < T; ++s) {
+        const int hmax = H < T - 1 - s ? H : T - 1 - s;
+        for (int h = 0; h <= hmax; ++h) {
+            const size_t b = (size_t)s * (H + 1) + h;
+            const int32_t* rp = row_ptr + b * (L + 1);
+            for (int l = 0; l < L; ++l)
+                for (int64_t k = blk_off[b] + rp[l]; k < blk_off[b] + rp[l + 1]; ++k)
+                    g[(size_t)s * N + col_idx[k]] += (double)val[k] * (double)rf[(size_t)(s + h) * L + l];
+        }
+    }
+    for (size_t i = 0; i < TN; ++i) {
+        const double v = (double)q[i] - (double)eta * g[i];
+        q[i] = (float)(v > 0.0 ? v : 0.0);
+    }
+}
+
+double oracle_objective_day_csr(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
+                                const int32_t* col_idx, const float* val, const float* q, const float* x) {
+    double f = 0.0;
+    for (int t = 0; t < T; ++t)
+        for (int l = 0; l < L; ++l) {
+            double acc = 0.0;
+            const int hmax = H < t ? H : t;
+            for (int h = 0; h <= hmax; ++h) {
+                const size_t b = (size_t)(t - h) * (H + 1) + h;
+                const int32_t* rp = row_ptr + b * (L + 1);
+                for (int64_t k = blk_off[b] + rp[l]; k < blk_off[b] + rp[l + 1]; ++k)
+                    acc += (double)val[k] * (double)q[(size_t)(t - h) * N + col_idx[k]];
+            }
+            const double r = acc - (double)x[(size_t)t * L + l];
+            f += r * r;
+        }
+    return f;
+}
+
+}  // extern "C"

@@ -1,0 +1,281 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+None of these touch the CUDA path.  Each test names the mistake it would catch."""
+import os
+
+import numpy as np
+import pytest
+import scipy.optimize
+import torch
+
+from oracle import oracle
+from paper_1901_09266_b200 import synth
+from tests.nnls_active_set import nnls_lawson_hanson
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def assemble_dense(Rc: np.ndarray) -> np.ndarray:
+    """Table 2: entry [(h2-1)|A|+a, (h1-1)|K|+k] of the (T*L) x (T*N) matrix,
+    block (h2,h1) = R[h1][h2-h1]; no block beyond the day.  0-based here."""
+    T, H1, L, N = Rc.shape
+    B = np.zeros((T * L, T * N), np.float64)
+    for h1 in range(T):
+        for lag in range(H1):
+            h2 = h1 + lag
+            if h2 < T:
+                B[h2 * L:(h2 + 1) * L, h1 * N:(h1 + 1) * N] = Rc[h1, lag]
+    return B
+
+
+@pytest.fixture(scope="module")
+def tiny12():
+    cfg = synth.CONFIGS["tiny12"]
+    R = synth.dar_dense(cfg)
+    lab = synth.labels(cfg)
+    qt = synth.q_true(cfg)
+    x = synth.counts(cfg, R, qt, lab, noise=True)
+    x0 = synth.counts(cfg, R, qt, lab, noise=False)
+    return cfg, R.numpy(), lab.numpy(), qt.numpy(), x.numpy(), x0.numpy()
+
+
+def converge(Rc, x_day, eta, iters, q0=None):
+    T, H1, L, N = Rc.shape
+    q = np.ones((1, T, N), np.float32) if q0 is None else q0.reshape(1, T, N)
+    sched = [(0, np.array([0], np.int32))] * iters
+    return oracle.run_schedule(Rc[None], np.zeros(1, np.int32), x_day[None], q, sched, [eta] * iters)[0]
+
+
+def test_p7_generator_invariants(tiny12):
+    """Eq. 17-18: lag fractions of a covered (s,l,n) sum to 1, others are 0, all >= 0."""
+    cfg, R, *_ = tiny12
+    mask = synth.incidence_mask(cfg).numpy()
+    tot = R[0].sum(axis=1)                      # [T][L][N]
+    assert (R >= 0).all()
+    np.testing.assert_allclose(tot[:, mask], 1.0, atol=1e-5)
+    assert (tot[:, ~mask] == 0).all()
+    k = mask.sum(axis=0)
+    assert k.min() >= cfg.kmin and k.max() <= cfg.kmax
+
+
+def test_p12_dense_assembly(tiny12):
+    """Operator indexing: O2a/O2b equal the plain mat-vec with Table 2's assembled matrix."""
+    cfg, R, lab, qt, x, _ = tiny12
+    Rc = R[0]
+    B = assemble_dense(Rc)
+    rng = np.random.default_rng(1)
+    q = rng.random((cfg.T, cfg.N)).astype(np.float32) * 30
+    r = oracle.forward_residual(Rc, q, x[3])
+    ref = B @ q.reshape(-1).astype(np.float64) - x[3].reshape(-1)
+    np.testing.assert_allclose(r.reshape(-1), ref, rtol=1e-6, atol=1e-5)
+    g = oracle.gradient(Rc, r)
+    np.testing.assert_allclose(g.reshape(-1), B.T @ r.reshape(-1).astype(np.float64), rtol=1e-12, atol=1e-9)
+    assert abs(oracle.objective_day(Rc, q, x[3]) - float(ref @ ref)) <= 1e-10 * float(ref @ ref)
+
+
+def test_p12_dense_assembly_full_tiny():
+    """Same on config 0 itself (T=288): catches a wrong truncation at either end of the day."""
+    cfg = synth.CONFIGS["tiny"]
+    Rc = synth.dar_dense(cfg).numpy()[0]
+    B = assemble_dense(Rc)
+    rng = np.random.default_rng(2)
+    q = rng.random((cfg.T, cfg.N)).astype(np.float32)
+    x = rng.random((cfg.T, cfg.L)).astype(np.float32)
+    r = oracle.forward_residual(Rc, q, x)
+    np.testing.assert_allclose(r.reshape(-1), B @ q.reshape(-1).astype(np.float64) - x.reshape(-1), atol=1e-6)
+    np.testing.assert_allclose(oracle.gradient(Rc, r).reshape(-1), B.T @ r.reshape(-1).astype(np.float64), atol=1e-9)
+
+
+def test_p6_example1_two_link():
+    """PAPER.md:114-124 Example 1: x1(t)=f(t), x2(t+dt)=f(t), x2(t0)=0 — pins lag direction, day-boundary
+    truncation (A5), the gradient factor convention (A1) and the projection."""
+    rows = {}
+    for line in open(os.path.join(GOLD, "example1_two_link.txt")):
+        if line.startswith("#") or ":" not in line:
+            continue
+        k, v = line.split(":")
+        rows[k.strip()] = np.array(v.split(), np.float32)
+    f1, x1, x2 = rows["f1"], rows["x1"], rows["x2"]
+    T = len(f1)
+    Rc = np.zeros((T, 2, 2, 1), np.float32)      # N=1, L=2, H=1
+    Rc[:, 0, 0, 0] = 1.0                          # lag 0 -> link 1
+    Rc[:, 1, 1, 0] = 1.0                          # lag 1 -> link 2
+    fwd = oracle.forward_residual(Rc, f1.reshape(T, 1), np.zeros((T, 2), np.float32))
+    np.testing.assert_array_equal(fwd[:, 0], x1)
+    np.testing.assert_array_equal(fwd[:, 1], x2)
+    # rho^T rho = diag(2,...,2,1) => L = 2, eta = 1/2: one step lands on (x1[s]+x2[s+1])/2, last entry halves its error.
+    assert abs(oracle.power_iteration(Rc, 200) - 2.0) < 1e-6
+    x = np.stack([x1, x2], axis=1)
+    q0 = np.array([7, 0, 2, 30, 1, 4], np.float32).reshape(T, 1)
+    q1 = oracle.visit(Rc, q0, x, 0.5)
+    expect = np.maximum(0, np.append((x1[:-1] + x2[1:]) / 2, (q0[-1, 0] + x1[-1]) / 2))
+    np.testing.assert_allclose(q1[:, 0], expect, rtol=1e-7)
+    # projection: a target that is negative must clamp to exactly 0
+    xneg = x.copy(); xneg[2, 0] = -50.0
+    assert oracle.visit(Rc, q0, xneg, 0.5)[2, 0] == 0.0
+
+
+def test_p5_degenerate_closed_form():
+    """T=1, H=0 reduces to textbook projected gradient; with the constraint inactive
+    q_k - q* = (I - eta B^T B)^k (q_0 - q*)."""
+    B = np.array([[2.0, 0.5, 0.1], [0.3, 1.5, 0.2], [0.1, 0.4, 1.0]], np.float32)
+    qstar = np.array([4.0, 5.0, 6.0])
+    y = (B.astype(np.float64) @ qstar).astype(np.float32)
+    Rc = B.reshape(1, 1, 3, 3)
+    eta = 0.15
+    q = np.array([[5.0, 4.0, 7.0]], np.float32)
+    M = np.eye(3) - eta * B.astype(np.float64).T @ B.astype(np.float64)
+    qs64 = np.linalg.solve(B.astype(np.float64), y.astype(np.float64))
+    e0 = q[0].astype(np.float64) - qs64
+    for k in range(1, 21):
+        q = oracle.visit(Rc, q, y.reshape(1, 3), eta)
+        np.testing.assert_allclose(q[0], qs64 + np.linalg.matrix_power(M, k) @ e0, rtol=2e-6)
+
+
+def test_p8_adjoint(tiny12):
+    """<rho u, v> = <u, rho^T v>: the transpose loop is the adjoint of the forward loop, truncation included."""
+    cfg, R, *_ = tiny12
+    rng = np.random.default_rng(3)
+    for Rc in (R[0], synth.dar_dense(synth.CONFIGS["tiny"]).numpy()[0][:40]):
+        T, H1, L, N = Rc.shape
+        u = rng.standard_normal((T, N)).astype(np.float32)
+        v = rng.standard_normal((T, L)).astype(np.float32)
+        ru = oracle.forward_residual(Rc, u, np.zeros((T, L), np.float32)).astype(np.float64)
+        rtv = oracle.gradient(Rc, v)
+        lhs, rhs = float((ru * v).sum()), float((u.astype(np.float64) * rtv).sum())
+        assert abs(lhs - rhs) <= 1e-5 * max(1.0, abs(lhs))
+
+
+def test_p3_finite_differences(tiny12):
+    """d f / d q = 2 g (reading A1): f is quadratic, so central differences are exact up to rounding."""
+    cfg, R, lab, qt, x, _ = tiny12
+    Rc = R[0]
+    rng = np.random.default_rng(4)
+    q = (rng.random((cfg.T, cfg.N)) * 40).astype(np.float32)
+    g = oracle.gradient(Rc, oracle.forward_residual(Rc, q, x[0]))
+    delta = 0.5
+    for (s, n) in [(0, 0), (3, 2), (7, 1), (11, 3), (5, 0)]:
+        qp, qm = q.copy(), q.copy()
+        qp[s, n] += delta
+        qm[s, n] -= delta
+        fd = (oracle.objective_day(Rc, qp, x[0]) - oracle.objective_day(Rc, qm, x[0])) / (2 * delta)
+        assert abs(fd - 2 * g[s, n]) <= 1e-5 * max(1.0, abs(fd))
+
+
+def _eta(Rc):
+    return np.float32(1.0 / oracle.power_iteration(Rc, 50))
+
+
+def test_power_iteration_matches_eigensolver(tiny12):
+    """O4 against numpy's symmetric eigensolver on the assembled Gram matrix."""
+    cfg, R, *_ = tiny12
+    B = assemble_dense(R[0])
+    lam = np.linalg.eigvalsh(B.T @ B)[-1]
+    est = oracle.power_iteration(R[0], 50)
+    assert est <= lam * (1 + 1e-12) and est >= 0.98 * lam
+    assert abs(oracle.power_iteration(R[0], 3000) - lam) <= 1e-6 * lam
+
+
+def test_p1_p2_active_set_and_kkt(tiny12):
+    """T=12 sub-instance (48 unknowns, 72 equations): the oracle iterated to convergence equals the
+    Lawson-Hanson solve (own implementation and scipy's), and satisfies KKT."""
+    cfg, R, lab, qt, x, _ = tiny12
+    Rc = R[0]
+    B = assemble_dense(Rc)
+    np.linalg.cholesky(B.T @ B)                       # Gram matrix must be PD (generator contract, G2)
+    ev = np.linalg.eigvalsh(B.T @ B)
+    assert ev[-1] / ev[0] < 1e4                       # synth.TINY_REDRAW was chosen for this
+    eta = _eta(Rc)
+    for day in (0, 5):
+        y = x[day].reshape(-1).astype(np.float64)
+        q_lh = nnls_lawson_hanson(B, y)
+        q_sp, _ = scipy.optimize.nnls(B, y, maxiter=10000)
+        np.testing.assert_allclose(q_lh, q_sp, atol=1e-8)
+        q = converge(Rc, x[day], eta, 60000)
+        g = oracle.gradient(Rc, oracle.forward_residual(Rc, q, x[day]))
+        eps = 1e-4 * np.abs(B.T @ y).max()             # A14
+        assert (g[q == 0] >= -eps).all()
+        assert (np.abs(g[q > 0]) <= eps).all()
+        f_or = oracle.objective_day(Rc, q, x[day])
+        f_lh = float(np.sum((B @ q_lh - y) ** 2))
+        assert f_or >= f_lh * (1 - 1e-9) and f_or <= f_lh * (1 + 1e-6)
+        np.testing.assert_allclose(q.reshape(-1), q_lh, atol=5e-3, rtol=1e-4)
+
+
+def test_p4_planted_recovery(tiny12):
+    """Fig. 12 protocol: x = rho q_true noiseless => f -> 0 and q -> q_true (full column rank)."""
+    cfg, R, lab, qt, _, x0 = tiny12
+    Rc = R[0]
+    q = converge(Rc, x0[2], _eta(Rc), 200000)
+    f0 = oracle.objective_day(Rc, np.ones_like(qt[2]), x0[2])
+    assert oracle.objective_day(Rc, q, x0[2]) <= 1e-8 * f0
+    np.testing.assert_allclose(q, qt[2], rtol=5e-3, atol=5e-3)
+
+
+def test_p9_monotone_descent(tiny12):
+    """Projected gradient with eta <= 1/L never increases the objective."""
+    cfg, R, lab, qt, x, _ = tiny12
+    Rc = R[0]
+    eta = _eta(Rc)
+    q = np.ones((cfg.T, cfg.N), np.float32)
+    f = oracle.objective_day(Rc, q, x[1])
+    for _ in range(200):
+        q = oracle.visit(Rc, q, x[1], eta)
+        f2 = oracle.objective_day(Rc, q, x[1])
+        assert f2 <= f * (1 + 1e-7)
+        f = f2
+
+
+def test_p10_separability_and_schedule(tiny12):
+    """A day's iterate depends only on its visit count: minibatch composition, and a day mask, change nothing."""
+    cfg, R, lab, qt, x, _ = tiny12
+    eta = _eta(R[0])
+    sched = synth.schedule(cfg, lab, K=60)
+    for c, days in sched:
+        assert len(set(days.tolist())) == len(days) <= cfg.b and all(lab[d] == c for d in days)
+    q0 = np.ones((cfg.D, cfg.T, cfg.N), np.float32)
+    qa = oracle.run_schedule(R, lab, x, q0, sched, [eta] * len(sched))
+    single = [(c, np.array([d], np.int32)) for c, days in sched for d in days]      # b = 1, same visits
+    qb = oracle.run_schedule(R, lab, x, q0, single, [eta] * len(single))
+    np.testing.assert_array_equal(qa, qb)
+    mask = np.zeros(cfg.D, np.uint8); mask[[2, 9]] = 1
+    qc = oracle.run_schedule(R, lab, x, q0, sched, [eta] * len(sched), day_mask=mask)
+    np.testing.assert_array_equal(qc[[2, 9]], qa[[2, 9]])
+    np.testing.assert_array_equal(qc[0], q0[0])
+    visits = np.bincount(np.concatenate([d for _, d in sched]), minlength=cfg.D)
+    q5 = q0[5]
+    for _ in range(visits[5]):
+        q5 = oracle.visit(R[0], q5, x[5], eta)
+    np.testing.assert_array_equal(q5, qa[5])
+
+
+def test_schedule_epoch_structure():
+    """A8: per epoch every day appears exactly once; chunks are same-cluster, <= b, ragged tails kept."""
+    cfg = synth.CONFIGS["corridor"]
+    lab = synth.labels(cfg).numpy()
+    ep = synth.one_epoch(cfg, lab)
+    alld = np.concatenate([d for _, d in ep])
+    assert sorted(alld.tolist()) == list(range(cfg.D))
+    assert len(ep) == sum(-(-int((lab == c).sum()) // cfg.b) for c in range(cfg.C))
+    s1, s2 = synth.schedule(cfg, lab, K=37), synth.schedule(cfg, lab, K=37)
+    assert all(a[0] == b[0] and (a[1] == b[1]).all() for a, b in zip(s1, s2)) and len(s1) == 37
+    full = synth.schedule(cfg, lab, K=20, full_only=True)
+    assert all(len(d) == cfg.b for _, d in full)
+
+
+def test_p13_dense_vs_csr(tiny12):
+    """a6: the CSR visit equals the dense visit on the same operator."""
+    cfg, R, lab, qt, x, _ = tiny12
+    csr = synth.dense_to_csr(torch.from_numpy(R))
+    assert csr.nnz == int((R != 0).sum())
+    eta = _eta(R[0])
+    q = np.ones((cfg.T, cfg.N), np.float32)
+    qd, qs = q, q
+    for _ in range(5):
+        qd = oracle.visit(R[0], qd, x[4], eta)
+        qs = oracle.visit_csr(cfg.N, cfg.L, cfg.T, cfg.H, csr.blk_off.numpy(), csr.row_ptr.numpy(),
+                              csr.col_idx.numpy(), csr.val.numpy(), qs, x[4], eta)
+    np.testing.assert_allclose(qs, qd, rtol=1e-6, atol=1e-6)
+    fd = oracle.objective_day(R[0], qd, x[4])
+    fs = oracle.objective_day_csr(cfg.N, cfg.L, cfg.T, cfg.H, csr.blk_off.numpy(), csr.row_ptr.numpy(),
+                                  csr.col_idx.numpy(), csr.val.numpy(), qd, x[4])
+    assert abs(fd - fs) <= 1e-12 * fd
