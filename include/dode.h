@@ -1,0 +1,125 @@
+/* dode.h — C ABI of the B200-native SPGD/NNLS hot path of Ma & Qian (arXiv 1901.09266).
+ *
+ * The library solves, day by day, the non-negative least squares problem
+ *     min  sum_d || rho_{c(d)} q_d - x_d ||^2   s.t.  q_d >= 0          (Eq. 40/42)
+ * by stochastic projected gradient descent (Alg. 1) with the re-scoping of
+ * BASELINE.json:north_star (minibatch = days of one cluster; plain projected step; one DAR
+ * operator per cluster — DESIGN.md readings A2, A3, A7).
+ *
+ * Notation: N OD pairs, L observed links, T intervals per day, H max lag,
+ * C clusters, D days.  R[c][s][h] is the L x N block that maps departures in interval s to link
+ * counts in interval s+h (Table 2: rho entry [(h2-1)|A|+a, (h1-1)Pi+k] with
+ * s = h1-1, h = h2-h1).  Blocks with s+h >= T may be present; they are ignored.
+ *
+ * Conventions: plain C types; every function returns DODE_OK (0) or a negative dode_status;
+ * nothing is written to stdout/stderr; no global state; no CPU fallback — every call fails with
+ * DODE_ECUDA if no usable sm_100 device/context exists.  "device" pointers are CUDA device
+ * pointers valid in the current context (e.g. torch-allocated); "host" pointers are ordinary
+ * host memory.  All work is issued on the stream given to dode_create.  A sticky CUDA error is
+ * reported by the next synchronising call.
+ */
+#ifndef DODE_H_
+#define DODE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dode_ctx dode_ctx;
+
+typedef enum dode_status {
+    DODE_OK = 0,
+    DODE_EINVAL = -1,  /* bad argument; state untouched */
+    DODE_ENOMEM = -2,  /* device or host allocation failed */
+    DODE_ECUDA = -3    /* CUDA runtime error (text in dode_last_error) */
+} dode_status;
+
+enum { DODE_DENSE = 0, DODE_CSR = 1 };
+
+typedef struct dode_dims {
+    int32_t N, L, T, H, C, D;
+    int32_t storage; /* DODE_DENSE or DODE_CSR */
+} dode_dims;
+
+/* The DAR operator of every cluster (the paper's assignment matrix B = delta.rho.p, Eq. 41,
+ * PAPER.md:337-340, shared by a cluster's days).
+ *   DENSE: dense = device fp32 [C][T][H+1][L][N], n fastest.
+ *   CSR  : per (c,s,h) block, rows = links, columns = OD pairs, blocks concatenated in [c][s][h]
+ *          order ("coordinate format sparse representation"):
+ *            blk_off  device int64 [C*T*(H+1) + 1]  first nnz of each block (blk_off[last] = nnz)
+ *            row_ptr  device int32 [C*T*(H+1)][L+1]  row offsets relative to the block start
+ *            col_idx  device int32 [nnz]             OD index n, ascending within a row
+ *            val      device fp32  [nnz]
+ * The library copies/re-packs what it needs during dode_create and keeps no caller pointer. */
+typedef struct dode_dar {
+    const float* dense;
+    const int64_t* blk_off;
+    const int32_t* row_ptr;
+    const int32_t* col_idx;
+    const float* val;
+    int64_t nnz;
+} dode_dar;
+
+/* a0: store R, labels, x; q[d][s][n] <- q0 ("Initialize x", Alg. 1 line 3).
+ *   labels  host   int32 [D], each in [0, C)
+ *   x       device fp32  [D][T][L]  (Table 2 link-flow order: entry t*L + l)
+ *   stream  cudaStream_t (NULL = legacy default stream)
+ * On failure *out is NULL. */
+int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const int32_t* labels,
+                const float* x, float q0, void* stream);
+
+/* a1-a4: one SPGD iteration on the listed days (Alg. 1 lines 8-11):
+ *   r = rho_c Q_B - X_B ;  g = rho_c^T r ;  q_d <- max(0, q_d - eta g_d)  for d in days.
+ *   days  host int32 [n]; all in [0, D), distinct, same cluster — else DODE_EINVAL, state untouched.
+ * Asynchronous on the ctx stream; no host synchronisation, no device->host traffic. */
+int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta);
+
+/* The same iteration for a streaming caller (bench.py's end-to-end leg): first uploads the n days'
+ * counts from x_host ([n][T][L], host, pinned or pageable), runs the step, then downloads the n
+ * days' updated q into q_host ([n][T][N], host) and synchronises. */
+int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta,
+                        const float* x_host, float* q_host);
+
+/* a5: f_d = sum_t sum_l r_d[t][l]^2 — no 1/2, no mean (Eq. 42).
+ *   days     host int32 [n], or NULL for all D days (then n is ignored); any mix of clusters
+ *   per_day  host double [n] (or [D]), nullable
+ *   total    host double, nullable
+ * fp32 products, fp64 sums.  Synchronises. */
+int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_day, double* total);
+
+/* Export / import one day's state in Table 2 order (entry s*N + n).
+ * out/in: fp32 [T][N]; is_device != 0 means a device pointer.  Synchronises. */
+int dode_get_q(dode_ctx* ctx, int32_t day, float* out, int32_t is_device);
+int dode_set_q(dode_ctx* ctx, int32_t day, const float* in, int32_t is_device);
+
+/* v = rho_c u and u = rho_c^T v through the production kernels with minibatch 1.
+ *   u device fp32 [T][N];  v device fp32 [T][L].  Asynchronous on the ctx stream. */
+int dode_apply(dode_ctx* ctx, int32_t c, const float* u, float* v);
+int dode_apply_t(dode_ctx* ctx, int32_t c, const float* v, float* u);
+
+/* a7: L_c ~ lambda_max(rho_c^T rho_c): Rayleigh quotient after `iters` power iterations from the
+ * all-ones vector, run through dode_apply/dode_apply_t's kernels (fp32 products, fp64 norms).
+ * eta_c = 1/L_c is the step "dependent on the problem scale".  Synchronises. */
+int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out);
+
+/* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
+int64_t dode_launch_count(const dode_ctx* ctx);
+
+/* Which kernel family the last dode_spgd_step used, e.g. "ffma_rowdot_bt8+ffma_coldot_bt8". */
+const char* dode_last_path(const dode_ctx* ctx);
+
+/* Wait for all work issued on the ctx stream; returns a pending CUDA error if any. */
+int dode_sync(dode_ctx* ctx);
+
+void dode_destroy(dode_ctx* ctx);
+
+/* Text of the last error on this ctx ("" if none).  With ctx == NULL: the text of the last
+ * failed dode_create on this thread. */
+const char* dode_last_error(const dode_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DODE_H_ */

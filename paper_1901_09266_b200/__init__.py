@@ -1,0 +1,197 @@
+"""paper_1901_09266_b200 — B200-native SPGD/NNLS hot path of Ma & Qian (arXiv 1901.09266).
+
+Thin ctypes binding over the C ABI of ``include/dode.h`` (argument marshalling only: every step
+of the path runs in the library's CUDA kernels).  PyTorch supplies device memory and streams.
+There is no CPU fallback: if ``libdode.so`` is missing or fails to load, every call raises.
+``paper_1901_09266_b200.synth`` (seeded input generators) does not need the library.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "libdode.so")
+
+DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
+DODE_DENSE, DODE_CSR = 0, 1
+
+EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_objective", "dode_get_q", "dode_set_q",
+           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_launch_count", "dode_last_path", "dode_sync",
+           "dode_destroy", "dode_last_error"]
+
+
+class DodeError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"dode error {code}: {msg}")
+        self.code = code
+
+
+class dode_dims(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in ("N", "L", "T", "H", "C", "D", "storage")]
+
+
+class dode_dar(C.Structure):
+    _fields_ = [("dense", C.c_void_p), ("blk_off", C.c_void_p), ("row_ptr", C.c_void_p),
+                ("col_idx", C.c_void_p), ("val", C.c_void_p), ("nnz", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libdode.so (never builds, never falls back)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(SO_PATH):
+            raise ImportError(f"{SO_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(SO_PATH)
+        vp, i32, f32 = C.c_void_p, C.c_int32, C.c_float
+        L.dode_create.argtypes = [C.POINTER(vp), C.POINTER(dode_dims), C.POINTER(dode_dar), vp, vp, f32, vp]
+        L.dode_spgd_step.argtypes = [vp, vp, i32, f32]
+        L.dode_spgd_step_host.argtypes = [vp, vp, i32, f32, vp, vp]
+        L.dode_objective.argtypes = [vp, vp, i32, vp, vp]
+        L.dode_get_q.argtypes = [vp, i32, vp, i32]
+        L.dode_set_q.argtypes = [vp, i32, vp, i32]
+        L.dode_apply.argtypes = [vp, i32, vp, vp]
+        L.dode_apply_t.argtypes = [vp, i32, vp, vp]
+        L.dode_lipschitz.argtypes = [vp, i32, i32, vp]
+        L.dode_launch_count.argtypes = [vp]
+        L.dode_launch_count.restype = C.c_int64
+        L.dode_last_path.argtypes = [vp]
+        L.dode_last_path.restype = C.c_char_p
+        L.dode_sync.argtypes = [vp]
+        L.dode_destroy.argtypes = [vp]
+        L.dode_destroy.restype = None
+        L.dode_last_error.argtypes = [vp]
+        L.dode_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _chk(h, rc: int):
+    if rc != 0:
+        raise DodeError(rc, lib().dode_last_error(h).decode())
+
+
+def _days(days) -> np.ndarray:
+    return np.ascontiguousarray(days, dtype=np.int32)
+
+
+def _dev(t, dtype, what):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TypeError(f"{what} must be a contiguous CUDA tensor of {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def dode_create(N: int, L: int, T: int, H: int, Cn: int, D: int, labels, x, q0: float = 1.0, *,
+                dense=None, csr=None, stream: Optional[int] = None):
+    """a0.  ``dense``: CUDA fp32 [C][T][H+1][L][N]; or ``csr``: object with CUDA tensors blk_off (int64),
+    row_ptr (int32), col_idx (int32), val (fp32).  ``labels``: host int32 [D].  ``x``: CUDA fp32 [D][T][L].
+    ``stream``: raw cudaStream_t (default: torch's current stream).  Returns an opaque handle."""
+    import torch
+    if (dense is None) == (csr is None):
+        raise ValueError("give exactly one of dense= or csr=")
+    dar = dode_dar()
+    if dense is not None:
+        if tuple(dense.shape) != (Cn, T, H + 1, L, N):
+            raise ValueError(f"dense R has shape {tuple(dense.shape)}, expected {(Cn, T, H + 1, L, N)}")
+        dar.dense = _dev(dense, torch.float32, "dense").value
+        storage = DODE_DENSE
+    else:
+        dar.blk_off = _dev(csr.blk_off, torch.int64, "blk_off").value
+        dar.row_ptr = _dev(csr.row_ptr, torch.int32, "row_ptr").value
+        dar.col_idx = _dev(csr.col_idx, torch.int32, "col_idx").value
+        dar.val = _dev(csr.val, torch.float32, "val").value
+        dar.nnz = int(csr.val.numel())
+        storage = DODE_CSR
+    if tuple(x.shape) != (D, T, L):
+        raise ValueError(f"x has shape {tuple(x.shape)}, expected {(D, T, L)}")
+    lab = np.ascontiguousarray(labels, dtype=np.int32)
+    if lab.shape != (D,):
+        raise ValueError("labels must have D entries")
+    dims = dode_dims(N, L, T, H, Cn, D, storage)
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    h = C.c_void_p()
+    rc = lib().dode_create(C.byref(h), C.byref(dims), C.byref(dar), lab.ctypes.data, _dev(x, torch.float32, "x"),
+                           C.c_float(q0), C.c_void_p(stream))
+    if rc != 0:
+        raise DodeError(rc, lib().dode_last_error(None).decode())
+    return h
+
+
+def dode_spgd_step(h, days, eta: float) -> None:
+    """a1-a4: one SPGD iteration on ``days`` (host ints, distinct, one cluster).  Asynchronous."""
+    d = _days(days)
+    _chk(h, lib().dode_spgd_step(h, d.ctypes.data, d.size, C.c_float(eta)))
+
+
+def dode_spgd_step_host(h, days, eta: float, x_host, q_host) -> None:
+    """Streaming step: uploads the days' counts from ``x_host`` ([n][T][L] CPU tensor, ideally pinned),
+    steps, downloads their q into ``q_host`` ([n][T][N] CPU tensor) and synchronises."""
+    d = _days(days)
+    _chk(h, lib().dode_spgd_step_host(h, d.ctypes.data, d.size, C.c_float(eta),
+                                      C.c_void_p(x_host.data_ptr()), C.c_void_p(q_host.data_ptr())))
+
+
+def dode_objective(h, days):
+    """a5: returns (per_day float64 array, total) for the listed days (any mix of clusters)."""
+    d = _days(days)
+    per = np.empty(d.size, np.float64)
+    tot = C.c_double()
+    _chk(h, lib().dode_objective(h, d.ctypes.data, d.size, per.ctypes.data, C.byref(tot)))
+    return per, tot.value
+
+
+def dode_get_q(h, day: int, out) -> None:
+    """Copies day's q ([T][N], Table 2 order) into ``out`` (CPU or CUDA fp32 tensor, contiguous)."""
+    _chk(h, lib().dode_get_q(h, day, C.c_void_p(out.data_ptr()), 1 if out.is_cuda else 0))
+
+
+def dode_set_q(h, day: int, src) -> None:
+    _chk(h, lib().dode_set_q(h, day, C.c_void_p(src.data_ptr()), 1 if src.is_cuda else 0))
+
+
+def dode_apply(h, c: int, u, v) -> None:
+    """v = rho_c u   (u CUDA fp32 [T][N], v CUDA fp32 [T][L])."""
+    import torch
+    _chk(h, lib().dode_apply(h, c, _dev(u, torch.float32, "u"), _dev(v, torch.float32, "v")))
+
+
+def dode_apply_t(h, c: int, v, u) -> None:
+    """u = rho_c^T v."""
+    import torch
+    _chk(h, lib().dode_apply_t(h, c, _dev(v, torch.float32, "v"), _dev(u, torch.float32, "u")))
+
+
+def dode_lipschitz(h, c: int, iters: int = 50) -> float:
+    """a7: L_c ~ lambda_max(rho_c^T rho_c) by power iteration through the production kernels."""
+    out = C.c_double()
+    _chk(h, lib().dode_lipschitz(h, c, iters, C.byref(out)))
+    return out.value
+
+
+def dode_launch_count(h) -> int:
+    return int(lib().dode_launch_count(h))
+
+
+def dode_last_path(h) -> str:
+    return lib().dode_last_path(h).decode()
+
+
+def dode_sync(h) -> None:
+    _chk(h, lib().dode_sync(h))
+
+
+def dode_destroy(h) -> None:
+    lib().dode_destroy(h)
+
+
+def dode_last_error(h) -> str:
+    return lib().dode_last_error(h).decode()

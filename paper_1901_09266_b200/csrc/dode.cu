@@ -1,0 +1,456 @@
+// C ABI (include/dode.h) and host logic of the DODE SPGD library.  sm_100a only; no CPU fallback.
+#include "../../include/dode.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels_dense.cuh"
+#include "kernels_csr.cuh"
+
+using namespace dode;
+
+struct dode_ctx {
+    dode_dims dm{};
+    int Np = 0, N4 = 0;
+    cudaStream_t stream = nullptr;
+    // dense storage
+    float* R = nullptr;          // [C][T][H+1][L][Np]
+    // CSR storage (a6)
+    CsrStore csr{};
+    // state
+    float* q = nullptr;          // [D][T][Np]
+    float* x = nullptr;          // [D][T][L]
+    float* r = nullptr;          // [T][L][bp] scratch
+    size_t r_cap = 0;            // floats
+    double* d_part = nullptr;    // objective partials
+    size_t part_cap = 0;
+    double* d_obj = nullptr;     // [D] per-day objective + 2 scalars
+    float *pu = nullptr, *pv = nullptr, *pw = nullptr;   // apply / power-iteration scratch
+    std::vector<int32_t> labels;
+    std::vector<int32_t> stamp;  // distinctness check
+    int32_t stamp_id = 0;
+    int64_t launches = 0;
+    std::string path;
+    char err[512] = {0};
+    bool sm_opt_in[8] = {false};
+};
+
+static thread_local char g_create_err[512] = {0};
+
+static int fail(dode_ctx* c, int code, const char* fmt, ...) {
+    char* dst = c ? c->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                              \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? DODE_ENOMEM : DODE_ECUDA,      \
+                        "%s: %s", #call, cudaGetErrorString(e_));                             \
+    } while (0)
+
+static inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
+
+static int ensure_r(dode_ctx* ctx, size_t floats) {
+    if (ctx->r_cap >= floats) return DODE_OK;
+    if (ctx->r) { CU(cudaStreamSynchronize(ctx->stream)); CU(cudaFree(ctx->r)); ctx->r = nullptr; ctx->r_cap = 0; }
+    CU(cudaMalloc(&ctx->r, floats * sizeof(float)));
+    ctx->r_cap = floats;
+    return DODE_OK;
+}
+
+static int pick_bt(int n) { return n <= 1 ? 1 : n <= 2 ? 2 : n <= 4 ? 4 : n <= 8 ? 8 : 16; }
+
+// ---- dense launches ---------------------------------------------------------------------------
+template <int BT, int RL>
+static void launch_fwd(dode_ctx* ctx, const float* Rc, const float* qbase, size_t dayStride, const float* xbase,
+                       float* r, int bp, const DayList& dl) {
+    const dode_dims& d = ctx->dm;
+    dim3 grid(ceil_div(d.L, (kThreads / 32) * RL), d.T, bp / BT);
+    fwd_rowdot<BT, RL><<<grid, kThreads, 0, ctx->stream>>>(Rc, qbase, dayStride, xbase, r, ctx->N4, d.L, d.T, d.H, bp, dl);
+    ctx->launches++;
+}
+
+static void fwd_dense(dode_ctx* ctx, int bt, const float* Rc, const float* qbase, size_t dayStride,
+                      const float* xbase, float* r, int bp, const DayList& dl) {
+    switch (bt) {
+        case 1: launch_fwd<1, 8>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
+        case 2: launch_fwd<2, 8>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
+        case 4: launch_fwd<4, 8>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
+        case 8: launch_fwd<8, 4>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
+        default: launch_fwd<16, 2>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
+    }
+}
+
+template <int BT, bool UPDATE>
+static int launch_grad(dode_ctx* ctx, int slot, const float* Rc, const float* r, float* qbase, size_t dayStride,
+                       float* gout, float eta, int bp, const DayList& dl) {
+    const dode_dims& d = ctx->dm;
+    int cwlog2 = 0;
+    while ((1 << cwlog2) < ctx->N4 && cwlog2 < 5) ++cwlog2;
+    const size_t smem = (size_t)kThreads * 4 * BT * sizeof(float);
+    if (smem > 48 * 1024 && !ctx->sm_opt_in[slot]) {
+        CU(cudaFuncSetAttribute(grad_coldot<BT, UPDATE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ctx->sm_opt_in[slot] = true;
+    }
+    dim3 grid(ceil_div(ctx->N4, 1 << cwlog2), d.T, bp / BT);
+    grad_coldot<BT, UPDATE><<<grid, kThreads, smem, ctx->stream>>>(Rc, r, qbase, dayStride, gout, eta, d.N, ctx->N4,
+                                                                   d.L, d.T, d.H, bp, cwlog2, dl);
+    ctx->launches++;
+    return DODE_OK;
+}
+
+static int grad_dense(dode_ctx* ctx, int bt, const float* Rc, const float* r, float* qbase, size_t dayStride,
+                      float eta, int bp, const DayList& dl) {
+    switch (bt) {
+        case 1: return launch_grad<1, true>(ctx, 0, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
+        case 2: return launch_grad<2, true>(ctx, 1, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
+        case 4: return launch_grad<4, true>(ctx, 2, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
+        case 8: return launch_grad<8, true>(ctx, 3, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
+        default: return launch_grad<16, true>(ctx, 4, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
+    }
+}
+
+static const float* dense_cluster(const dode_ctx* ctx, int c) {
+    const dode_dims& d = ctx->dm;
+    return ctx->R + (size_t)c * d.T * (d.H + 1) * d.L * ctx->Np;
+}
+
+// forward residual of one sub-batch (<= kMaxDays days of cluster c) into ctx->r; returns bt/bp
+static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, const float* qbase, size_t dayStride,
+                         const float* xbase, float* r_out, int* bt_out, int* bp_out) {
+    const dode_dims& d = ctx->dm;
+    const int bt = pick_bt(dl.n), bp = ceil_div(dl.n, bt) * bt;
+    float* r = r_out;
+    if (!r) {
+        int rc = ensure_r(ctx, (size_t)d.T * d.L * bp);
+        if (rc) return rc;
+        r = ctx->r;
+    }
+    if (d.storage == DODE_DENSE) fwd_dense(ctx, bt, dense_cluster(ctx, c), qbase, dayStride, xbase, r, bp, dl);
+    else csr_forward(ctx->csr, c, bt, qbase, dayStride, xbase, r, bp, dl, d, ctx->Np, ctx->stream, &ctx->launches);
+    *bt_out = bt; *bp_out = bp;
+    return DODE_OK;
+}
+
+static int validate_days(dode_ctx* ctx, const int32_t* days, int32_t n, bool same_cluster, int* cluster) {
+    if (!days || n <= 0) return fail(ctx, DODE_EINVAL, "days is null or n <= 0");
+    const dode_dims& d = ctx->dm;
+    if (++ctx->stamp_id == INT32_MAX) { std::fill(ctx->stamp.begin(), ctx->stamp.end(), 0); ctx->stamp_id = 1; }
+    for (int i = 0; i < n; ++i) {
+        const int day = days[i];
+        if (day < 0 || day >= d.D) return fail(ctx, DODE_EINVAL, "day %d out of range [0,%d)", day, d.D);
+        if (ctx->stamp[day] == ctx->stamp_id) return fail(ctx, DODE_EINVAL, "day %d listed twice", day);
+        ctx->stamp[day] = ctx->stamp_id;
+        if (same_cluster && ctx->labels[day] != ctx->labels[days[0]])
+            return fail(ctx, DODE_EINVAL, "days %d and %d belong to different clusters", days[0], day);
+    }
+    if (cluster) *cluster = ctx->labels[days[0]];
+    return DODE_OK;
+}
+
+static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c) {
+    const dode_dims& d = ctx->dm;
+    const size_t dayStride = (size_t)d.T * ctx->Np;
+    for (int off = 0; off < n; off += kMaxDays) {       // days are independent units
+        DayList dl;
+        dl.n = std::min(kMaxDays, n - off);
+        std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
+        int bt, bp, rc;
+        if ((rc = forward_batch(ctx, c, dl, ctx->q, dayStride, ctx->x, nullptr, &bt, &bp))) return rc;
+        if (d.storage == DODE_DENSE) {
+            if ((rc = grad_dense(ctx, bt, dense_cluster(ctx, c), ctx->r, ctx->q, dayStride, eta, bp, dl))) return rc;
+            char buf[96];
+            snprintf(buf, sizeof buf, "ffma_rowdot_bt%d+ffma_coldot_bt%d", bt, bt);
+            ctx->path = buf;
+        } else {
+            csr_gradient(ctx->csr, c, bt, ctx->r, ctx->q, dayStride, nullptr, eta, bp, dl, d, ctx->Np, ctx->stream,
+                         &ctx->launches);
+            char buf[96];
+            snprintf(buf, sizeof buf, "csr_fwd_bt%d+csrT_grad_bt%d", bt, bt);
+            ctx->path = buf;
+        }
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(ctx, DODE_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
+    return DODE_OK;
+}
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+void dode_destroy(dode_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->R); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r);
+    cudaFree(ctx->d_part); cudaFree(ctx->d_obj); cudaFree(ctx->pu); cudaFree(ctx->pv); cudaFree(ctx->pw);
+    csr_free(ctx->csr);
+    delete ctx;
+}
+
+int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const int32_t* labels, const float* x,
+                float q0, void* stream) {
+    dode_ctx* ctx = nullptr;   // errors before allocation go to the thread-local buffer
+    if (!out) return fail(ctx, DODE_EINVAL, "out is null");
+    *out = nullptr;
+    if (!dims || !R || !labels || !x) return fail(ctx, DODE_EINVAL, "null argument");
+    const dode_dims d = *dims;
+    if (d.N < 1 || d.L < 1 || d.T < 1 || d.H < 0 || d.C < 1 || d.D < 1)
+        return fail(ctx, DODE_EINVAL, "dims must be positive (N=%d L=%d T=%d H=%d C=%d D=%d)", d.N, d.L, d.T, d.H, d.C, d.D);
+    if (d.storage != DODE_DENSE && d.storage != DODE_CSR) return fail(ctx, DODE_EINVAL, "unknown storage %d", d.storage);
+    if (d.storage == DODE_DENSE && !R->dense) return fail(ctx, DODE_EINVAL, "R->dense is null");
+    if (d.storage == DODE_CSR && (!R->blk_off || !R->row_ptr || (R->nnz > 0 && (!R->col_idx || !R->val)) || R->nnz < 0))
+        return fail(ctx, DODE_EINVAL, "CSR arrays are null or nnz < 0");
+    for (int i = 0; i < d.D; ++i)
+        if (labels[i] < 0 || labels[i] >= d.C) return fail(ctx, DODE_EINVAL, "labels[%d]=%d not in [0,%d)", i, labels[i], d.C);
+    int dev = 0, major = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return fail(ctx, DODE_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+    if (major != 10) return fail(ctx, DODE_ECUDA, "this library is built for sm_100a only (device is sm_%d0)", major);
+
+    dode_ctx* c = new (std::nothrow) dode_ctx();
+    if (!c) return fail(ctx, DODE_ENOMEM, "host allocation failed");
+    c->dm = d;
+    c->Np = (d.N + 3) / 4 * 4;
+    c->N4 = c->Np / 4;
+    c->stream = (cudaStream_t)stream;
+    c->labels.assign(labels, labels + d.D);
+    c->stamp.assign(d.D, 0);
+    ctx = c;
+#define CUC(call)                                                                                          \
+    do {                                                                                                   \
+        cudaError_t e_ = (call);                                                                           \
+        if (e_ != cudaSuccess) {                                                                           \
+            int code_ = fail(nullptr, e_ == cudaErrorMemoryAllocation ? DODE_ENOMEM : DODE_ECUDA, "%s: %s", \
+                             #call, cudaGetErrorString(e_));                                               \
+            dode_destroy(c);                                                                               \
+            cudaGetLastError();                                                                            \
+            return code_;                                                                                  \
+        }                                                                                                  \
+    } while (0)
+    const size_t TNp = (size_t)d.T * c->Np, TL = (size_t)d.T * d.L;
+    CUC(cudaMalloc(&c->q, (size_t)d.D * TNp * sizeof(float)));
+    CUC(cudaMalloc(&c->x, (size_t)d.D * TL * sizeof(float)));
+    CUC(cudaMalloc(&c->d_obj, ((size_t)d.D + 8) * sizeof(double)));
+    CUC(cudaMalloc(&c->pu, TNp * sizeof(float)));
+    CUC(cudaMalloc(&c->pv, TL * sizeof(float)));
+    CUC(cudaMalloc(&c->pw, (size_t)d.T * d.N * sizeof(float)));
+    CUC(cudaMemcpyAsync(c->x, x, (size_t)d.D * TL * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    fill_state<<<1184, 256, 0, c->stream>>>(c->q, (size_t)d.D * d.T, d.N, c->Np, q0);
+    c->launches++;
+    if (d.storage == DODE_DENSE) {
+        const size_t rows = (size_t)d.C * d.T * (d.H + 1) * d.L;
+        CUC(cudaMalloc(&c->R, rows * c->Np * sizeof(float)));
+        if (c->Np == d.N) {
+            CUC(cudaMemcpyAsync(c->R, R->dense, rows * d.N * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+        } else {
+            CUC(cudaMemsetAsync(c->R, 0, rows * c->Np * sizeof(float), c->stream));
+            CUC(cudaMemcpy2DAsync(c->R, c->Np * sizeof(float), R->dense, d.N * sizeof(float), d.N * sizeof(float), rows,
+                                  cudaMemcpyDeviceToDevice, c->stream));
+        }
+    } else {
+        int rc = csr_build(c->csr, d, *R, c->stream, g_create_err);
+        if (rc) { dode_destroy(c); cudaGetLastError(); return rc; }
+    }
+    CUC(cudaStreamSynchronize(c->stream));   // caller may free its buffers on return
+    CUC(cudaGetLastError());
+#undef CUC
+    *out = c;
+    return DODE_OK;
+}
+
+int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta) {
+    if (!ctx) return DODE_EINVAL;
+    int c = 0, rc;
+    if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
+    return step_impl(ctx, days, n, eta, c);
+}
+
+int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, const float* x_host, float* q_host) {
+    if (!ctx) return DODE_EINVAL;
+    int c = 0, rc;
+    if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
+    if (!x_host || !q_host) return fail(ctx, DODE_EINVAL, "x_host or q_host is null");
+    const dode_dims& d = ctx->dm;
+    const size_t TL = (size_t)d.T * d.L, TNp = (size_t)d.T * ctx->Np, TN = (size_t)d.T * d.N;
+    for (int i = 0; i < n; ++i)
+        CU(cudaMemcpyAsync(ctx->x + TL * days[i], x_host + TL * i, TL * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    if ((rc = step_impl(ctx, days, n, eta, c))) return rc;
+    for (int i = 0; i < n; ++i)
+        CU(cudaMemcpy2DAsync(q_host + TN * i, d.N * sizeof(float), ctx->q + TNp * days[i], ctx->Np * sizeof(float),
+                             d.N * sizeof(float), d.T, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return DODE_OK;
+}
+
+int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_day, double* total) {
+    if (!ctx) return DODE_EINVAL;
+    const dode_dims& d = ctx->dm;
+    std::vector<int32_t> all;
+    if (!days) {
+        all.resize(d.D);
+        for (int i = 0; i < d.D; ++i) all[i] = i;
+        days = all.data();
+        n = d.D;
+    }
+    int rc;
+    if ((rc = validate_days(ctx, days, n, false, nullptr))) return rc;
+    // group positions by cluster, evaluate in sub-batches; d_obj[i] receives f of days[i]
+    constexpr int kObjBatch = 64;
+    const size_t dayStride = (size_t)d.T * ctx->Np;
+    const long rows = (long)d.T * d.L;
+    const int rowsPerBlock = 2048, nchunks = ceil_div(rows, rowsPerBlock);
+    if (ctx->part_cap < (size_t)nchunks * kObjBatch) {
+        if (ctx->d_part) CU(cudaFree(ctx->d_part));
+        ctx->d_part = nullptr;
+        CU(cudaMalloc(&ctx->d_part, (size_t)nchunks * kObjBatch * sizeof(double)));
+        ctx->part_cap = (size_t)nchunks * kObjBatch;
+    }
+    std::vector<double> host(n);
+    std::vector<int> pos;
+    for (int c = 0; c < d.C; ++c) {
+        pos.clear();
+        for (int i = 0; i < n; ++i)
+            if (ctx->labels[days[i]] == c) pos.push_back(i);
+        for (size_t off = 0; off < pos.size(); off += kObjBatch) {
+            DayList dl;
+            dl.n = (int)std::min<size_t>(kObjBatch, pos.size() - off);
+            for (int j = 0; j < dl.n; ++j) dl.day[j] = days[pos[off + j]];
+            int bt, bp;
+            if ((rc = forward_batch(ctx, c, dl, ctx->q, dayStride, ctx->x, nullptr, &bt, &bp))) return rc;
+            sumsq_partial<<<dim3(nchunks, ceil_div(dl.n, 32)), kThreads, 0, ctx->stream>>>(ctx->r, ctx->d_part, rows, bp,
+                                                                                         dl.n, rowsPerBlock);
+            sumsq_final<<<ceil_div(dl.n, 64), 64, 0, ctx->stream>>>(ctx->d_part, ctx->d_obj, nchunks, dl.n);
+            ctx->launches += 2;
+            std::vector<double> tmp(dl.n);
+            CU(cudaMemcpyAsync(tmp.data(), ctx->d_obj, dl.n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+            CU(cudaStreamSynchronize(ctx->stream));
+            for (int j = 0; j < dl.n; ++j) host[pos[off + j]] = tmp[j];
+        }
+    }
+    CU(cudaGetLastError());
+    double tot = 0.0;
+    for (int i = 0; i < n; ++i) tot += host[i];
+    if (per_day) std::memcpy(per_day, host.data(), sizeof(double) * n);
+    if (total) *total = tot;
+    return DODE_OK;
+}
+
+static int copy_q(dode_ctx* ctx, int32_t day, float* out, const float* in, int32_t is_device) {
+    const dode_dims& d = ctx->dm;
+    if (day < 0 || day >= d.D) return fail(ctx, DODE_EINVAL, "day %d out of range [0,%d)", day, d.D);
+    if (!out && !in) return fail(ctx, DODE_EINVAL, "null buffer");
+    float* qd = ctx->q + (size_t)day * d.T * ctx->Np;
+    if (out)
+        CU(cudaMemcpy2DAsync(out, d.N * sizeof(float), qd, ctx->Np * sizeof(float), d.N * sizeof(float), d.T,
+                             is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    else
+        CU(cudaMemcpy2DAsync(qd, ctx->Np * sizeof(float), in, d.N * sizeof(float), d.N * sizeof(float), d.T,
+                             is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return DODE_OK;
+}
+
+int dode_get_q(dode_ctx* ctx, int32_t day, float* out, int32_t is_device) {
+    if (!ctx) return DODE_EINVAL;
+    if (!out) return fail(ctx, DODE_EINVAL, "out is null");
+    return copy_q(ctx, day, out, nullptr, is_device);
+}
+
+int dode_set_q(dode_ctx* ctx, int32_t day, const float* in, int32_t is_device) {
+    if (!ctx) return DODE_EINVAL;
+    if (!in) return fail(ctx, DODE_EINVAL, "in is null");
+    return copy_q(ctx, day, nullptr, in, is_device);
+}
+
+// v = rho_c * (padded u in ctx->pu)
+static int apply_padded(dode_ctx* ctx, int c, float* v) {
+    DayList dl; dl.n = 1; dl.day[0] = 0;
+    int bt, bp;
+    return forward_batch(ctx, c, dl, ctx->pu, 0, nullptr, v, &bt, &bp);
+}
+
+static int apply_t_impl(dode_ctx* ctx, int c, const float* v, float* u) {
+    DayList dl; dl.n = 1; dl.day[0] = 0;
+    const dode_dims& d = ctx->dm;
+    if (d.storage == DODE_DENSE)
+        return launch_grad<1, false>(ctx, 5, dense_cluster(ctx, c), v, nullptr, 0, u, 0.f, 1, dl);
+    csr_gradient(ctx->csr, c, 1, v, nullptr, 0, u, 0.f, 1, dl, d, ctx->Np, ctx->stream, &ctx->launches);
+    return DODE_OK;
+}
+
+int dode_apply(dode_ctx* ctx, int32_t c, const float* u, float* v) {
+    if (!ctx) return DODE_EINVAL;
+    const dode_dims& d = ctx->dm;
+    if (c < 0 || c >= d.C || !u || !v) return fail(ctx, DODE_EINVAL, "bad cluster or null buffer");
+    scale_pad<<<592, 256, 0, ctx->stream>>>(u, ctx->pu, (size_t)d.T, d.N, ctx->Np, nullptr);
+    ctx->launches++;
+    int rc = apply_padded(ctx, c, v);
+    if (rc) return rc;
+    CU(cudaGetLastError());
+    return DODE_OK;
+}
+
+int dode_apply_t(dode_ctx* ctx, int32_t c, const float* v, float* u) {
+    if (!ctx) return DODE_EINVAL;
+    const dode_dims& d = ctx->dm;
+    if (c < 0 || c >= d.C || !u || !v) return fail(ctx, DODE_EINVAL, "bad cluster or null buffer");
+    int rc = apply_t_impl(ctx, c, v, u);
+    if (rc) return rc;
+    CU(cudaGetLastError());
+    return DODE_OK;
+}
+
+int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
+    if (!ctx) return DODE_EINVAL;
+    const dode_dims& d = ctx->dm;
+    if (c < 0 || c >= d.C || iters < 1 || !L_out) return fail(ctx, DODE_EINVAL, "bad cluster, iters or null output");
+    double* nrm = ctx->d_obj + d.D;       // [0] = |w|^2, [1] = |v|^2
+    const size_t TN = (size_t)d.T * d.N, TL = (size_t)d.T * d.L;
+    fill_f32<<<592, 256, 0, ctx->stream>>>(ctx->pw, TN, 1.f);
+    ctx->launches++;
+    for (int it = 0; it < iters; ++it) {
+        sumsq_single<<<1, 1024, 0, ctx->stream>>>(ctx->pw, TN, nrm);
+        scale_pad<<<592, 256, 0, ctx->stream>>>(ctx->pw, ctx->pu, (size_t)d.T, d.N, ctx->Np, nrm);
+        ctx->launches += 2;
+        int rc = apply_padded(ctx, c, ctx->pv);
+        if (rc) return rc;
+        sumsq_single<<<1, 1024, 0, ctx->stream>>>(ctx->pv, TL, nrm + 1);
+        ctx->launches++;
+        if ((rc = apply_t_impl(ctx, c, ctx->pv, ctx->pw))) return rc;
+    }
+    CU(cudaMemcpyAsync(L_out, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaGetLastError());
+    return DODE_OK;
+}
+
+int64_t dode_launch_count(const dode_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* dode_last_path(const dode_ctx* ctx) { return ctx ? ctx->path.c_str() : ""; }
+
+int dode_sync(dode_ctx* ctx) {
+    if (!ctx) return DODE_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaGetLastError());
+    return DODE_OK;
+}
+
+const char* dode_last_error(const dode_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+}  // extern "C"

@@ -1,0 +1,168 @@
+"""GPU-vs-oracle parity through the C ABI: identical iterates after K steps from the same
+q0, eta and schedule, |q_gpu - q_cpu| <= 1e-3 max(1,|q_cpu|), objective relative error <= 1e-4."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1901_09266_b200 import synth
+from tests import harness as hz
+
+pytestmark = pytest.mark.gpu
+
+TOL_OBJ = 1e-4
+
+
+def _oracle():
+    from oracle import oracle
+    return oracle
+
+
+def _objective_cpu(p, q, days):
+    o = _oracle()
+    return np.array([o.objective_day(p.R[p.labels[d]].numpy(), q[i], p.x[d].numpy()) for i, d in enumerate(days)])
+
+
+def _run_both(cfg, K=None, b=None, sample=None, csr=False):
+    p = hz.make_problem(cfg)
+    sched = synth.schedule(cfg, p.labels, K=K, b=b)
+    etas = hz.oracle_etas(p)
+    g = hz.GpuSolver(p, csr=csr)
+    g.run(sched, etas)
+    days = list(range(cfg.D)) if sample is None else list(sample)
+    q_gpu = g.q(days)
+    q_cpu = hz.oracle_run(p, sched, etas, sample)[days]
+    hz.assert_q_close(q_gpu, q_cpu, cfg.name)
+    # a5: library objective at the GPU's own q vs the oracle's O3 at the same q
+    f_gpu, tot = g.P.dode_objective(g.h, days)
+    f_cpu = _objective_cpu(p, q_gpu, days)
+    np.testing.assert_allclose(f_gpu, f_cpu, rtol=TOL_OBJ)
+    assert abs(tot - f_cpu.sum()) <= TOL_OBJ * f_cpu.sum()
+    # and the two sides' objectives at their own iterates
+    np.testing.assert_allclose(f_gpu, _objective_cpu(p, q_cpu, days), rtol=TOL_OBJ)
+    path = g.P.dode_last_path(g.h)
+    launches = g.P.dode_launch_count(g.h)
+    g.close()
+    assert launches >= 2 * len(sched)
+    return path
+
+
+def test_config0_tiny_full():
+    """BASELINE.json configs[0] exactly: N=4 L=6 T=288 H=6 D=14, b=4, 500 iterations, all days compared."""
+    path = _run_both(synth.CONFIGS["tiny"])
+    assert "ffma" in path
+
+
+def test_tiny12_sub_instance():
+    _run_both(synth.CONFIGS["tiny12"])
+
+
+@pytest.mark.parametrize("b", [1, 2, 3, 5, 8, 11, 20, 37])
+def test_ragged_shapes_and_minibatch_widths(b):
+    """N, L not multiples of 4/8 (padding paths), every BT specialisation, ragged last chunks, pad days."""
+    cfg = synth.Config("ragged", N=61, L=37, T=50, H=5, C=3, D=90, b=b, K=24, kmin=3, kmax=9)
+    _run_both(cfg)
+
+
+def test_corridor_shape_reduced_T():
+    """configs[1]'s blocks (N=60, L=120, H=12, C=4, b=32) on a shorter day so the oracle finishes in seconds;
+    spans several row tiles (L=120 -> 4 warps-tiles) and two b-tiles of 16."""
+    cfg = synth.CONFIGS["corridor"].replace(name="corridor_T72", T=72, D=96, K=16)
+    _run_both(cfg, sample=[0, 7, 33, 64, 95])
+
+
+def test_wide_blocks_several_column_tiles():
+    """N4 > 32 (several CTAs along n in the gradient kernel) and L > 32 (several CTAs along l in the forward)."""
+    cfg = synth.Config("wide", N=300, L=150, T=20, H=4, C=2, D=24, b=8, K=10, kmin=5, kmax=20)
+    _run_both(cfg, sample=[1, 5, 12, 23])
+
+
+@pytest.mark.parametrize("T,H", [(1, 0), (7, 0), (3, 5), (6, 6)])
+def test_degenerate_time_axis(T, H):
+    """T=1/H=0 (Fig. 12's plain NNLS), H=0 (no lag), H >= T (band wider than the day)."""
+    cfg = synth.Config("degenerate", N=9, L=11, T=T, H=H, C=2, D=10, b=4, K=20, kmin=2, kmax=5)
+    _run_both(cfg)
+
+
+def test_invalid_day_lists_leave_state_untouched():
+    cfg = synth.Config("inv", N=8, L=8, T=6, H=2, C=2, D=12, b=4, K=4, kmin=2, kmax=4)
+    p = hz.make_problem(cfg)
+    g = hz.GpuSolver(p)
+    P = g.P
+    before = g.q()
+    c0 = [int(d) for d in np.nonzero(p.labels == 0)[0]]
+    c1 = [int(d) for d in np.nonzero(p.labels == 1)[0]]
+    for bad in ([c0[0], c0[0]], [c0[0], c1[0]], [-1], [cfg.D], []):
+        with pytest.raises(P.DodeError) as e:
+            P.dode_spgd_step(g.h, bad, 0.1)
+        assert e.value.code == P.DODE_EINVAL
+        assert P.dode_last_error(g.h) != ""
+    np.testing.assert_array_equal(g.q(), before)
+    g.close()
+
+
+def test_apply_adjoint_and_lipschitz():
+    """<rho u, v> = <u, rho^T v> through the production kernels; dode_apply against the oracle's forward;
+    a7 against the oracle's O4."""
+    o = _oracle()
+    cfg = synth.Config("adj", N=45, L=70, T=30, H=6, C=2, D=4, b=2, K=2, kmin=3, kmax=12)
+    p = hz.make_problem(cfg)
+    g = hz.GpuSolver(p)
+    P = g.P
+    gen = torch.Generator().manual_seed(5)
+    for c in range(cfg.C):
+        u = torch.randn(cfg.T, cfg.N, generator=gen)
+        v = torch.randn(cfg.T, cfg.L, generator=gen)
+        ru = torch.empty(cfg.T, cfg.L, device="cuda")
+        rtv = torch.empty(cfg.T, cfg.N, device="cuda")
+        P.dode_apply(g.h, c, u.cuda(), ru)
+        P.dode_apply_t(g.h, c, v.cuda(), rtv)
+        P.dode_sync(g.h)
+        lhs = float((ru.cpu().double() * v.double()).sum())
+        rhs = float((u.double() * rtv.cpu().double()).sum())
+        assert abs(lhs - rhs) <= 1e-4 * max(1.0, abs(lhs))
+        ref = o.forward_residual(p.R[c].numpy(), u.numpy(), np.zeros((cfg.T, cfg.L), np.float32))
+        np.testing.assert_allclose(ru.cpu().numpy(), ref, rtol=1e-4, atol=1e-4)
+        np.testing.assert_allclose(rtv.cpu().numpy(), o.gradient(p.R[c].numpy(), v.numpy()), rtol=1e-4, atol=1e-4)
+        L_gpu = P.dode_lipschitz(g.h, c, 50)
+        L_cpu = o.power_iteration(p.R[c].numpy(), 50)
+        assert abs(L_gpu - L_cpu) <= 1e-4 * L_cpu
+    g.close()
+
+
+def test_get_set_q_and_host_step():
+    cfg = synth.Config("io", N=10, L=14, T=12, H=3, C=1, D=6, b=3, K=3, kmin=2, kmax=5, label_mode="zero")
+    p = hz.make_problem(cfg)
+    etas = hz.oracle_etas(p)
+    g1, g2 = hz.GpuSolver(p), hz.GpuSolver(p, q0=0.0)
+    P = g1.P
+    # set_q/get_q round trip (host and device buffers)
+    src = torch.rand(cfg.T, cfg.N)
+    P.dode_set_q(g2.h, 2, src)
+    back = torch.empty(cfg.T, cfg.N, device="cuda")
+    P.dode_get_q(g2.h, 2, back)
+    np.testing.assert_array_equal(back.cpu().numpy(), src.numpy())
+    for d in range(cfg.D):
+        P.dode_set_q(g2.h, d, torch.ones(cfg.T, cfg.N))
+    # streaming step == resident step
+    days = [4, 1, 3]
+    P.dode_spgd_step(g1.h, days, float(etas[0]))
+    xh = p.x[days].contiguous().pin_memory()
+    qh = torch.empty(len(days), cfg.T, cfg.N).pin_memory()
+    P.dode_spgd_step_host(g2.h, days, float(etas[0]), xh, qh)
+    np.testing.assert_array_equal(qh.numpy(), g1.q(days))
+    np.testing.assert_array_equal(g2.q(), g1.q())
+    g1.close(); g2.close()
+
+
+def test_batch_composition_invariance_on_gpu():
+    """P10 on the GPU: the same visits as b=1 steps give the same iterate to rounding."""
+    cfg = synth.Config("sep", N=24, L=20, T=16, H=4, C=2, D=20, b=7, K=12, kmin=2, kmax=6)
+    p = hz.make_problem(cfg)
+    etas = hz.oracle_etas(p)
+    sched = synth.schedule(cfg, p.labels)
+    single = [(c, np.array([d], np.int32)) for c, days in sched for d in days]
+    g1, g2 = hz.GpuSolver(p), hz.GpuSolver(p)
+    g1.run(sched, etas)
+    g2.run(single, etas)
+    hz.assert_q_close(g1.q(), g2.q(), "batch composition")
+    g1.close(); g2.close()
