@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py — SPGD epoch time over all days on one B200 (BASELINE.json metric), with the roofline of the
+dominant kernel and the CPU oracle timed beside it.
+
+A *step* is one SPGD epoch of the workload: every day receives exactly one projected-gradient step, i.e.
+sum_c ceil(D_c / b) calls of dode_spgd_step (a1-a4 of SURVEY.md §8(a)) in the seeded A8 schedule order.
+Default workload: BASELINE.json configs[1] ("corridor": N=60 L=120 T=288 H=12 C=4 D=365, minibatch 32).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--b B] [--impl reference]
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the byte/flop accounting.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from paper_1901_09266_b200 import synth
+
+METRIC = "spgd_epoch_time_over_all_days"
+UNIT = "ms/epoch"
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 flop x clocks.max.sm
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz, self.ok = index, False, [], set(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            uuid = torch.cuda.get_device_properties(index).uuid
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + str(uuid)).encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self.stop_flag:
+            try:
+                self.sm.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                r = self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(
+                    self.nv, "nvmlDeviceGetCurrentClocksEventReasons") else self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def summary(self):
+        if not self.ok or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml_unavailable"]}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.sm)}
+
+
+def make_epochs(cfg, lab, b, count):
+    rng = synth._Counter(cfg.seed, synth.S_SCHED)
+    return [synth.epoch_chunks(np.asarray(lab, np.int64), b, rng) for _ in range(count)]
+
+
+def algorithmic(cfg, n_days):
+    """Algorithmic bytes / flops of one launch on n_days days: R once per pass + the state."""
+    Rb = 4.0 * cfg.nb * cfg.L * cfg.N
+    fwd_b = Rb + 4.0 * n_days * cfg.T * (cfg.N + cfg.L)        # read q, read x   (r stays on chip in principle)
+    grad_b = Rb + 4.0 * n_days * cfg.T * cfg.N                 # write q
+    fl = 2.0 * cfg.nb * cfg.L * cfg.N * n_days
+    return fwd_b, grad_b, fl
+
+
+def cpu_oracle_sample(cfg, R, lab, x, etas, visits):
+    """Times the oracle as it stands on `visits` day-visits (single thread); returns ms per visit."""
+    from oracle import oracle
+    days = list(range(min(visits, cfg.D)))
+    q = np.ones((cfg.T, cfg.N), np.float32)
+    Rn = [R[c].numpy() for c in range(cfg.C)]
+    oracle.visit(Rn[int(lab[0])], q, x[0].numpy(), float(etas[int(lab[0])]))       # page in
+    t0 = time.perf_counter()
+    for d in days:
+        c = int(lab[d])
+        oracle.visit(Rn[c], q, x[d].numpy(), float(etas[c]))
+    return (time.perf_counter() - t0) * 1e3 / len(days)
+
+
+def run_reference(args, cfg, b, rank, world):
+    """--impl reference: the CPU oracle (oracle/), as it stands, on this host; one step = a bounded sample of an
+    epoch (args.ref_visits day-visits), extrapolated to the epoch (x D / visits)."""
+    if rank != 0:
+        return
+    from oracle import oracle
+    if cfg.N * cfg.L * cfg.T * (cfg.H + 1) * cfg.C * 4 > 8e9:
+        print(json.dumps({"impl": "reference", "unavailable": "workload too large to generate on the host"}))
+        return
+    R = synth.dar_dense(cfg)
+    lab = synth.labels(cfg).numpy()
+    x = synth.counts(cfg, R, synth.q_true(cfg), torch.from_numpy(lab))
+    Rn = [R[c].numpy() for c in range(cfg.C)]
+    etas = [np.float32(1.0 / oracle.power_iteration(Rn[c], 10)) for c in range(cfg.C)]
+    q = np.ones((cfg.D, cfg.T, cfg.N), np.float32)
+    v = args.ref_visits
+    times = []
+    day = 0
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        for _ in range(v):
+            c = int(lab[day])
+            q[day] = oracle.visit(Rn[c], q[day], x[day].numpy(), float(etas[c]))
+            day = (day + 1) % cfg.D
+        if it >= args.warmup:
+            times.append((time.perf_counter() - t0) * 1e3)
+    epoch_ms = float(np.mean(times)) * cfg.D / v
+    out = {"impl": "reference", "metric": METRIC, "value": epoch_ms, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": epoch_ms, "higher_is_better": False,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 storage", "data": "synthetic",
+           "config": workload_config(cfg, b),
+           "cpu_baseline": {"value": epoch_ms, "unit": UNIT, "cores": 1, "kind": "oracle",
+                            "sample": f"{v} day-visits per step of the {cfg.D}-visit epoch, extrapolated x{cfg.D / v:.1f}"},
+           "e2e": {"value": epoch_ms, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+
+
+def workload_config(cfg, b):
+    return {"workload": f"{cfg.name}: N={cfg.N} L={cfg.L} T={cfg.T} H={cfg.H} C={cfg.C} D={cfg.D} minibatch={b} "
+                        f"({'CSR' if cfg.sparse else 'dense'} fp32 DAR blocks)",
+            "step": "one SPGD epoch = sum_c ceil(D_c/b) dode_spgd_step calls, every day stepped once",
+            "l2": "L2 flushed (256 MiB write) before every timed epoch; R of all clusters also exceeds L2 "
+                  "except on the tiny workload"}
+
+
+def traffic_from_profiles(workload, kernel_kind):
+    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` summary, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    try:
+        return json.load(open(p)).get(workload, {}).get(kernel_kind)
+    except Exception:
+        return None
+
+
+def run_ours(args, cfg, b, rank, world, local_rank):
+    import paper_1901_09266_b200 as P
+    P.lib()                                   # fail loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+        cfg = cfg.replace(seed=cfg.seed + rank)      # weak scaling: every rank owns its own D days
+
+    # ---- inputs, generated once on the device (synth: no solver arithmetic) ----
+    lab = synth.labels(cfg).numpy()
+    if cfg.sparse:
+        csr, x = synth.sparse_problem(cfg, dev)
+        h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, csr=csr)
+        nnz_c = csr.nnz / cfg.C
+        del csr
+    else:
+        R = synth.dar_dense(cfg, device=dev)
+        x = synth.counts(cfg, R, synth.q_true(cfg, dev), torch.from_numpy(lab))
+        h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, dense=R)
+    x_cpu = x.cpu()
+    R_cpu = None
+    if rank == 0 and not args.no_cpu_baseline and not cfg.sparse and cfg.N * cfg.L * cfg.T * (cfg.H + 1) * 4 < 4e9:
+        R_cpu = R.cpu()
+    if not cfg.sparse:
+        del R
+    del x
+    torch.cuda.empty_cache()
+
+    etas = np.array([np.float32(1.0 / P.dode_lipschitz(h, c, 30)) for c in range(cfg.C)], np.float32)   # a7
+    epochs = make_epochs(cfg, lab, b, args.warmup + args.steps)
+    iters_per_epoch = len(epochs[0])
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def run_epoch(ep):
+        for c, days in ep:
+            P.dode_spgd_step(h, days, float(etas[c]))
+
+    for ep in epochs[:args.warmup]:
+        run_epoch(ep)
+    P.dode_sync(h)
+    launches0 = P.dode_launch_count(h)
+    P.dode_timing_enable(h, True)
+    P.dode_timing_read(h, 0, True); P.dode_timing_read(h, 1, True)
+
+    sampler = ClockSampler(local_rank)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev = []
+    wall0 = time.perf_counter()
+    for ep in epochs[args.warmup:]:
+        flush.zero_()                                    # L2 flush, outside the event pair
+        a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        run_epoch(ep)
+        z.record()
+        ev.append((a, z))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    wall = time.perf_counter() - wall0
+    sampler.stop_flag = True
+    sampler.join()
+    total_ms = sum(a.elapsed_time(z) for a, z in ev)
+    if world > 1:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    epoch_ms = total_ms / args.steps
+    launches = P.dode_launch_count(h) - launches0
+    fwd_ms, fwd_n = P.dode_timing_read(h, 0)
+    grad_ms, grad_n = P.dode_timing_read(h, 1)
+    P.dode_timing_enable(h, False)
+    path = P.dode_last_path(h)
+
+    # ---- roofline of the dominant kernel (algorithmic work summed over the timed launches) ----
+    fb = gb = fl = 0.0
+    for ep in epochs[args.warmup:]:
+        for c, days in ep:
+            if cfg.sparse:
+                f_b = 8.0 * nnz_c + 4.0 * len(days) * cfg.T * (cfg.N + cfg.L)
+                g_b = 8.0 * nnz_c + 4.0 * len(days) * cfg.T * cfg.N
+                f_l = 2.0 * nnz_c * len(days)
+            else:
+                f_b, g_b, f_l = algorithmic(cfg, len(days))
+            fb += f_b; gb += g_b; fl += f_l
+    hbm_peak, peak_src = measured_peaks()
+    dom = "forward" if fwd_ms >= grad_ms else "gradient_update"
+    d_ms, d_n, d_bytes = (fwd_ms, fwd_n, fb) if dom == "forward" else (grad_ms, grad_n, gb)
+    gbs = d_bytes / (d_ms * 1e-3) / 1e9 if d_ms > 0 else 0.0
+    tfl = fl / (d_ms * 1e-3) / 1e12 if d_ms > 0 else 0.0
+    t_hbm, t_alu = d_bytes / (hbm_peak * 1e9), fl / (FP32_PEAK_TFLOPS * 1e12)
+    kname = path.split("+")[0 if dom == "forward" else 1] if "+" in path else path
+    if t_hbm >= t_alu:
+        roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"}
+    else:
+        roof = {"bound": "alu", "achieved": tfl, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": tfl / FP32_PEAK_TFLOPS, "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+    roof.update({"kernel": kname, "launches": int(d_n), "avg_launch_ms": d_ms / max(1, d_n),
+                 "traffic": traffic_from_profiles(cfg.name, dom),
+                 "other": {"hbm_GBps": gbs, "hbm_frac": gbs / hbm_peak, "fp32_TFLOPs": tfl,
+                           "fp32_frac": tfl / FP32_PEAK_TFLOPS,
+                           "forward_ms_total": fwd_ms, "gradient_update_ms_total": grad_ms,
+                           "step_GBps_algorithmic": (fb + gb) / (total_ms * 1e-3) / 1e9,
+                           "step_TFLOPs_algorithmic": 2 * fl / (total_ms * 1e-3) / 1e12}})
+
+    # ---- e2e: the same epochs through dode_spgd_step_host (H2D of the minibatch counts, D2H of its q) ----
+    e2e = None
+    if args.e2e_steps > 0:
+        e_epochs = make_epochs(cfg, lab, b, args.e2e_steps + 1)
+        stage = [[(c, days, x_cpu[torch.from_numpy(days.astype(np.int64))].contiguous().pin_memory(),
+                   torch.empty((len(days), cfg.T, cfg.N), dtype=torch.float32).pin_memory()) for c, days in ep]
+                 for ep in e_epochs]
+        for c, days, xh, qh in stage[0]:
+            P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for ep in stage[1:]:
+            for c, days, xh, qh in ep:
+                P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
+        torch.cuda.synchronize()
+        e_ms = (time.perf_counter() - t0) * 1e3 / args.e2e_steps
+        if world > 1:
+            t = torch.tensor([e_ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        e2e = {"value": e_ms, "unit": UNIT, "h2d_bytes_per_step": int(cfg.D * cfg.T * cfg.L * 4),
+               "d2h_bytes_per_step": int(cfg.D * cfg.T * cfg.N * 4), "api": "dode_spgd_step_host (pinned host buffers)"}
+
+    if rank != 0:
+        P.dode_destroy(h)
+        return
+    # ---- CPU oracle beside it (bounded sample, rank 0 only) ----
+    cpu = None
+    if R_cpu is not None:
+        per_visit = cfg.nb * cfg.L * cfg.N * 4 / 0.6e9          # rough s per visit at ~0.6 GFLOP/s scalar double
+        visits = int(max(3, min(cfg.D, 15.0 / max(per_visit, 1e-4))))
+        ms_visit = cpu_oracle_sample(cfg, R_cpu, lab, x_cpu, etas, visits)
+        cpu = {"value": ms_visit * cfg.D, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{visits} day-visits of the {cfg.D}-visit epoch timed single-threaded on this host "
+                         f"({os.cpu_count()} cores visible), extrapolated x{cfg.D / visits:.1f}",
+               "ms_per_day_visit": ms_visit}
+    out = {"metric": METRIC, "value": epoch_ms, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": epoch_ms, "higher_is_better": False, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, b),
+           "day_steps_per_s": cfg.D * world / (epoch_ms * 1e-3), "spgd_iterations_per_epoch": iters_per_epoch,
+           "ms_per_spgd_iteration": epoch_ms / iters_per_epoch, "kernel_path": path,
+           "gpu_launches": int(launches), "wall_s_timed_region": wall, "clocks": sampler.summary(),
+           "roofline": roof, "e2e": e2e, "cpu_baseline": cpu}
+    print(json.dumps(out))
+    P.dode_destroy(h)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="corridor", choices=list(synth.CONFIGS))
+    ap.add_argument("--b", type=int, default=None, help="minibatch days (default: the workload's)")
+    ap.add_argument("--days", type=int, default=None, help="override D (bench smoke runs only)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-visits", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = max(args.warmup, 1)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = synth.CONFIGS[args.workload]
+    if args.days:
+        cfg = cfg.replace(D=args.days)
+    b = args.b or cfg.b
+    if args.impl == "reference":
+        run_reference(args, cfg, b, rank, world)
+    else:
+        run_ours(args, cfg, b, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -104,6 +104,13 @@ int dode_apply_t(dode_ctx* ctx, int32_t c, const float* v, float* u);
  * eta_c = 1/L_c is the step "dependent on the problem scale".  Synchronises. */
 int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out);
 
+/* Optional per-kernel timing for roofline reports: while enabled, every forward (kind 0) and
+ * gradient+update (kind 1) launch is bracketed by CUDA events on the ctx stream.  dode_timing_read
+ * synchronises, folds finished event pairs into the running totals and returns the total device
+ * time (ms) and launch count of one kind; reset != 0 clears that kind's totals afterwards. */
+int dode_timing_enable(dode_ctx* ctx, int32_t on);
+int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches, int32_t reset);
+
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 int64_t dode_launch_count(const dode_ctx* ctx);
 

@@ -20,7 +20,7 @@ DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
 DODE_DENSE, DODE_CSR = 0, 1
 
 EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_objective", "dode_get_q", "dode_set_q",
-           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_launch_count", "dode_last_path", "dode_sync",
+           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
 
@@ -60,6 +60,8 @@ def lib():
         L.dode_apply.argtypes = [vp, i32, vp, vp]
         L.dode_apply_t.argtypes = [vp, i32, vp, vp]
         L.dode_lipschitz.argtypes = [vp, i32, i32, vp]
+        L.dode_timing_enable.argtypes = [vp, i32]
+        L.dode_timing_read.argtypes = [vp, i32, vp, vp, i32]
         L.dode_launch_count.argtypes = [vp]
         L.dode_launch_count.restype = C.c_int64
         L.dode_last_path.argtypes = [vp]
@@ -175,6 +177,17 @@ def dode_lipschitz(h, c: int, iters: int = 50) -> float:
     out = C.c_double()
     _chk(h, lib().dode_lipschitz(h, c, iters, C.byref(out)))
     return out.value
+
+
+def dode_timing_enable(h, on: bool) -> None:
+    _chk(h, lib().dode_timing_enable(h, 1 if on else 0))
+
+
+def dode_timing_read(h, kind: int, reset: bool = False):
+    """(total device ms, launches) of kind 0 = forward, 1 = gradient+update."""
+    ms, cnt = C.c_double(), C.c_int64()
+    _chk(h, lib().dode_timing_read(h, kind, C.byref(ms), C.byref(cnt), 1 if reset else 0))
+    return ms.value, cnt.value
 
 
 def dode_launch_count(h) -> int:

@@ -40,6 +40,32 @@ struct dode_ctx {
     std::string path;
     char err[512] = {0};
     bool sm_opt_in[8] = {false};
+    // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;
+    struct Pending { int kind; cudaEvent_t a, b; };
+    std::vector<Pending> ev_pending;
+    double t_total[3] = {0, 0, 0};
+    int64_t t_count[3] = {0, 0, 0};
+};
+
+enum { KIND_FWD = 0, KIND_GRAD = 1, KIND_OTHER = 2 };
+
+struct KernelTimer {      // records an event pair around one launch when timing is on
+    dode_ctx* c; cudaEvent_t a = nullptr, b = nullptr; int kind;
+    KernelTimer(dode_ctx* ctx, int k) : c(ctx), kind(k) {
+        if (!c->timing) return;
+        for (cudaEvent_t* e : {&a, &b}) {
+            if (!c->ev_pool.empty()) { *e = c->ev_pool.back(); c->ev_pool.pop_back(); }
+            else if (cudaEventCreate(e) != cudaSuccess) { *e = nullptr; }
+        }
+        if (a && b) cudaEventRecord(a, c->stream);
+    }
+    ~KernelTimer() {
+        if (!c->timing || !a || !b) return;
+        cudaEventRecord(b, c->stream);
+        c->ev_pending.push_back({kind, a, b});
+    }
 };
 
 static thread_local char g_create_err[512] = {0};
@@ -79,6 +105,7 @@ static void launch_fwd(dode_ctx* ctx, const float* Rc, const float* qbase, size_
                        float* r, int bp, const DayList& dl) {
     const dode_dims& d = ctx->dm;
     dim3 grid(ceil_div(d.L, (kThreads / 32) * RL), d.T, bp / BT);
+    KernelTimer kt(ctx, KIND_FWD);
     fwd_rowdot<BT, RL><<<grid, kThreads, 0, ctx->stream>>>(Rc, qbase, dayStride, xbase, r, ctx->N4, d.L, d.T, d.H, bp, dl);
     ctx->launches++;
 }
@@ -106,6 +133,7 @@ static int launch_grad(dode_ctx* ctx, int slot, const float* Rc, const float* r,
         ctx->sm_opt_in[slot] = true;
     }
     dim3 grid(ceil_div(ctx->N4, 1 << cwlog2), d.T, bp / BT);
+    KernelTimer kt(ctx, KIND_GRAD);
     grad_coldot<BT, UPDATE><<<grid, kThreads, smem, ctx->stream>>>(Rc, r, qbase, dayStride, gout, eta, d.N, ctx->N4,
                                                                    d.L, d.T, d.H, bp, cwlog2, dl);
     ctx->launches++;
@@ -128,19 +156,28 @@ static const float* dense_cluster(const dode_ctx* ctx, int c) {
     return ctx->R + (size_t)c * d.T * (d.H + 1) * d.L * ctx->Np;
 }
 
-// forward residual of one sub-batch (<= kMaxDays days of cluster c) into ctx->r; returns bt/bp
+// forward residual of one sub-batch (<= kMaxDays days of cluster c) into ctx->r (or r_out with day stride 1
+// for dode_apply); returns the day-tile bt and the r stride bp
 static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, const float* qbase, size_t dayStride,
                          const float* xbase, float* r_out, int* bt_out, int* bp_out) {
     const dode_dims& d = ctx->dm;
-    const int bt = pick_bt(dl.n), bp = ceil_div(dl.n, bt) * bt;
+    const bool csr = d.storage == DODE_CSR;
+    const int bt = csr ? 32 : pick_bt(dl.n);
+    const int bp = csr ? csr_bp(dl.n) : ceil_div(dl.n, bt) * bt;
     float* r = r_out;
     if (!r) {
         int rc = ensure_r(ctx, (size_t)d.T * d.L * bp);
         if (rc) return rc;
         r = ctx->r;
     }
-    if (d.storage == DODE_DENSE) fwd_dense(ctx, bt, dense_cluster(ctx, c), qbase, dayStride, xbase, r, bp, dl);
-    else csr_forward(ctx->csr, c, bt, qbase, dayStride, xbase, r, bp, dl, d, ctx->Np, ctx->stream, &ctx->launches);
+    if (!csr) {
+        fwd_dense(ctx, bt, dense_cluster(ctx, c), qbase, dayStride, xbase, r, bp, dl);
+    } else {
+        KernelTimer kt(ctx, KIND_FWD);
+        int rc = csr_forward(ctx->csr, c, qbase, dayStride, xbase, r, bp, r_out ? 1 : bp, dl, d, ctx->Np, ctx->stream,
+                             &ctx->launches);
+        if (rc) return fail(ctx, rc, "CSR scratch allocation failed");
+    }
     *bt_out = bt; *bp_out = bp;
     return DODE_OK;
 }
@@ -164,9 +201,10 @@ static int validate_days(dode_ctx* ctx, const int32_t* days, int32_t n, bool sam
 static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c) {
     const dode_dims& d = ctx->dm;
     const size_t dayStride = (size_t)d.T * ctx->Np;
-    for (int off = 0; off < n; off += kMaxDays) {       // days are independent units
+    const int chunk = d.storage == DODE_CSR ? kCsrMaxDays : kMaxDays;
+    for (int off = 0; off < n; off += chunk) {          // days are independent units
         DayList dl;
-        dl.n = std::min(kMaxDays, n - off);
+        dl.n = std::min(chunk, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
         int bt, bp, rc;
         if ((rc = forward_batch(ctx, c, dl, ctx->q, dayStride, ctx->x, nullptr, &bt, &bp))) return rc;
@@ -176,10 +214,14 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
             snprintf(buf, sizeof buf, "ffma_rowdot_bt%d+ffma_coldot_bt%d", bt, bt);
             ctx->path = buf;
         } else {
-            csr_gradient(ctx->csr, c, bt, ctx->r, ctx->q, dayStride, nullptr, eta, bp, dl, d, ctx->Np, ctx->stream,
-                         &ctx->launches);
+            {
+                KernelTimer kt(ctx, KIND_GRAD);
+                rc = csr_gradient(ctx->csr, c, ctx->r, ctx->q, dayStride, nullptr, eta, bp, bp, dl, d, ctx->Np,
+                                  ctx->stream, &ctx->launches);
+            }
+            if (rc) return fail(ctx, rc, "CSR scratch allocation failed");
             char buf[96];
-            snprintf(buf, sizeof buf, "csr_fwd_bt%d+csrT_grad_bt%d", bt, bt);
+            snprintf(buf, sizeof buf, "csr_fwd_bp%d+csr_grad_bp%d", bp, bp);
             ctx->path = buf;
         }
     }
@@ -197,6 +239,8 @@ void dode_destroy(dode_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->R); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r);
+    for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+    for (auto e : ctx->ev_pool) cudaEventDestroy(e);
     cudaFree(ctx->d_part); cudaFree(ctx->d_obj); cudaFree(ctx->pu); cudaFree(ctx->pv); cudaFree(ctx->pw);
     csr_free(ctx->csr);
     delete ctx;
@@ -390,8 +434,7 @@ static int apply_t_impl(dode_ctx* ctx, int c, const float* v, float* u) {
     const dode_dims& d = ctx->dm;
     if (d.storage == DODE_DENSE)
         return launch_grad<1, false>(ctx, 5, dense_cluster(ctx, c), v, nullptr, 0, u, 0.f, 1, dl);
-    csr_gradient(ctx->csr, c, 1, v, nullptr, 0, u, 0.f, 1, dl, d, ctx->Np, ctx->stream, &ctx->launches);
-    return DODE_OK;
+    return csr_gradient(ctx->csr, c, v, nullptr, 0, u, 0.f, 32, 1, dl, d, ctx->Np, ctx->stream, &ctx->launches);
 }
 
 int dode_apply(dode_ctx* ctx, int32_t c, const float* u, float* v) {
@@ -437,6 +480,28 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
     CU(cudaMemcpyAsync(L_out, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     CU(cudaGetLastError());
+    return DODE_OK;
+}
+
+int dode_timing_enable(dode_ctx* ctx, int32_t on) {
+    if (!ctx) return DODE_EINVAL;
+    ctx->timing = on != 0;
+    return DODE_OK;
+}
+
+int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches, int32_t reset) {
+    if (!ctx) return DODE_EINVAL;
+    if (kind < 0 || kind > 2) return fail(ctx, DODE_EINVAL, "kind must be 0 (forward), 1 (gradient+update) or 2");
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (auto& p : ctx->ev_pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p.a, p.b) == cudaSuccess) { ctx->t_total[p.kind] += ms; ctx->t_count[p.kind]++; }
+        ctx->ev_pool.push_back(p.a); ctx->ev_pool.push_back(p.b);
+    }
+    ctx->ev_pending.clear();
+    if (total_ms) *total_ms = ctx->t_total[kind];
+    if (launches) *launches = ctx->t_count[kind];
+    if (reset) { ctx->t_total[kind] = 0; ctx->t_count[kind] = 0; }
     return DODE_OK;
 }
 

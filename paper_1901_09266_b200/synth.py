@@ -21,6 +21,7 @@ from __future__ import annotations
 
 import dataclasses
 import math
+import warnings
 from typing import List, Optional, Tuple
 
 import numpy as np
@@ -364,3 +365,119 @@ def dense_to_csr(R: torch.Tensor) -> CsrDar:
     idx = torch.nonzero(nzmask.view(-1, N))                           # row-major => CSR order
     return CsrDar(blk_off, row_ptr.to(torch.int32).contiguous(), idx[:, 1].to(torch.int32).contiguous(),
                   R[nzmask].contiguous())
+
+
+# --------------------------------------------------------------------------
+# G7: sparse DAR for large networks (cfg 4), generated directly in the boundary CSR format.
+# Example 3: departures of one interval reach a link spread over a few ADJACENT
+# arrival intervals, later the further downstream the link is.  Link at position j of OD n's path gets
+# lag offset h0 = min(floor(j*tau), H-w+1) (tau ~ U(0.3,0.9) intervals per link, per cluster and OD) and a
+# window of w ~ U{2,3,4} lags with flat-Dirichlet fractions (redrawn per departure interval s).
+# --------------------------------------------------------------------------
+def sparse_pattern(cfg: Config, c: int, device="cpu"):
+    """Sorted (h, l, n) pattern of cluster c (identical for every s) plus the (n,j) group id of each entry."""
+    start, k = incidence(cfg, device)
+    n_all = torch.arange(cfg.N, dtype=torch.int64, device=device)
+    tau = 0.3 + 0.6 * uniform01(cfg.seed, S_TAU, c * cfg.N + n_all, torch.float64)
+    kmax = int(k.max())
+    j = torch.arange(kmax, dtype=torch.int64, device=device)[None, :].expand(cfg.N, kmax)
+    valid = j < k[:, None]
+    nn = n_all[:, None].expand(cfg.N, kmax)[valid]
+    jj = j[valid]
+    gid = torch.arange(nn.numel(), dtype=torch.int64, device=device)          # one group per (n, j)
+    w = randint(cfg.seed, S_WIN, (c * cfg.N + nn) * 64 + jj, 2, 4).clamp(max=cfg.H + 1)
+    h0 = torch.minimum((jj.to(torch.float64) * tau[nn]).floor().to(torch.int64), cfg.H - w + 1)
+    ll = start[nn] + jj
+    wmax = int(w.max())
+    i = torch.arange(wmax, dtype=torch.int64, device=device)[None, :].expand(nn.numel(), wmax)
+    vi = i < w[:, None]
+    eh = (h0[:, None] + i)[vi]
+    el = ll[:, None].expand(-1, wmax)[vi]
+    en = nn[:, None].expand(-1, wmax)[vi]
+    eg = gid[:, None].expand(-1, wmax)[vi]
+    ei = i[vi]
+    order = torch.argsort((eh * cfg.L + el) * cfg.N + en)
+    return eh[order], el[order], en[order], eg[order], ei[order], int(gid.numel())
+
+
+def dar_sparse(cfg: Config, device="cpu", s_chunk: int = 8) -> CsrDar:
+    """CsrDar in [c][s][h] block order; same sparsity pattern for every s of a cluster, values per s."""
+    T, H1, L = cfg.T, cfg.H + 1, cfg.L
+    cols, vals, rps, blk_counts = [], [], [], []
+    for c in range(cfg.C):
+        eh, el, en, eg, ei, G = sparse_pattern(cfg, c, device)
+        P = eh.numel()
+        per_row = torch.zeros(H1 * L, dtype=torch.int64, device=device)
+        per_row.index_add_(0, eh * L + el, torch.ones(P, dtype=torch.int64, device=device))
+        rp = torch.zeros((H1, L + 1), dtype=torch.int64, device=device)
+        rp[:, 1:] = torch.cumsum(per_row.view(H1, L), 1)
+        per_blk = rp[:, -1]
+        col32 = en.to(torch.int32)
+        rps.append(rp.to(torch.int32).repeat(T, 1, 1))                          # [T][H1][L+1]
+        blk_counts.append(per_blk.repeat(T))
+        for s0 in range(0, T, s_chunk):
+            s1 = min(T, s0 + s_chunk)
+            S = s1 - s0
+            sidx = torch.arange(s0, s1, dtype=torch.int64, device=device)[:, None]
+            hidx = ((c * T + sidx) * G + eg[None, :]) * 4 + ei[None, :]
+            e = -torch.log(uniform01(cfg.seed, S_SPFRAC, hidx))                 # [S][P]
+            tot = torch.zeros((S, G), dtype=torch.float32, device=device)
+            tot.index_add_(1, eg, e)
+            vals.append((e / tot[:, eg]).reshape(-1))
+            cols.append(col32.repeat(S))
+    per_blk_all = torch.cat(blk_counts)
+    blk_off = torch.zeros(per_blk_all.numel() + 1, dtype=torch.int64, device=device)
+    blk_off[1:] = torch.cumsum(per_blk_all, 0)
+    return CsrDar(blk_off, torch.cat(rps).view(-1, L + 1).contiguous(), torch.cat(cols), torch.cat(vals))
+
+
+def counts_sparse(cfg: Config, csr: CsrDar, qt: torch.Tensor, lab: torch.Tensor, noise: bool = True) -> torch.Tensor:
+    """x_d = rho_{c(d)} q_true,d (+ noise) with library sparse matmuls per (cluster, s) — data synthesis only."""
+    dev = csr.val.device
+    T, H1, L, N = cfg.T, cfg.H + 1, cfg.L, cfg.N
+    acc_dtype = torch.float64 if dev.type == "cpu" else torch.float32
+    x = torch.zeros((cfg.D, T + cfg.H, L), dtype=acc_dtype, device=dev)
+    lab_d = lab.to(dev)
+    for c in range(cfg.C):
+        days = torch.nonzero(lab_d == c).flatten()
+        if days.numel() == 0:
+            continue
+        xc = torch.zeros((T + cfg.H, L, days.numel()), dtype=acc_dtype, device=dev)
+        for s in range(T):
+            b0 = (c * T + s) * H1
+            k0, k1 = int(csr.blk_off[b0]), int(csr.blk_off[b0 + H1])
+            # rows of the stacked [(H+1)*L] x N matrix of departure interval s
+            rp = csr.row_ptr[b0:b0 + H1].to(torch.int64)
+            base = (csr.blk_off[b0:b0 + H1] - k0)[:, None]
+            crow = torch.cat([(rp[:, :-1] + base).reshape(-1), torch.tensor([k1 - k0], device=dev)])
+            with warnings.catch_warnings():
+                warnings.simplefilter("ignore")
+                A = torch.sparse_csr_tensor(crow, csr.col_idx[k0:k1].to(torch.int64), csr.val[k0:k1].to(acc_dtype),
+                                            size=(H1 * L, N))
+            xc[s:s + H1] += (A @ qt[days, s].to(acc_dtype).T).view(H1, L, -1)
+        x[days] = xc.permute(2, 0, 1)
+    x = x[:, :T].contiguous()                       # arrivals after the day are dropped (PAPER.md:333)
+    if noise:
+        idx = torch.arange(x.numel(), dtype=torch.int64, device=dev).view(x.shape)
+        x = torch.clamp(x + 0.05 * x * normal(cfg.seed, S_NOISE, idx, acc_dtype), min=0.0)
+    return x.to(torch.float32)
+
+
+def sparse_problem(cfg: Config, device="cpu"):
+    """(CsrDar, x) for a sparse config, both on ``device``."""
+    csr = dar_sparse(cfg, device)
+    x = counts_sparse(cfg, csr, q_true(cfg, device), labels(cfg))
+    return csr, x
+
+
+def csr_to_dense(cfg: Config, csr: CsrDar) -> torch.Tensor:
+    """[C][T][H+1][L][N] dense copy of a CsrDar (small test instances only)."""
+    R = torch.zeros((cfg.C * cfg.T * (cfg.H + 1), cfg.L, cfg.N), dtype=torch.float32)
+    bo, rp, ci, va = csr.blk_off.cpu(), csr.row_ptr.cpu().to(torch.int64), csr.col_idx.cpu().to(torch.int64), csr.val.cpu()
+    for b in range(R.shape[0]):
+        k0 = int(bo[b])
+        cnt = rp[b, 1:] - rp[b, :-1]
+        rows = torch.repeat_interleave(torch.arange(cfg.L), cnt)
+        k1 = k0 + int(rp[b, -1])
+        R[b, rows, ci[k0:k1]] = va[k0:k1]
+    return R.view(cfg.C, cfg.T, cfg.H + 1, cfg.L, cfg.N)

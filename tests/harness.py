@@ -28,6 +28,12 @@ def make_problem(cfg: synth.Config, noise: bool = True) -> Problem:
     return Problem(cfg, R, lab.numpy(), x, qt)
 
 
+def make_problem_sparse(cfg: synth.Config) -> Problem:
+    """G7 sparse instance (small): generated as CSR, densified for the oracle's dense loops."""
+    csr, x = synth.sparse_problem(cfg)
+    return Problem(cfg, synth.csr_to_dense(cfg, csr), synth.labels(cfg).numpy(), x, synth.q_true(cfg))
+
+
 def oracle_etas(p: Problem, iters: int = 50) -> np.ndarray:
     """eta_c = (float) 1 / L_c with L_c from the oracle's power iteration (O4)."""
     from oracle import oracle

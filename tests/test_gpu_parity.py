@@ -22,8 +22,8 @@ def _objective_cpu(p, q, days):
     return np.array([o.objective_day(p.R[p.labels[d]].numpy(), q[i], p.x[d].numpy()) for i, d in enumerate(days)])
 
 
-def _run_both(cfg, K=None, b=None, sample=None, csr=False):
-    p = hz.make_problem(cfg)
+def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False):
+    p = hz.make_problem_sparse(cfg) if sparse_gen else hz.make_problem(cfg)
     sched = synth.schedule(cfg, p.labels, K=K, b=b)
     etas = hz.oracle_etas(p)
     g = hz.GpuSolver(p, csr=csr)
@@ -166,3 +166,48 @@ def test_batch_composition_invariance_on_gpu():
     g2.run(single, etas)
     hz.assert_q_close(g1.q(), g2.q(), "batch composition")
     g1.close(); g2.close()
+
+
+@pytest.mark.parametrize("b", [1, 5, 33, 70, 130])
+def test_csr_path_on_dense_blocks(b):
+    """P13 through the GPU: the same operator given as CSR gives the oracle's iterates (bp = 32/64/128 and a
+    minibatch larger than one CSR launch)."""
+    cfg = synth.Config("csr_ragged", N=61, L=37, T=30, H=5, C=2, D=280, b=b, K=8, kmin=3, kmax=9)
+    path = _run_both(cfg, csr=True, sample=[0, 3, 100, 279])
+    assert path.startswith("csr_")
+
+
+def test_csr_path_on_generated_sparse_instance():
+    """configs[4]'s structure at small size (G7 windowed lags, heavy-tailed demand, calendar factors)."""
+    cfg = synth.Config("sparse_small", N=400, L=90, T=40, H=10, C=3, D=60, b=24, K=10, kmin=6, kmax=20,
+                       base_mu=1.0, base_sigma=1.2, modulated=True, sparse=True)
+    p = hz.make_problem_sparse(cfg)
+    # the oracle's own CSR loop agrees with its dense loop on this instance (one visit)
+    o = _oracle()
+    csr = synth.dense_to_csr(p.R)
+    nb = cfg.T * (cfg.H + 1)
+    c = int(p.labels[7])
+    eta = hz.oracle_etas(p)[c]
+    q0 = np.ones((cfg.T, cfg.N), np.float32)
+    bo = csr.blk_off.numpy()[c * nb:(c + 1) * nb + 1]
+    qa = o.visit_csr(cfg.N, cfg.L, cfg.T, cfg.H, bo, csr.row_ptr.numpy()[c * nb:(c + 1) * nb], csr.col_idx.numpy(),
+                     csr.val.numpy(), q0, p.x[7].numpy(), eta)
+    np.testing.assert_allclose(qa, o.visit(p.R[c].numpy(), q0, p.x[7].numpy(), eta), rtol=1e-6, atol=1e-6)
+    _run_both(cfg, csr=True, sparse_gen=True, sample=[0, 7, 31, 59])
+
+
+def test_csr_apply_adjoint():
+    cfg = synth.Config("csr_adj", N=45, L=70, T=12, H=4, C=1, D=2, b=2, K=2, kmin=3, kmax=12, label_mode="zero")
+    p = hz.make_problem(cfg)
+    g = hz.GpuSolver(p, csr=True)
+    P, o = g.P, _oracle()
+    gen = torch.Generator().manual_seed(6)
+    u, v = torch.randn(cfg.T, cfg.N, generator=gen), torch.randn(cfg.T, cfg.L, generator=gen)
+    ru, rtv = torch.empty(cfg.T, cfg.L, device="cuda"), torch.empty(cfg.T, cfg.N, device="cuda")
+    P.dode_apply(g.h, 0, u.cuda(), ru)
+    P.dode_apply_t(g.h, 0, v.cuda(), rtv)
+    P.dode_sync(g.h)
+    np.testing.assert_allclose(ru.cpu().numpy(), o.forward_residual(p.R[0].numpy(), u.numpy(), np.zeros((cfg.T, cfg.L), np.float32)), rtol=1e-4, atol=1e-4)
+    np.testing.assert_allclose(rtv.cpu().numpy(), o.gradient(p.R[0].numpy(), v.numpy()), rtol=1e-4, atol=1e-4)
+    assert abs(P.dode_lipschitz(g.h, 0, 40) - o.power_iteration(p.R[0].numpy(), 40)) <= 1e-4 * o.power_iteration(p.R[0].numpy(), 40)
+    g.close()
