@@ -13,6 +13,9 @@
 
 #include "kernels_dense.cuh"
 #include "kernels_csr.cuh"
+#include "kernels_tc.cuh"
+
+#include <cstdlib>
 
 using namespace dode;
 
@@ -40,6 +43,15 @@ struct dode_ctx {
     std::string path;
     char err[512] = {0};
     bool sm_opt_in[8] = {false};
+    // tensor-core path (kernels_tc.cuh)
+    float* Rt = nullptr;         // [C][T][Np][KGp] transposed copy for the gradient pass
+    int KGp = 0;
+    float *Qg_full = nullptr, *Qg_lo = nullptr;   // [tc_cap][T*Np]
+    float *rp_full = nullptr, *rp_lo = nullptr;   // [tc_cap][rpitch]
+    long rpitch = 0;
+    int tc_cap = 0, tc_bn = 0, tc_min_b = 8;
+    bool tc_ready = false, tc_attr = false;
+    CUtensorMap mapA_fwd, mapA_grad, mapQ_f, mapQ_l, mapR_f, mapR_l;
     // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -198,6 +210,149 @@ static int validate_days(dode_ctx* ctx, const int32_t* days, int32_t n, bool sam
     return DODE_OK;
 }
 
+
+// ---- tensor-core path: tensor maps, panels, launches ---------------------------------------------
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_encodeTiled get_encode() {
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (PFN_encodeTiled)p;
+    }
+    return fn;
+}
+
+// fp32 tensor, innermost dim first; box = {32, ...}; SWIZZLE_128B; out-of-bounds elements read as zero
+static int make_map(dode_ctx* ctx, CUtensorMap* m, const void* base, int rank, const uint64_t* dims,
+                    const uint64_t* strides_bytes, const uint32_t* box) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled is unavailable");
+    cuuint64_t gd[3]; cuuint64_t gs[2]; cuuint32_t bx[3]; cuuint32_t es[3] = {1, 1, 1};
+    for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; }
+    for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_bytes[i];
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return DODE_OK;
+}
+
+// create-time: transposed copy + the two A maps
+static int tc_setup(dode_ctx* ctx) {
+    const dode_dims& d = ctx->dm;
+    const int Lp = (d.L + 3) / 4 * 4;
+    ctx->KGp = (d.H + 1) * Lp;
+    ctx->rpitch = (long)d.T * Lp;
+    const size_t rows = (size_t)d.C * d.T * ctx->Np;
+    CU(cudaMalloc(&ctx->Rt, rows * ctx->KGp * sizeof(float)));
+    CU(cudaMemsetAsync(ctx->Rt, 0, rows * ctx->KGp * sizeof(float), ctx->stream));
+    dim3 grid(ceil_div(ctx->Np, 32), (d.H + 1) * ceil_div(Lp, 32), d.C * d.T);
+    tc::transpose_blocks<<<grid, 256, 0, ctx->stream>>>(ctx->R, ctx->Rt, d.H + 1, d.L, Lp, ctx->Np, ctx->KGp);
+    ctx->launches++;
+    {
+        const uint64_t dims[2] = {(uint64_t)ctx->Np, (uint64_t)d.C * d.T * (d.H + 1) * d.L};
+        const uint64_t str[1] = {(uint64_t)ctx->Np * 4};
+        const uint32_t box[2] = {32, 128};
+        int rc = make_map(ctx, &ctx->mapA_fwd, ctx->R, 2, dims, str, box);
+        if (rc) return rc;
+    }
+    {
+        const uint64_t dims[2] = {(uint64_t)ctx->KGp, (uint64_t)rows};
+        const uint64_t str[1] = {(uint64_t)ctx->KGp * 4};
+        const uint32_t box[2] = {32, 128};
+        int rc = make_map(ctx, &ctx->mapA_grad, ctx->Rt, 2, dims, str, box);
+        if (rc) return rc;
+    }
+    ctx->tc_ready = true;
+    return DODE_OK;
+}
+
+static int tc_ensure(dode_ctx* ctx, int bn) {
+    const dode_dims& d = ctx->dm;
+    const size_t qlen = (size_t)d.T * ctx->Np;
+    if (ctx->tc_cap < bn) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
+        ctx->Qg_full = ctx->Qg_lo = ctx->rp_full = ctx->rp_lo = nullptr;
+        ctx->tc_cap = 0; ctx->tc_bn = 0;
+        CU(cudaMalloc(&ctx->Qg_full, bn * qlen * 4)); CU(cudaMalloc(&ctx->Qg_lo, bn * qlen * 4));
+        CU(cudaMalloc(&ctx->rp_full, (size_t)bn * ctx->rpitch * 4)); CU(cudaMalloc(&ctx->rp_lo, (size_t)bn * ctx->rpitch * 4));
+        CU(cudaMemsetAsync(ctx->Qg_full, 0, bn * qlen * 4, ctx->stream)); CU(cudaMemsetAsync(ctx->Qg_lo, 0, bn * qlen * 4, ctx->stream));
+        CU(cudaMemsetAsync(ctx->rp_full, 0, (size_t)bn * ctx->rpitch * 4, ctx->stream));
+        CU(cudaMemsetAsync(ctx->rp_lo, 0, (size_t)bn * ctx->rpitch * 4, ctx->stream));
+        ctx->tc_cap = bn;
+    }
+    if (ctx->tc_bn != bn) {
+        const uint64_t qd[3] = {(uint64_t)ctx->Np, (uint64_t)d.T, (uint64_t)ctx->tc_cap};
+        const uint64_t qs[2] = {(uint64_t)ctx->Np * 4, (uint64_t)qlen * 4};
+        const uint32_t qb[3] = {32, 1, (uint32_t)bn};
+        int rc;
+        if ((rc = make_map(ctx, &ctx->mapQ_f, ctx->Qg_full, 3, qd, qs, qb))) return rc;
+        if ((rc = make_map(ctx, &ctx->mapQ_l, ctx->Qg_lo, 3, qd, qs, qb))) return rc;
+        const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)ctx->tc_cap};
+        const uint64_t rs[1] = {(uint64_t)ctx->rpitch * 4};
+        const uint32_t rb[2] = {32, (uint32_t)bn};
+        if ((rc = make_map(ctx, &ctx->mapR_f, ctx->rp_full, 2, rd, rs, rb))) return rc;
+        if ((rc = make_map(ctx, &ctx->mapR_l, ctx->rp_lo, 2, rd, rs, rb))) return rc;
+        ctx->tc_bn = bn;
+    }
+    if (!ctx->tc_attr) {
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        ctx->tc_attr = true;
+    }
+    return DODE_OK;
+}
+
+// one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
+static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
+    const dode_dims& d = ctx->dm;
+    const int bn = (dl.n + 15) / 16 * 16;
+    int rc = tc_ensure(ctx, bn);
+    if (rc) return rc;
+    const size_t dayStride = (size_t)d.T * ctx->Np;
+    const int stageBytes = 2 * tc::kABytes + 2 * bn * tc::kTileK * 4;
+    int stages = (110 * 1024) / stageBytes;
+    if (stages < 2) stages = std::min(4, (220 * 1024) / stageBytes);
+    stages = std::max(2, std::min(stages, 6));
+    const size_t smem = (size_t)stages * stageBytes + 1024 + 256;
+    {
+        KernelTimer kt(ctx, KIND_OTHER);
+        tc::gather_split<<<dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), 256, 0, ctx->stream>>>(
+            ctx->q, dayStride, (long)dayStride / 4, ctx->Qg_full, ctx->Qg_lo, dl);
+        ctx->launches++;
+    }
+    tc::TcParams p{};
+    p.T = d.T; p.H = d.H; p.L = d.L; p.Lp = (d.L + 3) / 4 * 4; p.Np = ctx->Np; p.bn = bn; p.stages = stages;
+    p.kg_chunks = ceil_div((long)ctx->KGp, tc::kTileK);
+    p.x = ctx->x; p.rp_full = ctx->rp_full; p.rp_lo = ctx->rp_lo; p.rpitch = ctx->rpitch;
+    p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
+    { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
+    {
+        KernelTimer kt(ctx, KIND_FWD);
+        p.mode = 0; p.M = d.L; p.a_row0 = (long)c * d.T * (d.H + 1) * d.L;
+        tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
+            ctx->mapA_fwd, ctx->mapQ_f, ctx->mapQ_l, p, dl);
+        ctx->launches++;
+    }
+    {
+        KernelTimer kt(ctx, KIND_GRAD);
+        p.mode = 1; p.M = d.N; p.a_row0 = (long)c * d.T * ctx->Np;
+        tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
+            ctx->mapA_grad, ctx->mapR_f, ctx->mapR_l, p, dl);
+        ctx->launches++;
+    }
+    char buf[96];
+    snprintf(buf, sizeof buf, "tcgen05_3xtf32_fwd_bn%d+tcgen05_3xtf32_grad_bn%d", bn, bn);
+    ctx->path = buf;
+    return DODE_OK;
+}
+
 static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c) {
     const dode_dims& d = ctx->dm;
     const size_t dayStride = (size_t)d.T * ctx->Np;
@@ -207,6 +362,10 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
         dl.n = std::min(chunk, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
         int bt, bp, rc;
+        if (ctx->tc_ready && dl.n >= ctx->tc_min_b) {
+            if ((rc = tc_step(ctx, c, dl, eta))) return rc;
+            continue;
+        }
         if ((rc = forward_batch(ctx, c, dl, ctx->q, dayStride, ctx->x, nullptr, &bt, &bp))) return rc;
         if (d.storage == DODE_DENSE) {
             if ((rc = grad_dense(ctx, bt, dense_cluster(ctx, c), ctx->r, ctx->q, dayStride, eta, bp, dl))) return rc;
@@ -238,6 +397,7 @@ extern "C" {
 void dode_destroy(dode_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->Rt); cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
     cudaFree(ctx->R); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r);
     for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
@@ -306,6 +466,12 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
             CUC(cudaMemsetAsync(c->R, 0, rows * c->Np * sizeof(float), c->stream));
             CUC(cudaMemcpy2DAsync(c->R, c->Np * sizeof(float), R->dense, d.N * sizeof(float), d.N * sizeof(float), rows,
                                   cudaMemcpyDeviceToDevice, c->stream));
+        }
+        const char* env = getenv("DODE_TC_MIN_B");      // minibatch from which the tensor-core path is used (0 = never)
+        c->tc_min_b = env ? atoi(env) : 8;
+        if (c->tc_min_b > 0) {
+            int rc = tc_setup(c);
+            if (rc) { snprintf(g_create_err, 512, "%s", c->err); dode_destroy(c); cudaGetLastError(); return rc; }
         }
     } else {
         int rc = csr_build(c->csr, d, *R, c->stream, g_create_err);

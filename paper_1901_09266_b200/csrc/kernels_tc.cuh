@@ -1,0 +1,316 @@
+// Tensor-core path of a2-a4 for minibatch b >= 8: banded block GEMMs on tcgen05 (5th-gen tensor
+// cores, FP32 accumulators in TMEM) with 3xTF32 split arithmetic, TMA-staged operands.
+//
+// Per output tile (time index tt, 128 rows m0..m0+127) the pass is one GEMM
+//        D[128 x BN] = sum_k A[128 x K] * B[K x BN]        (BN = b rounded up to 16 days)
+//   forward  (a2): A = rows l of the blocks R[tt-h][h], h = 0..min(H,tt)   (K = (h, n), n contiguous)
+//                  B = gathered state Qg[d][tt-h][n]                        (K contiguous per day)
+//   gradient (a3): A = rows n of the transposed copy Rt[s][n][(h,l)]        (K = (h,l) contiguous)
+//                  B = residual panel rp[d][s*Lp + (h,l)]                   (K contiguous per day)
+// Both operands are K-major, so one kernel serves both passes; only the K enumeration and the epilogue
+// differ.  Truncation at the day boundary falls out of TMA's zero fill: the gradient's B
+// columns beyond T*L are out of bounds.
+//
+// 3xTF32 (north_star: "3xTF32 tensor-core emulation ... where the tolerance still holds"):
+//   a = a_hi + a_lo with a_hi = a truncated to TF32 (what the tensor core reads from an fp32 container),
+//   a_lo = a - a_hi (exact in fp32);   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo   (error ~2^-20 relative).
+//   B_lo panels are produced where B is produced (gather kernel / forward epilogue); A_lo is computed in
+//   shared memory by four "splitter" warps between the TMA landing and the MMA issue, so R is still read
+//   from HBM exactly once per pass.
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 = A_lo
+// splitters during the K loop, then the epilogue (TMEM -> registers -> global, fused -x / projected update).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "kernels_dense.cuh"
+
+namespace dode {
+namespace tc {
+
+constexpr int kThreadsTC = 192;
+constexpr int kTileM = 128;
+constexpr int kTileK = 32;                       // 32 fp32 = 128 B = one SWIZZLE_128B span
+constexpr int kABytes = kTileM * kTileK * 4;     // 16 KB
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.b32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+// K-major SWIZZLE_128B shared-memory matrix descriptor (sm_100 format): rows of 128 B, 8-row groups 1024 B apart.
+__device__ __forceinline__ uint64_t umma_desc_k_sw128(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);          // start address, 16-byte units
+    d |= (uint64_t)1 << 16;                            // leading byte offset (unused for swizzled K-major)
+    d |= (uint64_t)(1024 >> 4) << 32;                  // stride byte offset: 8 rows x 128 B
+    d |= (uint64_t)1 << 46;                            // descriptor version (Blackwell)
+    d |= (uint64_t)2 << 61;                            // layout type SWIZZLE_128B
+    return d;
+}
+
+// kind::tf32 instruction descriptor: D = F32, A = B = TF32, both K-major, M = 128, N = bn.
+__host__ __device__ constexpr uint32_t umma_idesc_tf32(int bn) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+}
+
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+struct TcParams {
+    int mode;            // 0 = forward, 1 = gradient
+    int M;               // valid output rows per time index (L forward, N gradient)
+    int T, H, L, Lp, Np;
+    int bn;              // MMA N (days rounded up to 16)
+    int stages;
+    long a_row0;         // first row of this cluster in the A tensor map
+    int kg_chunks;       // gradient: ceil((H+1)*L / 32)
+    // epilogue
+    const float* x;      // [D][T][L]        (forward)
+    float* rp_full;      // [bcap][rpitch]   (forward output / gradient B operand)
+    float* rp_lo;
+    long rpitch;
+    float* q;            // [D][T][Np]       (gradient, in place)
+    size_t dayStride;
+    float eta;
+    int dbg;             // bring-up switch: 0 = full kernel
+};
+
+template <int DUMMY = 0>
+__global__ void __launch_bounds__(kThreadsTC)
+banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapBf,
+                   const __grid_constant__ CUtensorMap mapBl, const __grid_constant__ TcParams p,
+                   const __grid_constant__ DayList dl) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
+    const int m0 = blockIdx.x * kTileM;
+    const int bBytes = p.bn * kTileK * 4;
+    const int stageBytes = 2 * kABytes + 2 * bBytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stageBytes);
+    uint64_t* full = bars;                        // [stages] TMA landed
+    uint64_t* split = bars + p.stages;            // [stages] A_lo written
+    uint64_t* empty = bars + 2 * p.stages;        // [stages] MMAs of the stage retired
+    uint64_t* accum = bars + 3 * p.stages;        // accumulator complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * p.stages + 1);
+
+    const int kchunks_per_lag = (p.Np + kTileK - 1) / kTileK;
+    int nk;
+    if (p.mode == 0) nk = (min(p.H, tt) + 1) * kchunks_per_lag;
+    else             nk = min(p.kg_chunks, ((min(p.H, p.T - 1 - tt) + 1) * p.Lp + kTileK - 1) / kTileK);
+
+    uint32_t tmem_cols = 32;
+    while ((int)tmem_cols < p.bn) tmem_cols <<= 1;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&split[s], 128); mbar_init(&empty[s], 1); }
+        mbar_init(accum, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBf) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBl) : "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_d = *tmem_slot;
+
+    if (p.dbg == 1) {
+    } else if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            for (int kc = 0; kc < nk; ++kc) {
+                const int s = kc % p.stages, round = kc / p.stages;
+                if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
+                uint8_t* st = smem + (size_t)s * stageBytes;
+                mbar_expect_tx(&full[s], kABytes + 2 * bBytes);
+                if (p.mode == 0) {
+                    const int h = kc / kchunks_per_lag, j = kc - h * kchunks_per_lag;
+                    const long arow = p.a_row0 + ((long)(tt - h) * (p.H + 1) + h) * p.L + m0;
+                    tma_load_2d(st, &mapA, &full[s], j * kTileK, (int)arow);
+                    tma_load_3d(st + 2 * kABytes, &mapBf, &full[s], j * kTileK, tt - h, 0);
+                    tma_load_3d(st + 2 * kABytes + bBytes, &mapBl, &full[s], j * kTileK, tt - h, 0);
+                } else {
+                    const long arow = p.a_row0 + (long)tt * p.Np + m0;
+                    tma_load_2d(st, &mapA, &full[s], kc * kTileK, (int)arow);
+                    tma_load_2d(st + 2 * kABytes, &mapBf, &full[s], tt * p.Lp + kc * kTileK, 0);
+                    tma_load_2d(st + 2 * kABytes + bBytes, &mapBl, &full[s], tt * p.Lp + kc * kTileK, 0);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0) {
+            const uint32_t idesc = umma_idesc_tf32(p.bn);
+            for (int kc = 0; kc < nk; ++kc) {
+                const int s = kc % p.stages, round = kc / p.stages;
+                mbar_wait(&full[s], round & 1);
+                mbar_wait(&split[s], round & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t a0 = smem_u32(smem + (size_t)s * stageBytes);
+                const uint32_t al0 = a0 + kABytes, bf0 = a0 + 2 * kABytes, bl0 = bf0 + bBytes;
+#pragma unroll
+                for (int k = 0; k < kTileK / 8; ++k) {           // UMMA_K = 8 for tf32: 32 bytes along the span
+                    const uint64_t da = umma_desc_k_sw128(a0 + k * 32), dal = umma_desc_k_sw128(al0 + k * 32);
+                    const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32), dbl = umma_desc_k_sw128(bl0 + k * 32);
+                    if (p.dbg == 2) continue;
+                    umma_tf32(tmem_d, da, dbf, idesc, (kc | k) != 0);   // a_hi * b_hi
+                    umma_tf32(tmem_d, dal, dbf, idesc, 1);              // a_lo * b_hi
+                    umma_tf32(tmem_d, da, dbl, idesc, 1);               // a_hi * b_lo
+                }
+                if (p.dbg == 2) mbar_arrive(&empty[s]); else umma_commit(&empty[s]);
+            }
+            if (p.dbg == 2) mbar_arrive(accum); else umma_commit(accum);
+        }
+    } else {
+        // ===== A_lo splitters (warps 2-5), then epilogue =====
+        const int st_tid = threadIdx.x - 64;                    // 0..127
+        for (int kc = 0; kc < nk; ++kc) {
+            const int s = kc % p.stages, round = kc / p.stages;
+            mbar_wait(&full[s], round & 1);
+            const float4* A = reinterpret_cast<const float4*>(smem + (size_t)s * stageBytes);
+            float4* Al = reinterpret_cast<float4*>(smem + (size_t)s * stageBytes + kABytes);
+#pragma unroll
+            for (int j = 0; j < kABytes / 16 / 128; ++j) {
+                const float4 v = A[st_tid + 128 * j];
+                float4 lo;
+                lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
+                lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
+                lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
+                lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
+                Al[st_tid + 128 * j] = lo;
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (UMMA) reads
+            mbar_arrive(&split[s]);
+        }
+        // ---- epilogue: TMEM lane = output row; a warp may touch lanes 32*(warp%4) .. +31 ----
+        mbar_wait(accum, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const int lane_base = (warp & 3) * 32;
+        const int m = m0 + lane_base + lane;
+        for (int c0 = 0; c0 < p.bn && p.dbg != 2 && p.dbg != 3; c0 += 16) {
+            uint32_t v[16];
+            const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
+            asm volatile(
+                "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                  "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                : "r"(taddr) : "memory");
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (m < p.M) {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int d = c0 + j;
+                    if (d < dl.n) {
+                        const float acc = __uint_as_float(v[j]);
+                        if (p.mode == 0) {
+                            const float r = acc - __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.L + m);
+                            const float hi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
+                            p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
+                            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - hi;
+                        } else {
+                            float* qp = p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
+                            *qp = fmaxf(0.f, fmaf(-p.eta, acc, *qp));
+                        }
+                    }
+                }
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(tmem_cols) : "memory");
+    }
+}
+
+// a1 for the tensor path: Qg_full[d][i] = q[day_d][i], Qg_lo[d][i] = q - trunc_tf32(q), i over T*Np (float4 wide)
+__global__ void __launch_bounds__(256)
+gather_split(const float* __restrict__ q, size_t dayStride, long len4, float* __restrict__ gfull, float* __restrict__ glo,
+             const __grid_constant__ DayList dl) {
+    const int d = blockIdx.y;
+    const float4* src = reinterpret_cast<const float4*>(q + (size_t)dl.day[d] * dayStride);
+    float4* f = reinterpret_cast<float4*>(gfull + (size_t)d * dayStride);
+    float4* l = reinterpret_cast<float4*>(glo + (size_t)d * dayStride);
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < len4; i += (long)gridDim.x * blockDim.x) {
+        const float4 v = __ldg(src + i);
+        float4 lo;
+        lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
+        lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
+        lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
+        lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
+        f[i] = v;
+        l[i] = lo;
+    }
+}
+
+// create-time: Rt[c][s][n][h*Lp + l] = R[c][s][h][l][n] (Lp = L rounded up to 4 so that every TMA box of the
+// gradient's B operand starts 16-byte aligned; pad columns are 0).  One 32x32 tile per block.
+__global__ void __launch_bounds__(256)
+transpose_blocks(const float* __restrict__ R, float* __restrict__ Rt, int H1, int L, int Lp, int Np, int KGp) {
+    __shared__ float tile[32][33];
+    const size_t cs = blockIdx.z;                                  // (c*T + s)
+    const int ltiles = (Lp + 31) / 32;
+    const int h = blockIdx.y / ltiles, l0 = (blockIdx.y - h * ltiles) * 32, n0 = blockIdx.x * 32;
+    const float* src = R + (cs * H1 + h) * (size_t)L * Np;
+    float* dst = Rt + cs * (size_t)Np * KGp + (size_t)h * Lp;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int ll = ty; ll < 32; ll += 8) {
+        const int l = l0 + ll, n = n0 + tx;
+        tile[ll][tx] = (l < L && n < Np) ? src[(size_t)l * Np + n] : 0.f;
+    }
+    __syncthreads();
+    for (int nn = ty; nn < 32; nn += 8) {
+        const int n = n0 + nn, l = l0 + tx;
+        if (n < Np && l < Lp) dst[(size_t)n * KGp + l] = tile[tx][nn];
+    }
+}
+
+}  // namespace tc
+}  // namespace dode

@@ -55,8 +55,13 @@ def oracle_run(p: Problem, sched, etas: np.ndarray, sample_days: Optional[Sequen
 class GpuSolver:
     """Owns one dode ctx on cuda:0 for a Problem."""
 
-    def __init__(self, p: Problem, csr: bool = False, q0: float = 1.0):
+    def __init__(self, p: Problem, csr: bool = False, q0: float = 1.0, tc_min_b: Optional[int] = None):
+        import os
         import paper_1901_09266_b200 as P
+        if tc_min_b is None:
+            os.environ.pop("DODE_TC_MIN_B", None)
+        else:
+            os.environ["DODE_TC_MIN_B"] = str(tc_min_b)      # read by dode_create
         self.P, self.p = P, p
         cfg = p.cfg
         dev = torch.device("cuda:0")

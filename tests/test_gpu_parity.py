@@ -22,11 +22,11 @@ def _objective_cpu(p, q, days):
     return np.array([o.objective_day(p.R[p.labels[d]].numpy(), q[i], p.x[d].numpy()) for i, d in enumerate(days)])
 
 
-def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False):
+def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False, tc_min_b=None):
     p = hz.make_problem_sparse(cfg) if sparse_gen else hz.make_problem(cfg)
     sched = synth.schedule(cfg, p.labels, K=K, b=b)
     etas = hz.oracle_etas(p)
-    g = hz.GpuSolver(p, csr=csr)
+    g = hz.GpuSolver(p, csr=csr, tc_min_b=tc_min_b)
     g.run(sched, etas)
     days = list(range(cfg.D)) if sample is None else list(sample)
     q_gpu = g.q(days)
@@ -57,10 +57,25 @@ def test_tiny12_sub_instance():
 
 
 @pytest.mark.parametrize("b", [1, 2, 3, 5, 8, 11, 20, 37])
-def test_ragged_shapes_and_minibatch_widths(b):
-    """N, L not multiples of 4/8 (padding paths), every BT specialisation, ragged last chunks, pad days."""
+def test_ragged_shapes_and_minibatch_widths_ffma(b):
+    """FFMA kernels only (tensor path off): N, L not multiples of 4/8 (padding paths), every BT specialisation,
+    ragged last chunks, pad days."""
     cfg = synth.Config("ragged", N=61, L=37, T=50, H=5, C=3, D=90, b=b, K=24, kmin=3, kmax=9)
-    _run_both(cfg)
+    assert "ffma" in _run_both(cfg, tc_min_b=0)
+
+
+@pytest.mark.parametrize("b", [8, 11, 16, 20, 37, 64])
+def test_ragged_shapes_tensor_core_path(b):
+    """tcgen05 3xTF32 path: ragged N/L (zero-filled K tails, partial M tiles), pad days, ragged chunks
+    (chunks of fewer than 8 days fall back to the FFMA kernels inside the same run)."""
+    cfg = synth.Config("ragged", N=61, L=37, T=50, H=5, C=3, D=200, b=b, K=24, kmin=3, kmax=9)
+    _run_both(cfg, sample=[0, 1, 50, 99, 150, 199])
+
+
+def test_tensor_core_path_multi_tile():
+    """Several 128-row tiles in both passes (L=300, N=270), K tails, H >= 1 lags, 2 CTAs per SM."""
+    cfg = synth.Config("tc_tiles", N=270, L=300, T=24, H=4, C=2, D=80, b=24, K=8, kmin=5, kmax=20)
+    assert "tcgen05" in _run_both(cfg, sample=[0, 11, 40, 79])
 
 
 def test_corridor_shape_reduced_T():
