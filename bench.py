@@ -33,12 +33,16 @@ UNIT = "ms/epoch"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 flop x clocks.max.sm
 
 
+TF32_OVER_BF16 = 1.1 / 2.25      # nominal dense tensor ratio (B200_PROFILING.md): tf32 1.1 PF vs bf16 2.25 PF
+
+
 def measured_peaks():
+    """(HBM GB/s, bf16 TFLOP/s burst, source) from the driver-written MEASURED_PEAKS.json, else the guide's fallback."""
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
-        return float(d["hbm_gbs"]), "measured"
-    return 6650.0, "fallback"
+        return float(d["hbm_gbs"]), float(d["bf16_tflops"]), "measured"
+    return 6650.0, 1590.0, "fallback"
 
 
 class ClockSampler(threading.Thread):
@@ -261,16 +265,23 @@ def run_ours(args, cfg, b, rank, world, local_rank):
             else:
                 f_b, g_b, f_l = algorithmic(cfg, len(days))
             fb += f_b; gb += g_b; fl += f_l
-    hbm_peak, peak_src = measured_peaks()
+    hbm_peak, bf16_peak, peak_src = measured_peaks()
+    tensor_path = path.startswith("tcgen05")
+    # 3xTF32: three tf32 MMAs per fp32 product, so the fp32-equivalent tensor peak is tf32 peak / 3
+    tc_peak = bf16_peak * TF32_OVER_BF16 / 3.0
     dom = "forward" if fwd_ms >= grad_ms else "gradient_update"
     d_ms, d_n, d_bytes = (fwd_ms, fwd_n, fb) if dom == "forward" else (grad_ms, grad_n, gb)
     gbs = d_bytes / (d_ms * 1e-3) / 1e9 if d_ms > 0 else 0.0
     tfl = fl / (d_ms * 1e-3) / 1e12 if d_ms > 0 else 0.0
-    t_hbm, t_alu = d_bytes / (hbm_peak * 1e9), fl / (FP32_PEAK_TFLOPS * 1e12)
+    t_hbm = d_bytes / (hbm_peak * 1e9)
+    t_alu = fl / ((tc_peak if tensor_path else FP32_PEAK_TFLOPS) * 1e12)
     kname = path.split("+")[0 if dom == "forward" else 1] if "+" in path else path
     if t_hbm >= t_alu:
         roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"}
+    elif tensor_path:
+        roof = {"bound": "tensor", "achieved": tfl, "peak": tc_peak, "unit": "TFLOP/s", "frac": tfl / tc_peak,
+                "peak_source": f"MEASURED_PEAKS.json bf16_tflops ({peak_src}) x 1.1/2.25 (tf32) / 3 (3xTF32 MMAs per product)"}
     else:
         roof = {"bound": "alu", "achieved": tfl, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": tfl / FP32_PEAK_TFLOPS, "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)"}

@@ -316,11 +316,17 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     int rc = tc_ensure(ctx, bn);
     if (rc) return rc;
     const size_t dayStride = (size_t)d.T * ctx->Np;
-    const int stageBytes = 2 * tc::kABytes + 2 * bn * tc::kTileK * 4;
-    int stages = (110 * 1024) / stageBytes;
-    if (stages < 2) stages = std::min(4, (220 * 1024) / stageBytes);
-    stages = std::max(2, std::min(stages, 6));
-    const size_t smem = (size_t)stages * stageBytes + 1024 + 256;
+    // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles; plus a 2-deep A_lo ring.  Short K loops and
+    // few tiles (small networks): 2 CTAs per SM so that one CTA's prologue/epilogue overlaps the other's
+    // main loop; otherwise one CTA per SM with the deepest ring that fits.
+    const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
+    const long tiles = (long)ceil_div(std::max(d.L, d.N), tc::kTileM) * d.T;
+    const int fixed = 2 * tc::kABytes + 1024 + 256;
+    int stages = (112 * 1024 - fixed) / stageBytes;
+    if (stages < 3) stages = (226 * 1024 - fixed) / stageBytes;
+    (void)tiles;
+    stages = std::max(2, std::min(stages, 10));
+    const size_t smem = (size_t)stages * stageBytes + fixed;
     {
         KernelTimer kt(ctx, KIND_OTHER);
         tc::gather_split<<<dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), 256, 0, ctx->stream>>>(

@@ -18,8 +18,10 @@
 //   shared memory by four "splitter" warps between the TMA landing and the MMA issue, so R is still read
 //   from HBM exactly once per pass.
 //
-// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 = A_lo
-// splitters during the K loop, then the epilogue (TMEM -> registers -> global, fused -x / projected update).
+// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 and 6-9 = two
+// groups of A_lo splitters that take alternate K chunks (each owns one A_lo buffer, so two split chains are
+// in flight), then the epilogue (TMEM -> registers -> global, fused -x / projected update), column chunks
+// interleaved between the groups.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -30,7 +32,7 @@
 namespace dode {
 namespace tc {
 
-constexpr int kThreadsTC = 192;
+constexpr int kThreadsTC = 320;
 constexpr int kTileM = 128;
 constexpr int kTileK = 32;                       // 32 fp32 = 128 B = one SWIZZLE_128B span
 constexpr int kABytes = kTileM * kTileK * 4;     // 16 KB
@@ -127,13 +129,17 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
     const int m0 = blockIdx.x * kTileM;
     const int bBytes = p.bn * kTileK * 4;
-    const int stageBytes = 2 * kABytes + 2 * bBytes;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stageBytes);
+    // smem: [stages x (A | B_full | B_lo)] [2 x A_lo] [barriers]; the A_lo ring is shorter than the TMA ring
+    // because A_lo only lives from the split to the retirement of its MMAs
+    const int stageBytes = kABytes + 2 * bBytes;
+    uint8_t* alo_base = smem + (size_t)p.stages * stageBytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(alo_base + 2 * kABytes);
     uint64_t* full = bars;                        // [stages] TMA landed
-    uint64_t* split = bars + p.stages;            // [stages] A_lo written
-    uint64_t* empty = bars + 2 * p.stages;        // [stages] MMAs of the stage retired
-    uint64_t* accum = bars + 3 * p.stages;        // accumulator complete
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * p.stages + 1);
+    uint64_t* empty = bars + p.stages;            // [stages] MMAs of the stage retired
+    uint64_t* split = bars + 2 * p.stages;        // [2] A_lo written
+    uint64_t* alo_empty = split + 2;              // [2] MMAs that read this A_lo buffer retired
+    uint64_t* accum = alo_empty + 2;              // accumulator complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
 
     const int kchunks_per_lag = (p.Np + kTileK - 1) / kTileK;
     int nk;
@@ -144,7 +150,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     while ((int)tmem_cols < p.bn) tmem_cols <<= 1;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&split[s], 128); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int j = 0; j < 2; ++j) { mbar_init(&split[j], 128); mbar_init(&alo_empty[j], 1); }
         mbar_init(accum, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
@@ -173,13 +180,13 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                     const int h = kc / kchunks_per_lag, j = kc - h * kchunks_per_lag;
                     const long arow = p.a_row0 + ((long)(tt - h) * (p.H + 1) + h) * p.L + m0;
                     tma_load_2d(st, &mapA, &full[s], j * kTileK, (int)arow);
-                    tma_load_3d(st + 2 * kABytes, &mapBf, &full[s], j * kTileK, tt - h, 0);
-                    tma_load_3d(st + 2 * kABytes + bBytes, &mapBl, &full[s], j * kTileK, tt - h, 0);
+                    tma_load_3d(st + kABytes, &mapBf, &full[s], j * kTileK, tt - h, 0);
+                    tma_load_3d(st + kABytes + bBytes, &mapBl, &full[s], j * kTileK, tt - h, 0);
                 } else {
                     const long arow = p.a_row0 + (long)tt * p.Np + m0;
                     tma_load_2d(st, &mapA, &full[s], kc * kTileK, (int)arow);
-                    tma_load_2d(st + 2 * kABytes, &mapBf, &full[s], tt * p.Lp + kc * kTileK, 0);
-                    tma_load_2d(st + 2 * kABytes + bBytes, &mapBl, &full[s], tt * p.Lp + kc * kTileK, 0);
+                    tma_load_2d(st + kABytes, &mapBf, &full[s], tt * p.Lp + kc * kTileK, 0);
+                    tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], tt * p.Lp + kc * kTileK, 0);
                 }
             }
         }
@@ -189,11 +196,12 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             const uint32_t idesc = umma_idesc_tf32(p.bn);
             for (int kc = 0; kc < nk; ++kc) {
                 const int s = kc % p.stages, round = kc / p.stages;
+                const int jb = kc & 1;
                 mbar_wait(&full[s], round & 1);
-                mbar_wait(&split[s], round & 1);
+                mbar_wait(&split[jb], (kc >> 1) & 1);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t a0 = smem_u32(smem + (size_t)s * stageBytes);
-                const uint32_t al0 = a0 + kABytes, bf0 = a0 + 2 * kABytes, bl0 = bf0 + bBytes;
+                const uint32_t al0 = smem_u32(alo_base + (size_t)jb * kABytes), bf0 = a0 + kABytes, bl0 = bf0 + bBytes;
 #pragma unroll
                 for (int k = 0; k < kTileK / 8; ++k) {           // UMMA_K = 8 for tf32: 32 bytes along the span
                     const uint64_t da = umma_desc_k_sw128(a0 + k * 32), dal = umma_desc_k_sw128(al0 + k * 32);
@@ -203,18 +211,22 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                     umma_tf32(tmem_d, dal, dbf, idesc, 1);              // a_lo * b_hi
                     umma_tf32(tmem_d, da, dbl, idesc, 1);               // a_hi * b_lo
                 }
-                if (p.dbg == 2) mbar_arrive(&empty[s]); else umma_commit(&empty[s]);
+                if (p.dbg == 2) { mbar_arrive(&empty[s]); mbar_arrive(&alo_empty[jb]); }
+                else { umma_commit(&empty[s]); umma_commit(&alo_empty[jb]); }
             }
             if (p.dbg == 2) mbar_arrive(accum); else umma_commit(accum);
         }
     } else {
-        // ===== A_lo splitters (warps 2-5), then epilogue =====
-        const int st_tid = threadIdx.x - 64;                    // 0..127
-        for (int kc = 0; kc < nk; ++kc) {
+        // ===== A_lo splitters (group 0 = warps 2-5: even chunks, group 1 = warps 6-9: odd chunks), then epilogue =====
+        const int group = (warp - 2) >> 2;
+        const int st_tid = threadIdx.x - 64 - 128 * group;      // 0..127
+        for (int kc = group; kc < nk; kc += 2) {
             const int s = kc % p.stages, round = kc / p.stages;
+            const int jb = group;
             mbar_wait(&full[s], round & 1);
+            if (kc >= 2) mbar_wait(&alo_empty[jb], ((kc >> 1) - 1) & 1);
             const float4* A = reinterpret_cast<const float4*>(smem + (size_t)s * stageBytes);
-            float4* Al = reinterpret_cast<float4*>(smem + (size_t)s * stageBytes + kABytes);
+            float4* Al = reinterpret_cast<float4*>(alo_base + (size_t)jb * kABytes);
 #pragma unroll
             for (int j = 0; j < kABytes / 16 / 128; ++j) {
                 const float4 v = A[st_tid + 128 * j];
@@ -226,14 +238,14 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 Al[st_tid + 128 * j] = lo;
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (UMMA) reads
-            mbar_arrive(&split[s]);
+            mbar_arrive(&split[jb]);
         }
         // ---- epilogue: TMEM lane = output row; a warp may touch lanes 32*(warp%4) .. +31 ----
         mbar_wait(accum, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int lane_base = (warp & 3) * 32;
         const int m = m0 + lane_base + lane;
-        for (int c0 = 0; c0 < p.bn && p.dbg != 2 && p.dbg != 3; c0 += 16) {
+        for (int c0 = 16 * group; c0 < p.bn && p.dbg != 2 && p.dbg != 3; c0 += 32) {
             uint32_t v[16];
             const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
             asm volatile(
