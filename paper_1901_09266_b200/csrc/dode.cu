@@ -51,7 +51,7 @@ struct dode_ctx {
     long rpitch = 0;
     int tc_cap = 0, tc_bn = 0, tc_min_b = 8;
     bool tc_ready = false, tc_attr = false;
-    CUtensorMap mapA_fwd, mapA_grad, mapQ_f, mapQ_l, mapR_f, mapR_l;
+    CUtensorMap mapA_fwd, mapA_grad, mapA_fwd64, mapA_grad64, mapQ_f, mapQ_l, mapR_f, mapR_l;
     // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -258,16 +258,18 @@ static int tc_setup(dode_ctx* ctx) {
     {
         const uint64_t dims[2] = {(uint64_t)ctx->Np, (uint64_t)d.C * d.T * (d.H + 1) * d.L};
         const uint64_t str[1] = {(uint64_t)ctx->Np * 4};
-        const uint32_t box[2] = {32, 128};
+        const uint32_t box[2] = {32, 128}, box64[2] = {32, 64};
         int rc = make_map(ctx, &ctx->mapA_fwd, ctx->R, 2, dims, str, box);
         if (rc) return rc;
+        if ((rc = make_map(ctx, &ctx->mapA_fwd64, ctx->R, 2, dims, str, box64))) return rc;
     }
     {
         const uint64_t dims[2] = {(uint64_t)ctx->KGp, (uint64_t)rows};
         const uint64_t str[1] = {(uint64_t)ctx->KGp * 4};
-        const uint32_t box[2] = {32, 128};
+        const uint32_t box[2] = {32, 128}, box64[2] = {32, 64};
         int rc = make_map(ctx, &ctx->mapA_grad, ctx->Rt, 2, dims, str, box);
         if (rc) return rc;
+        if ((rc = make_map(ctx, &ctx->mapA_grad64, ctx->Rt, 2, dims, str, box64))) return rc;
     }
     ctx->tc_ready = true;
     return DODE_OK;
@@ -304,6 +306,7 @@ static int tc_ensure(dode_ctx* ctx, int bn) {
     }
     if (!ctx->tc_attr) {
         CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->tc_attr = true;
     }
     return DODE_OK;
@@ -316,15 +319,18 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     int rc = tc_ensure(ctx, bn);
     if (rc) return rc;
     const size_t dayStride = (size_t)d.T * ctx->Np;
-    // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles; plus a 2-deep A_lo ring.  Short K loops and
-    // few tiles (small networks): 2 CTAs per SM so that one CTA's prologue/epilogue overlaps the other's
-    // main loop; otherwise one CTA per SM with the deepest ring that fits.
+    // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  TS kernel (default): A_hi/A_lo live in TMEM,
+    // 2 CTAs per SM when 3 stages fit in half the shared memory and 256 TMEM columns suffice.
+    static const bool use_ss = getenv("DODE_TC_KERNEL") && !strcmp(getenv("DODE_TC_KERNEL"), "ss");
     const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
-    const long tiles = (long)ceil_div(std::max(d.L, d.N), tc::kTileM) * d.T;
-    const int fixed = 2 * tc::kABytes + 1024 + 256;
+    const int fixed = (use_ss ? 2 * tc::kABytes : 0) + 1024 + 256;
+    const int acc_cols = bn <= 128 ? 2 * bn : bn;
     int stages = (112 * 1024 - fixed) / stageBytes;
-    if (stages < 3) stages = (226 * 1024 - fixed) / stageBytes;
-    (void)tiles;
+    int nring = 2;
+    if (stages < 3 || (!use_ss && acc_cols + 128 > 256)) {          // one CTA per SM
+        stages = (226 * 1024 - fixed) / stageBytes;
+        nring = acc_cols + 256 <= 512 ? 4 : 2;
+    }
     stages = std::max(2, std::min(stages, 10));
     const size_t smem = (size_t)stages * stageBytes + fixed;
     {
@@ -339,18 +345,27 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     p.x = ctx->x; p.rp_full = ctx->rp_full; p.rp_lo = ctx->rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
+    p.nring = nring;
     {
         KernelTimer kt(ctx, KIND_FWD);
         p.mode = 0; p.M = d.L; p.a_row0 = (long)c * d.T * (d.H + 1) * d.L;
-        tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
-            ctx->mapA_fwd, ctx->mapQ_f, ctx->mapQ_l, p, dl);
+        if (use_ss)
+            tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
+                ctx->mapA_fwd, ctx->mapQ_f, ctx->mapQ_l, p, dl);
+        else
+            tc::banded_gemm_3xtf32_ts<<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
+                ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl);
         ctx->launches++;
     }
     {
         KernelTimer kt(ctx, KIND_GRAD);
         p.mode = 1; p.M = d.N; p.a_row0 = (long)c * d.T * ctx->Np;
-        tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
-            ctx->mapA_grad, ctx->mapR_f, ctx->mapR_l, p, dl);
+        if (use_ss)
+            tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
+                ctx->mapA_grad, ctx->mapR_f, ctx->mapR_l, p, dl);
+        else
+            tc::banded_gemm_3xtf32_ts<<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
+                ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl);
         ctx->launches++;
     }
     char buf[96];

@@ -116,6 +116,7 @@ struct TcParams {
     size_t dayStride;
     float eta;
     int dbg;             // bring-up switch: 0 = full kernel
+    int nring;           // TS kernel: TMEM A buffers (2 or 4)
 };
 
 template <int DUMMY = 0>
@@ -265,6 +266,218 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                             const float hi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
                             p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
                             p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - hi;
+                        } else {
+                            float* qp = p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
+                            *qp = fmaxf(0.f, fmaf(-p.eta, acc, *qp));
+                        }
+                    }
+                }
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(tmem_cols) : "memory");
+    }
+}
+
+
+// =====================================================================================================
+// v2 ("TS mode"): A operands in tensor memory.
+// Shared-memory bandwidth bounds the SS kernel above: every MMA re-reads its 128x8 A slice from smem
+// (3 MMAs x 4 K-steps x 4 KB per chunk) on top of the splitters' 16 KB read + 16 KB write.  Here the
+// splitter threads read their A row ONCE from the TMA-landed (swizzled) tile into registers and store both
+// A_hi (the fp32 container; the tensor core truncates it to TF32) and A_lo = a - trunc(a) into TMEM with
+// tcgen05.st; tcgen05.mma then takes A from TMEM, so smem only carries the TMA writes, one 16 KB read and
+// the B slices.  For bn <= 128 the B_full and B_lo tiles, adjacent in smem, are fed as ONE N = 2*bn
+// operand: D[:, 0:bn] += A_hi*B_full (+ A_lo*B_full by a second MMA), D[:, bn:2bn] += A_hi*B_lo, and the
+// epilogue adds the two halves -> 2 MMAs per K-step instead of 3.
+// TMEM columns: [0, acc_cols) accumulators, then nring x (32 cols A_hi | 32 cols A_lo).
+// =====================================================================================================
+__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
+
+__global__ void __launch_bounds__(kThreadsTC)
+banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA64,
+                      const __grid_constant__ CUtensorMap mapBf,
+                      const __grid_constant__ CUtensorMap mapBl, const __grid_constant__ TcParams p,
+                      const __grid_constant__ DayList dl) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tt = blockIdx.y;
+    const int m0 = blockIdx.x * kTileM;
+    const int bBytes = p.bn * kTileK * 4;
+    const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full | B_lo
+    const int nring = p.nring;                                   // TMEM A buffers (2 or 4), half per splitter group
+    // a tile with <= 64 valid rows (small networks, ragged last tile) fetches and splits only 64 rows of A; the
+    // MMA still runs M = 128 and the upper accumulator rows are never stored
+    const bool half = p.M - m0 <= 64;
+    const int aBytes = half ? kABytes / 2 : kABytes;
+    const CUtensorMap* mA = half ? &mapA64 : &mapA;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stageBytes);
+    uint64_t* full = bars;                        // [stages] TMA landed
+    uint64_t* empty = bars + p.stages;            // [stages] MMAs of the stage retired
+    uint64_t* split = bars + 2 * p.stages;        // [nring] A_hi/A_lo in TMEM
+    uint64_t* a_empty = split + 4;                // [nring] MMAs that read this TMEM buffer retired
+    uint64_t* accum = a_empty + 4;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
+
+    const int kchunks_per_lag = (p.Np + kTileK - 1) / kTileK;
+    int nk;
+    if (p.mode == 0) nk = (min(p.H, tt) + 1) * kchunks_per_lag;
+    else             nk = min(p.kg_chunks, ((min(p.H, p.T - 1 - tt) + 1) * p.Lp + kTileK - 1) / kTileK);
+
+    const bool fused_n = p.bn <= 128;
+    const int acc_cols = fused_n ? 2 * p.bn : p.bn;
+    uint32_t tmem_cols = 32;
+    while ((int)tmem_cols < acc_cols + 64 * nring) tmem_cols <<= 1;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int j = 0; j < nring; ++j) { mbar_init(&split[j], 128); mbar_init(&a_empty[j], 1); }
+        mbar_init(accum, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(mA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBf) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBl) : "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_d = *tmem_slot;
+    const uint32_t tmem_ring = tmem_d + (uint32_t)acc_cols;
+    const int per_group = nring >> 1;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            for (int kc = 0; kc < nk; ++kc) {
+                const int s = kc % p.stages, round = kc / p.stages;
+                if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
+                uint8_t* st = smem + (size_t)s * stageBytes;
+                mbar_expect_tx(&full[s], aBytes + 2 * bBytes);
+                if (p.mode == 0) {
+                    const int h = kc / kchunks_per_lag, j = kc - h * kchunks_per_lag;
+                    const long arow = p.a_row0 + ((long)(tt - h) * (p.H + 1) + h) * p.L + m0;
+                    tma_load_2d(st, mA, &full[s], j * kTileK, (int)arow);
+                    tma_load_3d(st + kABytes, &mapBf, &full[s], j * kTileK, tt - h, 0);
+                    tma_load_3d(st + kABytes + bBytes, &mapBl, &full[s], j * kTileK, tt - h, 0);
+                } else {
+                    const long arow = p.a_row0 + (long)tt * p.Np + m0;
+                    tma_load_2d(st, mA, &full[s], kc * kTileK, (int)arow);
+                    tma_load_2d(st + kABytes, &mapBf, &full[s], tt * p.Lp + kc * kTileK, 0);
+                    tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], tt * p.Lp + kc * kTileK, 0);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0) {
+            const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc2 = umma_idesc_tf32(2 * p.bn);
+            for (int kc = 0; kc < nk; ++kc) {
+                const int s = kc % p.stages, round = kc / p.stages;
+                const int g = kc & 1, use = kc >> 1;
+                const int jr = g * per_group + use % per_group;
+                mbar_wait(&full[s], round & 1);
+                mbar_wait(&split[jr], (use / per_group) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes, bl0 = bf0 + bBytes;
+                const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
+#pragma unroll
+                for (int k = 0; k < kTileK / 8; ++k) {
+                    const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
+                    if (fused_n) {
+                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, (kc | k) != 0);   // [a_hi*b_full | a_hi*b_lo]
+                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);               //  a_lo*b_full
+                    } else {
+                        const uint64_t dbl = umma_desc_k_sw128(bl0 + k * 32);
+                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc1, (kc | k) != 0);
+                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);
+                        umma_tf32_ts(tmem_d, ahi + k * 8, dbl, idesc1, 1);
+                    }
+                }
+                umma_commit(&empty[s]);
+                umma_commit(&a_empty[jr]);
+            }
+            umma_commit(accum);
+        }
+    } else {
+        // ===== splitters: smem row -> registers -> TMEM (A_hi, A_lo); group g takes chunks kc = g, g+2, ... =====
+        const int group = (warp - 2) >> 2;
+        const int lane_base = (warp & 3) * 32;                  // TMEM lanes this warp may touch
+        const int row = lane_base + lane;                       // A tile row == TMEM lane
+        for (int kc = group; kc < nk; kc += 2) {
+            const int s = kc % p.stages, round = kc / p.stages;
+            const int use = kc >> 1;
+            const int jr = group * per_group + use % per_group;
+            mbar_wait(&full[s], round & 1);
+            if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1);
+            if (half && lane_base >= 64) { mbar_arrive(&split[jr]); continue; }    // rows never stored
+            const uint8_t* A = smem + (size_t)s * stageBytes + (size_t)row * 128;
+            uint32_t hi[32], lo[32];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {                       // 16-byte chunk c of the row sits at (c ^ (row & 7))
+                const uint4 v = *reinterpret_cast<const uint4*>(A + ((c ^ (row & 7)) << 4));
+                hi[4 * c + 0] = v.x; hi[4 * c + 1] = v.y; hi[4 * c + 2] = v.z; hi[4 * c + 3] = v.w;
+            }
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+                lo[i] = __float_as_uint(__uint_as_float(hi[i]) - __uint_as_float(hi[i] & 0xffffe000u));
+            const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);
+            tmem_st16(t0, hi); tmem_st16(t0 + 16, hi + 16);
+            tmem_st16(t0 + 32, lo); tmem_st16(t0 + 48, lo + 16);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            mbar_arrive(&split[jr]);
+        }
+        // ---- epilogue ----
+        mbar_wait(accum, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const int m = m0 + row;
+        for (int c0 = 16 * group; c0 < p.bn; c0 += 32) {
+            uint32_t v[16], w[16];
+            const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
+            tmem_ld16(taddr, v);
+            if (fused_n) tmem_ld16(taddr + p.bn, w);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (m < p.M) {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int d = c0 + j;
+                    if (d < dl.n) {
+                        const float acc = __uint_as_float(v[j]) + (fused_n ? __uint_as_float(w[j]) : 0.f);
+                        if (p.mode == 0) {
+                            const float r = acc - __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.L + m);
+                            const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
+                            p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
+                            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - rhi;
                         } else {
                             float* qp = p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
                             *qp = fmaxf(0.f, fmaf(-p.eta, acc, *qp));
