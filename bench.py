@@ -90,6 +90,27 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.sm)}
 
 
+def rank_config(cfg, rank: int, world: int):
+    """Weak scaling over days (days are independent units): every rank owns its own D days and its
+    own copy of the cluster operators, generated from seed + rank; no collective sits on the step path."""
+    return cfg if world <= 1 else cfg.replace(seed=cfg.seed + rank)
+
+
+def max_over_ranks(value: float, device="cpu") -> float:
+    """MAX over ranks of a per-rank device time (the job finishes with its slowest rank)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_day_steps_per_s(D: int, world: int, epoch_ms: float) -> float:
+    """Whole-job throughput: every rank steps its D days once per epoch."""
+    return D * world / (epoch_ms * 1e-3)
+
+
 def make_epochs(cfg, lab, b, count):
     rng = synth._Counter(cfg.seed, synth.S_SCHED)
     return [synth.epoch_chunks(np.asarray(lab, np.int64), b, rng) for _ in range(count)]
@@ -184,18 +205,20 @@ def run_ours(args, cfg, b, rank, world, local_rank):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
-        cfg = cfg.replace(seed=cfg.seed + rank)      # weak scaling: every rank owns its own D days
+    cfg = rank_config(cfg, rank, world)
 
     # ---- inputs, generated once on the device (synth: no solver arithmetic) ----
     lab = synth.labels(cfg).numpy()
     if cfg.sparse:
         csr, x = synth.sparse_problem(cfg, dev)
+        torch.cuda.empty_cache()              # the library allocates with cudaMalloc: give torch's cached blocks back first
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, csr=csr)
         nnz_c = csr.nnz / cfg.C
         del csr
     else:
         R = synth.dar_dense(cfg, device=dev)
         x = synth.counts(cfg, R, synth.q_true(cfg, dev), torch.from_numpy(lab))
+        torch.cuda.empty_cache()
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, dense=R)
     x_cpu = x.cpu()
     R_cpu = None
@@ -243,10 +266,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
     sampler.stop_flag = True
     sampler.join()
     total_ms = sum(a.elapsed_time(z) for a, z in ev)
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dev)
     epoch_ms = total_ms / args.steps
     launches = P.dode_launch_count(h) - launches0
     fwd_ms, fwd_n = P.dode_timing_read(h, 0)
@@ -311,10 +331,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
                 P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
         torch.cuda.synchronize()
         e_ms = (time.perf_counter() - t0) * 1e3 / args.e2e_steps
-        if world > 1:
-            t = torch.tensor([e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
+        e_ms = max_over_ranks(e_ms, dev)
         e2e = {"value": e_ms, "unit": UNIT, "h2d_bytes_per_step": int(cfg.D * cfg.T * cfg.L * 4),
                "d2h_bytes_per_step": int(cfg.D * cfg.T * cfg.N * 4), "api": "dode_spgd_step_host (pinned host buffers)"}
 
@@ -334,7 +351,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
     out = {"metric": METRIC, "value": epoch_ms, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": epoch_ms, "higher_is_better": False, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, b),
-           "day_steps_per_s": cfg.D * world / (epoch_ms * 1e-3), "spgd_iterations_per_epoch": iters_per_epoch,
+           "day_steps_per_s": job_day_steps_per_s(cfg.D, world, epoch_ms), "spgd_iterations_per_epoch": iters_per_epoch,
            "ms_per_spgd_iteration": epoch_ms / iters_per_epoch, "kernel_path": path,
            "gpu_launches": int(launches), "wall_s_timed_region": wall, "clocks": sampler.summary(),
            "roofline": roof, "e2e": e2e, "cpu_baseline": cpu}

@@ -331,6 +331,8 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
         stages = (226 * 1024 - fixed) / stageBytes;
         nring = acc_cols + 256 <= 512 ? 4 : 2;
     }
+    if (const char* e = getenv("DODE_TC_OCC1")) if (atoi(e)) { stages = (226 * 1024 - fixed) / stageBytes; nring = acc_cols + 256 <= 512 ? 4 : 2; }
+    if (const char* e = getenv("DODE_TC_STAGES")) if (atoi(e) > 1) stages = std::min(stages, atoi(e));
     stages = std::max(2, std::min(stages, 10));
     const size_t smem = (size_t)stages * stageBytes + fixed;
     {

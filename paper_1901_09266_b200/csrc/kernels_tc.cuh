@@ -410,6 +410,7 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes, bl0 = bf0 + bBytes;
                 const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
+                if (p.dbg & 2) { mbar_arrive(&empty[s]); mbar_arrive(&a_empty[jr]); continue; }   // bring-up: no MMA
 #pragma unroll
                 for (int k = 0; k < kTileK / 8; ++k) {
                     const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
@@ -426,7 +427,7 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
                 umma_commit(&empty[s]);
                 umma_commit(&a_empty[jr]);
             }
-            umma_commit(accum);
+            if (p.dbg & 2) mbar_arrive(accum); else umma_commit(accum);
         }
     } else {
         // ===== splitters: smem row -> registers -> TMEM (A_hi, A_lo); group g takes chunks kc = g, g+2, ... =====
@@ -439,7 +440,7 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
             const int jr = group * per_group + use % per_group;
             mbar_wait(&full[s], round & 1);
             if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1);
-            if (half && lane_base >= 64) { mbar_arrive(&split[jr]); continue; }    // rows never stored
+            if ((half && lane_base >= 64) || (p.dbg & 1)) { mbar_arrive(&split[jr]); continue; }    // rows never stored
             const uint8_t* A = smem + (size_t)s * stageBytes + (size_t)row * 128;
             uint32_t hi[32], lo[32];
 #pragma unroll
@@ -461,7 +462,7 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
         mbar_wait(accum, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int m = m0 + row;
-        for (int c0 = 16 * group; c0 < p.bn; c0 += 32) {
+        for (int c0 = 16 * group; c0 < p.bn && !(p.dbg & 4); c0 += 32) {
             uint32_t v[16], w[16];
             const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
             tmem_ld16(taddr, v);
