@@ -312,6 +312,20 @@ static int tc_ensure(dode_ctx* ctx, int bn) {
     return DODE_OK;
 }
 
+// Launch with programmatic stream serialization (PDL): the kernel may start while its predecessor drains; it
+// calls griddepcontrol.wait before touching anything the predecessor wrote.  Per-kernel event timing records
+// events between launches, which serialises them again — timing mode therefore shows un-overlapped durations.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
 static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     const dode_dims& d = ctx->dm;
@@ -337,8 +351,8 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     const size_t smem = (size_t)stages * stageBytes + fixed;
     {
         KernelTimer kt(ctx, KIND_OTHER);
-        tc::gather_split<<<dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), 256, 0, ctx->stream>>>(
-            ctx->q, dayStride, (long)dayStride / 4, ctx->Qg_full, ctx->Qg_lo, dl);
+        CU(launch_pdl(tc::gather_split, dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), dim3(256), 0,
+                      ctx->stream, ctx->q, dayStride, (long)dayStride / 4, ctx->Qg_full, ctx->Qg_lo, dl));
         ctx->launches++;
     }
     tc::TcParams p{};
@@ -355,8 +369,8 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
             tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
                 ctx->mapA_fwd, ctx->mapQ_f, ctx->mapQ_l, p, dl);
         else
-            tc::banded_gemm_3xtf32_ts<<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
-                ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl);
+            CU(launch_pdl(tc::banded_gemm_3xtf32_ts, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+                          ctx->stream, ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl));
         ctx->launches++;
     }
     {
@@ -366,8 +380,8 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
             tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
                 ctx->mapA_grad, ctx->mapR_f, ctx->mapR_l, p, dl);
         else
-            tc::banded_gemm_3xtf32_ts<<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
-                ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl);
+            CU(launch_pdl(tc::banded_gemm_3xtf32_ts, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+                          ctx->stream, ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl));
         ctx->launches++;
     }
     char buf[96];

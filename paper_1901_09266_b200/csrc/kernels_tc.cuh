@@ -375,6 +375,28 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
     const uint32_t tmem_ring = tmem_d + (uint32_t)acc_cols;
     const int per_group = nring >> 1;
 
+    // Programmatic dependent launch: everything above overlapped the previous kernel's tail.  The next kernel in
+    // the stream may start its own prologue now; nothing produced by the previous kernel is touched before the wait.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // Epilogue operands (x for the forward pass, the old q for the update) are fetched by the epilogue threads
+    // BEFORE the main loop so that their DRAM/L2 latency is hidden behind it: 16 values per thread.
+    float pre[16];
+    const int erow = ((warp & 3) << 5) + lane, em = m0 + erow;
+    const int egroup = warp >= 2 ? (warp - 2) >> 2 : 0;
+    auto prefetch = [&](int c0) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int d = c0 + j;
+            pre[j] = 0.f;
+            if (em < p.M && d < dl.n)
+                pre[j] = p.mode == 0 ? __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.L + em)
+                                     : p.q[(size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + em];
+        }
+    };
+    if (p.mode == 0 && warp >= 2) prefetch(16 * egroup);             // x is a static input
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (p.mode == 1 && warp >= 2) prefetch(16 * egroup);             // q: written by the previous step
+
     if (warp == 0) {
         // ===== TMA producer =====
         if (lane == 0) {
@@ -467,6 +489,10 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
             const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
             tmem_ld16(taddr, v);
             if (fused_n) tmem_ld16(taddr + p.bn, w);
+            float cur[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) cur[j] = pre[j];
+            if (c0 + 32 < p.bn) prefetch(c0 + 32);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             if (m < p.M) {
 #pragma unroll
@@ -475,13 +501,12 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
                     if (d < dl.n) {
                         const float acc = __uint_as_float(v[j]) + (fused_n ? __uint_as_float(w[j]) : 0.f);
                         if (p.mode == 0) {
-                            const float r = acc - __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.L + m);
+                            const float r = acc - cur[j];
                             const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
                             p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
                             p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - rhi;
                         } else {
-                            float* qp = p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
-                            *qp = fmaxf(0.f, fmaf(-p.eta, acc, *qp));
+                            p.q[(size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m] = fmaxf(0.f, fmaf(-p.eta, acc, cur[j]));
                         }
                     }
                 }
@@ -500,6 +525,8 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
 __global__ void __launch_bounds__(256)
 gather_split(const float* __restrict__ q, size_t dayStride, long len4, float* __restrict__ gfull, float* __restrict__ glo,
              const __grid_constant__ DayList dl) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");          // q is written by the previous step's update
     const int d = blockIdx.y;
     const float4* src = reinterpret_cast<const float4*>(q + (size_t)dl.day[d] * dayStride);
     float4* f = reinterpret_cast<float4*>(gfull + (size_t)d * dayStride);
