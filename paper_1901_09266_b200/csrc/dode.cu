@@ -21,37 +21,38 @@ using namespace dode;
 
 struct dode_ctx {
     dode_dims dm{};
-    int Np = 0, N4 = 0;
+    int Np = 0, Lp = 0;          // padded N / L (dense: 128-byte rows when that costs <= 7 %, else 32- or 16-byte)
     cudaStream_t stream = nullptr;
-    // dense storage
-    float* R = nullptr;          // [C][T][H+1][L][Np]
+    // dense storage (layouts: kernels_dense.cuh)
+    float* Ag = nullptr;         // [C][T][H+1][Lp][Np]  departure-major, a3
+    float* Af = nullptr;         // [C][T][H+1][Np][Lp]  arrival-major (lag-merged), a2
     // CSR storage (a6)
     CsrStore csr{};
     // state
     float* q = nullptr;          // [D][T][Np]
     float* x = nullptr;          // [D][T][L]
-    float* r = nullptr;          // [T][L][bp] scratch
+    float* r = nullptr;          // [T*Lp][bp] residual panel (FFMA / CSR paths)
     size_t r_cap = 0;            // floats
+    float* Qb = nullptr;         // [T*Np][bp] gathered state panel (FFMA path, 1 < b)
+    size_t qb_cap = 0;
     double* d_part = nullptr;    // objective partials
     size_t part_cap = 0;
     double* d_obj = nullptr;     // [D] per-day objective + 2 scalars
-    float *pu = nullptr, *pv = nullptr, *pw = nullptr;   // apply / power-iteration scratch
+    float *pu = nullptr, *pv = nullptr, *pw = nullptr;   // apply / power-iteration scratch: [T][Np], [T][Lp], [T][N]
     std::vector<int32_t> labels;
     std::vector<int32_t> stamp;  // distinctness check
     int32_t stamp_id = 0;
     int64_t launches = 0;
     std::string path;
     char err[512] = {0};
-    bool sm_opt_in[8] = {false};
+    bool sm_opt_in[16] = {false};
     // tensor-core path (kernels_tc.cuh)
-    float* Rt = nullptr;         // [C][T][Np][KGp] transposed copy for the gradient pass
-    int KGp = 0;
     float *Qg_full = nullptr, *Qg_lo = nullptr;   // [tc_cap][T*Np]
-    float *rp_full = nullptr, *rp_lo = nullptr;   // [tc_cap][rpitch]
+    float *rp_full = nullptr, *rp_lo = nullptr;   // [tc_cap][T*Lp]
     long rpitch = 0;
     int tc_cap = 0, tc_bn = 0, tc_min_b = 8;
     bool tc_ready = false, tc_attr = false;
-    CUtensorMap mapA_fwd, mapA_grad, mapA_fwd64, mapA_grad64, mapQ_f, mapQ_l, mapR_f, mapR_l;
+    CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64, mapQ_f, mapQ_l, mapR_f, mapR_l;
     // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -100,94 +101,100 @@ static int fail(dode_ctx* c, int code, const char* fmt, ...) {
     } while (0)
 
 static inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
+static inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
-static int ensure_r(dode_ctx* ctx, size_t floats) {
-    if (ctx->r_cap >= floats) return DODE_OK;
-    if (ctx->r) { CU(cudaStreamSynchronize(ctx->stream)); CU(cudaFree(ctx->r)); ctx->r = nullptr; ctx->r_cap = 0; }
-    CU(cudaMalloc(&ctx->r, floats * sizeof(float)));
-    ctx->r_cap = floats;
+// Padded extent of an operator dimension: whole 128-byte lines per row when that costs at most ~7 % more bytes,
+// else whole 32-byte sectors, else the 16 bytes float4 / TMA need.
+static int pad_dim(int n) {
+    for (int a : {32, 8}) {
+        const int p = round_up(n, a);
+        if ((long)p * 100 <= (long)n * 107) return p;
+    }
+    return round_up(n, 4);
+}
+
+static int ensure_buf(dode_ctx* ctx, float** buf, size_t* cap, size_t floats) {
+    if (*cap >= floats) return DODE_OK;
+    if (*buf) { CU(cudaStreamSynchronize(ctx->stream)); CU(cudaFree(*buf)); *buf = nullptr; *cap = 0; }
+    CU(cudaMalloc(buf, floats * sizeof(float)));
+    *cap = floats;
     return DODE_OK;
 }
 
 static int pick_bt(int n) { return n <= 1 ? 1 : n <= 2 ? 2 : n <= 4 ? 4 : n <= 8 ? 8 : 16; }
 
-// ---- dense launches ---------------------------------------------------------------------------
-template <int BT, int RL>
-static void launch_fwd(dode_ctx* ctx, const float* Rc, const float* qbase, size_t dayStride, const float* xbase,
-                       float* r, int bp, const DayList& dl) {
+static size_t cluster_floats(const dode_ctx* ctx) {
     const dode_dims& d = ctx->dm;
-    dim3 grid(ceil_div(d.L, (kThreads / 32) * RL), d.T, bp / BT);
-    KernelTimer kt(ctx, KIND_FWD);
-    fwd_rowdot<BT, RL><<<grid, kThreads, 0, ctx->stream>>>(Rc, qbase, dayStride, xbase, r, ctx->N4, d.L, d.T, d.H, bp, dl);
-    ctx->launches++;
+    return (size_t)d.T * (d.H + 1) * ctx->Lp * ctx->Np;
 }
 
-static void fwd_dense(dode_ctx* ctx, int bt, const float* Rc, const float* qbase, size_t dayStride,
-                      const float* xbase, float* r, int bp, const DayList& dl) {
-    switch (bt) {
-        case 1: launch_fwd<1, 8>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
-        case 2: launch_fwd<2, 8>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
-        case 4: launch_fwd<4, 8>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
-        case 8: launch_fwd<8, 4>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
-        default: launch_fwd<16, 2>(ctx, Rc, qbase, dayStride, xbase, r, bp, dl); break;
-    }
-}
-
-template <int BT, bool UPDATE>
-static int launch_grad(dode_ctx* ctx, int slot, const float* Rc, const float* r, float* qbase, size_t dayStride,
-                       float* gout, float eta, int bp, const DayList& dl) {
-    const dode_dims& d = ctx->dm;
+// ---- dense FFMA launches ------------------------------------------------------------------------
+template <int BT, int EPI>
+static int launch_band(dode_ctx* ctx, int slot, const BandArgs& a, int nbt, const DayList& dl, int kind) {
     int cwlog2 = 0;
-    while ((1 << cwlog2) < ctx->N4 && cwlog2 < 5) ++cwlog2;
+    while ((1 << cwlog2) < a.M4 && cwlog2 < 5) ++cwlog2;
     const size_t smem = (size_t)kThreads * 4 * BT * sizeof(float);
     if (smem > 48 * 1024 && !ctx->sm_opt_in[slot]) {
-        CU(cudaFuncSetAttribute(grad_coldot<BT, UPDATE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaFuncSetAttribute(band_coldot<BT, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ctx->sm_opt_in[slot] = true;
     }
-    dim3 grid(ceil_div(ctx->N4, 1 << cwlog2), d.T, bp / BT);
-    KernelTimer kt(ctx, KIND_GRAD);
-    grad_coldot<BT, UPDATE><<<grid, kThreads, smem, ctx->stream>>>(Rc, r, qbase, dayStride, gout, eta, d.N, ctx->N4,
-                                                                   d.L, d.T, d.H, bp, cwlog2, dl);
+    dim3 grid(ceil_div(a.M4, 1 << cwlog2), a.T, nbt);
+    KernelTimer kt(ctx, kind);
+    band_coldot<BT, EPI><<<grid, kThreads, smem, ctx->stream>>>(a, cwlog2, dl);
     ctx->launches++;
     return DODE_OK;
 }
 
-static int grad_dense(dode_ctx* ctx, int bt, const float* Rc, const float* r, float* qbase, size_t dayStride,
-                      float eta, int bp, const DayList& dl) {
+template <int EPI>
+static int launch_band_bt(dode_ctx* ctx, int bt, const BandArgs& a, const DayList& dl, int kind) {
+    const int nbt = a.bp / bt;
     switch (bt) {
-        case 1: return launch_grad<1, true>(ctx, 0, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
-        case 2: return launch_grad<2, true>(ctx, 1, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
-        case 4: return launch_grad<4, true>(ctx, 2, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
-        case 8: return launch_grad<8, true>(ctx, 3, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
-        default: return launch_grad<16, true>(ctx, 4, Rc, r, qbase, dayStride, nullptr, eta, bp, dl);
+        case 1: return launch_band<1, EPI>(ctx, EPI * 5 + 0, a, nbt, dl, kind);
+        case 2: return launch_band<2, EPI>(ctx, EPI * 5 + 1, a, nbt, dl, kind);
+        case 4: return launch_band<4, EPI>(ctx, EPI * 5 + 2, a, nbt, dl, kind);
+        case 8: return launch_band<8, EPI>(ctx, EPI * 5 + 3, a, nbt, dl, kind);
+        default: return launch_band<16, EPI>(ctx, EPI * 5 + 4, a, nbt, dl, kind);
     }
 }
 
-static const float* dense_cluster(const dode_ctx* ctx, int c) {
+static BandArgs band_args(const dode_ctx* ctx, int c, bool forward, int bp) {
     const dode_dims& d = ctx->dm;
-    return ctx->R + (size_t)c * d.T * (d.H + 1) * d.L * ctx->Np;
+    BandArgs a{};
+    a.A = (forward ? ctx->Af : ctx->Ag) + (size_t)c * cluster_floats(ctx);
+    a.M = forward ? d.L : d.N;
+    a.M4 = (forward ? ctx->Lp : ctx->Np) / 4;
+    a.kunit = forward ? ctx->Np : ctx->Lp;
+    a.T = d.T; a.H = d.H; a.bp = bp; a.forward = forward ? 1 : 0;
+    return a;
 }
 
-// forward residual of one sub-batch (<= kMaxDays days of cluster c) into ctx->r (or r_out with day stride 1
-// for dode_apply); returns the day-tile bt and the r stride bp
-static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, const float* qbase, size_t dayStride,
-                         const float* xbase, float* r_out, int* bt_out, int* bp_out) {
+// a2 on the FFMA / CSR paths: residual panel of one sub-batch (<= kMaxDays days of cluster c) into ctx->r
+// ([T*Lp][bp], day fastest); returns the day tile bt and the panel stride bp
+static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, int* bt_out, int* bp_out) {
     const dode_dims& d = ctx->dm;
     const bool csr = d.storage == DODE_CSR;
     const int bt = csr ? 32 : pick_bt(dl.n);
     const int bp = csr ? csr_bp(dl.n) : ceil_div(dl.n, bt) * bt;
-    float* r = r_out;
-    if (!r) {
-        int rc = ensure_r(ctx, (size_t)d.T * d.L * bp);
-        if (rc) return rc;
-        r = ctx->r;
-    }
+    const size_t dayStride = (size_t)d.T * ctx->Np;
+    int rc = ensure_buf(ctx, &ctx->r, &ctx->r_cap, (size_t)d.T * ctx->Lp * bp);
+    if (rc) return rc;
     if (!csr) {
-        fwd_dense(ctx, bt, dense_cluster(ctx, c), qbase, dayStride, xbase, r, bp, dl);
+        const float* panel = ctx->q + (size_t)dl.day[0] * dayStride;      // b = 1: the day's state IS the panel
+        if (bp > 1) {
+            if ((rc = ensure_buf(ctx, &ctx->Qb, &ctx->qb_cap, dayStride * bp))) return rc;
+            KernelTimer kt(ctx, KIND_OTHER);
+            gather_panel<<<dim3(ceil_div((long)dayStride, 32), ceil_div(bp, 32)), 256, 0, ctx->stream>>>(
+                ctx->q, dayStride, (long)dayStride, ctx->Qb, bp, dl);
+            ctx->launches++;
+            panel = ctx->Qb;
+        }
+        BandArgs a = band_args(ctx, c, true, bp);
+        a.B = panel; a.x = ctx->x; a.out = ctx->r;
+        if ((rc = launch_band_bt<EPI_RESID>(ctx, bt, a, dl, KIND_FWD))) return rc;
     } else {
         KernelTimer kt(ctx, KIND_FWD);
-        int rc = csr_forward(ctx->csr, c, qbase, dayStride, xbase, r, bp, r_out ? 1 : bp, dl, d, ctx->Np, ctx->stream,
-                             &ctx->launches);
+        rc = csr_forward(ctx->csr, c, ctx->q, dayStride, ctx->x, ctx->r, bp, bp, dl, d, ctx->Np, ctx->stream,
+                         &ctx->launches);
         if (rc) return fail(ctx, rc, "CSR scratch allocation failed");
     }
     *bt_out = bt; *bp_out = bp;
@@ -228,48 +235,36 @@ static PFN_encodeTiled get_encode() {
     return fn;
 }
 
-// fp32 tensor, innermost dim first; box = {32, ...}; SWIZZLE_128B; out-of-bounds elements read as zero
+// fp32 tensor, innermost dim first; out-of-bounds elements read as zero
 static int make_map(dode_ctx* ctx, CUtensorMap* m, const void* base, int rank, const uint64_t* dims,
-                    const uint64_t* strides_bytes, const uint32_t* box) {
+                    const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128) {
     PFN_encodeTiled enc = get_encode();
     if (!enc) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled is unavailable");
     cuuint64_t gd[3]; cuuint64_t gs[2]; cuuint32_t bx[3]; cuuint32_t es[3] = {1, 1, 1};
     for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; }
     for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_bytes[i];
     CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
     return DODE_OK;
 }
 
-// create-time: transposed copy + the two A maps
+// create-time: the A maps over Af / Ag, one (cluster, time) slab per index of the outer dimension so that K rows
+// beyond the slab read as zero
 static int tc_setup(dode_ctx* ctx) {
     const dode_dims& d = ctx->dm;
-    const int Lp = (d.L + 3) / 4 * 4;
-    ctx->KGp = (d.H + 1) * Lp;
-    ctx->rpitch = (long)d.T * Lp;
-    const size_t rows = (size_t)d.C * d.T * ctx->Np;
-    CU(cudaMalloc(&ctx->Rt, rows * ctx->KGp * sizeof(float)));
-    CU(cudaMemsetAsync(ctx->Rt, 0, rows * ctx->KGp * sizeof(float), ctx->stream));
-    dim3 grid(ceil_div(ctx->Np, 32), (d.H + 1) * ceil_div(Lp, 32), d.C * d.T);
-    tc::transpose_blocks<<<grid, 256, 0, ctx->stream>>>(ctx->R, ctx->Rt, d.H + 1, d.L, Lp, ctx->Np, ctx->KGp);
-    ctx->launches++;
-    {
-        const uint64_t dims[2] = {(uint64_t)ctx->Np, (uint64_t)d.C * d.T * (d.H + 1) * d.L};
-        const uint64_t str[1] = {(uint64_t)ctx->Np * 4};
-        const uint32_t box[2] = {32, 128}, box64[2] = {32, 64};
-        int rc = make_map(ctx, &ctx->mapA_fwd, ctx->R, 2, dims, str, box);
+    ctx->rpitch = (long)d.T * ctx->Lp;
+    const uint64_t slabs = (uint64_t)d.C * d.T;
+    for (int fwd = 0; fwd < 2; ++fwd) {
+        const uint64_t Mp = fwd ? ctx->Lp : ctx->Np, krows = (uint64_t)(d.H + 1) * (fwd ? ctx->Np : ctx->Lp);
+        const uint64_t dims[3] = {Mp, krows, slabs};
+        const uint64_t str[2] = {Mp * 4, krows * Mp * 4};
+        const uint32_t box[3] = {(uint32_t)tc::kTileM, (uint32_t)tc::kTileK, 1}, box64[3] = {(uint32_t)tc::kTileM / 2, (uint32_t)tc::kTileK, 1};
+        const float* base = fwd ? ctx->Af : ctx->Ag;
+        int rc = make_map(ctx, fwd ? &ctx->mapA_fwd : &ctx->mapA_grad, base, 3, dims, str, box, false);
         if (rc) return rc;
-        if ((rc = make_map(ctx, &ctx->mapA_fwd64, ctx->R, 2, dims, str, box64))) return rc;
-    }
-    {
-        const uint64_t dims[2] = {(uint64_t)ctx->KGp, (uint64_t)rows};
-        const uint64_t str[1] = {(uint64_t)ctx->KGp * 4};
-        const uint32_t box[2] = {32, 128}, box64[2] = {32, 64};
-        int rc = make_map(ctx, &ctx->mapA_grad, ctx->Rt, 2, dims, str, box);
-        if (rc) return rc;
-        if ((rc = make_map(ctx, &ctx->mapA_grad64, ctx->Rt, 2, dims, str, box64))) return rc;
+        if ((rc = make_map(ctx, fwd ? &ctx->mapA_fwd64 : &ctx->mapA_grad64, base, 3, dims, str, box64, false))) return rc;
     }
     ctx->tc_ready = true;
     return DODE_OK;
@@ -291,22 +286,21 @@ static int tc_ensure(dode_ctx* ctx, int bn) {
         ctx->tc_cap = bn;
     }
     if (ctx->tc_bn != bn) {
-        const uint64_t qd[3] = {(uint64_t)ctx->Np, (uint64_t)d.T, (uint64_t)ctx->tc_cap};
-        const uint64_t qs[2] = {(uint64_t)ctx->Np * 4, (uint64_t)qlen * 4};
-        const uint32_t qb[3] = {32, 1, (uint32_t)bn};
+        // B operands: K-major windows of the per-day vectors, SWIZZLE_128B tiles of {32 floats, bn days}
+        const uint64_t qd[2] = {(uint64_t)qlen, (uint64_t)ctx->tc_cap};
+        const uint64_t qs[1] = {(uint64_t)qlen * 4};
+        const uint32_t bb[2] = {(uint32_t)tc::kTileK, (uint32_t)bn};
         int rc;
-        if ((rc = make_map(ctx, &ctx->mapQ_f, ctx->Qg_full, 3, qd, qs, qb))) return rc;
-        if ((rc = make_map(ctx, &ctx->mapQ_l, ctx->Qg_lo, 3, qd, qs, qb))) return rc;
+        if ((rc = make_map(ctx, &ctx->mapQ_f, ctx->Qg_full, 2, qd, qs, bb, true))) return rc;
+        if ((rc = make_map(ctx, &ctx->mapQ_l, ctx->Qg_lo, 2, qd, qs, bb, true))) return rc;
         const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)ctx->tc_cap};
         const uint64_t rs[1] = {(uint64_t)ctx->rpitch * 4};
-        const uint32_t rb[2] = {32, (uint32_t)bn};
-        if ((rc = make_map(ctx, &ctx->mapR_f, ctx->rp_full, 2, rd, rs, rb))) return rc;
-        if ((rc = make_map(ctx, &ctx->mapR_l, ctx->rp_lo, 2, rd, rs, rb))) return rc;
+        if ((rc = make_map(ctx, &ctx->mapR_f, ctx->rp_full, 2, rd, rs, bb, true))) return rc;
+        if ((rc = make_map(ctx, &ctx->mapR_l, ctx->rp_lo, 2, rd, rs, bb, true))) return rc;
         ctx->tc_bn = bn;
     }
     if (!ctx->tc_attr) {
-        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->tc_attr = true;
     }
     return DODE_OK;
@@ -333,15 +327,14 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     int rc = tc_ensure(ctx, bn);
     if (rc) return rc;
     const size_t dayStride = (size_t)d.T * ctx->Np;
-    // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  TS kernel (default): A_hi/A_lo live in TMEM,
-    // 2 CTAs per SM when 3 stages fit in half the shared memory and 256 TMEM columns suffice.
-    static const bool use_ss = getenv("DODE_TC_KERNEL") && !strcmp(getenv("DODE_TC_KERNEL"), "ss");
+    // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  Two CTAs per SM when 3 stages fit in half the
+    // shared memory and 256 TMEM columns suffice.
     const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
-    const int fixed = (use_ss ? 2 * tc::kABytes : 0) + 1024 + 256;
+    const int fixed = 1024 + 256;
     const int acc_cols = bn <= 128 ? 2 * bn : bn;
     int stages = (112 * 1024 - fixed) / stageBytes;
     int nring = 2;
-    if (stages < 3 || (!use_ss && acc_cols + 128 > 256)) {          // one CTA per SM
+    if (stages < 3 || acc_cols + 128 > 256) {          // one CTA per SM
         stages = (226 * 1024 - fixed) / stageBytes;
         nring = acc_cols + 256 <= 512 ? 4 : 2;
     }
@@ -356,32 +349,23 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
         ctx->launches++;
     }
     tc::TcParams p{};
-    p.T = d.T; p.H = d.H; p.L = d.L; p.Lp = (d.L + 3) / 4 * 4; p.Np = ctx->Np; p.bn = bn; p.stages = stages;
-    p.kg_chunks = ceil_div((long)ctx->KGp, tc::kTileK);
+    p.T = d.T; p.H = d.H; p.Lp = ctx->Lp; p.Np = ctx->Np; p.bn = bn; p.stages = stages; p.nring = nring;
+    p.slab0 = c * d.T;
     p.x = ctx->x; p.rp_full = ctx->rp_full; p.rp_lo = ctx->rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
-    p.nring = nring;
     {
         KernelTimer kt(ctx, KIND_FWD);
-        p.mode = 0; p.M = d.L; p.a_row0 = (long)c * d.T * (d.H + 1) * d.L;
-        if (use_ss)
-            tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.L, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
-                ctx->mapA_fwd, ctx->mapQ_f, ctx->mapQ_l, p, dl);
-        else
-            CU(launch_pdl(tc::banded_gemm_3xtf32_ts, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
-                          ctx->stream, ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl));
+        p.mode = 0; p.M = d.L; p.kunit = ctx->Np;
+        CU(launch_pdl(tc::banded_gemm_3xtf32, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+                      ctx->stream, ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl));
         ctx->launches++;
     }
     {
         KernelTimer kt(ctx, KIND_GRAD);
-        p.mode = 1; p.M = d.N; p.a_row0 = (long)c * d.T * ctx->Np;
-        if (use_ss)
-            tc::banded_gemm_3xtf32<0><<<dim3(ceil_div(d.N, tc::kTileM), d.T), tc::kThreadsTC, smem, ctx->stream>>>(
-                ctx->mapA_grad, ctx->mapR_f, ctx->mapR_l, p, dl);
-        else
-            CU(launch_pdl(tc::banded_gemm_3xtf32_ts, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
-                          ctx->stream, ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl));
+        p.mode = 1; p.M = d.N; p.kunit = ctx->Lp;
+        CU(launch_pdl(tc::banded_gemm_3xtf32, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+                      ctx->stream, ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl));
         ctx->launches++;
     }
     char buf[96];
@@ -403,11 +387,13 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
             if ((rc = tc_step(ctx, c, dl, eta))) return rc;
             continue;
         }
-        if ((rc = forward_batch(ctx, c, dl, ctx->q, dayStride, ctx->x, nullptr, &bt, &bp))) return rc;
+        if ((rc = forward_batch(ctx, c, dl, &bt, &bp))) return rc;
         if (d.storage == DODE_DENSE) {
-            if ((rc = grad_dense(ctx, bt, dense_cluster(ctx, c), ctx->r, ctx->q, dayStride, eta, bp, dl))) return rc;
+            BandArgs a = band_args(ctx, c, false, bp);
+            a.B = ctx->r; a.q = ctx->q; a.dayStride = dayStride; a.eta = eta;
+            if ((rc = launch_band_bt<EPI_UPDATE>(ctx, bt, a, dl, KIND_GRAD))) return rc;
             char buf[96];
-            snprintf(buf, sizeof buf, "ffma_rowdot_bt%d+ffma_coldot_bt%d", bt, bt);
+            snprintf(buf, sizeof buf, "ffma_coldot_fwd_bt%d+ffma_coldot_grad_bt%d", bt, bt);
             ctx->path = buf;
         } else {
             {
@@ -434,8 +420,8 @@ extern "C" {
 void dode_destroy(dode_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->Rt); cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
-    cudaFree(ctx->R); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r);
+    cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
+    cudaFree(ctx->Ag); cudaFree(ctx->Af); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r); cudaFree(ctx->Qb);
     for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
     cudaFree(ctx->d_part); cudaFree(ctx->d_obj); cudaFree(ctx->pu); cudaFree(ctx->pv); cudaFree(ctx->pw);
@@ -467,8 +453,8 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     dode_ctx* c = new (std::nothrow) dode_ctx();
     if (!c) return fail(ctx, DODE_ENOMEM, "host allocation failed");
     c->dm = d;
-    c->Np = (d.N + 3) / 4 * 4;
-    c->N4 = c->Np / 4;
+    c->Np = d.storage == DODE_DENSE ? pad_dim(d.N) : round_up(d.N, 4);
+    c->Lp = d.storage == DODE_DENSE ? pad_dim(d.L) : d.L;
     c->stream = (cudaStream_t)stream;
     c->labels.assign(labels, labels + d.D);
     c->stamp.assign(d.D, 0);
@@ -489,21 +475,21 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     CUC(cudaMalloc(&c->x, (size_t)d.D * TL * sizeof(float)));
     CUC(cudaMalloc(&c->d_obj, ((size_t)d.D + 8) * sizeof(double)));
     CUC(cudaMalloc(&c->pu, TNp * sizeof(float)));
-    CUC(cudaMalloc(&c->pv, TL * sizeof(float)));
+    CUC(cudaMalloc(&c->pv, (size_t)d.T * c->Lp * sizeof(float)));
     CUC(cudaMalloc(&c->pw, (size_t)d.T * d.N * sizeof(float)));
     CUC(cudaMemcpyAsync(c->x, x, (size_t)d.D * TL * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     fill_state<<<1184, 256, 0, c->stream>>>(c->q, (size_t)d.D * d.T, d.N, c->Np, q0);
     c->launches++;
     if (d.storage == DODE_DENSE) {
-        const size_t rows = (size_t)d.C * d.T * (d.H + 1) * d.L;
-        CUC(cudaMalloc(&c->R, rows * c->Np * sizeof(float)));
-        if (c->Np == d.N) {
-            CUC(cudaMemcpyAsync(c->R, R->dense, rows * d.N * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
-        } else {
-            CUC(cudaMemsetAsync(c->R, 0, rows * c->Np * sizeof(float), c->stream));
-            CUC(cudaMemcpy2DAsync(c->R, c->Np * sizeof(float), R->dense, d.N * sizeof(float), d.N * sizeof(float), rows,
-                                  cudaMemcpyDeviceToDevice, c->stream));
-        }
+        // a0: the two packed copies of the operator (kernels_dense.cuh); the caller's tensor is not kept
+        const size_t total = (size_t)d.C * cluster_floats(c);
+        const long blocks = (long)d.C * d.T * (d.H + 1);
+        CUC(cudaMalloc(&c->Ag, total * sizeof(float)));
+        CUC(cudaMalloc(&c->Af, total * sizeof(float)));
+        pack_departure_major<<<148 * 16, 256, 0, c->stream>>>(R->dense, c->Ag, blocks, d.T, d.H, d.L, d.N, c->Lp, c->Np);
+        pack_arrival_major<<<dim3(ceil_div(c->Lp, 32), ceil_div(c->Np, 32), (unsigned)blocks), 256, 0, c->stream>>>(
+            R->dense, c->Af, d.T, d.H, d.L, d.N, c->Lp, c->Np);
+        c->launches += 2;
         const char* env = getenv("DODE_TC_MIN_B");      // minibatch from which the tensor-core path is used (0 = never)
         c->tc_min_b = env ? atoi(env) : 8;
         if (c->tc_min_b > 0) {
@@ -560,7 +546,7 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
     // group positions by cluster, evaluate in sub-batches; d_obj[i] receives f of days[i]
     constexpr int kObjBatch = 64;
     const size_t dayStride = (size_t)d.T * ctx->Np;
-    const long rows = (long)d.T * d.L;
+    const long rows = (long)d.T * ctx->Lp;
     const int rowsPerBlock = 2048, nchunks = ceil_div(rows, rowsPerBlock);
     if (ctx->part_cap < (size_t)nchunks * kObjBatch) {
         if (ctx->d_part) CU(cudaFree(ctx->d_part));
@@ -579,7 +565,7 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
             dl.n = (int)std::min<size_t>(kObjBatch, pos.size() - off);
             for (int j = 0; j < dl.n; ++j) dl.day[j] = days[pos[off + j]];
             int bt, bp;
-            if ((rc = forward_batch(ctx, c, dl, ctx->q, dayStride, ctx->x, nullptr, &bt, &bp))) return rc;
+            if ((rc = forward_batch(ctx, c, dl, &bt, &bp))) return rc;
             sumsq_partial<<<dim3(nchunks, ceil_div(dl.n, 32)), kThreads, 0, ctx->stream>>>(ctx->r, ctx->d_part, rows, bp,
                                                                                          dl.n, rowsPerBlock);
             sumsq_final<<<ceil_div(dl.n, 64), 64, 0, ctx->stream>>>(ctx->d_part, ctx->d_obj, nchunks, dl.n);
@@ -625,19 +611,30 @@ int dode_set_q(dode_ctx* ctx, int32_t day, const float* in, int32_t is_device) {
     return copy_q(ctx, day, nullptr, in, is_device);
 }
 
-// v = rho_c * (padded u in ctx->pu)
-static int apply_padded(dode_ctx* ctx, int c, float* v) {
+// v[T][opitch] = rho_c * (padded u in ctx->pu), minibatch 1 through the production kernels
+static int apply_padded(dode_ctx* ctx, int c, float* v, int opitch) {
+    const dode_dims& d = ctx->dm;
     DayList dl; dl.n = 1; dl.day[0] = 0;
-    int bt, bp;
-    return forward_batch(ctx, c, dl, ctx->pu, 0, nullptr, v, &bt, &bp);
+    if (d.storage == DODE_DENSE) {
+        BandArgs a = band_args(ctx, c, true, 1);
+        a.B = ctx->pu; a.out = v; a.opitch = opitch;
+        return launch_band<1, EPI_STORE>(ctx, 15, a, 1, dl, KIND_FWD);
+    }
+    int rc = csr_forward(ctx->csr, c, ctx->pu, 0, nullptr, v, 32, 1, dl, d, ctx->Np, ctx->stream, &ctx->launches);
+    return rc ? fail(ctx, rc, "CSR scratch allocation failed") : DODE_OK;
 }
 
-static int apply_t_impl(dode_ctx* ctx, int c, const float* v, float* u) {
-    DayList dl; dl.n = 1; dl.day[0] = 0;
+// u[T][N] = rho_c^T * (padded v in ctx->pv, [T][Lp])
+static int apply_t_padded(dode_ctx* ctx, int c, float* u) {
     const dode_dims& d = ctx->dm;
-    if (d.storage == DODE_DENSE)
-        return launch_grad<1, false>(ctx, 5, dense_cluster(ctx, c), v, nullptr, 0, u, 0.f, 1, dl);
-    return csr_gradient(ctx->csr, c, v, nullptr, 0, u, 0.f, 32, 1, dl, d, ctx->Np, ctx->stream, &ctx->launches);
+    DayList dl; dl.n = 1; dl.day[0] = 0;
+    if (d.storage == DODE_DENSE) {
+        BandArgs a = band_args(ctx, c, false, 1);
+        a.B = ctx->pv; a.out = u; a.opitch = d.N;
+        return launch_band<1, EPI_STORE>(ctx, 15, a, 1, dl, KIND_GRAD);
+    }
+    int rc = csr_gradient(ctx->csr, c, ctx->pv, nullptr, 0, u, 0.f, 32, 1, dl, d, ctx->Np, ctx->stream, &ctx->launches);
+    return rc ? fail(ctx, rc, "CSR scratch allocation failed") : DODE_OK;
 }
 
 int dode_apply(dode_ctx* ctx, int32_t c, const float* u, float* v) {
@@ -646,7 +643,7 @@ int dode_apply(dode_ctx* ctx, int32_t c, const float* u, float* v) {
     if (c < 0 || c >= d.C || !u || !v) return fail(ctx, DODE_EINVAL, "bad cluster or null buffer");
     scale_pad<<<592, 256, 0, ctx->stream>>>(u, ctx->pu, (size_t)d.T, d.N, ctx->Np, nullptr);
     ctx->launches++;
-    int rc = apply_padded(ctx, c, v);
+    int rc = apply_padded(ctx, c, v, d.L);
     if (rc) return rc;
     CU(cudaGetLastError());
     return DODE_OK;
@@ -656,7 +653,9 @@ int dode_apply_t(dode_ctx* ctx, int32_t c, const float* v, float* u) {
     if (!ctx) return DODE_EINVAL;
     const dode_dims& d = ctx->dm;
     if (c < 0 || c >= d.C || !u || !v) return fail(ctx, DODE_EINVAL, "bad cluster or null buffer");
-    int rc = apply_t_impl(ctx, c, v, u);
+    scale_pad<<<592, 256, 0, ctx->stream>>>(v, ctx->pv, (size_t)d.T, d.L, ctx->Lp, nullptr);
+    ctx->launches++;
+    int rc = apply_t_padded(ctx, c, u);
     if (rc) return rc;
     CU(cudaGetLastError());
     return DODE_OK;
@@ -667,18 +666,18 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
     const dode_dims& d = ctx->dm;
     if (c < 0 || c >= d.C || iters < 1 || !L_out) return fail(ctx, DODE_EINVAL, "bad cluster, iters or null output");
     double* nrm = ctx->d_obj + d.D;       // [0] = |w|^2, [1] = |v|^2
-    const size_t TN = (size_t)d.T * d.N, TL = (size_t)d.T * d.L;
+    const size_t TN = (size_t)d.T * d.N, TLp = (size_t)d.T * ctx->Lp;
     fill_f32<<<592, 256, 0, ctx->stream>>>(ctx->pw, TN, 1.f);
     ctx->launches++;
     for (int it = 0; it < iters; ++it) {
         sumsq_single<<<1, 1024, 0, ctx->stream>>>(ctx->pw, TN, nrm);
         scale_pad<<<592, 256, 0, ctx->stream>>>(ctx->pw, ctx->pu, (size_t)d.T, d.N, ctx->Np, nrm);
         ctx->launches += 2;
-        int rc = apply_padded(ctx, c, ctx->pv);
+        int rc = apply_padded(ctx, c, ctx->pv, ctx->Lp);          // pad columns come out as 0
         if (rc) return rc;
-        sumsq_single<<<1, 1024, 0, ctx->stream>>>(ctx->pv, TL, nrm + 1);
+        sumsq_single<<<1, 1024, 0, ctx->stream>>>(ctx->pv, TLp, nrm + 1);
         ctx->launches++;
-        if ((rc = apply_t_impl(ctx, c, ctx->pv, ctx->pw))) return rc;
+        if ((rc = apply_t_padded(ctx, c, ctx->pw))) return rc;
     }
     CU(cudaMemcpyAsync(L_out, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -707,6 +706,12 @@ int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* lau
     if (reset) { ctx->t_total[kind] = 0; ctx->t_count[kind] = 0; }
     return DODE_OK;
 }
+
+#ifdef DODE_TC_TRACE
+int dode_debug_trace(long long* host, int n) {
+    return (int)cudaMemcpyFromSymbol(host, tc::g_trace, sizeof(long long) * n);
+}
+#endif
 
 int64_t dode_launch_count(const dode_ctx* ctx) { return ctx ? ctx->launches : 0; }
 

@@ -1,16 +1,20 @@
 // Dense FP32-FFMA kernels of the SPGD hot path, sm_100a.
 //
-// Regime: minibatch b small enough that streaming R from HBM bounds the step
-// (arithmetic intensity b/2 flop per byte of R per pass).  Every element of R is needed by
-// exactly ONE output row (a2) / output column (a3), so R goes HBM -> registers directly with
-// 128-bit coalesced loads (no shared-memory staging: there is no reuse to capture); the only
-// reused operand is the minibatch state (Q or r), which is small and lives in L1/L2.
+// Regime: minibatch b < 8, where streaming R from HBM bounds the step (arithmetic intensity b/2 flop per
+// byte of R per pass).  Every element of R is needed by exactly ONE output row (a2) / output column (a3),
+// so R goes HBM -> registers directly with 128-bit coalesced loads (no shared-memory staging: there is no
+// reuse to capture); the only reused operand is the minibatch panel (Q or r), which is small and lives in L1/L2.
 //
-// Layouts (device, fp32):
-//   Rc   [T][H+1][L][Np]    one cluster's blocks, Np = N rounded up to 4 (pad columns are 0)
-//   q    [D][T][Np]         state; day d at q + d*T*Np
-//   x    [D][T][L]
-//   r    [T][L][bp]         residual of the current minibatch, day index fastest (bp = b rounded up to BT)
+// The library keeps the operator twice, each copy with the OUTPUT index contiguous, so that both passes are
+// the same "column dot" stream (thread = 4 output columns, walks K rows, no cross-lane reduction):
+//   Ag [C][T][H+1][Lp][Np]  departure-major (the boundary order, zero padded): for departure s the K rows are
+//                           (h,l) and n is contiguous            -> a3, g[s][n] = sum_k Ag[s][k][n] r[s*Lp + k]
+//   Af [C][T][H+1][Np][Lp]  arrival-major, lag-merged at create: for arrival t the K rows are (j,n), j-th lag
+//                           slot = departure s = t-hmax+j (hmax = min(H,t)), and l is contiguous
+//                                                                -> a2, r[t][l] = sum_k Af[t][k][l] q[(t-hmax)*Np + k]
+// In both cases the second operand is a contiguous window of the day's state vector.
+//   q    [D][T][Np]   state; x [D][T][L]
+//   panels (FFMA path): [rows][bp], day index fastest (bp = b rounded up to BT)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -32,139 +36,54 @@ __device__ __forceinline__ float4 ldg_stream(const float4* p) {     // R: read o
     return v;
 }
 
-// Sum V (power of two <= 32) per-lane values across the warp with V-1 + log2(32/V) shuffles.
-// Returns, in every lane, the total of value index (lane & (V-1)).
-template <int V>
-__device__ __forceinline__ float warp_reduce_multi(float (&v)[V], int lane) {
-#pragma unroll
-    for (int n = V / 2; n >= 1; n >>= 1) {
-        const bool up = (lane & n) != 0;
-#pragma unroll
-        for (int i = 0; i < n; ++i) {
-            const float send = up ? v[i] : v[i + n];
-            const float keep = up ? v[i + n] : v[i];
-            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, n);
-        }
-    }
-    float s = v[0];
-#pragma unroll
-    for (int off = V; off < 32; off <<= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-    return s;
-}
-
-// ---------------------------------------------------------------------------------------------
-// a2: forward residual  r[t][l][d] = sum_{h<=min(H,t)} sum_n R[t-h][h][l][n] q_d[t-h][n] - x_d[t][l]
-// ("B_o x - y", Alg. 1 line 9).  One warp owns RL link rows of one arrival interval
-// t for BT days; lanes run along the contiguous OD index (the reduction index), so the K loop is
-// the flattened (h, n/4) float4 index and the sum over lanes is a shuffle reduction at the end.
-// grid = (ceil(L / (8*RL)), T, ceil(b/BT)), block = 256.
-// ---------------------------------------------------------------------------------------------
-template <int BT, int RL>
-__global__ void __launch_bounds__(kThreads)
-fwd_rowdot(const float* __restrict__ Rc, const float* __restrict__ qbase, size_t dayStride,
-           const float* __restrict__ xbase, float* __restrict__ r,
-           int N4, int L, int T, int H, int bp, const __grid_constant__ DayList dl) {
-    static_assert(BT * RL <= 32, "one shuffle-reduction group");
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int t = blockIdx.y;
-    const int l0 = (blockIdx.x * (kThreads / 32) + warp) * RL;
-    if (l0 >= L) return;
-    const int d0 = blockIdx.z * BT;
-
-    const float4* Rrow[RL];
-#pragma unroll
-    for (int i = 0; i < RL; ++i) {
-        const int l = min(l0 + i, L - 1);
-        Rrow[i] = reinterpret_cast<const float4*>(Rc) + ((size_t)t * (H + 1) * L + l) * N4;
-    }
-    const float4* qd[BT];
-#pragma unroll
-    for (int j = 0; j < BT; ++j) {
-        const int day = dl.day[min(d0 + j, dl.n - 1)];
-        qd[j] = reinterpret_cast<const float4*>(qbase + (size_t)day * dayStride) + (size_t)t * N4;
-    }
-    // block (s = t-h, h) sits H*L*N4 float4 before block (t-h+1, h-1); q[t-h] sits N4 before q[t-h+1]
-    const long hstepR = (long)H * L * N4;
-    const int F = (min(H, t) + 1) * N4;
-    const int dh = 32 / N4, dn = 32 - dh * N4;
-    int h = lane / N4, n4 = lane - h * N4;
-
-    float acc[RL][BT];
-#pragma unroll
-    for (int i = 0; i < RL; ++i)
-#pragma unroll
-        for (int j = 0; j < BT; ++j) acc[i][j] = 0.f;
-
-#pragma unroll 2
-    for (int f = lane; f < F; f += 32) {
-        const long ro = (long)n4 - (long)h * hstepR;
-        const long qo = (long)n4 - (long)h * N4;
-        float4 a[RL];
-#pragma unroll
-        for (int i = 0; i < RL; ++i) a[i] = ldg_stream(Rrow[i] + ro);
-#pragma unroll
-        for (int j = 0; j < BT; ++j) {
-            const float4 qv = __ldg(qd[j] + qo);
-#pragma unroll
-            for (int i = 0; i < RL; ++i) {
-                acc[i][j] = fmaf(a[i].x, qv.x, acc[i][j]);
-                acc[i][j] = fmaf(a[i].y, qv.y, acc[i][j]);
-                acc[i][j] = fmaf(a[i].z, qv.z, acc[i][j]);
-                acc[i][j] = fmaf(a[i].w, qv.w, acc[i][j]);
-            }
-        }
-        n4 += dn; h += dh;
-        if (n4 >= N4) { n4 -= N4; ++h; }
-    }
-
-    float v[RL * BT];
-#pragma unroll
-    for (int i = 0; i < RL; ++i)
-#pragma unroll
-        for (int j = 0; j < BT; ++j) v[i * BT + j] = acc[i][j];
-    const float tot = warp_reduce_multi<RL * BT>(v, lane);
-    if (lane < RL * BT) {
-        const int i = lane / BT, j = lane - i * BT;
-        const int l = l0 + i;
-        if (l < L) {
-            float xv = 0.f;
-            if (xbase != nullptr) {
-                const int day = dl.day[min(d0 + j, dl.n - 1)];
-                xv = __ldg(xbase + ((size_t)day * T + t) * L + l);
-            }
-            r[((size_t)t * L + l) * bp + d0 + j] = tot - xv;   // pad days (d0+j >= n) repeat the last day
-        }
-    }
-}
-
 template <int BT> struct RVec;
 template <> struct RVec<1> { using type = float; };
 template <> struct RVec<2> { using type = float2; };
 template <> struct RVec<4> { using type = float4; };
 
+enum { EPI_RESID = 0, EPI_UPDATE = 1, EPI_STORE = 2 };
+
+struct BandArgs {
+    const float* A;      // one cluster's copy (Af for a2, Ag for a3): [T][krows][M4*4]
+    const float* B;      // panel [T*kunit][bp]: window rows w0(tt) .. w0(tt)+Kc
+    int M;               // valid outputs per time index (L for a2, N for a3)
+    int M4;              // padded outputs / 4
+    int kunit;           // K rows per lag (Np for a2, Lp for a3)
+    int T, H, bp;
+    int forward;         // 1: a2 (window ends at tt), 0: a3 (window starts at tt)
+    // epilogues
+    const float* x;      // EPI_RESID: [D][T][M]
+    float* out;          // EPI_RESID: r panel [T*M4*4][bp]; EPI_STORE: [T][opitch]
+    int opitch;
+    float* q;            // EPI_UPDATE: state, in place
+    size_t dayStride;
+    float eta;
+};
+
 // ---------------------------------------------------------------------------------------------
-// a3 + a4: transpose gradient g[s][n][d] = sum_{h<=min(H,T-1-s)} sum_l R[s][h][l][n] r[s+h][l][d]
-// ("g = B_o^T(...)") with the projected update q <- max(0, q - eta g) in the epilogue
-// ("x = max(x,0)").  The (h,l) rows of R[s] are contiguous, so a thread owns one
-// float4 of OD columns and walks rows; 256 threads = CW column-threads x KS row-slices; partial
-// sums meet in shared memory, then the CTA applies the update with coalesced q accesses.
-// grid = (ceil(N4/CW), T, ceil(b/BT)), block = 256, dynamic smem = 256*4*BT*4 bytes.
-// UPDATE = false stores g to gout[s][n] (minibatch 1; dode_apply_t).
+// a2 / a3 (+a4): out[tt][m][d] = sum_{k < Kc} A[tt][k][m] * B[w0 + k][d]
+//   a2 ("B_o x - y", Alg. 1 line 9): Kc = (min(H,tt)+1)*Np, w0 = (tt-min(H,tt))*Np, EPI_RESID subtracts x
+//   a3 ("g = B_o^T(...)"):            Kc = (min(H,T-1-tt)+1)*Lp, w0 = tt*Lp, EPI_UPDATE applies
+//        q <- max(0, q - eta g) ("x = max(x,0)") in place
+// A thread owns one float4 of outputs and walks K rows; 256 threads = CW column-threads x KS row-slices;
+// partial sums meet in shared memory, then the CTA runs the epilogue with coalesced accesses.
+// grid = (ceil(M4/CW), T, ceil(b/BT)), block = 256, dynamic smem = 256*4*BT*4 bytes.
 // ---------------------------------------------------------------------------------------------
-template <int BT, bool UPDATE>
+template <int BT, int EPI>
 __global__ void __launch_bounds__(kThreads)
-grad_coldot(const float* __restrict__ Rc, const float* __restrict__ r, float* __restrict__ qbase,
-            size_t dayStride, float* __restrict__ gout, float eta,
-            int N, int N4, int L, int T, int H, int bp, int cwlog2, const __grid_constant__ DayList dl) {
+band_coldot(const __grid_constant__ BandArgs a, int cwlog2, const __grid_constant__ DayList dl) {
     extern __shared__ float sm[];
     const int CW = 1 << cwlog2, KS = kThreads >> cwlog2;
     const int col = threadIdx.x & (CW - 1), ks = threadIdx.x >> cwlog2;
-    const int s = blockIdx.y, d0 = blockIdx.z * BT;
-    const int n4 = min((int)blockIdx.x * CW + col, N4 - 1);
-    const int Kc = (min(H, T - 1 - s) + 1) * L;
+    const int tt = blockIdx.y, d0 = blockIdx.z * BT;
+    const int m4 = min((int)blockIdx.x * CW + col, a.M4 - 1);
+    const int lags = (a.forward ? min(a.H, tt) : min(a.H, a.T - 1 - tt)) + 1;
+    const int Kc = lags * a.kunit;
+    const long w0 = a.forward ? (long)(tt - lags + 1) * a.kunit : (long)tt * a.kunit;
+    const int bp = a.bp;
 
-    const float4* Rp = reinterpret_cast<const float4*>(Rc) + (size_t)s * (H + 1) * L * N4 + n4;
-    const float* rp = r + (size_t)s * L * bp + d0;
+    const float4* Ap = reinterpret_cast<const float4*>(a.A) + (size_t)tt * (a.H + 1) * a.kunit * a.M4 + m4;
+    const float* Bp = a.B + (size_t)w0 * bp + d0;
 
     float acc[4][BT];
 #pragma unroll
@@ -172,17 +91,17 @@ grad_coldot(const float* __restrict__ Rc, const float* __restrict__ r, float* __
 #pragma unroll
         for (int j = 0; j < BT; ++j) acc[c][j] = 0.f;
 
-    constexpr int VW = BT >= 4 ? 4 : BT;           // days per r load
+    constexpr int VW = BT >= 4 ? 4 : BT;           // days per panel load
     using rvec = typename RVec<VW>::type;
     constexpr int U = 4;
     int k = ks;
     for (; k + (U - 1) * KS < Kc; k += U * KS) {
-        float4 a[U];
+        float4 av[U];
 #pragma unroll
-        for (int u = 0; u < U; ++u) a[u] = ldg_stream(Rp + (size_t)(k + u * KS) * N4);
+        for (int u = 0; u < U; ++u) av[u] = ldg_stream(Ap + (size_t)(k + u * KS) * a.M4);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const rvec* rr = reinterpret_cast<const rvec*>(rp + (size_t)(k + u * KS) * bp);
+            const rvec* rr = reinterpret_cast<const rvec*>(Bp + (size_t)(k + u * KS) * bp);
 #pragma unroll
             for (int jv = 0; jv < BT / VW; ++jv) {
                 const rvec rv = __ldg(rr + jv);
@@ -190,17 +109,17 @@ grad_coldot(const float* __restrict__ Rc, const float* __restrict__ r, float* __
 #pragma unroll
                 for (int e = 0; e < VW; ++e) {
                     const int j = jv * VW + e;
-                    acc[0][j] = fmaf(a[u].x, rf[e], acc[0][j]);
-                    acc[1][j] = fmaf(a[u].y, rf[e], acc[1][j]);
-                    acc[2][j] = fmaf(a[u].z, rf[e], acc[2][j]);
-                    acc[3][j] = fmaf(a[u].w, rf[e], acc[3][j]);
+                    acc[0][j] = fmaf(av[u].x, rf[e], acc[0][j]);
+                    acc[1][j] = fmaf(av[u].y, rf[e], acc[1][j]);
+                    acc[2][j] = fmaf(av[u].z, rf[e], acc[2][j]);
+                    acc[3][j] = fmaf(av[u].w, rf[e], acc[3][j]);
                 }
             }
         }
     }
     for (; k < Kc; k += KS) {
-        const float4 a = ldg_stream(Rp + (size_t)k * N4);
-        const rvec* rr = reinterpret_cast<const rvec*>(rp + (size_t)k * bp);
+        const float4 av = ldg_stream(Ap + (size_t)k * a.M4);
+        const rvec* rr = reinterpret_cast<const rvec*>(Bp + (size_t)k * bp);
 #pragma unroll
         for (int jv = 0; jv < BT / VW; ++jv) {
             const rvec rv = __ldg(rr + jv);
@@ -208,10 +127,10 @@ grad_coldot(const float* __restrict__ Rc, const float* __restrict__ r, float* __
 #pragma unroll
             for (int e = 0; e < VW; ++e) {
                 const int j = jv * VW + e;
-                acc[0][j] = fmaf(a.x, rf[e], acc[0][j]);
-                acc[1][j] = fmaf(a.y, rf[e], acc[1][j]);
-                acc[2][j] = fmaf(a.z, rf[e], acc[2][j]);
-                acc[3][j] = fmaf(a.w, rf[e], acc[3][j]);
+                acc[0][j] = fmaf(av.x, rf[e], acc[0][j]);
+                acc[1][j] = fmaf(av.y, rf[e], acc[1][j]);
+                acc[2][j] = fmaf(av.z, rf[e], acc[2][j]);
+                acc[3][j] = fmaf(av.w, rf[e], acc[3][j]);
             }
         }
     }
@@ -223,20 +142,103 @@ grad_coldot(const float* __restrict__ Rc, const float* __restrict__ r, float* __
         *reinterpret_cast<float4*>(sm + (size_t)ks * O + j * CW * 4 + col * 4) =
             make_float4(acc[0][j], acc[1][j], acc[2][j], acc[3][j]);
     __syncthreads();
-    const int Np = N4 * 4;
+    const int Mp = a.M4 * 4;
     for (int o = threadIdx.x; o < O; o += kThreads) {
         float g = 0.f;
         for (int q = 0; q < KS; ++q) g += sm[(size_t)q * O + o];
-        const int j = o >> (cwlog2 + 2), nn = o & (CW * 4 - 1);
-        const int n = blockIdx.x * CW * 4 + nn;
-        if (n < N && d0 + j < dl.n) {
-            if (UPDATE) {
-                float* qp = qbase + (size_t)dl.day[d0 + j] * dayStride + (size_t)s * Np + n;
-                *qp = fmaxf(0.f, fmaf(-eta, g, *qp));
-            } else {
-                gout[(size_t)s * N + n] = g;
+        const int j = o >> (cwlog2 + 2), mm = o & (CW * 4 - 1);
+        const int m = blockIdx.x * CW * 4 + mm;
+        if (m >= Mp) continue;
+        if (EPI == EPI_RESID) {
+            // pad days (d0+j >= n) repeat the last day; pad rows (m >= M) are written as 0
+            float v = 0.f;
+            if (m < a.M) {
+                const int day = dl.day[min(d0 + j, dl.n - 1)];
+                v = g - __ldg(a.x + ((size_t)day * a.T + tt) * a.M + m);
             }
+            a.out[((size_t)tt * Mp + m) * bp + d0 + j] = v;
+        } else if (EPI == EPI_UPDATE) {
+            if (m < a.M && d0 + j < dl.n) {
+                float* qp = a.q + (size_t)dl.day[d0 + j] * a.dayStride + (size_t)tt * Mp + m;
+                *qp = fmaxf(0.f, fmaf(-a.eta, g, *qp));
+            }
+        } else {
+            if (m < a.opitch && j == 0) a.out[(size_t)tt * a.opitch + m] = g;
         }
+    }
+}
+
+// ---- create-time packing (a0) -------------------------------------------------------------------
+// Ag[c][s][h][l][n] = R[c][s][h][l][n] for l < L, n < N and s+h < T; everything else 0.
+// (blocks with s+h >= T "may be present; they are ignored" — include/dode.h)
+__global__ void __launch_bounds__(256)
+pack_departure_major(const float* __restrict__ R, float* __restrict__ Ag, long blocks, int T, int H, int L, int N,
+                     int Lp, int Np) {
+    const long total = blocks * Lp * (Np / 4);
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+        const int n4 = (int)(i % (Np / 4));
+        const long rowi = i / (Np / 4);
+        const int l = (int)(rowi % Lp);
+        const long blk = rowi / Lp;                       // (c*T + s)*(H+1) + h
+        const int h = (int)(blk % (H + 1)), s = (int)((blk / (H + 1)) % T);
+        float v[4] = {0.f, 0.f, 0.f, 0.f};
+        if (l < L && s + h < T) {
+            const float* src = R + (blk * L + l) * (size_t)N + n4 * 4;
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                if (n4 * 4 + e < N) v[e] = __ldg(src + e);
+        }
+        reinterpret_cast<float4*>(Ag)[i] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+// Af[c][t][j][n][l] = R[c][s][h][l][n] with s = t-hmax+j, h = hmax-j, hmax = min(H,t), for j <= hmax; 0 otherwise.
+// One 32x32 (l x n) transpose tile per block; grid = (ceil(Lp/32), ceil(Np/32), C*T*(H+1)).
+__global__ void __launch_bounds__(256)
+pack_arrival_major(const float* __restrict__ R, float* __restrict__ Af, int T, int H, int L, int N, int Lp, int Np) {
+    __shared__ float tile[32][33];
+    const long ctj = blockIdx.z;                          // (c*T + t)*(H+1) + j
+    const int j = (int)(ctj % (H + 1));
+    const long ct = ctj / (H + 1);
+    const int t = (int)(ct % T);
+    const long c = ct / T;
+    const int hmax = min(H, t);
+    const int l0 = blockIdx.x * 32, n0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const bool valid = j <= hmax;
+    if (valid) {
+        const int s = t - hmax + j, h = hmax - j;
+        const float* src = R + (((c * T + s) * (H + 1) + h) * (size_t)L) * N;
+        for (int ll = ty; ll < 32; ll += 8) {
+            const int l = l0 + ll, n = n0 + tx;
+            tile[ll][tx] = (l < L && n < N) ? __ldg(src + (size_t)l * N + n) : 0.f;
+        }
+    }
+    __syncthreads();
+    float* dst = Af + ctj * (size_t)Np * Lp;
+    for (int nn = ty; nn < 32; nn += 8) {
+        const int n = n0 + nn, l = l0 + tx;
+        if (n < Np && l < Lp) dst[(size_t)n * Lp + l] = valid ? tile[tx][nn] : 0.f;
+    }
+}
+
+// dst[i*bp + d] = src[day_d*dayStride + i] for i < rowLen, d < bp (pad days repeat the last day). 32x32 smem transpose.
+__global__ void __launch_bounds__(256)
+gather_panel(const float* __restrict__ src, size_t dayStride, long rowLen, float* __restrict__ dst, int bp,
+             const __grid_constant__ DayList dl) {
+    __shared__ float tile[32][33];
+    const long i0 = (long)blockIdx.x * 32;
+    const int d0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int dd = ty; dd < 32; dd += 8) {
+        const int d = min(d0 + dd, dl.n - 1);
+        const long i = i0 + tx;
+        tile[dd][tx] = i < rowLen ? __ldg(src + (size_t)dl.day[d] * dayStride + i) : 0.f;
+    }
+    __syncthreads();
+    for (int ii = ty; ii < 32; ii += 8) {
+        const long i = i0 + ii;
+        if (i < rowLen && d0 + tx < bp) dst[i * bp + d0 + tx] = tile[tx][ii];
     }
 }
 

@@ -1,27 +1,31 @@
 // Tensor-core path of a2-a4 for minibatch b >= 8: banded block GEMMs on tcgen05 (5th-gen tensor
 // cores, FP32 accumulators in TMEM) with 3xTF32 split arithmetic, TMA-staged operands.
 //
-// Per output tile (time index tt, 128 rows m0..m0+127) the pass is one GEMM
-//        D[128 x BN] = sum_k A[128 x K] * B[K x BN]        (BN = b rounded up to 16 days)
-//   forward  (a2): A = rows l of the blocks R[tt-h][h], h = 0..min(H,tt)   (K = (h, n), n contiguous)
-//                  B = gathered state Qg[d][tt-h][n]                        (K contiguous per day)
-//   gradient (a3): A = rows n of the transposed copy Rt[s][n][(h,l)]        (K = (h,l) contiguous)
-//                  B = residual panel rp[d][s*Lp + (h,l)]                   (K contiguous per day)
-// Both operands are K-major, so one kernel serves both passes; only the K enumeration and the epilogue
-// differ.  Truncation at the day boundary falls out of TMA's zero fill: the gradient's B
-// columns beyond T*L are out of bounds.
+// Per output tile (time index tt, 128 outputs m0..m0+127) the pass is one GEMM
+//        D[128 x BN] = sum_k A[k][m] * B[k][d]             (BN = b rounded up to 16 days)
+//   forward  (a2): A = Af[tt] (K rows (j,n), outputs l contiguous),  B[k][d] = Qg[d][(tt-hmax)*Np + k]
+//   gradient (a3): A = Ag[tt] (K rows (h,l), outputs n contiguous),  B[k][d] = rp[d][tt*Lp + k]
+// (layouts: kernels_dense.cuh).  In both passes B is a contiguous window of a per-day vector, K-major, and A
+// arrives "M-major" (the output index contiguous in HBM, so TMA moves 512-byte runs).  That is fine because
+// A never feeds the tensor core from shared memory: 3xTF32 has to split A = A_hi + A_lo anyway, so splitter
+// threads (thread = output row = TMEM lane) read their COLUMN of the landed tile (consecutive lanes ->
+// consecutive words, conflict-free), and write A_hi / A_lo into tensor memory with tcgen05.st; tcgen05.mma
+// then takes A from TMEM (TS form) and B from shared memory (SWIZZLE_128B K-major descriptors).
+// Truncation at the day boundary falls out of zero rows packed at create time and of TMA's
+// zero fill beyond the end of the per-day vector / of the K rows of a slab.
 //
 // 3xTF32 (north_star: "3xTF32 tensor-core emulation ... where the tolerance still holds"):
 //   a = a_hi + a_lo with a_hi = a truncated to TF32 (what the tensor core reads from an fp32 container),
 //   a_lo = a - a_hi (exact in fp32);   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo   (error ~2^-20 relative).
-//   B_lo panels are produced where B is produced (gather kernel / forward epilogue); A_lo is computed in
-//   shared memory by four "splitter" warps between the TMA landing and the MMA issue, so R is still read
-//   from HBM exactly once per pass.
+//   B_lo panels are produced where B is produced (gather kernel / forward epilogue).  For bn <= 128 the
+//   B_full and B_lo tiles, adjacent in smem, are fed as ONE N = 2*bn operand: D[:, 0:bn] += A_hi*B_full
+//   (+ A_lo*B_full by a second MMA), D[:, bn:2bn] += A_hi*B_lo, and the epilogue adds the two halves
+//   -> 2 MMAs per K-step instead of 3.
+// TMEM columns: [0, acc_cols) accumulators, then nring x (32 cols A_hi | 32 cols A_lo).
 //
 // Warp roles (320 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 and 6-9 = two
-// groups of A_lo splitters that take alternate K chunks (each owns one A_lo buffer, so two split chains are
-// in flight), then the epilogue (TMEM -> registers -> global, fused -x / projected update), column chunks
-// interleaved between the groups.
+// groups of splitters that take alternate K chunks, then the epilogue (TMEM -> registers -> global, fused
+// -x / projected update), column chunks interleaved between the groups.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -60,6 +64,19 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     } while (!done);
 }
 
+// One lane of a converged warp (elect.sync).  Inside a warp-uniform branch this lets ptxas emit the uniform-datapath
+// instructions (UTMALDG, UTCHMMA, UTCBAR) once, predicated, instead of an ELECT/BRA.U.ANY loop per instruction.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "elect.sync _|p, 0xffffffff;\n"
+        "selp.b32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(pred));
+    return pred != 0;
+}
+
 __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
@@ -87,26 +104,20 @@ __host__ __device__ constexpr uint32_t umma_idesc_tf32(int bn) {
     return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 }
 
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
-        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
 struct TcParams {
-    int mode;            // 0 = forward, 1 = gradient
-    int M;               // valid output rows per time index (L forward, N gradient)
-    int T, H, L, Lp, Np;
+    int mode;            // 0 = forward (a2), 1 = gradient (a3 + a4)
+    int M;               // valid outputs per time index (L forward, N gradient)
+    int T, H;
+    int kunit;           // K rows per lag (Np forward, Lp gradient)
+    int slab0;           // c*T: first (cluster, time) slab of the A tensor map
+    int Lp, Np;
     int bn;              // MMA N (days rounded up to 16)
     int stages;
-    long a_row0;         // first row of this cluster in the A tensor map
-    int kg_chunks;       // gradient: ceil((H+1)*L / 32)
+    int nring;           // TMEM A buffers (2 or 4), half per splitter group
     // epilogue
     const float* x;      // [D][T][L]        (forward)
     float* rp_full;      // [bcap][rpitch]   (forward output / gradient B operand)
@@ -115,187 +126,9 @@ struct TcParams {
     float* q;            // [D][T][Np]       (gradient, in place)
     size_t dayStride;
     float eta;
-    int dbg;             // bring-up switch: 0 = full kernel
-    int nring;           // TS kernel: TMEM A buffers (2 or 4)
+    int dbg;             // bring-up switches: 1 = no split, 2 = no MMA, 4 = no epilogue (results invalid)
 };
 
-template <int DUMMY = 0>
-__global__ void __launch_bounds__(kThreadsTC)
-banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapBf,
-                   const __grid_constant__ CUtensorMap mapBl, const __grid_constant__ TcParams p,
-                   const __grid_constant__ DayList dl) {
-    extern __shared__ __align__(1024) uint8_t smem_raw[];
-    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
-    const int m0 = blockIdx.x * kTileM;
-    const int bBytes = p.bn * kTileK * 4;
-    // smem: [stages x (A | B_full | B_lo)] [2 x A_lo] [barriers]; the A_lo ring is shorter than the TMA ring
-    // because A_lo only lives from the split to the retirement of its MMAs
-    const int stageBytes = kABytes + 2 * bBytes;
-    uint8_t* alo_base = smem + (size_t)p.stages * stageBytes;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(alo_base + 2 * kABytes);
-    uint64_t* full = bars;                        // [stages] TMA landed
-    uint64_t* empty = bars + p.stages;            // [stages] MMAs of the stage retired
-    uint64_t* split = bars + 2 * p.stages;        // [2] A_lo written
-    uint64_t* alo_empty = split + 2;              // [2] MMAs that read this A_lo buffer retired
-    uint64_t* accum = alo_empty + 2;              // accumulator complete
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
-
-    const int kchunks_per_lag = (p.Np + kTileK - 1) / kTileK;
-    int nk;
-    if (p.mode == 0) nk = (min(p.H, tt) + 1) * kchunks_per_lag;
-    else             nk = min(p.kg_chunks, ((min(p.H, p.T - 1 - tt) + 1) * p.Lp + kTileK - 1) / kTileK);
-
-    uint32_t tmem_cols = 32;
-    while ((int)tmem_cols < p.bn) tmem_cols <<= 1;
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-        for (int j = 0; j < 2; ++j) { mbar_init(&split[j], 128); mbar_init(&alo_empty[j], 1); }
-        mbar_init(accum, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBf) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBl) : "memory");
-    }
-    if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t tmem_d = *tmem_slot;
-
-    if (p.dbg == 1) {
-    } else if (warp == 0) {
-        // ===== TMA producer =====
-        if (lane == 0) {
-            for (int kc = 0; kc < nk; ++kc) {
-                const int s = kc % p.stages, round = kc / p.stages;
-                if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
-                uint8_t* st = smem + (size_t)s * stageBytes;
-                mbar_expect_tx(&full[s], kABytes + 2 * bBytes);
-                if (p.mode == 0) {
-                    const int h = kc / kchunks_per_lag, j = kc - h * kchunks_per_lag;
-                    const long arow = p.a_row0 + ((long)(tt - h) * (p.H + 1) + h) * p.L + m0;
-                    tma_load_2d(st, &mapA, &full[s], j * kTileK, (int)arow);
-                    tma_load_3d(st + kABytes, &mapBf, &full[s], j * kTileK, tt - h, 0);
-                    tma_load_3d(st + kABytes + bBytes, &mapBl, &full[s], j * kTileK, tt - h, 0);
-                } else {
-                    const long arow = p.a_row0 + (long)tt * p.Np + m0;
-                    tma_load_2d(st, &mapA, &full[s], kc * kTileK, (int)arow);
-                    tma_load_2d(st + kABytes, &mapBf, &full[s], tt * p.Lp + kc * kTileK, 0);
-                    tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], tt * p.Lp + kc * kTileK, 0);
-                }
-            }
-        }
-    } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
-            const uint32_t idesc = umma_idesc_tf32(p.bn);
-            for (int kc = 0; kc < nk; ++kc) {
-                const int s = kc % p.stages, round = kc / p.stages;
-                const int jb = kc & 1;
-                mbar_wait(&full[s], round & 1);
-                mbar_wait(&split[jb], (kc >> 1) & 1);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t a0 = smem_u32(smem + (size_t)s * stageBytes);
-                const uint32_t al0 = smem_u32(alo_base + (size_t)jb * kABytes), bf0 = a0 + kABytes, bl0 = bf0 + bBytes;
-#pragma unroll
-                for (int k = 0; k < kTileK / 8; ++k) {           // UMMA_K = 8 for tf32: 32 bytes along the span
-                    const uint64_t da = umma_desc_k_sw128(a0 + k * 32), dal = umma_desc_k_sw128(al0 + k * 32);
-                    const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32), dbl = umma_desc_k_sw128(bl0 + k * 32);
-                    if (p.dbg == 2) continue;
-                    umma_tf32(tmem_d, da, dbf, idesc, (kc | k) != 0);   // a_hi * b_hi
-                    umma_tf32(tmem_d, dal, dbf, idesc, 1);              // a_lo * b_hi
-                    umma_tf32(tmem_d, da, dbl, idesc, 1);               // a_hi * b_lo
-                }
-                if (p.dbg == 2) { mbar_arrive(&empty[s]); mbar_arrive(&alo_empty[jb]); }
-                else { umma_commit(&empty[s]); umma_commit(&alo_empty[jb]); }
-            }
-            if (p.dbg == 2) mbar_arrive(accum); else umma_commit(accum);
-        }
-    } else {
-        // ===== A_lo splitters (group 0 = warps 2-5: even chunks, group 1 = warps 6-9: odd chunks), then epilogue =====
-        const int group = (warp - 2) >> 2;
-        const int st_tid = threadIdx.x - 64 - 128 * group;      // 0..127
-        for (int kc = group; kc < nk; kc += 2) {
-            const int s = kc % p.stages, round = kc / p.stages;
-            const int jb = group;
-            mbar_wait(&full[s], round & 1);
-            if (kc >= 2) mbar_wait(&alo_empty[jb], ((kc >> 1) - 1) & 1);
-            const float4* A = reinterpret_cast<const float4*>(smem + (size_t)s * stageBytes);
-            float4* Al = reinterpret_cast<float4*>(alo_base + (size_t)jb * kABytes);
-#pragma unroll
-            for (int j = 0; j < kABytes / 16 / 128; ++j) {
-                const float4 v = A[st_tid + 128 * j];
-                float4 lo;
-                lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
-                lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
-                lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
-                lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
-                Al[st_tid + 128 * j] = lo;
-            }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> async-proxy (UMMA) reads
-            mbar_arrive(&split[jb]);
-        }
-        // ---- epilogue: TMEM lane = output row; a warp may touch lanes 32*(warp%4) .. +31 ----
-        mbar_wait(accum, 0);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const int lane_base = (warp & 3) * 32;
-        const int m = m0 + lane_base + lane;
-        for (int c0 = 16 * group; c0 < p.bn && p.dbg != 2 && p.dbg != 3; c0 += 32) {
-            uint32_t v[16];
-            const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
-            asm volatile(
-                "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                  "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                : "r"(taddr) : "memory");
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (m < p.M) {
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int d = c0 + j;
-                    if (d < dl.n) {
-                        const float acc = __uint_as_float(v[j]);
-                        if (p.mode == 0) {
-                            const float r = acc - __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.L + m);
-                            const float hi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
-                            p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
-                            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - hi;
-                        } else {
-                            float* qp = p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
-                            *qp = fmaxf(0.f, fmaf(-p.eta, acc, *qp));
-                        }
-                    }
-                }
-            }
-        }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    }
-    __syncthreads();
-    if (warp == 1) {
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(tmem_cols) : "memory");
-    }
-}
-
-
-// =====================================================================================================
-// v2 ("TS mode"): A operands in tensor memory.
-// Shared-memory bandwidth bounds the SS kernel above: every MMA re-reads its 128x8 A slice from smem
-// (3 MMAs x 4 K-steps x 4 KB per chunk) on top of the splitters' 16 KB read + 16 KB write.  Here the
-// splitter threads read their A row ONCE from the TMA-landed (swizzled) tile into registers and store both
-// A_hi (the fp32 container; the tensor core truncates it to TF32) and A_lo = a - trunc(a) into TMEM with
-// tcgen05.st; tcgen05.mma then takes A from TMEM, so smem only carries the TMA writes, one 16 KB read and
-// the B slices.  For bn <= 128 the B_full and B_lo tiles, adjacent in smem, are fed as ONE N = 2*bn
-// operand: D[:, 0:bn] += A_hi*B_full (+ A_lo*B_full by a second MMA), D[:, bn:2bn] += A_hi*B_lo, and the
-// epilogue adds the two halves -> 2 MMAs per K-step instead of 3.
-// TMEM columns: [0, acc_cols) accumulators, then nring x (32 cols A_hi | 32 cols A_lo).
-// =====================================================================================================
 __device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n"
@@ -319,23 +152,35 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
         : "r"(taddr) : "memory");
 }
 
+#ifdef DODE_TC_TRACE
+// bring-up instrumentation (not built by default): per-chunk SM clock stamps of one CTA
+constexpr int kTraceNk = 512;
+__device__ long long g_trace[4 * kTraceNk * 4];
+#define TC_TRACE(role, kc, slot) do { if (tracing && (kc) < kTraceNk) g_trace[(((role) * kTraceNk) + (kc)) * 4 + (slot)] = clock64(); } while (0)
+#else
+#define TC_TRACE(role, kc, slot) do {} while (0)
+#endif
+
 __global__ void __launch_bounds__(kThreadsTC)
-banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA64,
-                      const __grid_constant__ CUtensorMap mapBf,
-                      const __grid_constant__ CUtensorMap mapBl, const __grid_constant__ TcParams p,
-                      const __grid_constant__ DayList dl) {
+banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA64,
+                   const __grid_constant__ CUtensorMap mapBf, const __grid_constant__ CUtensorMap mapBl,
+                   const __grid_constant__ TcParams p, const __grid_constant__ DayList dl) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tt = blockIdx.y;
+    const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
     const int m0 = blockIdx.x * kTileM;
+#ifdef DODE_TC_TRACE
+    const bool tracing = p.mode == 0 && blockIdx.y == gridDim.y / 2 && blockIdx.x == gridDim.x / 2;
+#endif
     const int bBytes = p.bn * kTileK * 4;
     const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full | B_lo
-    const int nring = p.nring;                                   // TMEM A buffers (2 or 4), half per splitter group
-    // a tile with <= 64 valid rows (small networks, ragged last tile) fetches and splits only 64 rows of A; the
+    const int nring = p.nring;
+    // a tile with <= 64 valid outputs (small networks, ragged last tile) fetches and splits a 64-wide A box; the
     // MMA still runs M = 128 and the upper accumulator rows are never stored
     const bool half = p.M - m0 <= 64;
-    const int aBytes = half ? kABytes / 2 : kABytes;
+    const int BM = half ? kTileM / 2 : kTileM;                   // A tile in smem: [kTileK rows][BM floats], no swizzle
+    const int aBytes = BM * kTileK * 4;
     const CUtensorMap* mA = half ? &mapA64 : &mapA;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stageBytes);
     uint64_t* full = bars;                        // [stages] TMA landed
@@ -345,10 +190,9 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
     uint64_t* accum = a_empty + 4;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
 
-    const int kchunks_per_lag = (p.Np + kTileK - 1) / kTileK;
-    int nk;
-    if (p.mode == 0) nk = (min(p.H, tt) + 1) * kchunks_per_lag;
-    else             nk = min(p.kg_chunks, ((min(p.H, p.T - 1 - tt) + 1) * p.Lp + kTileK - 1) / kTileK);
+    const int lags = (p.mode == 0 ? min(p.H, tt) : min(p.H, p.T - 1 - tt)) + 1;
+    const int nk = (lags * p.kunit + kTileK - 1) / kTileK;
+    const int w0 = p.mode == 0 ? (tt - lags + 1) * p.kunit : tt * p.kunit;     // first element of the B window
 
     const bool fused_n = p.bn <= 128;
     const int acc_cols = fused_n ? 2 * p.bn : p.bn;
@@ -389,7 +233,7 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
             const int d = c0 + j;
             pre[j] = 0.f;
             if (em < p.M && d < dl.n)
-                pre[j] = p.mode == 0 ? __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.L + em)
+                pre[j] = p.mode == 0 ? __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.M + em)
                                      : p.q[(size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + em];
         }
     };
@@ -399,77 +243,81 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
 
     if (warp == 0) {
         // ===== TMA producer =====
-        if (lane == 0) {
-            for (int kc = 0; kc < nk; ++kc) {
-                const int s = kc % p.stages, round = kc / p.stages;
-                if (round > 0) mbar_wait(&empty[s], (round - 1) & 1);
+        int s = 0, ph = 1;                                       // ph: parity of the previous round of slot s
+        for (int kc = 0; kc < nk; ++kc) {
+            TC_TRACE(0, kc, 0);
+            if (kc >= p.stages) mbar_wait(&empty[s], ph);
+            TC_TRACE(0, kc, 1);
+            if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
                 mbar_expect_tx(&full[s], aBytes + 2 * bBytes);
-                if (p.mode == 0) {
-                    const int h = kc / kchunks_per_lag, j = kc - h * kchunks_per_lag;
-                    const long arow = p.a_row0 + ((long)(tt - h) * (p.H + 1) + h) * p.L + m0;
-                    tma_load_2d(st, mA, &full[s], j * kTileK, (int)arow);
-                    tma_load_3d(st + kABytes, &mapBf, &full[s], j * kTileK, tt - h, 0);
-                    tma_load_3d(st + kABytes + bBytes, &mapBl, &full[s], j * kTileK, tt - h, 0);
-                } else {
-                    const long arow = p.a_row0 + (long)tt * p.Np + m0;
-                    tma_load_2d(st, mA, &full[s], kc * kTileK, (int)arow);
-                    tma_load_2d(st + kABytes, &mapBf, &full[s], tt * p.Lp + kc * kTileK, 0);
-                    tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], tt * p.Lp + kc * kTileK, 0);
-                }
+                tma_load_3d(st, mA, &full[s], m0, kc * kTileK, p.slab0 + tt);
+                tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
+                tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
             }
+            __syncwarp();
+            if (++s == p.stages) { s = 0; ph ^= 1; }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
-            const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc2 = umma_idesc_tf32(2 * p.bn);
-            for (int kc = 0; kc < nk; ++kc) {
-                const int s = kc % p.stages, round = kc / p.stages;
-                const int g = kc & 1, use = kc >> 1;
-                const int jr = g * per_group + use % per_group;
-                mbar_wait(&full[s], round & 1);
-                mbar_wait(&split[jr], (use / per_group) & 1);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes, bl0 = bf0 + bBytes;
-                const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
-                if (p.dbg & 2) { mbar_arrive(&empty[s]); mbar_arrive(&a_empty[jr]); continue; }   // bring-up: no MMA
+        // ===== MMA issuer: the whole warp walks the loop, one elected lane issues =====
+        const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc2 = umma_idesc_tf32(2 * p.bn);
+        int s = 0, ph = 0;
+        for (int kc = 0; kc < nk; ++kc) {
+            const int g = kc & 1, use = kc >> 1;
+            const int jr = g * per_group + use % per_group;
+            TC_TRACE(1, kc, 0);
+            mbar_wait(&full[s], ph);
+            TC_TRACE(1, kc, 1);
+            mbar_wait(&split[jr], (use / per_group) & 1);
+            TC_TRACE(1, kc, 2);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes, bl0 = bf0 + bBytes;
+            const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
+            if (elect_one()) {
+                if (p.dbg & 2) { mbar_arrive(&empty[s]); mbar_arrive(&a_empty[jr]); }            // bring-up: no MMA
+                else {
 #pragma unroll
-                for (int k = 0; k < kTileK / 8; ++k) {
-                    const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
-                    if (fused_n) {
-                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, (kc | k) != 0);   // [a_hi*b_full | a_hi*b_lo]
-                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);               //  a_lo*b_full
-                    } else {
-                        const uint64_t dbl = umma_desc_k_sw128(bl0 + k * 32);
-                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc1, (kc | k) != 0);
-                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);
-                        umma_tf32_ts(tmem_d, ahi + k * 8, dbl, idesc1, 1);
+                    for (int k = 0; k < kTileK / 8; ++k) {       // UMMA_K = 8 for tf32: 32 bytes along the swizzle span
+                        const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
+                        if (fused_n) {
+                            umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, (kc | k) != 0);   // [a_hi*b_full | a_hi*b_lo]
+                            umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);               //  a_lo*b_full
+                        } else {
+                            const uint64_t dbl = umma_desc_k_sw128(bl0 + k * 32);
+                            umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc1, (kc | k) != 0);
+                            umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);
+                            umma_tf32_ts(tmem_d, ahi + k * 8, dbl, idesc1, 1);
+                        }
                     }
+                    umma_commit(&empty[s]);
+                    umma_commit(&a_empty[jr]);
                 }
-                umma_commit(&empty[s]);
-                umma_commit(&a_empty[jr]);
             }
-            if (p.dbg & 2) mbar_arrive(accum); else umma_commit(accum);
+            __syncwarp();
+            TC_TRACE(1, kc, 3);
+            if (++s == p.stages) { s = 0; ph ^= 1; }
         }
+        if (elect_one()) { if (p.dbg & 2) mbar_arrive(accum); else umma_commit(accum); }
+        __syncwarp();
     } else {
-        // ===== splitters: smem row -> registers -> TMEM (A_hi, A_lo); group g takes chunks kc = g, g+2, ... =====
+        // ===== splitters: smem column -> registers -> TMEM (A_hi, A_lo); group g takes chunks kc = g, g+2, ... =====
         const int group = (warp - 2) >> 2;
         const int lane_base = (warp & 3) * 32;                  // TMEM lanes this warp may touch
-        const int row = lane_base + lane;                       // A tile row == TMEM lane
+        const int row = lane_base + lane;                       // output row within the tile == TMEM lane
         for (int kc = group; kc < nk; kc += 2) {
             const int s = kc % p.stages, round = kc / p.stages;
             const int use = kc >> 1;
             const int jr = group * per_group + use % per_group;
+            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 0);
             mbar_wait(&full[s], round & 1);
+            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 1);
             if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1);
-            if ((half && lane_base >= 64) || (p.dbg & 1)) { mbar_arrive(&split[jr]); continue; }    // rows never stored
-            const uint8_t* A = smem + (size_t)s * stageBytes + (size_t)row * 128;
+            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 2);
+            if (lane_base >= BM || (p.dbg & 1)) { mbar_arrive(&split[jr]); continue; }    // rows never stored
+            const float* A = reinterpret_cast<const float*>(smem + (size_t)s * stageBytes) + row;
             uint32_t hi[32], lo[32];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {                       // 16-byte chunk c of the row sits at (c ^ (row & 7))
-                const uint4 v = *reinterpret_cast<const uint4*>(A + ((c ^ (row & 7)) << 4));
-                hi[4 * c + 0] = v.x; hi[4 * c + 1] = v.y; hi[4 * c + 2] = v.z; hi[4 * c + 3] = v.w;
-            }
+            for (int k = 0; k < 32; ++k) hi[k] = __float_as_uint(A[k * BM]);
 #pragma unroll
             for (int i = 0; i < 32; ++i)
                 lo[i] = __float_as_uint(__uint_as_float(hi[i]) - __uint_as_float(hi[i] & 0xffffe000u));
@@ -479,6 +327,7 @@ banded_gemm_3xtf32_ts(const __grid_constant__ CUtensorMap mapA, const __grid_con
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             mbar_arrive(&split[jr]);
+            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 3);
         }
         // ---- epilogue ----
         mbar_wait(accum, 0);
@@ -540,28 +389,6 @@ gather_split(const float* __restrict__ q, size_t dayStride, long len4, float* __
         lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
         f[i] = v;
         l[i] = lo;
-    }
-}
-
-// create-time: Rt[c][s][n][h*Lp + l] = R[c][s][h][l][n] (Lp = L rounded up to 4 so that every TMA box of the
-// gradient's B operand starts 16-byte aligned; pad columns are 0).  One 32x32 tile per block.
-__global__ void __launch_bounds__(256)
-transpose_blocks(const float* __restrict__ R, float* __restrict__ Rt, int H1, int L, int Lp, int Np, int KGp) {
-    __shared__ float tile[32][33];
-    const size_t cs = blockIdx.z;                                  // (c*T + s)
-    const int ltiles = (Lp + 31) / 32;
-    const int h = blockIdx.y / ltiles, l0 = (blockIdx.y - h * ltiles) * 32, n0 = blockIdx.x * 32;
-    const float* src = R + (cs * H1 + h) * (size_t)L * Np;
-    float* dst = Rt + cs * (size_t)Np * KGp + (size_t)h * Lp;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    for (int ll = ty; ll < 32; ll += 8) {
-        const int l = l0 + ll, n = n0 + tx;
-        tile[ll][tx] = (l < L && n < Np) ? src[(size_t)l * Np + n] : 0.f;
-    }
-    __syncthreads();
-    for (int nn = ty; nn < 32; nn += 8) {
-        const int n = n0 + nn, l = l0 + tx;
-        if (n < Np && l < Lp) dst[(size_t)n * KGp + l] = tile[tx][nn];
     }
 }
 
