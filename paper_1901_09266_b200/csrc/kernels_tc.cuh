@@ -234,12 +234,14 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             pre[j] = 0.f;
             if (em < p.M && d < dl.n)
                 pre[j] = p.mode == 0 ? __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.M + em)
-                                     : p.q[(size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + em];
+                                     : __ldcg(p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + em);
         }
     };
     if (p.mode == 0 && warp >= 2) prefetch(16 * egroup);             // x is a static input
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (p.mode == 1 && warp >= 2) prefetch(16 * egroup);             // q: written by the previous step
+    // q was written by the previous step's kernel, which may still have been running on this SM when this CTA was
+    // launched (PDL): the launch-time L1 invalidation does not cover it, so q is read through L2 (ld.global.cg)
+    if (p.mode == 1 && warp >= 2) prefetch(16 * egroup);
 
     if (warp == 0) {
         // ===== TMA producer =====
@@ -304,12 +306,17 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         const int group = (warp - 2) >> 2;
         const int lane_base = (warp & 3) * 32;                  // TMEM lanes this warp may touch
         const int row = lane_base + lane;                       // output row within the tile == TMEM lane
-        for (int kc = group; kc < nk; kc += 2) {
-            const int s = kc % p.stages, round = kc / p.stages;
+        int s = -1, ph = 1;
+        for (int kc = 0; kc < nk; ++kc) {
+            if (++s == p.stages) s = 0;
+            if (s == 0) ph ^= 1;
             const int use = kc >> 1;
             const int jr = group * per_group + use % per_group;
             if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 0);
-            mbar_wait(&full[s], round & 1);
+            // every group observes EVERY phase of every full barrier (also for the other group's chunks): a parity
+            // wait is only sound for a waiter that never falls a whole phase behind or skips one
+            mbar_wait(&full[s], ph);
+            if ((kc & 1) != group) continue;
             if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 1);
             if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1);
             if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 2);
@@ -381,7 +388,7 @@ gather_split(const float* __restrict__ q, size_t dayStride, long len4, float* __
     float4* f = reinterpret_cast<float4*>(gfull + (size_t)d * dayStride);
     float4* l = reinterpret_cast<float4*>(glo + (size_t)d * dayStride);
     for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < len4; i += (long)gridDim.x * blockDim.x) {
-        const float4 v = __ldg(src + i);
+        const float4 v = __ldcg(src + i);          // through L2: see the note on PDL and L1 in banded_gemm_3xtf32
         float4 lo;
         lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
         lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
