@@ -76,9 +76,12 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
  * Asynchronous on the ctx stream; no host synchronisation, no device->host traffic. */
 int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta);
 
-/* The same iteration for a streaming caller (bench.py's end-to-end leg): first uploads the n days'
- * counts from x_host ([n][T][L], host, pinned or pageable), runs the step, then downloads the n
- * days' updated q into q_host ([n][T][N], host) and synchronises. */
+/* The same iteration for a streaming caller (bench.py's end-to-end leg): uploads the n days' counts from x_host
+ * ([n][T][L], host; pinned memory makes the copies asynchronous), runs the step, and downloads the n days' updated q
+ * into q_host ([n][T][N], host).  ASYNCHRONOUS and pipelined over consecutive calls on two internal copy streams:
+ * the upload of call i+1 and the download of call i-1 overlap the kernels of call i (calls that share a day are
+ * ordered).  x_host must stay valid and q_host is defined only after the next synchronising call (dode_sync,
+ * dode_objective, dode_get_q, dode_set_q, dode_timing_read, dode_destroy). */
 int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta,
                         const float* x_host, float* q_host);
 

@@ -53,6 +53,13 @@ struct dode_ctx {
     int tc_cap = 0, tc_bn = 0, tc_min_b = 8;
     bool tc_ready = false, tc_attr = false;
     CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64, mapQ_f, mapQ_l, mapR_f, mapR_l;
+    // streaming steps (dode_spgd_step_host): copy streams, staging buffers, ping-pong events
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_h2d = nullptr, ev_step[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
+    float *stage_x = nullptr, *stage_q = nullptr;
+    size_t stage_x_cap = 0, stage_q_cap = 0;
+    int64_t host_calls = 0;
+    std::vector<int32_t> prev_days;
     // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -199,6 +206,14 @@ static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, int* bt_out, i
     }
     *bt_out = bt; *bp_out = bp;
     return DODE_OK;
+}
+
+// waits for the compute stream and for the copy streams of the streaming step
+static cudaError_t sync_all(dode_ctx* ctx) {
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (ctx->s_h2d) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_h2d); if (e == cudaSuccess) e = e2; }
+    if (ctx->s_d2h) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_d2h); if (e == cudaSuccess) e = e2; }
+    return e;
 }
 
 static int validate_days(dode_ctx* ctx, const int32_t* days, int32_t n, bool same_cluster, int* cluster) {
@@ -420,7 +435,12 @@ extern "C" {
 
 void dode_destroy(dode_ctx* ctx) {
     if (!ctx) return;
-    cudaStreamSynchronize(ctx->stream);
+    sync_all(ctx);
+    if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
+    if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+    if (ctx->ev_h2d) cudaEventDestroy(ctx->ev_h2d);
+    for (int i = 0; i < 2; ++i) { if (ctx->ev_step[i]) cudaEventDestroy(ctx->ev_step[i]); if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]); }
+    cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
     cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
     cudaFree(ctx->Ag); cudaFree(ctx->Af); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r); cudaFree(ctx->Qb);
     for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
@@ -515,20 +535,84 @@ int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta) {
     return step_impl(ctx, days, n, eta, c);
 }
 
+// staging <-> state for the streaming step: x[day_i] <- stage[i] (scatter) / stage[i] <- q[day_i] without the pad columns
+__global__ void __launch_bounds__(256)
+stage_scatter_x(const float* __restrict__ stage, float* __restrict__ x, long TL, const __grid_constant__ DayList dl) {
+    const float* src = stage + (size_t)blockIdx.y * TL;
+    float* dst = x + (size_t)dl.day[blockIdx.y] * TL;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < TL; i += (long)gridDim.x * blockDim.x) dst[i] = src[i];
+}
+__global__ void __launch_bounds__(256)
+stage_gather_q(const float* __restrict__ q, float* __restrict__ stage, int T, int N, int Np, const __grid_constant__ DayList dl) {
+    const float* src = q + (size_t)dl.day[blockIdx.y] * T * Np;
+    float* dst = stage + (size_t)blockIdx.y * T * N;
+    const long total = (long)T * N;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+        const long t = i / N;
+        dst[i] = src[t * Np + (i - t * N)];
+    }
+}
+
 int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, const float* x_host, float* q_host) {
     if (!ctx) return DODE_EINVAL;
     int c = 0, rc;
     if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
     if (!x_host || !q_host) return fail(ctx, DODE_EINVAL, "x_host or q_host is null");
     const dode_dims& d = ctx->dm;
-    const size_t TL = (size_t)d.T * d.L, TNp = (size_t)d.T * ctx->Np, TN = (size_t)d.T * d.N;
-    for (int i = 0; i < n; ++i)
-        CU(cudaMemcpyAsync(ctx->x + TL * days[i], x_host + TL * i, TL * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    const size_t TL = (size_t)d.T * d.L, TN = (size_t)d.T * d.N;
+    if (!ctx->s_h2d) {
+        CU(cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->ev_h2d, cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_step[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_d2h[i], cudaEventDisableTiming));
+        }
+    }
+    if (ctx->stage_x_cap < TL * n || ctx->stage_q_cap < TN * n) {
+        CU(sync_all(ctx));
+        cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
+        ctx->stage_x = ctx->stage_q = nullptr; ctx->stage_x_cap = ctx->stage_q_cap = 0;
+        CU(cudaMalloc(&ctx->stage_x, TL * n * sizeof(float)));
+        CU(cudaMalloc(&ctx->stage_q, TN * n * sizeof(float)));
+        ctx->stage_x_cap = TL * n; ctx->stage_q_cap = TN * n;
+    }
+    // One-deep software pipeline over calls i: upload(i+1) || step(i) || download(i-1).
+    //   upload(i)   waits for step(i-2) always and for step(i-1) if the two calls share a day (x of that day is still being read)
+    //   step(i)     waits for upload(i), for download(i-2) always and for download(i-1) if they share a day (q still being read)
+    //   download(i) waits for step(i)
+    const int me = (int)(ctx->host_calls & 1), other = me ^ 1;
+    bool shares_day = false;                       // validate_days stamped this call's days with stamp_id
+    for (int32_t pd : ctx->prev_days) shares_day |= ctx->stamp[pd] == ctx->stamp_id;
+    if (ctx->host_calls >= 2) CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_step[me], 0));
+    if (ctx->host_calls >= 1 && shares_day) CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_step[other], 0));
+    CU(cudaMemcpyAsync(ctx->stage_x, x_host, TL * n * sizeof(float), cudaMemcpyHostToDevice, ctx->s_h2d));
+    for (int off = 0; off < n; off += kMaxDays) {
+        DayList dl; dl.n = std::min(kMaxDays, n - off);
+        std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
+        stage_scatter_x<<<dim3(std::min<long>(64, ceil_div((long)TL, 256)), dl.n), 256, 0, ctx->s_h2d>>>(
+            ctx->stage_x + TL * off, ctx->x, (long)TL, dl);
+        ctx->launches++;
+    }
+    CU(cudaEventRecord(ctx->ev_h2d, ctx->s_h2d));
+    CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_h2d, 0));
+    if (ctx->host_calls >= 2) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_d2h[me], 0));
+    if (ctx->host_calls >= 1 && shares_day) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_d2h[other], 0));
     if ((rc = step_impl(ctx, days, n, eta, c))) return rc;
-    for (int i = 0; i < n; ++i)
-        CU(cudaMemcpy2DAsync(q_host + TN * i, d.N * sizeof(float), ctx->q + TNp * days[i], ctx->Np * sizeof(float),
-                             d.N * sizeof(float), d.T, cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
+    CU(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_step[me], 0));
+    for (int off = 0; off < n; off += kMaxDays) {
+        DayList dl; dl.n = std::min(kMaxDays, n - off);
+        std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
+        stage_gather_q<<<dim3(std::min<long>(64, ceil_div((long)TN, 256)), dl.n), 256, 0, ctx->s_d2h>>>(
+            ctx->q, ctx->stage_q + TN * off, d.T, d.N, ctx->Np, dl);
+        ctx->launches++;
+    }
+    CU(cudaMemcpyAsync(q_host, ctx->stage_q, TN * n * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_d2h));
+    CU(cudaEventRecord(ctx->ev_d2h[me], ctx->s_d2h));
+    ctx->prev_days.assign(days, days + n);
+    ctx->host_calls++;
+    CU(cudaGetLastError());
     return DODE_OK;
 }
 
@@ -544,6 +628,7 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
     }
     int rc;
     if ((rc = validate_days(ctx, days, n, false, nullptr))) return rc;
+    CU(sync_all(ctx));                        // pending streamed uploads of x belong to the state being evaluated
     // group positions by cluster, evaluate in sub-batches; d_obj[i] receives f of days[i]
     constexpr int kObjBatch = 64;
     const size_t dayStride = (size_t)d.T * ctx->Np;
@@ -589,6 +674,7 @@ static int copy_q(dode_ctx* ctx, int32_t day, float* out, const float* in, int32
     const dode_dims& d = ctx->dm;
     if (day < 0 || day >= d.D) return fail(ctx, DODE_EINVAL, "day %d out of range [0,%d)", day, d.D);
     if (!out && !in) return fail(ctx, DODE_EINVAL, "null buffer");
+    CU(sync_all(ctx));
     float* qd = ctx->q + (size_t)day * d.T * ctx->Np;
     if (out)
         CU(cudaMemcpy2DAsync(out, d.N * sizeof(float), qd, ctx->Np * sizeof(float), d.N * sizeof(float), d.T,
@@ -720,7 +806,7 @@ const char* dode_last_path(const dode_ctx* ctx) { return ctx ? ctx->path.c_str()
 
 int dode_sync(dode_ctx* ctx) {
     if (!ctx) return DODE_EINVAL;
-    CU(cudaStreamSynchronize(ctx->stream));
+    CU(sync_all(ctx));
     CU(cudaGetLastError());
     return DODE_OK;
 }

@@ -164,7 +164,23 @@ def test_get_set_q_and_host_step():
     xh = p.x[days].contiguous().pin_memory()
     qh = torch.empty(len(days), cfg.T, cfg.N).pin_memory()
     P.dode_spgd_step_host(g2.h, days, float(etas[0]), xh, qh)
+    P.dode_sync(g2.h)                      # the streaming step is asynchronous: q_host is defined after a sync
     np.testing.assert_array_equal(qh.numpy(), g1.q(days))
+    np.testing.assert_array_equal(g2.q(), g1.q())
+    # a pipelined sequence of streaming calls — consecutive calls that share a day, disjoint calls, a repeat two calls
+    # later — equals the same sequence of resident steps, and every call's download is that call's state
+    seq = [[0, 1, 2], [2, 3], [4, 5], [0, 5], [1], [0, 1, 2, 3, 4, 5], [3]]
+    bufs = []
+    for days in seq:
+        P.dode_spgd_step(g1.h, days, float(etas[0]))
+        want = g1.q(days).copy()
+        xh = p.x[days].contiguous().pin_memory()
+        qh = torch.empty(len(days), cfg.T, cfg.N).pin_memory()
+        P.dode_spgd_step_host(g2.h, days, float(etas[0]), xh, qh)
+        bufs.append((xh, qh, want))
+    P.dode_sync(g2.h)
+    for xh, qh, want in bufs:
+        np.testing.assert_array_equal(qh.numpy(), want)
     np.testing.assert_array_equal(g2.q(), g1.q())
     g1.close(); g2.close()
 
