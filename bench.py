@@ -125,18 +125,20 @@ def algorithmic(cfg, n_days):
     return fwd_b, grad_b, fl
 
 
-def cpu_oracle_sample(cfg, R, lab, x, etas, visits):
-    """Times the oracle as it stands on `visits` day-visits (single thread); returns ms per visit."""
+def cpu_oracle_sample(cfg, Rc, c0, lab, x, eta, visits):
+    """Times the oracle as it stands on `visits` day-visits of cluster c0's days (single thread); returns ms per visit
+    and the number of visits timed."""
     from oracle import oracle
-    days = list(range(min(visits, cfg.D)))
+    own = [d for d in range(cfg.D) if int(lab[d]) == c0]
+    days = [own[i % len(own)] for i in range(max(1, visits))]
     q = np.ones((cfg.T, cfg.N), np.float32)
-    Rn = [R[c].numpy() for c in range(cfg.C)]
-    oracle.visit(Rn[int(lab[0])], q, x[0].numpy(), float(etas[int(lab[0])]))       # page in
+    Rn = Rc.numpy()
+    if cfg.nb * cfg.L * cfg.N < 2e8:
+        oracle.visit(Rn, q, x[days[0]].numpy(), float(eta))       # page in
     t0 = time.perf_counter()
     for d in days:
-        c = int(lab[d])
-        oracle.visit(Rn[c], q, x[d].numpy(), float(etas[c]))
-    return (time.perf_counter() - t0) * 1e3 / len(days)
+        oracle.visit(Rn, q, x[d].numpy(), float(eta))
+    return (time.perf_counter() - t0) * 1e3 / len(days), len(days)
 
 
 def run_reference(args, cfg, b, rank, world):
@@ -214,6 +216,13 @@ def run_ours(args, cfg, b, rank, world, local_rank):
         torch.cuda.empty_cache()              # the library allocates with cudaMalloc: give torch's cached blocks back first
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, csr=csr)
         nnz_c = csr.nnz / cfg.C
+        csr_host = None
+        if rank == 0 and not args.no_cpu_baseline:          # one cluster's CSR blocks for the oracle's timing leg
+            c0, nbk = int(lab[0]), cfg.T * (cfg.H + 1)
+            bo = csr.blk_off[c0 * nbk:(c0 + 1) * nbk + 1].cpu().numpy()
+            k0, k1 = int(bo[0]), int(bo[-1])
+            csr_host = (c0, bo - k0, csr.row_ptr[c0 * nbk:(c0 + 1) * nbk].cpu().numpy(),
+                        csr.col_idx[k0:k1].cpu().numpy(), csr.val[k0:k1].cpu().numpy())
         del csr
     else:
         R = synth.dar_dense(cfg, device=dev)
@@ -222,8 +231,8 @@ def run_ours(args, cfg, b, rank, world, local_rank):
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, dense=R)
     x_cpu = x.cpu()
     R_cpu = None
-    if rank == 0 and not args.no_cpu_baseline and not cfg.sparse and cfg.N * cfg.L * cfg.T * (cfg.H + 1) * 4 < 4e9:
-        R_cpu = R.cpu()
+    if rank == 0 and not args.no_cpu_baseline and not cfg.sparse:
+        R_cpu = R[int(lab[0])].cpu()                  # one cluster's operator for the oracle's timing leg
     if not cfg.sparse:
         del R
     del x
@@ -348,10 +357,24 @@ def run_ours(args, cfg, b, rank, world, local_rank):
         return
     # ---- CPU oracle beside it (bounded sample, rank 0 only) ----
     cpu = None
+    if cfg.sparse and csr_host is not None:
+        from oracle import oracle
+        c0, bo, rp, ci, va = csr_host
+        days_c0 = [d for d in range(cfg.D) if int(lab[d]) == c0][:3]
+        q1 = np.ones((cfg.T, cfg.N), np.float32)
+        t0 = time.perf_counter()
+        for d in days_c0:
+            oracle.visit_csr(cfg.N, cfg.L, cfg.T, cfg.H, bo, rp, ci, va, q1, x_cpu[d].numpy(), float(etas[c0]))
+        ms_visit = (time.perf_counter() - t0) * 1e3 / len(days_c0)
+        cpu = {"value": ms_visit * cfg.D, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{len(days_c0)} day-visits (CSR oracle loop) of the {cfg.D}-visit epoch timed single-threaded on this host "
+                         f"({os.cpu_count()} cores visible), extrapolated x{cfg.D / len(days_c0):.1f}",
+               "ms_per_day_visit": ms_visit}
     if R_cpu is not None:
-        per_visit = cfg.nb * cfg.L * cfg.N * 4 / 0.6e9          # rough s per visit at ~0.6 GFLOP/s scalar double
-        visits = int(max(3, min(cfg.D, 15.0 / max(per_visit, 1e-4))))
-        ms_visit = cpu_oracle_sample(cfg, R_cpu, lab, x_cpu, etas, visits)
+        per_visit = cfg.nb * cfg.L * cfg.N * 4 / 3e9            # rough s per visit at ~3 GFLOP/s scalar double
+        visits = int(max(3, min(2 * cfg.D, 15.0 / max(per_visit, 1e-4))))
+        c0 = int(lab[0])
+        ms_visit, visits = cpu_oracle_sample(cfg, R_cpu, c0, lab, x_cpu, etas[c0], visits)
         cpu = {"value": ms_visit * cfg.D, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{visits} day-visits of the {cfg.D}-visit epoch timed single-threaded on this host "
                          f"({os.cpu_count()} cores visible), extrapolated x{cfg.D / visits:.1f}",
