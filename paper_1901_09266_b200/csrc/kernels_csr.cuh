@@ -1,18 +1,23 @@
 // a6: block-sparse CSR variant of a2-a4 for large networks (BASELINE.json configs[4]).
 //
 // The boundary format is one CSR per (c,s,h) block (include/dode.h).  At create time each cluster is
-// re-packed, on the device, into two lag-merged CSR matrices so that both passes stream their non-zeros
-// contiguously and deterministically (no atomics on the hot path):
-//   F (forward):  row (t,l) holds every entry of blocks (t-h,h), h<=min(H,t):  (off = n - h*Np, val)
-//                 so that the operand is Qb[(t*Np + off)*bp + d]
-//   G (gradient): row (s,n) holds every entry of blocks (s,h), s+h<T:           (kl = h*L + l, val)
-//                 so that the operand is r[(s*L + kl)*bp + d]
-// Entries with s+h >= T are dropped.  The re-pack is a stable radix sort of 64-bit keys
-// (CUB, create-time only).
+// re-packed, on the device, into two lag-merged ROW-BLOCKED sparse matrices so that both passes stream their
+// non-zeros contiguously and deterministically (no atomics on the hot path) and so that one gathered panel row
+// feeds up to kRB output rows:
+//   F (forward):  row block (t, l/4) holds one entry per distinct (h,n) of the blocks (t-h,h), h<=min(H,t), that
+//                 touches any of its 4 links: payload off = n - h*Np, values val[4] (0 where a link has no entry)
+//                 -> operand Qb[(t*Np + off)*bp + d].  Paths are contiguous link runs with slowly growing lag
+//                 (PAPER.md:195-228), so adjacent links share most (h,n): ~2.5x fewer gathers than plain CSR.
+//   G (gradient): row block (s/4, n) holds one entry per distinct residual row (t,l), t = s+h, reached from any of
+//                 its 4 departure intervals: payload kl = (t - 4*(s/4))*L + l, values val[4] by s%4
+//                 -> operand r[((4*(s/4))*L + kl)*bp + d].  The lag window of a (link, OD) pair spans 2-4 adjacent
+//                 lags, so consecutive departure intervals share most residual rows: ~2x fewer gathers.
+// Entries with s+h >= T are dropped.  The re-pack is a radix sort of 64-bit keys, a head-flag scan
+// and a scatter (CUB, create-time only).
 //
 // Hot path: the minibatch state is gathered once per step into day-fastest panels Qb[T*Np][bp] and
-// Xb[T*L][bp] (coalesced transposes), so that one non-zero pulls bp contiguous floats; a warp owns one
-// CSR row and its lanes run along the days.  The update q <- max(0, q - eta g) is applied to Qb in the
+// Xb[T*L][bp] (coalesced transposes), so that one entry pulls bp contiguous floats; a warp owns one
+// row block and its lanes run along the days.  The update q <- max(0, q - eta g) is applied to Qb in the
 // gradient kernel's epilogue and scattered back to q[d][s][n].
 #pragma once
 #include <cuda_runtime.h>
@@ -20,6 +25,7 @@
 
 #include <cstdio>
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 
 #include "../../include/dode.h"
 #include "kernels_dense.cuh"
@@ -27,15 +33,17 @@
 namespace dode {
 
 constexpr int kCsrMaxDays = 128;
+constexpr int kRB = 4;            // output rows per row block
 
 struct CsrCluster {
-    int64_t* rowptrF = nullptr;   // [T*L + 1]
-    int32_t* offF = nullptr;      // [nnzF]
-    float* valF = nullptr;
-    int64_t* rowptrG = nullptr;   // [T*N + 1]
-    int32_t* klG = nullptr;       // [nnzG]
-    float* valG = nullptr;
+    int64_t* rowptrF = nullptr;   // [T*ceil(L/4) + 1]
+    int32_t* payF = nullptr;      // [nuF]  n - h*Np
+    float4* valF = nullptr;       // [nuF]  by l%4
+    int64_t* rowptrG = nullptr;   // [ceil(T/4)*Np + 1]
+    int32_t* payG = nullptr;      // [nuG]  (t - 4*(s/4))*L + l
+    float4* valG = nullptr;       // [nuG]  by s%4
     int64_t nnz = 0;              // valid entries (s+h < T)
+    int64_t nuF = 0, nuG = 0;     // distinct (row block, payload) entries
 };
 
 struct CsrStore {
@@ -48,7 +56,7 @@ struct CsrStore {
 };
 
 // ---- create-time re-pack ---------------------------------------------------------------------------
-// one warp per input CSR row (s,h,l) of cluster c
+// one warp per input CSR row (s,h,l) of cluster c; key = ((row block * K + payload) << 2) | row in block
 __global__ void csr_expand_keys(const int64_t* __restrict__ blk_off, const int32_t* __restrict__ row_ptr,
                                 const int32_t* __restrict__ col_idx, int c, int N, int Np, int L, int T, int H,
                                 int64_t base, unsigned long long* __restrict__ keyF,
@@ -63,40 +71,58 @@ __global__ void csr_expand_keys(const int64_t* __restrict__ blk_off, const int32
     const long b = (long)c * T * (H + 1) + sh;
     const int32_t* rp = row_ptr + b * (L + 1);
     const int64_t k0 = blk_off[b] + rp[l], k1 = blk_off[b] + rp[l + 1];
-    const unsigned long long KF = (unsigned long long)(H + 1) * Np, KG = (unsigned long long)(H + 1) * L;
+    const unsigned long long KF = (unsigned long long)(H + 1) * Np, KG = (unsigned long long)(H + kRB) * L;
+    const unsigned long long LB = (unsigned long long)(L + kRB - 1) / kRB;
     const bool valid = s + h < T;
+    const int t = s + h, sb = s / kRB;
     for (int64_t k = k0 + lane; k < k1; k += 32) {
         const int n = col_idx[k];
-        keyF[k - base] = valid ? ((unsigned long long)(s + h) * L + l) * KF + (unsigned long long)h * Np + n : ~0ull;
-        keyG[k - base] = valid ? ((unsigned long long)s * Np + n) * KG + (unsigned long long)h * L + l : ~0ull;
+        const unsigned long long rbF = (unsigned long long)t * LB + l / kRB, payF = (unsigned long long)h * Np + n;
+        const unsigned long long rbG = (unsigned long long)sb * Np + n, payG = (unsigned long long)(t - sb * kRB) * L + l;
+        keyF[k - base] = valid ? ((rbF * KF + payF) << 2) | (unsigned)(l % kRB) : ~0ull;
+        keyG[k - base] = valid ? ((rbG * KG + payG) << 2) | (unsigned)(s % kRB) : ~0ull;
     }
 }
 
-// rowptr[row] = lower_bound(keys, row*K); decoded payload: F -> n - h*Np, G -> h*L + l
-__global__ void csr_rowptr(const unsigned long long* __restrict__ keys, int64_t nvalid, long rows,
+// head[i] = 1 where a new (row block, payload) starts in the sorted key array
+__global__ void csr_heads(const unsigned long long* __restrict__ keys, int64_t n, int32_t* __restrict__ head) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        head[i] = (i == 0 || (keys[i] >> 2) != (keys[i - 1] >> 2)) ? 1 : 0;
+}
+
+// uidx = inclusive scan of head; entry u = uidx[i]-1 receives val[i] in slot key&3; heads also write payload and key
+__global__ void csr_scatter_unique(const unsigned long long* __restrict__ keys, const float* __restrict__ val,
+                                   const int32_t* __restrict__ uidx, int64_t n, unsigned long long K, int Np, int forward,
+                                   float* __restrict__ val4, int32_t* __restrict__ pay, unsigned long long* __restrict__ ukey) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const unsigned long long key = keys[i], kk = key >> 2;
+        const int64_t u = (int64_t)uidx[i] - 1;
+        val4[u * 4 + (int)(key & 3)] = val[i];
+        if (i == 0 || kk != (keys[i - 1] >> 2)) {
+            const unsigned long long rem = kk % K;
+            if (forward) {
+                const int h = (int)(rem / Np), nn = (int)(rem - (unsigned long long)h * Np);
+                pay[u] = nn - h * Np;
+            } else {
+                pay[u] = (int32_t)rem;
+            }
+            ukey[u] = kk;
+        }
+    }
+}
+
+// rowptr[rb] = lower_bound(ukey, rb*K)
+__global__ void csr_rowptr(const unsigned long long* __restrict__ ukey, int64_t nu, long rows,
                            unsigned long long K, int64_t* __restrict__ rowptr) {
     const long row = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (row > rows) return;
     const unsigned long long target = (unsigned long long)row * K;
-    int64_t lo = 0, hi = nvalid;
+    int64_t lo = 0, hi = nu;
     while (lo < hi) {
         const int64_t mid = (lo + hi) >> 1;
-        if (keys[mid] < target) lo = mid + 1; else hi = mid;
+        if (ukey[mid] < target) lo = mid + 1; else hi = mid;
     }
     rowptr[row] = lo;
-}
-
-__global__ void csr_decode(const unsigned long long* __restrict__ keys, int64_t nvalid, unsigned long long K,
-                           int Np, int forward, int32_t* __restrict__ out) {
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < nvalid; i += (int64_t)gridDim.x * blockDim.x) {
-        const unsigned long long rem = keys[i] % K;
-        if (forward) {
-            const int h = (int)(rem / Np), n = (int)(rem - (unsigned long long)h * Np);
-            out[i] = n - h * Np;
-        } else {
-            out[i] = (int32_t)rem;
-        }
-    }
 }
 
 __global__ void count_invalid(const unsigned long long* __restrict__ keys, int64_t n, unsigned long long* cnt) {
@@ -110,8 +136,8 @@ __global__ void count_invalid(const unsigned long long* __restrict__ keys, int64
 inline void csr_free(CsrStore& st) {
     if (st.cl) {
         for (int c = 0; c < st.C; ++c) {
-            cudaFree(st.cl[c].rowptrF); cudaFree(st.cl[c].offF); cudaFree(st.cl[c].valF);
-            cudaFree(st.cl[c].rowptrG); cudaFree(st.cl[c].klG); cudaFree(st.cl[c].valG);
+            cudaFree(st.cl[c].rowptrF); cudaFree(st.cl[c].payF); cudaFree(st.cl[c].valF);
+            cudaFree(st.cl[c].rowptrG); cudaFree(st.cl[c].payG); cudaFree(st.cl[c].valG);
         }
         delete[] st.cl;
         st.cl = nullptr;
@@ -128,6 +154,7 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
         if (e_ != cudaSuccess) {                                                                 \
             snprintf(err, 512, "%s: %s", #call, cudaGetErrorString(e_));                         \
             cudaFree(kF); cudaFree(kG); cudaFree(kS); cudaFree(vS); cudaFree(tmp); cudaFree(dcnt); \
+            cudaFree(head); cudaFree(ukey);                                                      \
             return e_ == cudaErrorMemoryAllocation ? DODE_ENOMEM : DODE_ECUDA;                   \
         }                                                                                        \
     } while (0)
@@ -136,8 +163,9 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
     st.cl = new CsrCluster[d.C];
     const long nblk = (long)d.T * (d.H + 1);
     std::vector<int64_t> off(d.C + 1);
-    unsigned long long *kF = nullptr, *kG = nullptr, *kS = nullptr, *dcnt = nullptr;
+    unsigned long long *kF = nullptr, *kG = nullptr, *kS = nullptr, *dcnt = nullptr, *ukey = nullptr;
     float* vS = nullptr;
+    int32_t* head = nullptr;
     void* tmp = nullptr;
     for (int c = 0; c <= d.C; ++c)
         CSR_CU(cudaMemcpyAsync(&off[c], R.blk_off + (long)c * nblk, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
@@ -145,48 +173,65 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
     if (off[d.C] != R.nnz) { snprintf(err, 512, "blk_off[last]=%lld but nnz=%lld", (long long)off[d.C], (long long)R.nnz); return DODE_EINVAL; }
     int64_t maxn = 1;
     for (int c = 0; c < d.C; ++c) maxn = std::max<int64_t>(maxn, off[c + 1] - off[c]);
+    if (maxn >= (int64_t)1 << 31) { snprintf(err, 512, "more than 2^31 non-zeros in one cluster"); return DODE_EINVAL; }
     CSR_CU(cudaMalloc(&kF, maxn * 8)); CSR_CU(cudaMalloc(&kG, maxn * 8)); CSR_CU(cudaMalloc(&kS, maxn * 8));
+    CSR_CU(cudaMalloc(&ukey, maxn * 8)); CSR_CU(cudaMalloc(&head, maxn * 4));
     CSR_CU(cudaMalloc(&vS, maxn * 4)); CSR_CU(cudaMalloc(&dcnt, 8));
-    size_t tmp_bytes = 0;
-    cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, kF, kS, (const float*)nullptr, vS, maxn, 0, 64, stream);
+    size_t tmp_sort = 0, tmp_scan = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, tmp_sort, kF, kS, (const float*)nullptr, vS, maxn, 0, 64, stream);
+    cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, head, head, (int)maxn, stream);
+    const size_t tmp_bytes = std::max(tmp_sort, tmp_scan);
     CSR_CU(cudaMalloc(&tmp, tmp_bytes));
-    const unsigned long long KF = (unsigned long long)(d.H + 1) * Np, KG = (unsigned long long)(d.H + 1) * d.L;
+    const unsigned long long KF = (unsigned long long)(d.H + 1) * Np, KG = (unsigned long long)(d.H + kRB) * d.L;
+    const long LB = (d.L + kRB - 1) / kRB, SB = (d.T + kRB - 1) / kRB;
     for (int c = 0; c < d.C; ++c) {
         CsrCluster& cl = st.cl[c];
         const int64_t n = off[c + 1] - off[c];
         const long rows_in = nblk * d.L;
+        unsigned long long ninv = 0;
         if (n > 0) {
             csr_expand_keys<<<(unsigned)((rows_in * 32 + 255) / 256), 256, 0, stream>>>(
                 R.blk_off, R.row_ptr, R.col_idx, c, d.N, Np, d.L, d.T, d.H, off[c], kF, kG);
             CSR_CU(cudaMemsetAsync(dcnt, 0, 8, stream));
             count_invalid<<<1184, 256, 0, stream>>>(kF, n, dcnt);
+            CSR_CU(cudaMemcpyAsync(&ninv, dcnt, 8, cudaMemcpyDeviceToHost, stream));
         }
-        unsigned long long ninv = 0;
-        if (n > 0) CSR_CU(cudaMemcpyAsync(&ninv, dcnt, 8, cudaMemcpyDeviceToHost, stream));
         CSR_CU(cudaStreamSynchronize(stream));
         const int64_t nv = n - (int64_t)ninv;
         cl.nnz = nv;
-        const long rowsF = (long)d.T * d.L, rowsG = (long)d.T * Np;
-        CSR_CU(cudaMalloc(&cl.rowptrF, (rowsF + 1) * 8)); CSR_CU(cudaMalloc(&cl.rowptrG, (rowsG + 1) * 8));
-        CSR_CU(cudaMalloc(&cl.offF, std::max<int64_t>(nv, 1) * 4)); CSR_CU(cudaMalloc(&cl.valF, std::max<int64_t>(nv, 1) * 4));
-        CSR_CU(cudaMalloc(&cl.klG, std::max<int64_t>(nv, 1) * 4)); CSR_CU(cudaMalloc(&cl.valG, std::max<int64_t>(nv, 1) * 4));
         for (int pass = 0; pass < 2; ++pass) {
             unsigned long long* kin = pass == 0 ? kF : kG;
             const unsigned long long K = pass == 0 ? KF : KG;
-            const long rows = pass == 0 ? rowsF : rowsG;
-            float* vout = pass == 0 ? cl.valF : cl.valG;
-            if (n > 0) {
+            const long rows = pass == 0 ? (long)d.T * LB : SB * Np;          // row blocks
+            int64_t nu = 0;
+            if (nv > 0) {
                 // invalid keys are all-ones: sort on all 64 bits so they land at the end
-                CSR_CU(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, kin, kS, R.val + off[c], vS, n, 0, 64, stream));
-                CSR_CU(cudaMemcpyAsync(vout, vS, nv * 4, cudaMemcpyDeviceToDevice, stream));
-                csr_decode<<<1184, 256, 0, stream>>>(kS, nv, K, Np, pass == 0, pass == 0 ? cl.offF : cl.klG);
+                CSR_CU(cub::DeviceRadixSort::SortPairs(tmp, tmp_sort, kin, kS, R.val + off[c], vS, n, 0, 64, stream));
+                csr_heads<<<1184, 256, 0, stream>>>(kS, nv, head);
+                CSR_CU(cub::DeviceScan::InclusiveSum(tmp, tmp_scan, head, head, (int)nv, stream));
+                int32_t last = 0;
+                CSR_CU(cudaMemcpyAsync(&last, head + nv - 1, 4, cudaMemcpyDeviceToHost, stream));
+                CSR_CU(cudaStreamSynchronize(stream));
+                nu = last;
             }
-            csr_rowptr<<<(unsigned)((rows + 1 + 255) / 256), 256, 0, stream>>>(kS, nv, rows, K, pass == 0 ? cl.rowptrF : cl.rowptrG);
+            int32_t** pay = pass == 0 ? &cl.payF : &cl.payG;
+            float4** val4 = pass == 0 ? &cl.valF : &cl.valG;
+            int64_t** rowptr = pass == 0 ? &cl.rowptrF : &cl.rowptrG;
+            (pass == 0 ? cl.nuF : cl.nuG) = nu;
+            CSR_CU(cudaMalloc(pay, std::max<int64_t>(nu, 1) * 4));
+            CSR_CU(cudaMalloc(val4, std::max<int64_t>(nu, 1) * 16));
+            CSR_CU(cudaMalloc(rowptr, (rows + 1) * 8));
+            if (nu > 0) {
+                CSR_CU(cudaMemsetAsync(*val4, 0, nu * 16, stream));
+                csr_scatter_unique<<<1184, 256, 0, stream>>>(kS, vS, head, nv, K, Np, pass == 0,
+                                                             reinterpret_cast<float*>(*val4), *pay, ukey);
+            }
+            csr_rowptr<<<(unsigned)((rows + 1 + 255) / 256), 256, 0, stream>>>(ukey, nu, rows, K, *rowptr);
         }
         CSR_CU(cudaStreamSynchronize(stream));
     }
     CSR_CU(cudaGetLastError());
-    cudaFree(kF); cudaFree(kG); cudaFree(kS); cudaFree(vS); cudaFree(tmp); cudaFree(dcnt);
+    cudaFree(kF); cudaFree(kG); cudaFree(kS); cudaFree(vS); cudaFree(tmp); cudaFree(dcnt); cudaFree(head); cudaFree(ukey);
     st.ready = true;
     return DODE_OK;
 #undef CSR_CU
@@ -238,134 +283,169 @@ template <> struct DVec<1> { using type = float; };
 template <> struct DVec<2> { using type = float2; };
 template <> struct DVec<4> { using type = float4; };
 
-// a2 (CSR): one warp per row (t,l) of F; lanes along days (DV days per lane, bp = 32*DV).
-// r[(t*L+l)*rbp + d] = sum_k val_k * Qb[(t*Np + off_k)*bp + d] - Xb[(t*L+l)*bp + d]   for d < rbp
+// a2 (CSR): one warp per row block (t, l/4) of F; lanes along days (DV days per lane, bp = 32*DV).
+// r[(t*L+l)*rbp + d] = sum_k val_k[l%4] * Qb[(t*Np + off_k)*bp + d] - Xb[(t*L+l)*bp + d]   for d < rbp
 template <int DV>
 __global__ void __launch_bounds__(256)
-csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, const float* __restrict__ val,
+csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, const float4* __restrict__ val,
         const float* __restrict__ Qb, const float* __restrict__ Xb, float* __restrict__ r,
-        long rows, int L, int Np, int rbp) {
+        long rblocks, int L, int LB, int Np, int rbp) {
     constexpr int bp = 32 * DV;
     using vec = typename DVec<DV>::type;
-    const long row = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
+    // Warps walk the row blocks LINK-BLOCK-major, time-minor: the warps in flight then cover a few dozen neighbouring
+    // link blocks over all t, whose OD sets overlap (paths are link runs), so the panel rows they gather (~100 MB) stay
+    // in L2; time-major order would sweep the whole 25-lag window of every OD (256 MB) for every t.
+    const long w = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (row >= rows) return;
-    const long t = row / L;
-    const int64_t k0 = rowptr[row], k1 = rowptr[row + 1];
+    if (w >= rblocks) return;
+    const int T = (int)(rblocks / LB);
+    const long lb = w / T, t = w - lb * T;
+    const long rb = t * LB + lb;
+    const int l0 = (int)lb * kRB;
+    const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const float* qrow = Qb + (size_t)t * Np * bp + lane * DV;
-    float acc[DV];
+    float acc[kRB][DV];
 #pragma unroll
-    for (int e = 0; e < DV; ++e) acc[e] = 0.f;
+    for (int i = 0; i < kRB; ++i)
+#pragma unroll
+        for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
     for (int64_t kb = k0; kb < k1; kb += 32) {
         const int64_t k = kb + lane;
         const int o = k < k1 ? __ldg(off + k) : 0;
-        const float v = k < k1 ? __ldg(val + k) : 0.f;
+        const float4 v = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
         const int cnt = (int)min((int64_t)32, k1 - kb);
         int j = 0;
-        for (; j + 4 <= cnt; j += 4) {
-            vec qv[4]; float vv[4];
+        for (; j + 2 <= cnt; j += 2) {
+            vec qv[2]; float vv[2][kRB];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < 2; ++u) {
                 const int oo = __shfl_sync(0xffffffffu, o, j + u);
-                vv[u] = __shfl_sync(0xffffffffu, v, j + u);
+                vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
+                vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
                 qv[u] = *reinterpret_cast<const vec*>(qrow + (long)oo * bp);
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < 2; ++u) {
                 const float* qf = reinterpret_cast<const float*>(&qv[u]);
 #pragma unroll
-                for (int e = 0; e < DV; ++e) acc[e] = fmaf(vv[u], qf[e], acc[e]);
+                for (int i = 0; i < kRB; ++i)
+#pragma unroll
+                    for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[u][i], qf[e], acc[i][e]);
             }
         }
         for (; j < cnt; ++j) {
             const int oo = __shfl_sync(0xffffffffu, o, j);
-            const float vv = __shfl_sync(0xffffffffu, v, j);
+            const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
+                                   __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
             const vec qv = *reinterpret_cast<const vec*>(qrow + (long)oo * bp);
             const float* qf = reinterpret_cast<const float*>(&qv);
 #pragma unroll
-            for (int e = 0; e < DV; ++e) acc[e] = fmaf(vv, qf[e], acc[e]);
+            for (int i = 0; i < kRB; ++i)
+#pragma unroll
+                for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(v4[i], qf[e], acc[i][e]);
         }
     }
-    if (Xb != nullptr) {
-        const vec xv = *reinterpret_cast<const vec*>(Xb + (size_t)row * bp + lane * DV);
-        const float* xf = reinterpret_cast<const float*>(&xv);
 #pragma unroll
-        for (int e = 0; e < DV; ++e) acc[e] -= xf[e];
-    }
-    if (rbp == bp) {
-        vec out;
-        float* of = reinterpret_cast<float*>(&out);
+    for (int i = 0; i < kRB; ++i) {
+        const int l = l0 + i;
+        if (l >= L) break;
+        const size_t row = (size_t)t * L + l;
+        if (Xb != nullptr) {
+            const vec xv = *reinterpret_cast<const vec*>(Xb + row * bp + lane * DV);
+            const float* xf = reinterpret_cast<const float*>(&xv);
 #pragma unroll
-        for (int e = 0; e < DV; ++e) of[e] = acc[e];
-        *reinterpret_cast<vec*>(r + (size_t)row * bp + lane * DV) = out;
-    } else {
+            for (int e = 0; e < DV; ++e) acc[i][e] -= xf[e];
+        }
+        if (rbp == bp) {
+            vec out;
+            float* of = reinterpret_cast<float*>(&out);
 #pragma unroll
-        for (int e = 0; e < DV; ++e)
-            if (lane * DV + e < rbp) r[(size_t)row * rbp + lane * DV + e] = acc[e];
+            for (int e = 0; e < DV; ++e) of[e] = acc[i][e];
+            *reinterpret_cast<vec*>(r + row * bp + lane * DV) = out;
+        } else {
+#pragma unroll
+            for (int e = 0; e < DV; ++e)
+                if (lane * DV + e < rbp) r[row * rbp + lane * DV + e] = acc[i][e];
+        }
     }
 }
 
-// a3+a4 (CSR): one warp per row (s,n) of G.  g[d] = sum_k val_k * r[(s*L + kl_k)*rbp + d];
-// UPDATE: Qb[(s*Np+n)*bp + d] = max(0, Qb - eta g); else gout[s*N + n] = g[0].
+// a3+a4 (CSR): one warp per row block (s/4, n) of G.  g_i[d] = sum_k val_k[i] * r[((4*sb)*L + kl_k)*rbp + d], s = 4*sb+i;
+// UPDATE: Qb[(s*Np+n)*bp + d] = max(0, Qb - eta g_i); else gout[s*N + n] = g_i[0].
 template <int DV, bool UPDATE>
 __global__ void __launch_bounds__(256)
-csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, const float* __restrict__ val,
+csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, const float4* __restrict__ val,
          const float* __restrict__ r, float* __restrict__ Qb, float* __restrict__ gout, float eta,
-         long rows, int L, int N, int Np, int rbp) {
+         long rblocks, int T, int L, int N, int Np, int rbp) {
     constexpr int bp = 32 * DV;
     using vec = typename DVec<DV>::type;
-    const long row = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
+    const long rb = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (row >= rows) return;
-    const long s = row / Np;
-    const int n = (int)(row - s * Np);
+    if (rb >= rblocks) return;
+    const long sb = rb / Np;
+    const int n = (int)(rb - sb * Np);
     if (n >= N) return;
-    const int64_t k0 = rowptr[row], k1 = rowptr[row + 1];
+    const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const bool full = rbp == bp;
-    const float* rrow = r + (size_t)s * L * rbp + lane * DV;
-    float acc[DV];
+    const float* rrow = r + (size_t)sb * kRB * L * rbp + lane * DV;
+    float acc[kRB][DV];
 #pragma unroll
-    for (int e = 0; e < DV; ++e) acc[e] = 0.f;
+    for (int i = 0; i < kRB; ++i)
+#pragma unroll
+        for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
     for (int64_t kb = k0; kb < k1; kb += 32) {
         const int64_t k = kb + lane;
         const int o = k < k1 ? __ldg(kl + k) : 0;
-        const float v = k < k1 ? __ldg(val + k) : 0.f;
+        const float4 v = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
         const int cnt = (int)min((int64_t)32, k1 - kb);
         int j = 0;
         if (full) {
-            for (; j + 4 <= cnt; j += 4) {
-                vec rv[4]; float vv[4];
+            for (; j + 2 <= cnt; j += 2) {
+                vec rv[2]; float vv[2][kRB];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < 2; ++u) {
                     const int oo = __shfl_sync(0xffffffffu, o, j + u);
-                    vv[u] = __shfl_sync(0xffffffffu, v, j + u);
+                    vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
+                    vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
                     rv[u] = *reinterpret_cast<const vec*>(rrow + (long)oo * bp);
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < 2; ++u) {
                     const float* rf = reinterpret_cast<const float*>(&rv[u]);
 #pragma unroll
-                    for (int e = 0; e < DV; ++e) acc[e] = fmaf(vv[u], rf[e], acc[e]);
+                    for (int i = 0; i < kRB; ++i)
+#pragma unroll
+                        for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[u][i], rf[e], acc[i][e]);
                 }
             }
         }
         for (; j < cnt; ++j) {
             const int oo = __shfl_sync(0xffffffffu, o, j);
-            const float vv = __shfl_sync(0xffffffffu, v, j);
+            const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
+                                   __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
 #pragma unroll
             for (int e = 0; e < DV; ++e)
-                if (full || lane * DV + e < rbp) acc[e] = fmaf(vv, rrow[(long)oo * rbp + e], acc[e]);
+                if (full || lane * DV + e < rbp) {
+                    const float rv = rrow[(long)oo * rbp + e];
+#pragma unroll
+                    for (int i = 0; i < kRB; ++i) acc[i][e] = fmaf(v4[i], rv, acc[i][e]);
+                }
         }
     }
-    if (UPDATE) {
-        vec* qp = reinterpret_cast<vec*>(Qb + (size_t)row * bp + lane * DV);
-        vec qv = *qp;
-        float* qf = reinterpret_cast<float*>(&qv);
 #pragma unroll
-        for (int e = 0; e < DV; ++e) qf[e] = fmaxf(0.f, fmaf(-eta, acc[e], qf[e]));
-        *qp = qv;
-    } else if (lane == 0) {
-        gout[(size_t)s * N + n] = acc[0];
+    for (int i = 0; i < kRB; ++i) {
+        const long s = sb * kRB + i;
+        if (s >= T) break;
+        if (UPDATE) {
+            vec* qp = reinterpret_cast<vec*>(Qb + ((size_t)s * Np + n) * bp + lane * DV);
+            vec qv = *qp;
+            float* qf = reinterpret_cast<float*>(&qv);
+#pragma unroll
+            for (int e = 0; e < DV; ++e) qf[e] = fmaxf(0.f, fmaf(-eta, acc[i][e], qf[e]));
+            *qp = qv;
+        } else if (lane == 0) {
+            gout[(size_t)s * N + n] = acc[i][0];
+        }
     }
 }
 
@@ -393,12 +473,14 @@ inline int csr_forward(CsrStore& st, int c, const float* qbase, size_t dayStride
     gather_days<<<dim3((unsigned)((qlen + 31) / 32), bp / 32), 256, 0, stream>>>(qbase, dayStride, qlen, st.Qb, bp, dl);
     if (xbase)
         gather_days<<<dim3((unsigned)((xlen + 31) / 32), bp / 32), 256, 0, stream>>>(xbase, (size_t)d.T * d.L, xlen, st.Xb, bp, dl);
-    const unsigned grid = (unsigned)((xlen * 32 + 255) / 256);
+    const int LB = (d.L + kRB - 1) / kRB;
+    const long rblocks = (long)d.T * LB;
+    const unsigned grid = (unsigned)((rblocks * 32 + 255) / 256);
     const float* Xb = xbase ? st.Xb : nullptr;
     switch (bp) {
-        case 32: csr_fwd<1><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.offF, cl.valF, st.Qb, Xb, r, xlen, d.L, Np, rbp); break;
-        case 64: csr_fwd<2><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.offF, cl.valF, st.Qb, Xb, r, xlen, d.L, Np, rbp); break;
-        default: csr_fwd<4><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.offF, cl.valF, st.Qb, Xb, r, xlen, d.L, Np, rbp); break;
+        case 32: csr_fwd<1><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, r, rblocks, d.L, LB, Np, rbp); break;
+        case 64: csr_fwd<2><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, r, rblocks, d.L, LB, Np, rbp); break;
+        default: csr_fwd<4><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, r, rblocks, d.L, LB, Np, rbp); break;
     }
     *launches += xbase ? 3 : 2;
     return DODE_OK;
@@ -412,16 +494,17 @@ inline int csr_gradient(CsrStore& st, int c, const float* r, float* qbase, size_
     if (rc) return rc;
     const CsrCluster& cl = st.cl[c];
     const long rows = (long)d.T * Np;
-    const unsigned grid = (unsigned)((rows * 32 + 255) / 256);
+    const long rblocks = (long)((d.T + kRB - 1) / kRB) * Np;
+    const unsigned grid = (unsigned)((rblocks * 32 + 255) / 256);
     if (gout) {
-        csr_grad<1, false><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.klG, cl.valG, r, nullptr, gout, eta, rows, d.L, d.N, Np, rbp);
+        csr_grad<1, false><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, nullptr, gout, eta, rblocks, d.T, d.L, d.N, Np, rbp);
         *launches += 1;
         return DODE_OK;
     }
     switch (bp) {
-        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.klG, cl.valG, r, st.Qb, nullptr, eta, rows, d.L, d.N, Np, rbp); break;
-        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.klG, cl.valG, r, st.Qb, nullptr, eta, rows, d.L, d.N, Np, rbp); break;
-        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.klG, cl.valG, r, st.Qb, nullptr, eta, rows, d.L, d.N, Np, rbp); break;
+        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
     }
     scatter_days<<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(st.Qb, bp, rows, qbase, dayStride, dl);
     *launches += 2;
