@@ -42,6 +42,7 @@ struct CsrCluster {
     int64_t* rowptrG = nullptr;   // [ceil(T/4)*Np + 1]
     int32_t* payG = nullptr;      // [nuG]  (t - 4*(s/4))*L + l
     float4* valG = nullptr;       // [nuG]  by s%4
+    int32_t* permG = nullptr;     // [Np]   OD indices ordered by the first link of their path (processing order of a3)
     int64_t nnz = 0;              // valid entries (s+h < T)
     int64_t nuF = 0, nuG = 0;     // distinct (row block, payload) entries
 };
@@ -125,6 +126,20 @@ __global__ void csr_rowptr(const unsigned long long* __restrict__ ukey, int64_t 
     rowptr[row] = lo;
 }
 
+// first link of OD n's path = smallest link index among the entries of its first non-empty row block (L if none)
+__global__ void csr_first_link(const int64_t* __restrict__ rowptrG, const int32_t* __restrict__ payG, int Np, long SB, int L,
+                               int32_t* __restrict__ first, int32_t* __restrict__ ident) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= Np) return;
+    int best = L;
+    for (long sb = 0; sb < SB && best == L; ++sb) {
+        const int64_t k0 = rowptrG[sb * Np + n], k1 = rowptrG[sb * Np + n + 1];
+        for (int64_t k = k0; k < k1; ++k) best = min(best, payG[k] % L);
+    }
+    first[n] = best;
+    ident[n] = n;
+}
+
 __global__ void count_invalid(const unsigned long long* __restrict__ keys, int64_t n, unsigned long long* cnt) {
     unsigned long long local = 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
@@ -137,7 +152,7 @@ inline void csr_free(CsrStore& st) {
     if (st.cl) {
         for (int c = 0; c < st.C; ++c) {
             cudaFree(st.cl[c].rowptrF); cudaFree(st.cl[c].payF); cudaFree(st.cl[c].valF);
-            cudaFree(st.cl[c].rowptrG); cudaFree(st.cl[c].payG); cudaFree(st.cl[c].valG);
+            cudaFree(st.cl[c].rowptrG); cudaFree(st.cl[c].payG); cudaFree(st.cl[c].valG); cudaFree(st.cl[c].permG);
         }
         delete[] st.cl;
         st.cl = nullptr;
@@ -228,6 +243,21 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
             }
             csr_rowptr<<<(unsigned)((rows + 1 + 255) / 256), 256, 0, stream>>>(ukey, nu, rows, K, *rowptr);
         }
+        // processing order of the gradient rows: ODs sorted by the first link of their path
+        {
+            int32_t* sc = nullptr;                       // [Np] keys in | [Np] keys out | [Np] identity
+            CSR_CU(cudaMalloc(&sc, (size_t)3 * Np * 4));
+            CSR_CU(cudaMalloc(&cl.permG, (size_t)Np * 4));
+            csr_first_link<<<(Np + 255) / 256, 256, 0, stream>>>(cl.rowptrG, cl.payG, Np, SB, d.L, sc, sc + 2 * Np);
+            size_t need = 0;
+            void* t2 = nullptr;
+            cub::DeviceRadixSort::SortPairs(nullptr, need, sc, sc + Np, sc + 2 * Np, cl.permG, Np, 0, 32, stream);
+            cudaError_t e2 = cudaMalloc(&t2, need);
+            if (e2 == cudaSuccess) e2 = cub::DeviceRadixSort::SortPairs(t2, need, sc, sc + Np, sc + 2 * Np, cl.permG, Np, 0, 32, stream);
+            if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(stream);
+            cudaFree(t2); cudaFree(sc);
+            CSR_CU(e2);
+        }
         CSR_CU(cudaStreamSynchronize(stream));
     }
     CSR_CU(cudaGetLastError());
@@ -286,7 +316,7 @@ template <> struct DVec<4> { using type = float4; };
 // a2 (CSR): one warp per row block (t, l/4) of F; lanes along days (DV days per lane, bp = 32*DV).
 // r[(t*L+l)*rbp + d] = sum_k val_k[l%4] * Qb[(t*Np + off_k)*bp + d] - Xb[(t*L+l)*bp + d]   for d < rbp
 template <int DV>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, const float4* __restrict__ val,
         const float* __restrict__ Qb, const float* __restrict__ Xb, float* __restrict__ r,
         long rblocks, int L, int LB, int Np, int rbp) {
@@ -373,18 +403,23 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, con
 // a3+a4 (CSR): one warp per row block (s/4, n) of G.  g_i[d] = sum_k val_k[i] * r[((4*sb)*L + kl_k)*rbp + d], s = 4*sb+i;
 // UPDATE: Qb[(s*Np+n)*bp + d] = max(0, Qb - eta g_i); else gout[s*N + n] = g_i[0].
 template <int DV, bool UPDATE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, const float4* __restrict__ val,
-         const float* __restrict__ r, float* __restrict__ Qb, float* __restrict__ gout, float eta,
+         const int32_t* __restrict__ perm, const float* __restrict__ r, float* __restrict__ Qb, float* __restrict__ gout, float eta,
          long rblocks, int T, int L, int N, int Np, int rbp) {
     constexpr int bp = 32 * DV;
     using vec = typename DVec<DV>::type;
-    const long rb = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
+    // Warps walk the row blocks OD-major in path order (perm: ODs sorted by the first link of their path), time-minor:
+    // the warps in flight then gather residual rows of a few dozen neighbouring links over all t (~10 MB, L2-resident)
+    // instead of the 28-interval window of every link (72 MB, which thrashes a 63 MB L2 partition).
+    const long w = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (rb >= rblocks) return;
-    const long sb = rb / Np;
-    const int n = (int)(rb - sb * Np);
+    if (w >= rblocks) return;
+    const long SB = rblocks / Np;
+    const long i = w / SB, sb = w - i * SB;
+    const int n = __ldg(perm + i);
     if (n >= N) return;
+    const long rb = sb * Np + n;
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const bool full = rbp == bp;
     const float* rrow = r + (size_t)sb * kRB * L * rbp + lane * DV;
@@ -497,14 +532,14 @@ inline int csr_gradient(CsrStore& st, int c, const float* r, float* qbase, size_
     const long rblocks = (long)((d.T + kRB - 1) / kRB) * Np;
     const unsigned grid = (unsigned)((rblocks * 32 + 255) / 256);
     if (gout) {
-        csr_grad<1, false><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, nullptr, gout, eta, rblocks, d.T, d.L, d.N, Np, rbp);
+        csr_grad<1, false><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, nullptr, gout, eta, rblocks, d.T, d.L, d.N, Np, rbp);
         *launches += 1;
         return DODE_OK;
     }
     switch (bp) {
-        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
     }
     scatter_days<<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(st.Qb, bp, rows, qbase, dayStride, dl);
     *launches += 2;
