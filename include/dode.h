@@ -92,6 +92,14 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
  * fp32 products, fp64 sums.  Synchronises. */
 int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_day, double* total);
 
+/* Step 6 "quality check" ("R-square between the observed link flow and estimated link flow",
+ * PAPER.md:553): coefficient of determination of the fitted counts of each listed day, observed counts as reference,
+ *     R2_d = 1 - sum_t sum_l (x_d - rho q_d)^2 / sum_t sum_l (x_d - mean(x_d))^2      (reading A17).
+ *   days     host int32 [n], or NULL for all D days (then n is ignored)
+ *   per_day  host double [n] (or [D]), nullable;   mean  host double (average over the listed days), nullable
+ * SS_res is dode_objective's value; sums in fp64.  Synchronises. */
+int dode_r2(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_day, double* mean);
+
 /* Export / import one day's state in Table 2 order (entry s*N + n).
  * out/in: fp32 [T][N]; is_device != 0 means a device pointer.  Synchronises. */
 int dode_get_q(dode_ctx* ctx, int32_t day, float* out, int32_t is_device);

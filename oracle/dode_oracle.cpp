@@ -20,13 +20,14 @@
 //        -- "x = max(x,0)"; plain step instead of Adagrad (reading A3,
 //           BASELINE.json north_star).  r is complete before any q changes.
 //   O3   f = sum_t sum_l r[t][l]^2, no 1/2, no mean -- Eq. 42.
+//   O5   R2_d = 1 - sum r^2 / sum (x - mean x)^2 -- Step 6 quality check (reading A17).
 //   O4   L_c = lambda_max(rho_c^T rho_c) by power iteration from the all-ones
 //        vector (reading A10; PAPER.md:416 only says the rate depends on scale).
 //
 // Pins (tests/test_oracle_pins.py): P1 active-set NNLS on the T=12 instance,
 // P2 KKT, P3 finite differences, P4 planted recovery, P5 closed-form linear
 // iteration, P6 Example 1, P8 adjoint, P9 descent,
-// P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR.
+// P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR, P14 R2 closed forms.
 // No function here is "parity unpinned".
 #include <cmath>
 #include <cstddef>
@@ -119,6 +120,22 @@ double oracle_objective_day(int N, int L, int T, int H, const float* Rc, const f
     double f = 0.0;
     for (double v : rd) f += v * v;
     return f;
+}
+
+// O5 (Step 6 "quality check"; "R-square between the observed link flow and estimated link flow",
+// PAPER.md:553): coefficient of determination of one day's fitted counts, observed counts as the reference
+// (reading A17):  R2 = 1 - sum (x - rho q)^2 / sum (x - mean(x))^2  over the day's T*L entries, all in double.
+double oracle_r2_day(int N, int L, int T, int H, const float* Rc, const float* q, const float* x) {
+    Dims d{N, L, T, H};
+    const size_t TL = (size_t)T * L;
+    std::vector<double> rd(TL);
+    forward_d(d, Rc, q, x, rd.data());
+    double ss_res = 0.0, mean = 0.0, ss_tot = 0.0;
+    for (double v : rd) ss_res += v * v;
+    for (size_t i = 0; i < TL; ++i) mean += (double)x[i];
+    mean /= (double)TL;
+    for (size_t i = 0; i < TL; ++i) ss_tot += ((double)x[i] - mean) * ((double)x[i] - mean);
+    return 1.0 - ss_res / ss_tot;
 }
 
 // Replays a schedule: iteration k visits days sched_days[sched_ptr[k] .. sched_ptr[k+1])

@@ -36,6 +36,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(build_oracle())
         _lib.oracle_objective_day.restype = C.c_double
+        _lib.oracle_r2_day.restype = C.c_double
         _lib.oracle_objective_day_csr.restype = C.c_double
         _lib.oracle_power_iteration.restype = C.c_double
     return _lib
@@ -80,6 +81,13 @@ def objective_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray) -> float:
     N, L, T, H = _dims(Rc)
     Rc, pR = _f(Rc); q, pq = _f(q); x, px = _f(x)
     return float(lib().oracle_objective_day(N, L, T, H, pR, pq, px))
+
+
+def r2_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray) -> float:
+    """O5: coefficient of determination of the fitted counts of one day (Step 6; reading A17)."""
+    N, L, T, H = _dims(Rc)
+    Rc, pR = _f(Rc); q, pq = _f(q); x, px = _f(x)
+    return float(lib().oracle_r2_day(N, L, T, H, pR, pq, px))
 
 
 def power_iteration(Rc: np.ndarray, iters: int = 50) -> float:

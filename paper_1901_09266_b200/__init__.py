@@ -19,7 +19,7 @@ SO_PATH = os.path.join(_HERE, "libdode.so")
 DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
 DODE_DENSE, DODE_CSR = 0, 1
 
-EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_objective", "dode_get_q", "dode_set_q",
+EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
            "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
@@ -57,6 +57,7 @@ def lib():
         L.dode_objective.argtypes = [vp, vp, i32, vp, vp]
         L.dode_get_q.argtypes = [vp, i32, vp, i32]
         L.dode_set_q.argtypes = [vp, i32, vp, i32]
+        L.dode_r2.argtypes = [vp, vp, i32, vp, vp]
         L.dode_apply.argtypes = [vp, i32, vp, vp]
         L.dode_apply_t.argtypes = [vp, i32, vp, vp]
         L.dode_lipschitz.argtypes = [vp, i32, i32, vp]
@@ -149,6 +150,15 @@ def dode_objective(h, days):
     tot = C.c_double()
     _chk(h, lib().dode_objective(h, d.ctypes.data, d.size, per.ctypes.data, C.byref(tot)))
     return per, tot.value
+
+
+def dode_r2(h, days):
+    """Step 6: returns (per-day R2 as a float64 array, their mean) for the listed days."""
+    d = _days(days)
+    per = np.empty(d.size, np.float64)
+    mean = C.c_double()
+    _chk(h, lib().dode_r2(h, d.ctypes.data, d.size, per.ctypes.data, C.byref(mean)))
+    return per, mean.value
 
 
 def dode_get_q(h, day: int, out) -> None:

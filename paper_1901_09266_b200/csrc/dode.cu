@@ -671,6 +671,42 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
     return DODE_OK;
 }
 
+int dode_r2(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_day, double* mean) {
+    if (!ctx) return DODE_EINVAL;
+    const dode_dims& d = ctx->dm;
+    std::vector<int32_t> all;
+    if (!days) {
+        all.resize(d.D);
+        for (int i = 0; i < d.D; ++i) all[i] = i;
+        days = all.data();
+        n = d.D;
+    }
+    if (n <= 0) return fail(ctx, DODE_EINVAL, "n <= 0");
+    std::vector<double> f(n), mom(2 * (size_t)kMaxDays);
+    int rc = dode_objective(ctx, days, n, f.data(), nullptr);            // validates the list, SS_res per day
+    if (rc) return rc;
+    const long TL = (long)d.T * d.L;
+    double acc = 0.0;
+    constexpr int kChunk = 32;                 // 2*kChunk doubles fit the objective's partial buffer (>= 64 doubles)
+    for (int off = 0; off < n; off += kChunk) {
+        DayList dl; dl.n = std::min(kChunk, n - off);
+        std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
+        x_moments<<<dl.n, kThreads, 0, ctx->stream>>>(ctx->x, TL, ctx->d_part, dl);
+        ctx->launches++;
+        CU(cudaMemcpyAsync(mom.data(), ctx->d_part, sizeof(double) * 2 * dl.n, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        for (int i = 0; i < dl.n; ++i) {
+            const double ss_tot = mom[2 * i + 1] - mom[2 * i] * mom[2 * i] / (double)TL;
+            const double r2 = 1.0 - f[off + i] / ss_tot;
+            if (per_day) per_day[off + i] = r2;
+            acc += r2;
+        }
+    }
+    CU(cudaGetLastError());
+    if (mean) *mean = acc / n;
+    return DODE_OK;
+}
+
 static int copy_q(dode_ctx* ctx, int32_t day, float* out, const float* in, int32_t is_device) {
     const dode_dims& d = ctx->dm;
     if (day < 0 || day >= d.D) return fail(ctx, DODE_EINVAL, "day %d out of range [0,%d)", day, d.D);

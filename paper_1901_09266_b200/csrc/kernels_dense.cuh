@@ -275,6 +275,26 @@ __global__ void sumsq_final(const double* __restrict__ part, double* __restrict_
     out[d] = acc;
 }
 
+// Step 6 quality check: per-day sum and sum of squares of the observed counts x[day][T*L] in double
+// (for SS_tot of the coefficient of determination).  One block per listed day.
+__global__ void __launch_bounds__(kThreads)
+x_moments(const float* __restrict__ x, long TL, double* __restrict__ out, const __grid_constant__ DayList dl) {
+    __shared__ double s1[kThreads], s2[kThreads];
+    const float* xd = x + (size_t)dl.day[blockIdx.x] * TL;
+    double a = 0.0, b = 0.0;
+    for (long i = threadIdx.x; i < TL; i += kThreads) {
+        const double v = (double)xd[i];
+        a += v; b += v * v;
+    }
+    s1[threadIdx.x] = a; s2[threadIdx.x] = b;
+    __syncthreads();
+    for (int s = kThreads / 2; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s) { s1[threadIdx.x] += s1[threadIdx.x + s]; s2[threadIdx.x] += s2[threadIdx.x + s]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[2 * blockIdx.x] = s1[0]; out[2 * blockIdx.x + 1] = s2[0]; }
+}
+
 // ---- small helpers for a7 (power iteration) and state init ----
 __global__ void fill_f32(float* p, size_t n, float v) {
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;

@@ -242,3 +242,24 @@ def test_csr_apply_adjoint():
     np.testing.assert_allclose(rtv.cpu().numpy(), o.gradient(p.R[0].numpy(), v.numpy()), rtol=1e-4, atol=1e-4)
     assert abs(P.dode_lipschitz(g.h, 0, 40) - o.power_iteration(p.R[0].numpy(), 40)) <= 1e-4 * o.power_iteration(p.R[0].numpy(), 40)
     g.close()
+
+
+def test_r2_quality_check_matches_oracle():
+    """NEXT-3 / Step 6: per-day R2 through the library equals the oracle's O5 on the library's own q,
+    on the FFMA, tensor-core and CSR forward kernels."""
+    o = _oracle()
+    cfg = synth.Config("r2", N=37, L=53, T=30, H=5, C=2, D=24, b=12, K=6, kmin=3, kmax=9)
+    p = hz.make_problem(cfg)
+    sched = synth.schedule(cfg, p.labels)
+    etas = hz.oracle_etas(p)
+    for csr in (False, True):
+        g = hz.GpuSolver(p, csr=csr)
+        g.run(sched, etas)
+        days = list(range(cfg.D))
+        per, mean = g.P.dode_r2(g.h, days)
+        q = g.q()
+        want = np.array([o.r2_day(p.R[int(p.labels[d])].numpy(), q[d], p.x[d].numpy()) for d in days])
+        np.testing.assert_allclose(per, want, rtol=0, atol=1e-5)
+        assert abs(mean - want.mean()) < 1e-5
+        assert per.max() <= 1.0 + 1e-6
+        g.close()

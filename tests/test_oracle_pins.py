@@ -279,3 +279,32 @@ def test_p13_dense_vs_csr(tiny12):
     fs = oracle.objective_day_csr(cfg.N, cfg.L, cfg.T, cfg.H, csr.blk_off.numpy(), csr.row_ptr.numpy(),
                                   csr.col_idx.numpy(), csr.val.numpy(), qd, x[4])
     assert abs(fd - fs) <= 1e-12 * fd
+
+
+def test_p14_r2_closed_forms(tiny12):
+    """O5 (Step 6; reading A17): R2 = 1 - SS_res / SS_tot with the observed counts as reference.
+    Pinned by cases with a closed form: a perfect fit gives exactly 1; q = 0 gives 1 - sum x^2 / sum (x - mean)^2;
+    and the general case equals the textbook formula evaluated with the Table-2 assembled matrix."""
+    cfg, R, lab, qt, x, xclean = tiny12
+    o = oracle
+    Rc = R[0]
+    d = 3
+    # perfect fit on the noiseless counts (x0 is rho q_true rounded to fp32, hence the tolerance)
+    assert abs(o.r2_day(Rc, qt[d], xclean[d]) - 1.0) < 1e-9
+    # q = 0: the residual is -x
+    xd = x[d].astype(np.float64)
+    want0 = 1.0 - (xd ** 2).sum() / ((xd - xd.mean()) ** 2).sum()
+    assert abs(o.r2_day(Rc, np.zeros((cfg.T, cfg.N), np.float32), x[d]) - want0) < 1e-12
+    # general q: dense assembly (P12's matrix) + numpy
+    A = assemble_dense(Rc)
+    q = (np.random.default_rng(5).random((cfg.T, cfg.N)) * 30).astype(np.float32)
+    fit = A @ q.reshape(-1).astype(np.float64)
+    want = 1.0 - ((xd.reshape(-1) - fit) ** 2).sum() / ((xd - xd.mean()) ** 2).sum()
+    assert abs(o.r2_day(Rc, q, x[d]) - want) < 1e-10
+    # a better fit scores higher: a few SPGD visits raise R2 from the q0 = 1 start
+    eta = _eta(Rc)
+    q1 = np.ones((cfg.T, cfg.N), np.float32)
+    r2_a = o.r2_day(Rc, q1, x[d])
+    for _ in range(20):
+        q1 = o.visit(Rc, q1, x[d], eta)
+    assert o.r2_day(Rc, q1, x[d]) > r2_a
