@@ -27,7 +27,8 @@
 // Pins (tests/test_oracle_pins.py): P1 active-set NNLS on the T=12 instance,
 // P2 KKT, P3 finite differences, P4 planted recovery, P5 closed-form linear
 // iteration, P6 Example 1, P8 adjoint, P9 descent,
-// P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR, P14 R2 closed forms.
+// P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR, P14 R2 closed forms,
+// P15 row-chunk Adagrad against torch.optim.Adagrad on the assembled matrix.
 // No function here is "parity unpinned".
 #include <cmath>
 #include <cstddef>
@@ -136,6 +137,31 @@ double oracle_r2_day(int N, int L, int T, int H, const float* Rc, const float* q
     mean /= (double)TL;
     for (size_t i = 0; i < TL; ++i) ss_tot += ((double)x[i] - mean) * ((double)x[i] - mean);
     return 1.0 - ss_res / ss_tot;
+}
+
+// O6 (NEXT-1): one iteration of Alg. 1 as the paper states it on one day:
+//   line 8  B_o = rows `mask` of the day's system (a chunk of the permuted row range),
+//   line 9  g = B_o^T (B_o x - y_o)   == rho^T (mask .* (rho q - x)),
+//   line 10 x = Adagrad(x, g, eta)    -- accumulate G += g^2, step eta * g / (sqrt(G) + eps)  ([14]; the paper's
+//                                        implementation is PyTorch, whose Adagrad is exactly this with eps = 1e-10;
+//                                        reading A18),
+//   line 11 x = max(x, 0).
+// mask is [T][L] bytes (nullable = every row); G is the fp32 accumulator state [T][N], updated in place.
+void oracle_visit_adagrad(int N, int L, int T, int H, const float* Rc, float* q, float* G, const float* x,
+                          const uint8_t* mask, float eta, float eps) {
+    Dims d{N, L, T, H};
+    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<double> rd(TL), g(TN);
+    std::vector<float> rf(TL);
+    forward_d(d, Rc, q, x, rd.data());
+    for (size_t i = 0; i < TL; ++i) rf[i] = (mask && !mask[i]) ? 0.f : (float)rd[i];
+    gradient_f(d, Rc, rf.data(), g.data());
+    for (size_t i = 0; i < TN; ++i) {
+        const double Gd = (double)G[i] + g[i] * g[i];
+        G[i] = (float)Gd;
+        const double v = (double)q[i] - (double)eta * g[i] / (std::sqrt(Gd) + (double)eps);
+        q[i] = (float)(v > 0.0 ? v : 0.0);
+    }
 }
 
 // Replays a schedule: iteration k visits days sched_days[sched_ptr[k] .. sched_ptr[k+1])

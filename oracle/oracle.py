@@ -83,6 +83,23 @@ def objective_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray) -> float:
     return float(lib().oracle_objective_day(N, L, T, H, pR, pq, px))
 
 
+def visit_adagrad(Rc: np.ndarray, q: np.ndarray, G: np.ndarray, x: np.ndarray, mask, eta: float, eps: float = 1e-10):
+    """O6 (NEXT-1): one row-chunk Adagrad iteration of Alg. 1; returns (new q, new G).
+    mask: uint8 [T][L] (rows of the chunk) or None for every row."""
+    N, L, T, H = _dims(Rc)
+    Rc, pR = _f(Rc); x, px = _f(x)
+    q = np.array(q, dtype=np.float32, order="C", copy=True)
+    G = np.array(G, dtype=np.float32, order="C", copy=True)
+    pm = None
+    if mask is not None:
+        mask = np.ascontiguousarray(mask, dtype=np.uint8)
+        assert mask.shape == (T, L)
+        pm = mask.ctypes.data_as(C.c_void_p)
+    lib().oracle_visit_adagrad(N, L, T, H, pR, q.ctypes.data_as(C.c_void_p), G.ctypes.data_as(C.c_void_p), px, pm,
+                               C.c_float(eta), C.c_float(eps))
+    return q, G
+
+
 def r2_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray) -> float:
     """O5: coefficient of determination of the fitted counts of one day (Step 6; reading A17)."""
     N, L, T, H = _dims(Rc)

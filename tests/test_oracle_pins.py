@@ -308,3 +308,40 @@ def test_p14_r2_closed_forms(tiny12):
     for _ in range(20):
         q1 = o.visit(Rc, q1, x[d], eta)
     assert o.r2_day(Rc, q1, x[d]) > r2_a
+
+
+def test_p15_row_chunk_adagrad_against_torch(tiny12):
+    """O6 / NEXT-1 (Alg. 1 as printed): row-chunk minibatches + Adagrad + projection.  The paper's
+    implementation is PyTorch, so the pin is torch.optim.Adagrad itself on the Table-2 assembled matrix: the same
+    permuted row chunks, g = B_o^T(B_o x - y_o), optimizer step, clamp — in float64."""
+    import torch
+    cfg, R, lab, qt, x, _ = tiny12
+    Rc = R[0]
+    d = 2
+    A = torch.from_numpy(assemble_dense(Rc))                       # (T*L) x (T*N), float64
+    y = torch.from_numpy(x[d].astype(np.float64).reshape(-1))
+    rows = cfg.T * cfg.L
+    rng = np.random.default_rng(11)
+    eta, eps, bs = 0.5, 1e-10, 29                                  # 72 rows -> chunks of 29, 29, 14 (ragged tail)
+    p = torch.nn.Parameter(torch.ones(cfg.T * cfg.N, dtype=torch.float64))
+    opt = torch.optim.Adagrad([p], lr=eta, eps=eps, initial_accumulator_value=0.0, lr_decay=0.0)
+    q = np.ones((cfg.T, cfg.N), np.float32)
+    G = np.zeros((cfg.T, cfg.N), np.float32)
+    for epoch in range(6):
+        perm = rng.permutation(rows)
+        for c0 in range(0, rows, bs):
+            chunk = perm[c0:c0 + bs]
+            mask = np.zeros(rows, np.uint8); mask[chunk] = 1
+            Bo, yo = A[chunk], y[chunk]
+            with torch.no_grad():
+                p.grad = Bo.T @ (Bo @ p - yo)                      # Alg. 1 line 9: no factor 2 (reading A1)
+            opt.step()
+            with torch.no_grad():
+                p.clamp_(min=0.0)                                  # line 11
+            q, G = oracle.visit_adagrad(Rc, q, G, x[d], mask.reshape(cfg.T, cfg.L), eta, eps)
+    want = p.detach().numpy().reshape(cfg.T, cfg.N)
+    np.testing.assert_allclose(q, want, rtol=2e-4, atol=2e-4)
+    # mask = None is the full-batch step
+    qa, Ga = oracle.visit_adagrad(Rc, q, G, x[d], None, eta, eps)
+    qb, Gb = oracle.visit_adagrad(Rc, q, G, x[d], np.ones((cfg.T, cfg.L), np.uint8), eta, eps)
+    np.testing.assert_array_equal(qa, qb); np.testing.assert_array_equal(Ga, Gb)
