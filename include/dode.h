@@ -76,6 +76,20 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
  * Asynchronous on the ctx stream; no host synchronisation, no device->host traffic. */
 int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta);
 
+/* NEXT-1 — Alg. 1 as the paper prints it, on the listed days of one cluster:
+ *   line 8   B_o = the rows of each day's system selected by row_mask (a chunk of the permuted row range, 398-404)
+ *   line 9   g = B_o^T (B_o x - y_o)          == rho^T (mask .* (rho q - x))
+ *   line 10  x = Adagrad(x, g, eta)           G += g^2 ; q -= eta g / (sqrt(G) + eps)   ([14]; reading A18)
+ *   line 11  x = max(x, 0)
+ *   row_mask  device uint8 [n][T][L] indexed by the POSITION in `days` (entry t*L + l, Table 2 link-flow order),
+ *             non-zero = row belongs to the chunk; NULL = every row (full-batch Adagrad).  Read during the call's
+ *             kernels: keep it alive and unmodified until they have run (stream order is enough).
+ *   eta, eps  > 0, else DODE_EINVAL.
+ * The accumulator G ([D][T][N] fp32, zero at first use) lives in the ctx; dode_adagrad_reset zeroes it.
+ * Same validation, asynchrony and kernels as dode_spgd_step (the mask and the accumulator ride in the epilogues). */
+int dode_adagrad_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, float eps, const uint8_t* row_mask);
+int dode_adagrad_reset(dode_ctx* ctx);
+
 /* The same iteration for a streaming caller (bench.py's end-to-end leg): uploads the n days' counts from x_host
  * ([n][T][L], host; pinned memory makes the copies asynchronous), runs the step, and downloads the n days' updated q
  * into q_host ([n][T][N], host).  ASYNCHRONOUS and pipelined over consecutive calls on two internal copy streams:

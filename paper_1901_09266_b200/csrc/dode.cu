@@ -30,6 +30,7 @@ struct dode_ctx {
     CsrStore csr{};
     // state
     float* q = nullptr;          // [D][T][Np]
+    float* G = nullptr;          // [D][T][Np] Adagrad accumulator (NEXT-1), allocated by the first dode_adagrad_step
     float* x = nullptr;          // [D][T][L]
     float* r = nullptr;          // [T*Lp][bp] residual panel (FFMA / CSR paths)
     size_t r_cap = 0;            // floats
@@ -70,6 +71,13 @@ struct dode_ctx {
 };
 
 enum { KIND_FWD = 0, KIND_GRAD = 1, KIND_OTHER = 2 };
+
+// NEXT-1, Alg. 1 as printed: optional row-chunk mask on the residual and Adagrad in the update
+struct StepOpt {
+    const uint8_t* mask = nullptr;   // device [n][T][L] by position in the day list; null = every row
+    float* G = nullptr;              // Adagrad accumulator [D][T][Np]; null = plain projected step
+    float eps = 0.f;
+};
 
 struct KernelTimer {      // records an event pair around one launch when timing is on
     dode_ctx* c; cudaEvent_t a = nullptr, b = nullptr; int kind;
@@ -178,7 +186,7 @@ static BandArgs band_args(const dode_ctx* ctx, int c, bool forward, int bp) {
 
 // a2 on the FFMA / CSR paths: residual panel of one sub-batch (<= kMaxDays days of cluster c) into ctx->r
 // ([T*Lp][bp], day fastest); returns the day tile bt and the panel stride bp
-static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, int* bt_out, int* bp_out) {
+static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, int* bt_out, int* bp_out, const uint8_t* mask = nullptr) {
     const dode_dims& d = ctx->dm;
     const bool csr = d.storage == DODE_CSR;
     const int bt = csr ? 32 : pick_bt(dl.n);
@@ -197,12 +205,12 @@ static int forward_batch(dode_ctx* ctx, int c, const DayList& dl, int* bt_out, i
             panel = ctx->Qb;
         }
         BandArgs a = band_args(ctx, c, true, bp);
-        a.B = panel; a.x = ctx->x; a.out = ctx->r;
+        a.B = panel; a.x = ctx->x; a.out = ctx->r; a.mask = mask;
         if ((rc = launch_band_bt<EPI_RESID>(ctx, bt, a, dl, KIND_FWD))) return rc;
     } else {
         KernelTimer kt(ctx, KIND_FWD);
         rc = csr_forward(ctx->csr, c, ctx->q, dayStride, ctx->x, ctx->r, bp, bp, dl, d, ctx->Np, ctx->stream,
-                         &ctx->launches);
+                         &ctx->launches, mask);
         if (rc) return fail(ctx, rc, "CSR scratch allocation failed");
     }
     *bt_out = bt; *bp_out = bp;
@@ -316,7 +324,8 @@ static int tc_ensure(dode_ctx* ctx, int bn) {
         ctx->tc_bn = bn;
     }
     if (!ctx->tc_attr) {
-        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->tc_attr = true;
     }
     return DODE_OK;
@@ -338,7 +347,7 @@ static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 }
 
 // one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
-static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
+static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt) {
     const dode_dims& d = ctx->dm;
     const int bn = (dl.n + 15) / 16 * 16;
     int rc = tc_ensure(ctx, bn);
@@ -370,18 +379,20 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     p.slab0 = c * d.T;
     p.x = ctx->x; p.rp_full = ctx->rp_full; p.rp_lo = ctx->rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
+    p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
     { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
+    auto kern = (opt.mask || opt.G) ? tc::banded_gemm_3xtf32<true> : tc::banded_gemm_3xtf32<false>;
     {
         KernelTimer kt(ctx, KIND_FWD);
         p.mode = 0; p.M = d.L; p.kunit = ctx->Np;
-        CU(launch_pdl(tc::banded_gemm_3xtf32, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+        CU(launch_pdl(kern, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
                       ctx->stream, ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl));
         ctx->launches++;
     }
     {
         KernelTimer kt(ctx, KIND_GRAD);
         p.mode = 1; p.M = d.N; p.kunit = ctx->Lp;
-        CU(launch_pdl(tc::banded_gemm_3xtf32, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+        CU(launch_pdl(kern, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
                       ctx->stream, ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl));
         ctx->launches++;
     }
@@ -391,7 +402,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta) {
     return DODE_OK;
 }
 
-static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c) {
+static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c, const StepOpt& opt0 = StepOpt()) {
     const dode_dims& d = ctx->dm;
     const size_t dayStride = (size_t)d.T * ctx->Np;
     const int chunk = d.storage == DODE_CSR ? kCsrMaxDays : kMaxDays;
@@ -400,14 +411,16 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
         dl.n = std::min(chunk, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
         int bt, bp, rc;
+        StepOpt opt = opt0;
+        if (opt.mask) opt.mask += (size_t)off * d.T * d.L;
         if (ctx->tc_ready && dl.n >= ctx->tc_min_b) {
-            if ((rc = tc_step(ctx, c, dl, eta))) return rc;
+            if ((rc = tc_step(ctx, c, dl, eta, opt))) return rc;
             continue;
         }
-        if ((rc = forward_batch(ctx, c, dl, &bt, &bp))) return rc;
+        if ((rc = forward_batch(ctx, c, dl, &bt, &bp, opt.mask))) return rc;
         if (d.storage == DODE_DENSE) {
             BandArgs a = band_args(ctx, c, false, bp);
-            a.B = ctx->r; a.q = ctx->q; a.dayStride = dayStride; a.eta = eta;
+            a.B = ctx->r; a.q = ctx->q; a.dayStride = dayStride; a.eta = eta; a.G = opt.G; a.eps = opt.eps;
             if ((rc = launch_band_bt<EPI_UPDATE>(ctx, bt, a, dl, KIND_GRAD))) return rc;
             char buf[96];
             snprintf(buf, sizeof buf, "ffma_coldot_fwd_bt%d+ffma_coldot_grad_bt%d", bt, bt);
@@ -416,7 +429,7 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
             {
                 KernelTimer kt(ctx, KIND_GRAD);
                 rc = csr_gradient(ctx->csr, c, ctx->r, ctx->q, dayStride, nullptr, eta, bp, bp, dl, d, ctx->Np,
-                                  ctx->stream, &ctx->launches);
+                                  ctx->stream, &ctx->launches, opt.G, opt.eps);
             }
             if (rc) return fail(ctx, rc, "CSR scratch allocation failed");
             char buf[96];
@@ -443,7 +456,7 @@ void dode_destroy(dode_ctx* ctx) {
     for (int i = 0; i < 2; ++i) { if (ctx->ev_step[i]) cudaEventDestroy(ctx->ev_step[i]); if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]); }
     cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
     cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
-    cudaFree(ctx->Ag); cudaFree(ctx->Af); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r); cudaFree(ctx->Qb);
+    cudaFree(ctx->Ag); cudaFree(ctx->Af); cudaFree(ctx->G); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r); cudaFree(ctx->Qb);
     for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
     cudaFree(ctx->d_part); cudaFree(ctx->d_obj); cudaFree(ctx->pu); cudaFree(ctx->pv); cudaFree(ctx->pw);
@@ -534,6 +547,28 @@ int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta) {
     int c = 0, rc;
     if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
     return step_impl(ctx, days, n, eta, c);
+}
+
+int dode_adagrad_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, float eps, const uint8_t* row_mask) {
+    if (!ctx) return DODE_EINVAL;
+    int c = 0, rc;
+    if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
+    if (!(eps > 0.f) || !(eta > 0.f)) return fail(ctx, DODE_EINVAL, "eta and eps must be positive");
+    const dode_dims& d = ctx->dm;
+    if (!ctx->G) {
+        const size_t bytes = (size_t)d.D * d.T * ctx->Np * sizeof(float);
+        CU(cudaMalloc(&ctx->G, bytes));
+        CU(cudaMemsetAsync(ctx->G, 0, bytes, ctx->stream));
+    }
+    StepOpt opt;
+    opt.mask = row_mask; opt.G = ctx->G; opt.eps = eps;
+    return step_impl(ctx, days, n, eta, c, opt);
+}
+
+int dode_adagrad_reset(dode_ctx* ctx) {
+    if (!ctx) return DODE_EINVAL;
+    if (ctx->G) CU(cudaMemsetAsync(ctx->G, 0, (size_t)ctx->dm.D * ctx->dm.T * ctx->Np * sizeof(float), ctx->stream));
+    return DODE_OK;
 }
 
 // staging <-> state for the streaming step: x[day_i] <- stage[i] (scatter) / stage[i] <- q[day_i] without the pad columns

@@ -54,6 +54,10 @@ struct CsrStore {
     float* Qb = nullptr;          // [T*Np][bp]
     float* Xb = nullptr;          // [T*L][bp]
     int cap_bp = 0;
+    // NEXT-1 (row-chunk + Adagrad), allocated on first use
+    float* Mb = nullptr;          // [T*L][bp]  row mask as 0/1 floats
+    float* Gb = nullptr;          // [T*Np][bp] Adagrad accumulator panel
+    int cap_bp_ada = 0;
 };
 
 // ---- create-time re-pack ---------------------------------------------------------------------------
@@ -157,8 +161,8 @@ inline void csr_free(CsrStore& st) {
         delete[] st.cl;
         st.cl = nullptr;
     }
-    cudaFree(st.Qb); cudaFree(st.Xb);
-    st.Qb = st.Xb = nullptr;
+    cudaFree(st.Qb); cudaFree(st.Xb); cudaFree(st.Mb); cudaFree(st.Gb);
+    st.Qb = st.Xb = st.Mb = st.Gb = nullptr;
     st.ready = false;
 }
 
@@ -269,8 +273,10 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
 
 // ---- hot path ------------------------------------------------------------------------------------
 // dst[i*bp + d] = src[day_d*dayStride + i] for i < rowLen, d < bp (pad days -> 0).  32x32 smem transpose.
+// BYPOS: the source is indexed by the position in the day list (a caller's per-step buffer) instead of the day id.
+template <typename SrcT, bool BYPOS>
 __global__ void __launch_bounds__(256)
-gather_days(const float* __restrict__ src, size_t dayStride, long rowLen, float* __restrict__ dst, int bp,
+gather_days(const SrcT* __restrict__ src, size_t dayStride, long rowLen, float* __restrict__ dst, int bp,
             const __grid_constant__ DayList dl) {
     __shared__ float tile[32][33];
     const long i0 = (long)blockIdx.x * 32;
@@ -279,7 +285,7 @@ gather_days(const float* __restrict__ src, size_t dayStride, long rowLen, float*
     for (int dd = ty; dd < 32; dd += 8) {
         const int d = d0 + dd;
         const long i = i0 + tx;
-        tile[dd][tx] = (d < dl.n && i < rowLen) ? __ldg(src + (size_t)dl.day[d] * dayStride + i) : 0.f;
+        tile[dd][tx] = (d < dl.n && i < rowLen) ? (float)__ldg(src + (size_t)(BYPOS ? d : dl.day[d]) * dayStride + i) : 0.f;
     }
     __syncthreads();
     for (int ii = ty; ii < 32; ii += 8) {
@@ -318,7 +324,7 @@ template <> struct DVec<4> { using type = float4; };
 template <int DV>
 __global__ void __launch_bounds__(256, 4)
 csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, const float4* __restrict__ val,
-        const float* __restrict__ Qb, const float* __restrict__ Xb, float* __restrict__ r,
+        const float* __restrict__ Qb, const float* __restrict__ Xb, const float* __restrict__ Mb, float* __restrict__ r,
         long rblocks, int L, int LB, int Np, int rbp) {
     constexpr int bp = 32 * DV;
     using vec = typename DVec<DV>::type;
@@ -386,6 +392,12 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, con
 #pragma unroll
             for (int e = 0; e < DV; ++e) acc[i][e] -= xf[e];
         }
+        if (Mb != nullptr) {                      // rows outside the chunk B_o contribute no residual
+            const vec mv = *reinterpret_cast<const vec*>(Mb + row * bp + lane * DV);
+            const float* mf = reinterpret_cast<const float*>(&mv);
+#pragma unroll
+            for (int e = 0; e < DV; ++e) acc[i][e] = mf[e] != 0.f ? acc[i][e] : 0.f;
+        }
         if (rbp == bp) {
             vec out;
             float* of = reinterpret_cast<float*>(&out);
@@ -406,7 +418,7 @@ template <int DV, bool UPDATE>
 __global__ void __launch_bounds__(256, 4)
 csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, const float4* __restrict__ val,
          const int32_t* __restrict__ perm, const float* __restrict__ r, float* __restrict__ Qb, float* __restrict__ gout, float eta,
-         long rblocks, int T, int L, int N, int Np, int rbp) {
+         float* __restrict__ Gb, float eps, long rblocks, int T, int L, int N, int Np, int rbp) {
     constexpr int bp = 32 * DV;
     using vec = typename DVec<DV>::type;
     // Warps walk the row blocks OD-major in path order (perm: ODs sorted by the first link of their path), time-minor:
@@ -476,7 +488,10 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
             vec qv = *qp;
             float* qf = reinterpret_cast<float*>(&qv);
 #pragma unroll
-            for (int e = 0; e < DV; ++e) qf[e] = fmaxf(0.f, fmaf(-eta, acc[i][e], qf[e]));
+            for (int e = 0; e < DV; ++e) {
+                if (Gb != nullptr) qf[e] = adagrad_update(qf[e], acc[i][e], Gb + ((size_t)s * Np + n) * bp + lane * DV + e, eta, eps);
+                else qf[e] = fmaxf(0.f, fmaf(-eta, acc[i][e], qf[e]));
+            }
             *qp = qv;
         } else if (lane == 0) {
             gout[(size_t)s * N + n] = acc[i][0];
@@ -498,24 +513,42 @@ inline int csr_ensure(CsrStore& st, const dode_dims& d, int Np, int bp, cudaStre
 }
 
 // gathers + forward.  rbp: stride of r (== bp for steps/objective, 1 for dode_apply).
+inline int csr_ensure_ada(CsrStore& st, const dode_dims& d, int Np, int bp, cudaStream_t stream) {
+    if (st.cap_bp_ada >= bp) return DODE_OK;
+    cudaStreamSynchronize(stream);
+    cudaFree(st.Mb); cudaFree(st.Gb);
+    st.Mb = st.Gb = nullptr; st.cap_bp_ada = 0;
+    if (cudaMalloc(&st.Mb, (size_t)d.T * d.L * bp * 4) != cudaSuccess) return DODE_ENOMEM;
+    if (cudaMalloc(&st.Gb, (size_t)d.T * Np * bp * 4) != cudaSuccess) return DODE_ENOMEM;
+    st.cap_bp_ada = bp;
+    return DODE_OK;
+}
+
+// mask (nullable): device bytes [n][T][L] by position in the day list
 inline int csr_forward(CsrStore& st, int c, const float* qbase, size_t dayStride, const float* xbase, float* r,
                        int bp, int rbp, const DayList& dl, const dode_dims& d, int Np, cudaStream_t stream,
-                       int64_t* launches) {
+                       int64_t* launches, const uint8_t* mask = nullptr) {
     int rc = csr_ensure(st, d, Np, bp, stream);
     if (rc) return rc;
+    if (mask && (rc = csr_ensure_ada(st, d, Np, bp, stream))) return rc;
     const CsrCluster& cl = st.cl[c];
     const long qlen = (long)d.T * Np, xlen = (long)d.T * d.L;
-    gather_days<<<dim3((unsigned)((qlen + 31) / 32), bp / 32), 256, 0, stream>>>(qbase, dayStride, qlen, st.Qb, bp, dl);
+    gather_days<float, false><<<dim3((unsigned)((qlen + 31) / 32), bp / 32), 256, 0, stream>>>(qbase, dayStride, qlen, st.Qb, bp, dl);
     if (xbase)
-        gather_days<<<dim3((unsigned)((xlen + 31) / 32), bp / 32), 256, 0, stream>>>(xbase, (size_t)d.T * d.L, xlen, st.Xb, bp, dl);
+        gather_days<float, false><<<dim3((unsigned)((xlen + 31) / 32), bp / 32), 256, 0, stream>>>(xbase, (size_t)d.T * d.L, xlen, st.Xb, bp, dl);
+    if (mask) {
+        gather_days<uint8_t, true><<<dim3((unsigned)((xlen + 31) / 32), bp / 32), 256, 0, stream>>>(mask, (size_t)d.T * d.L, xlen, st.Mb, bp, dl);
+        *launches += 1;
+    }
+    const float* Mb = mask ? st.Mb : nullptr;
     const int LB = (d.L + kRB - 1) / kRB;
     const long rblocks = (long)d.T * LB;
     const unsigned grid = (unsigned)((rblocks * 32 + 255) / 256);
     const float* Xb = xbase ? st.Xb : nullptr;
     switch (bp) {
-        case 32: csr_fwd<1><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, r, rblocks, d.L, LB, Np, rbp); break;
-        case 64: csr_fwd<2><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, r, rblocks, d.L, LB, Np, rbp); break;
-        default: csr_fwd<4><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, r, rblocks, d.L, LB, Np, rbp); break;
+        case 32: csr_fwd<1><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, Mb, r, rblocks, d.L, LB, Np, rbp); break;
+        case 64: csr_fwd<2><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, Mb, r, rblocks, d.L, LB, Np, rbp); break;
+        default: csr_fwd<4><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, Mb, r, rblocks, d.L, LB, Np, rbp); break;
     }
     *launches += xbase ? 3 : 2;
     return DODE_OK;
@@ -524,24 +557,35 @@ inline int csr_forward(CsrStore& st, int c, const float* qbase, size_t dayStride
 // gradient + update on Qb + scatter back to q (UPDATE), or g -> gout for minibatch 1 (dode_apply_t, rbp = 1)
 inline int csr_gradient(CsrStore& st, int c, const float* r, float* qbase, size_t dayStride, float* gout, float eta,
                         int bp, int rbp, const DayList& dl, const dode_dims& d, int Np, cudaStream_t stream,
-                        int64_t* launches) {
+                        int64_t* launches, float* Gbase = nullptr, float eps = 0.f) {
     int rc = csr_ensure(st, d, Np, bp, stream);
     if (rc) return rc;
+    if (Gbase && (rc = csr_ensure_ada(st, d, Np, bp, stream))) return rc;
     const CsrCluster& cl = st.cl[c];
     const long rows = (long)d.T * Np;
     const long rblocks = (long)((d.T + kRB - 1) / kRB) * Np;
     const unsigned grid = (unsigned)((rblocks * 32 + 255) / 256);
     if (gout) {
-        csr_grad<1, false><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, nullptr, gout, eta, rblocks, d.T, d.L, d.N, Np, rbp);
+        csr_grad<1, false><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, nullptr, gout, eta, nullptr, 0.f, rblocks, d.T, d.L, d.N, Np, rbp);
         *launches += 1;
         return DODE_OK;
     }
+    float* Gb = nullptr;
+    if (Gbase) {                      // Adagrad accumulator of the minibatch days as a day-fastest panel, like Qb
+        gather_days<float, false><<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(Gbase, dayStride, rows, st.Gb, bp, dl);
+        Gb = st.Gb;
+        *launches += 1;
+    }
     switch (bp) {
-        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
     }
     scatter_days<<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(st.Qb, bp, rows, qbase, dayStride, dl);
+    if (Gbase) {
+        scatter_days<<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(st.Gb, bp, rows, Gbase, dayStride, dl);
+        *launches += 1;
+    }
     *launches += 2;
     return DODE_OK;
 }

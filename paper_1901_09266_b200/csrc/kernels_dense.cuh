@@ -36,6 +36,14 @@ __device__ __forceinline__ float4 ldg_stream(const float4* p) {     // R: read o
     return v;
 }
 
+// Alg. 1 lines 10-11: x = Adagrad(x, g, eta); x = max(x, 0).  Adagrad [14] as the paper's PyTorch
+// implementation has it: G += g^2, x -= eta g / (sqrt(G) + eps)  (reading A18).
+__device__ __forceinline__ float adagrad_update(float q, float g, float* Gp, float eta, float eps) {
+    const float Gn = fmaf(g, g, __ldcg(Gp));      // through L2: under PDL the previous step may have written it (kernels_tc.cuh)
+    *Gp = Gn;
+    return fmaxf(0.f, q - eta * g / (sqrtf(Gn) + eps));
+}
+
 template <int BT> struct RVec;
 template <> struct RVec<1> { using type = float; };
 template <> struct RVec<2> { using type = float2; };
@@ -58,6 +66,10 @@ struct BandArgs {
     float* q;            // EPI_UPDATE: state, in place
     size_t dayStride;
     float eta;
+    // NEXT-1, Alg. 1 as printed: row-chunk minibatch and Adagrad
+    const uint8_t* mask; // EPI_RESID: [n][T][M] bytes by position in the day list, 0 = row not in the chunk B_o (r = 0); nullable
+    float* G;            // EPI_UPDATE: Adagrad accumulator [D][T][Mp], nullable = plain projected step
+    float eps;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -153,14 +165,17 @@ band_coldot(const __grid_constant__ BandArgs a, int cwlog2, const __grid_constan
             // pad days (d0+j >= n) repeat the last day; pad rows (m >= M) are written as 0
             float v = 0.f;
             if (m < a.M) {
-                const int day = dl.day[min(d0 + j, dl.n - 1)];
-                v = g - __ldg(a.x + ((size_t)day * a.T + tt) * a.M + m);
+                const int pos = min(d0 + j, dl.n - 1);
+                v = g - __ldg(a.x + ((size_t)dl.day[pos] * a.T + tt) * a.M + m);
+                if (a.mask != nullptr && a.mask[((size_t)pos * a.T + tt) * a.M + m] == 0) v = 0.f;   // row outside B_o
             }
             a.out[((size_t)tt * Mp + m) * bp + d0 + j] = v;
         } else if (EPI == EPI_UPDATE) {
             if (m < a.M && d0 + j < dl.n) {
-                float* qp = a.q + (size_t)dl.day[d0 + j] * a.dayStride + (size_t)tt * Mp + m;
-                *qp = fmaxf(0.f, fmaf(-a.eta, g, *qp));
+                const size_t qi = (size_t)dl.day[d0 + j] * a.dayStride + (size_t)tt * Mp + m;
+                float* qp = a.q + qi;
+                if (a.G != nullptr) *qp = adagrad_update(*qp, g, a.G + qi, a.eta, a.eps);
+                else *qp = fmaxf(0.f, fmaf(-a.eta, g, *qp));
             }
         } else {
             if (m < a.opitch && j == 0) a.out[(size_t)tt * a.opitch + m] = g;

@@ -126,6 +126,10 @@ struct TcParams {
     float* q;            // [D][T][Np]       (gradient, in place)
     size_t dayStride;
     float eta;
+    // NEXT-1 (Alg. 1 as printed); both nullable
+    const uint8_t* mask; // forward: [n][T][L] bytes by position in the day list, 0 = row outside the chunk B_o (r = 0)
+    float* G;            // gradient: Adagrad accumulator [D][T][Np], in place
+    float eps;
     int dbg;             // bring-up switches: 1 = no split, 2 = no MMA, 4 = no epilogue (results invalid)
 };
 
@@ -161,7 +165,10 @@ __device__ long long g_trace[4 * kTraceNk * 4];
 #define TC_TRACE(role, kc, slot) do {} while (0)
 #endif
 
-__global__ void __launch_bounds__(kThreadsTC)
+// ADA = true compiles in the NEXT-1 epilogues (row mask on r, Adagrad accumulator).  It is a template parameter, not a
+// run-time branch, because the extra live values cost 25 registers: 117 x 320 threads no longer fits two CTAs per SM.
+template <bool ADA>
+__global__ void __launch_bounds__(kThreadsTC, 2)
 banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA64,
                    const __grid_constant__ CUtensorMap mapBf, const __grid_constant__ CUtensorMap mapBl,
                    const __grid_constant__ TcParams p, const __grid_constant__ DayList dl) {
@@ -237,8 +244,18 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                                      : __ldcg(p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + em);
         }
     };
+    uint32_t keep = 0xffffu;                                          // bit j: row (em, day c0+j) belongs to the chunk B_o
+    auto prefetch_mask = [&](int c0) {
+        keep = 0;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int d = c0 + j;
+            if (em < p.M && d < dl.n && __ldg(p.mask + ((size_t)d * p.T + tt) * p.M + em) != 0) keep |= 1u << j;
+        }
+    };
     if (p.mode == 0 && warp >= 2) prefetch(16 * egroup);             // x is a static input
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (ADA && p.mode == 0 && p.mask != nullptr && warp >= 2) prefetch_mask(16 * egroup);   // the caller's buffer: after the wait
     // q was written by the previous step's kernel, which may still have been running on this SM when this CTA was
     // launched (PDL): the launch-time L1 invalidation does not cover it, so q is read through L2 (ld.global.cg)
     if (p.mode == 1 && warp >= 2) prefetch(16 * egroup);
@@ -348,7 +365,11 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             float cur[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j) cur[j] = pre[j];
-            if (c0 + 32 < p.bn) prefetch(c0 + 32);
+            const uint32_t curkeep = keep;
+            if (c0 + 32 < p.bn) {
+                prefetch(c0 + 32);
+                if (ADA && p.mode == 0 && p.mask != nullptr) prefetch_mask(c0 + 32);
+            }
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             if (m < p.M) {
 #pragma unroll
@@ -357,12 +378,14 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                     if (d < dl.n) {
                         const float acc = __uint_as_float(v[j]) + (fused_n ? __uint_as_float(w[j]) : 0.f);
                         if (p.mode == 0) {
-                            const float r = acc - cur[j];
+                            const float r = (!ADA || ((curkeep >> j) & 1u)) ? acc - cur[j] : 0.f;
                             const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
                             p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
                             p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - rhi;
                         } else {
-                            p.q[(size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m] = fmaxf(0.f, fmaf(-p.eta, acc, cur[j]));
+                            const size_t qi = (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
+                            if (ADA && p.G != nullptr) p.q[qi] = adagrad_update(cur[j], acc, p.G + qi, p.eta, p.eps);
+                            else p.q[qi] = fmaxf(0.f, fmaf(-p.eta, acc, cur[j]));
                         }
                     }
                 }
