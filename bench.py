@@ -264,6 +264,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
         a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         run_epoch(ep)
+        P.dode_join(h)                                   # the end event must follow the steps on the library's lanes
         z.record()
         ev.append((a, z))
     torch.cuda.synchronize()

@@ -15,7 +15,7 @@
  * nothing is written to stdout/stderr; no global state; no CPU fallback — every call fails with
  * DODE_ECUDA if no usable sm_100 device/context exists.  "device" pointers are CUDA device
  * pointers valid in the current context (e.g. torch-allocated); "host" pointers are ordinary
- * host memory.  All work is issued on the stream given to dode_create.  A sticky CUDA error is
+ * host memory.  All work is issued on the stream given to dode_create or ordered with it as dode_spgd_step states.  A sticky CUDA error is
  * reported by the next synchronising call.
  */
 #ifndef DODE_H_
@@ -73,8 +73,16 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
 /* a1-a4: one SPGD iteration on the listed days (Alg. 1 lines 8-11):
  *   r = rho_c Q_B - X_B ;  g = rho_c^T r ;  q_d <- max(0, q_d - eta g_d)  for d in days.
  *   days  host int32 [n]; all in [0, D), distinct, same cluster — else DODE_EINVAL, state untouched.
- * Asynchronous on the ctx stream; no host synchronisation, no device->host traffic. */
+ * Asynchronous; no host synchronisation, no device->host traffic.
+ * Ordering: a step starts after everything that was on the ctx stream when it was called and after every earlier
+ * step that shares a day with it.  Steps on disjoint days (the chunks of one epoch) may overlap
+ * each other: the library alternates them on two internal streams.  Every other library call is ordered after all
+ * earlier steps by itself; work that the CALLER puts on the ctx stream (an event record, a kernel) is ordered after
+ * them only once dode_join has been called. */
 int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta);
+
+/* Makes the ctx stream wait for every step issued so far (asynchronous, no host wait). */
+int dode_join(dode_ctx* ctx);
 
 /* NEXT-1 — Alg. 1 as the paper prints it, on the listed days of one cluster:
  *   line 8   B_o = the rows of each day's system selected by row_mask (a chunk of the permuted row range, 398-404)

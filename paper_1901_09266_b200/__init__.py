@@ -19,7 +19,7 @@ SO_PATH = os.path.join(_HERE, "libdode.so")
 DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
 DODE_DENSE, DODE_CSR = 0, 1
 
-EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
+EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
            "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
@@ -56,6 +56,7 @@ def lib():
         L.dode_spgd_step_host.argtypes = [vp, vp, i32, f32, vp, vp]
         L.dode_adagrad_step.argtypes = [vp, vp, i32, f32, f32, vp]
         L.dode_adagrad_reset.argtypes = [vp]
+        L.dode_join.argtypes = [vp]
         L.dode_objective.argtypes = [vp, vp, i32, vp, vp]
         L.dode_get_q.argtypes = [vp, i32, vp, i32]
         L.dode_set_q.argtypes = [vp, i32, vp, i32]
@@ -135,6 +136,11 @@ def dode_spgd_step(h, days, eta: float) -> None:
     """a1-a4: one SPGD iteration on ``days`` (host ints, distinct, one cluster).  Asynchronous."""
     d = _days(days)
     _chk(h, lib().dode_spgd_step(h, d.ctypes.data, d.size, C.c_float(eta)))
+
+
+def dode_join(h) -> None:
+    """Makes the ctx stream wait for every step issued so far (asynchronous)."""
+    _chk(h, lib().dode_join(h))
 
 
 def dode_adagrad_step(h, days, eta: float, eps: float = 1e-10, row_mask=None) -> None:

@@ -19,6 +19,27 @@
 
 using namespace dode;
 
+// Minibatch panels and their tensor maps for the tensor-core path, one set per issue stream
+struct TcBuf {
+    float *Qg_full = nullptr, *Qg_lo = nullptr;   // [cap][T*Np]
+    float *rp_full = nullptr, *rp_lo = nullptr;   // [cap][T*Lp]
+    int cap = 0, bn = 0;
+    CUtensorMap mapQ_f, mapQ_l, mapR_f, mapR_l;
+};
+
+// Two internal streams that plain dode_spgd_step calls alternate on (tensor-core path): consecutive iterations touch
+// disjoint days (chunks of a permutation) and read-only operators, so iteration i+1 may start while
+// iteration i drains.  A kernel of one lane then fills the SM slots the other lane's kernel leaves at its prologue,
+// dependency wait and tail — the short kernels of small networks (corridor: 288 CTAs = one wave) are otherwise
+// serialised by the grid-wide dependency between forward and gradient.
+struct Lane {
+    cudaStream_t st = nullptr;
+    cudaEvent_t done = nullptr, entry = nullptr;
+    TcBuf buf;
+    int64_t last_id = 0;          // id of the latest step issued on this lane
+    int64_t seen_other = 0;       // latest step id of the OTHER lane that this lane has already waited for
+};
+
 struct dode_ctx {
     dode_dims dm{};
     int Np = 0, Lp = 0;          // padded N / L (dense: 128-byte rows when that costs <= 3 %, else 32- or 16-byte)
@@ -48,18 +69,25 @@ struct dode_ctx {
     char err[512] = {0};
     bool sm_opt_in[16] = {false};
     // tensor-core path (kernels_tc.cuh)
-    float *Qg_full = nullptr, *Qg_lo = nullptr;   // [tc_cap][T*Np]
-    float *rp_full = nullptr, *rp_lo = nullptr;   // [tc_cap][T*Lp]
+    TcBuf tcb;                                     // panels of the ctx stream
+    Lane lane[2];
+    bool lanes_on = true, lanes_dirty = false;     // dirty: lane work not yet joined into the ctx stream
+    int lane_next = 0;
+    int64_t lane_step_id = 0;
+    std::vector<int64_t> day_last_id;              // [D] id of the last lane step that touched the day
+    std::vector<int8_t> day_last_lane;             // [D] and its lane (-1: none)
     long rpitch = 0;
-    int tc_cap = 0, tc_bn = 0, tc_min_b = 8;
+    int tc_min_b = 8;
     bool tc_ready = false, tc_attr = false;
-    CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64, mapQ_f, mapQ_l, mapR_f, mapR_l;
+    CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64;
     // streaming steps (dode_spgd_step_host): copy streams, staging buffers, ping-pong events
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_h2d = nullptr, ev_step[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
     float *stage_x = nullptr, *stage_q = nullptr;
     size_t stage_x_cap = 0, stage_q_cap = 0;
     int64_t host_calls = 0;
+    cudaEvent_t ev_fence = nullptr;
+    bool plain_since_host = true;   // non-streaming work was issued on the ctx stream since the last streaming step
     std::vector<int32_t> prev_days;
     // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
     bool timing = false;
@@ -222,6 +250,9 @@ static cudaError_t sync_all(dode_ctx* ctx) {
     cudaError_t e = cudaStreamSynchronize(ctx->stream);
     if (ctx->s_h2d) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_h2d); if (e == cudaSuccess) e = e2; }
     if (ctx->s_d2h) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_d2h); if (e == cudaSuccess) e = e2; }
+    for (Lane& ln : ctx->lane)
+        if (ln.st) { cudaError_t e2 = cudaStreamSynchronize(ln.st); if (e == cudaSuccess) e = e2; }
+    ctx->lanes_dirty = false;
     return e;
 }
 
@@ -261,14 +292,15 @@ static PFN_encodeTiled get_encode() {
 
 // fp32 tensor, innermost dim first; out-of-bounds elements read as zero
 static int make_map(dode_ctx* ctx, CUtensorMap* m, const void* base, int rank, const uint64_t* dims,
-                    const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128) {
+                    const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128, bool atom32 = false) {
     PFN_encodeTiled enc = get_encode();
     if (!enc) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled is unavailable");
     cuuint64_t gd[3]; cuuint64_t gs[2]; cuuint32_t bx[3]; cuuint32_t es[3] = {1, 1, 1};
     for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; }
     for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_bytes[i];
     CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     atom32 ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
     return DODE_OK;
@@ -294,34 +326,34 @@ static int tc_setup(dode_ctx* ctx) {
     return DODE_OK;
 }
 
-static int tc_ensure(dode_ctx* ctx, int bn) {
+static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn) {
     const dode_dims& d = ctx->dm;
     const size_t qlen = (size_t)d.T * ctx->Np;
-    if (ctx->tc_cap < bn) {
-        CU(cudaStreamSynchronize(ctx->stream));
-        cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
-        ctx->Qg_full = ctx->Qg_lo = ctx->rp_full = ctx->rp_lo = nullptr;
-        ctx->tc_cap = 0; ctx->tc_bn = 0;
-        CU(cudaMalloc(&ctx->Qg_full, bn * qlen * 4)); CU(cudaMalloc(&ctx->Qg_lo, bn * qlen * 4));
-        CU(cudaMalloc(&ctx->rp_full, (size_t)bn * ctx->rpitch * 4)); CU(cudaMalloc(&ctx->rp_lo, (size_t)bn * ctx->rpitch * 4));
-        CU(cudaMemsetAsync(ctx->Qg_full, 0, bn * qlen * 4, ctx->stream)); CU(cudaMemsetAsync(ctx->Qg_lo, 0, bn * qlen * 4, ctx->stream));
-        CU(cudaMemsetAsync(ctx->rp_full, 0, (size_t)bn * ctx->rpitch * 4, ctx->stream));
-        CU(cudaMemsetAsync(ctx->rp_lo, 0, (size_t)bn * ctx->rpitch * 4, ctx->stream));
-        ctx->tc_cap = bn;
+    if (tb.cap < bn) {
+        CU(cudaStreamSynchronize(st));
+        cudaFree(tb.Qg_full); cudaFree(tb.Qg_lo); cudaFree(tb.rp_full); cudaFree(tb.rp_lo);
+        tb.Qg_full = tb.Qg_lo = tb.rp_full = tb.rp_lo = nullptr;
+        tb.cap = 0; tb.bn = 0;
+        CU(cudaMalloc(&tb.Qg_full, bn * qlen * 4)); CU(cudaMalloc(&tb.Qg_lo, bn * qlen * 4));
+        CU(cudaMalloc(&tb.rp_full, (size_t)bn * ctx->rpitch * 4)); CU(cudaMalloc(&tb.rp_lo, (size_t)bn * ctx->rpitch * 4));
+        CU(cudaMemsetAsync(tb.Qg_full, 0, bn * qlen * 4, st)); CU(cudaMemsetAsync(tb.Qg_lo, 0, bn * qlen * 4, st));
+        CU(cudaMemsetAsync(tb.rp_full, 0, (size_t)bn * ctx->rpitch * 4, st));
+        CU(cudaMemsetAsync(tb.rp_lo, 0, (size_t)bn * ctx->rpitch * 4, st));
+        tb.cap = bn;
     }
-    if (ctx->tc_bn != bn) {
+    if (tb.bn != bn) {
         // B operands: K-major windows of the per-day vectors, SWIZZLE_128B tiles of {32 floats, bn days}
-        const uint64_t qd[2] = {(uint64_t)qlen, (uint64_t)ctx->tc_cap};
+        const uint64_t qd[2] = {(uint64_t)qlen, (uint64_t)tb.cap};
         const uint64_t qs[1] = {(uint64_t)qlen * 4};
         const uint32_t bb[2] = {(uint32_t)tc::kTileK, (uint32_t)bn};
         int rc;
-        if ((rc = make_map(ctx, &ctx->mapQ_f, ctx->Qg_full, 2, qd, qs, bb, true))) return rc;
-        if ((rc = make_map(ctx, &ctx->mapQ_l, ctx->Qg_lo, 2, qd, qs, bb, true))) return rc;
-        const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)ctx->tc_cap};
+        if ((rc = make_map(ctx, &tb.mapQ_f, tb.Qg_full, 2, qd, qs, bb, true))) return rc;
+        if ((rc = make_map(ctx, &tb.mapQ_l, tb.Qg_lo, 2, qd, qs, bb, true))) return rc;
+        const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)tb.cap};
         const uint64_t rs[1] = {(uint64_t)ctx->rpitch * 4};
-        if ((rc = make_map(ctx, &ctx->mapR_f, ctx->rp_full, 2, rd, rs, bb, true))) return rc;
-        if ((rc = make_map(ctx, &ctx->mapR_l, ctx->rp_lo, 2, rd, rs, bb, true))) return rc;
-        ctx->tc_bn = bn;
+        if ((rc = make_map(ctx, &tb.mapR_f, tb.rp_full, 2, rd, rs, bb, true))) return rc;
+        if ((rc = make_map(ctx, &tb.mapR_l, tb.rp_lo, 2, rd, rs, bb, true))) return rc;
+        tb.bn = bn;
     }
     if (!ctx->tc_attr) {
         CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
@@ -347,10 +379,10 @@ static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 }
 
 // one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
-static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt) {
+static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt, TcBuf& tb, cudaStream_t st) {
     const dode_dims& d = ctx->dm;
     const int bn = (dl.n + 15) / 16 * 16;
-    int rc = tc_ensure(ctx, bn);
+    int rc = tc_ensure(ctx, tb, st, bn);
     if (rc) return rc;
     const size_t dayStride = (size_t)d.T * ctx->Np;
     // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  Two CTAs per SM when 3 stages fit in half the
@@ -371,13 +403,13 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     {
         KernelTimer kt(ctx, KIND_OTHER);
         CU(launch_pdl(tc::gather_split, dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), dim3(256), 0,
-                      ctx->stream, ctx->q, dayStride, (long)dayStride / 4, ctx->Qg_full, ctx->Qg_lo, dl));
+                      st, ctx->q, dayStride, (long)dayStride / 4, tb.Qg_full, tb.Qg_lo, dl));
         ctx->launches++;
     }
     tc::TcParams p{};
     p.T = d.T; p.H = d.H; p.Lp = ctx->Lp; p.Np = ctx->Np; p.bn = bn; p.stages = stages; p.nring = nring;
     p.slab0 = c * d.T;
-    p.x = ctx->x; p.rp_full = ctx->rp_full; p.rp_lo = ctx->rp_lo; p.rpitch = ctx->rpitch;
+    p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = tb.rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
     { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
@@ -386,14 +418,14 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
         KernelTimer kt(ctx, KIND_FWD);
         p.mode = 0; p.M = d.L; p.kunit = ctx->Np;
         CU(launch_pdl(kern, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
-                      ctx->stream, ctx->mapA_fwd, ctx->mapA_fwd64, ctx->mapQ_f, ctx->mapQ_l, p, dl));
+                      st, ctx->mapA_fwd, ctx->mapA_fwd64, tb.mapQ_f, tb.mapQ_l, p, dl));
         ctx->launches++;
     }
     {
         KernelTimer kt(ctx, KIND_GRAD);
         p.mode = 1; p.M = d.N; p.kunit = ctx->Lp;
         CU(launch_pdl(kern, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
-                      ctx->stream, ctx->mapA_grad, ctx->mapA_grad64, ctx->mapR_f, ctx->mapR_l, p, dl));
+                      st, ctx->mapA_grad, ctx->mapA_grad64, tb.mapR_f, tb.mapR_l, p, dl));
         ctx->launches++;
     }
     char buf[96];
@@ -402,7 +434,53 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     return DODE_OK;
 }
 
-static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c, const StepOpt& opt0 = StepOpt()) {
+// ---- lanes ------------------------------------------------------------------------------------------
+// makes the ctx stream wait for everything issued on the lanes so far (asynchronous; no host wait)
+static int join_lanes(dode_ctx* ctx) {
+    if (!ctx->lanes_dirty) return DODE_OK;
+    for (Lane& ln : ctx->lane)
+        if (ln.st && ln.last_id) CU(cudaStreamWaitEvent(ctx->stream, ln.done, 0));
+    ctx->lanes_dirty = false;
+    return DODE_OK;
+}
+
+// picks the lane of the next step, forks it from the ctx stream and orders it after earlier steps on its days
+static int lane_begin(dode_ctx* ctx, const DayList& dl, Lane** out) {
+    const int li = ctx->lane_next;
+    ctx->lane_next ^= 1;
+    Lane& ln = ctx->lane[li];
+    Lane& ot = ctx->lane[li ^ 1];
+    if (!ln.st) {
+        CU(cudaStreamCreateWithFlags(&ln.st, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ln.done, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&ln.entry, cudaEventDisableTiming));
+    }
+    // fork: whatever is on the ctx stream now (the caller's work, earlier non-lane calls) precedes this step
+    CU(cudaEventRecord(ln.entry, ctx->stream));
+    CU(cudaStreamWaitEvent(ln.st, ln.entry, 0));
+    // a day last stepped on the other lane by a step this lane has not waited for yet (steps of this lane: stream order)
+    bool conflict = false;
+    for (int i = 0; i < dl.n; ++i)
+        conflict |= ctx->day_last_lane[dl.day[i]] == (li ^ 1) && ctx->day_last_id[dl.day[i]] > ln.seen_other;
+    if (conflict) {
+        CU(cudaStreamWaitEvent(ln.st, ot.done, 0));
+        ln.seen_other = ot.last_id;
+    }
+    const int64_t id = ++ctx->lane_step_id;
+    for (int i = 0; i < dl.n; ++i) { ctx->day_last_lane[dl.day[i]] = (int8_t)li; ctx->day_last_id[dl.day[i]] = id; }
+    ln.last_id = id;
+    *out = &ln;
+    return DODE_OK;
+}
+
+static int lane_end(dode_ctx* ctx, Lane* ln) {
+    CU(cudaEventRecord(ln->done, ln->st));
+    ctx->lanes_dirty = true;
+    return DODE_OK;
+}
+
+static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, int c, const StepOpt& opt0 = StepOpt(),
+                     bool allow_lanes = false) {
     const dode_dims& d = ctx->dm;
     const size_t dayStride = (size_t)d.T * ctx->Np;
     const int chunk = d.storage == DODE_CSR ? kCsrMaxDays : kMaxDays;
@@ -413,8 +491,17 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
         int bt, bp, rc;
         StepOpt opt = opt0;
         if (opt.mask) opt.mask += (size_t)off * d.T * d.L;
-        if (ctx->tc_ready && dl.n >= ctx->tc_min_b) {
-            if ((rc = tc_step(ctx, c, dl, eta, opt))) return rc;
+        const bool tcp = ctx->tc_ready && dl.n >= ctx->tc_min_b;
+        if (tcp && allow_lanes && ctx->lanes_on && !ctx->timing && !opt.mask && !opt.G) {
+            Lane* ln = nullptr;
+            if ((rc = lane_begin(ctx, dl, &ln))) return rc;
+            if ((rc = tc_step(ctx, c, dl, eta, opt, ln->buf, ln->st))) return rc;
+            if ((rc = lane_end(ctx, ln))) return rc;
+            continue;
+        }
+        if ((rc = join_lanes(ctx))) return rc;
+        if (tcp) {
+            if ((rc = tc_step(ctx, c, dl, eta, opt, ctx->tcb, ctx->stream))) return rc;
             continue;
         }
         if ((rc = forward_batch(ctx, c, dl, &bt, &bp, opt.mask))) return rc;
@@ -453,9 +540,17 @@ void dode_destroy(dode_ctx* ctx) {
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
     if (ctx->ev_h2d) cudaEventDestroy(ctx->ev_h2d);
+    if (ctx->ev_fence) cudaEventDestroy(ctx->ev_fence);
     for (int i = 0; i < 2; ++i) { if (ctx->ev_step[i]) cudaEventDestroy(ctx->ev_step[i]); if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]); }
     cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
-    cudaFree(ctx->Qg_full); cudaFree(ctx->Qg_lo); cudaFree(ctx->rp_full); cudaFree(ctx->rp_lo);
+    for (TcBuf* tb : {&ctx->tcb, &ctx->lane[0].buf, &ctx->lane[1].buf}) {
+        cudaFree(tb->Qg_full); cudaFree(tb->Qg_lo); cudaFree(tb->rp_full); cudaFree(tb->rp_lo);
+    }
+    for (Lane& ln : ctx->lane) {
+        if (ln.st) cudaStreamDestroy(ln.st);
+        if (ln.done) cudaEventDestroy(ln.done);
+        if (ln.entry) cudaEventDestroy(ln.entry);
+    }
     cudaFree(ctx->Ag); cudaFree(ctx->Af); cudaFree(ctx->G); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r); cudaFree(ctx->Qb);
     for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
@@ -474,6 +569,7 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     if (d.N < 1 || d.L < 1 || d.T < 1 || d.H < 0 || d.C < 1 || d.D < 1)
         return fail(ctx, DODE_EINVAL, "dims must be positive (N=%d L=%d T=%d H=%d C=%d D=%d)", d.N, d.L, d.T, d.H, d.C, d.D);
     if (d.storage != DODE_DENSE && d.storage != DODE_CSR) return fail(ctx, DODE_EINVAL, "unknown storage %d", d.storage);
+    if (d.T > 65535) return fail(ctx, DODE_EINVAL, "T=%d exceeds 65535 (the time index rides on grid.y)", d.T);
     if (d.storage == DODE_DENSE && !R->dense) return fail(ctx, DODE_EINVAL, "R->dense is null");
     if (d.storage == DODE_CSR && (!R->blk_off || !R->row_ptr || (R->nnz > 0 && (!R->col_idx || !R->val)) || R->nnz < 0))
         return fail(ctx, DODE_EINVAL, "CSR arrays are null or nnz < 0");
@@ -493,6 +589,9 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     c->stream = (cudaStream_t)stream;
     c->labels.assign(labels, labels + d.D);
     c->stamp.assign(d.D, 0);
+    c->day_last_id.assign(d.D, 0);
+    c->day_last_lane.assign(d.D, -1);
+    if (const char* e = getenv("DODE_LANES")) c->lanes_on = atoi(e) != 0;
     ctx = c;
 #define CUC(call)                                                                                          \
     do {                                                                                                   \
@@ -522,7 +621,7 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
         CUC(cudaMalloc(&c->Ag, total * sizeof(float)));
         CUC(cudaMalloc(&c->Af, total * sizeof(float)));
         pack_departure_major<<<148 * 16, 256, 0, c->stream>>>(R->dense, c->Ag, blocks, d.T, d.H, d.L, d.N, c->Lp, c->Np);
-        pack_arrival_major<<<dim3(ceil_div(c->Lp, 32), ceil_div(c->Np, 32), (unsigned)blocks), 256, 0, c->stream>>>(
+        pack_arrival_major<<<dim3((unsigned)blocks, ceil_div(c->Lp, 32), ceil_div(c->Np, 32)), 256, 0, c->stream>>>(
             R->dense, c->Af, d.T, d.H, d.L, d.N, c->Lp, c->Np);
         c->launches += 2;
         const char* env = getenv("DODE_TC_MIN_B");      // minibatch from which the tensor-core path is used (0 = never)
@@ -546,7 +645,13 @@ int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta) {
     if (!ctx) return DODE_EINVAL;
     int c = 0, rc;
     if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
-    return step_impl(ctx, days, n, eta, c);
+    ctx->plain_since_host = true;
+    return step_impl(ctx, days, n, eta, c, StepOpt(), true);
+}
+
+int dode_join(dode_ctx* ctx) {
+    if (!ctx) return DODE_EINVAL;
+    return join_lanes(ctx);
 }
 
 int dode_adagrad_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, float eps, const uint8_t* row_mask) {
@@ -562,6 +667,7 @@ int dode_adagrad_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, 
     }
     StepOpt opt;
     opt.mask = row_mask; opt.G = ctx->G; opt.eps = eps;
+    ctx->plain_since_host = true;
     return step_impl(ctx, days, n, eta, c, opt);
 }
 
@@ -594,6 +700,7 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
     int c = 0, rc;
     if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
     if (!x_host || !q_host) return fail(ctx, DODE_EINVAL, "x_host or q_host is null");
+    if ((rc = join_lanes(ctx))) return rc;
     const dode_dims& d = ctx->dm;
     const size_t TL = (size_t)d.T * d.L, TN = (size_t)d.T * d.N;
     if (!ctx->s_h2d) {
@@ -604,6 +711,12 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
             CU(cudaEventCreateWithFlags(&ctx->ev_step[i], cudaEventDisableTiming));
             CU(cudaEventCreateWithFlags(&ctx->ev_d2h[i], cudaEventDisableTiming));
         }
+        CU(cudaEventCreateWithFlags(&ctx->ev_fence, cudaEventDisableTiming));
+    }
+    if (ctx->plain_since_host) {      // earlier steps on the ctx stream / the lanes may still read x or write q of these days
+        CU(cudaEventRecord(ctx->ev_fence, ctx->stream));
+        CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_fence, 0));
+        ctx->plain_since_host = false;
     }
     if (ctx->stage_x_cap < TL * n || ctx->stage_q_cap < TN * n) {
         CU(sync_all(ctx));
@@ -800,6 +913,7 @@ int dode_apply(dode_ctx* ctx, int32_t c, const float* u, float* v) {
     if (!ctx) return DODE_EINVAL;
     const dode_dims& d = ctx->dm;
     if (c < 0 || c >= d.C || !u || !v) return fail(ctx, DODE_EINVAL, "bad cluster or null buffer");
+    if (int rj = join_lanes(ctx)) return rj;
     scale_pad<<<592, 256, 0, ctx->stream>>>(u, ctx->pu, (size_t)d.T, d.N, ctx->Np, nullptr);
     ctx->launches++;
     int rc = apply_padded(ctx, c, v, d.L);
@@ -812,6 +926,7 @@ int dode_apply_t(dode_ctx* ctx, int32_t c, const float* v, float* u) {
     if (!ctx) return DODE_EINVAL;
     const dode_dims& d = ctx->dm;
     if (c < 0 || c >= d.C || !u || !v) return fail(ctx, DODE_EINVAL, "bad cluster or null buffer");
+    if (int rj = join_lanes(ctx)) return rj;
     scale_pad<<<592, 256, 0, ctx->stream>>>(v, ctx->pv, (size_t)d.T, d.L, ctx->Lp, nullptr);
     ctx->launches++;
     int rc = apply_t_padded(ctx, c, u);
@@ -824,6 +939,7 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
     if (!ctx) return DODE_EINVAL;
     const dode_dims& d = ctx->dm;
     if (c < 0 || c >= d.C || iters < 1 || !L_out) return fail(ctx, DODE_EINVAL, "bad cluster, iters or null output");
+    if (int rj = join_lanes(ctx)) return rj;
     double* nrm = ctx->d_obj + d.D;       // [0] = |w|^2, [1] = |v|^2
     const size_t TN = (size_t)d.T * d.N, TLp = (size_t)d.T * ctx->Lp;
     fill_f32<<<592, 256, 0, ctx->stream>>>(ctx->pw, TN, 1.f);
@@ -847,7 +963,7 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
 int dode_timing_enable(dode_ctx* ctx, int32_t on) {
     if (!ctx) return DODE_EINVAL;
     ctx->timing = on != 0;
-    return DODE_OK;
+    return join_lanes(ctx);
 }
 
 int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches, int32_t reset) {

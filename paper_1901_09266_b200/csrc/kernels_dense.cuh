@@ -208,17 +208,18 @@ pack_departure_major(const float* __restrict__ R, float* __restrict__ Ag, long b
 }
 
 // Af[c][t][j][n][l] = R[c][s][h][l][n] with s = t-hmax+j, h = hmax-j, hmax = min(H,t), for j <= hmax; 0 otherwise.
-// One 32x32 (l x n) transpose tile per block; grid = (ceil(Lp/32), ceil(Np/32), C*T*(H+1)).
+// One 32x32 (l x n) transpose tile per block; grid = (C*T*(H+1), ceil(Lp/32), ceil(Np/32)) — the block count can
+// exceed the 65535 limit of grid.y/z, so it rides on grid.x.
 __global__ void __launch_bounds__(256)
 pack_arrival_major(const float* __restrict__ R, float* __restrict__ Af, int T, int H, int L, int N, int Lp, int Np) {
     __shared__ float tile[32][33];
-    const long ctj = blockIdx.z;                          // (c*T + t)*(H+1) + j
+    const long ctj = blockIdx.x;                          // (c*T + t)*(H+1) + j
     const int j = (int)(ctj % (H + 1));
     const long ct = ctj / (H + 1);
     const int t = (int)(ct % T);
     const long c = ct / T;
     const int hmax = min(H, t);
-    const int l0 = blockIdx.x * 32, n0 = blockIdx.y * 32;
+    const int l0 = blockIdx.y * 32, n0 = blockIdx.z * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const bool valid = j <= hmax;
     if (valid) {

@@ -156,6 +156,31 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
         : "r"(taddr) : "memory");
 }
 
+// tcgen05.ld is asynchronous: its destination registers are written some time after the instruction issues and may be
+// read only after tcgen05.wait::ld.  Load and wait therefore live in ONE asm statement: with them in separate
+// statements the compiler is free to spill a destination register in between (it believes the value is there) and to
+// hand the register to another variable, which the late write then clobbers — seen as an intermittent hang of the
+// kernel variant that spills (ADA, 96 registers).
+__device__ __forceinline__ void tmem_ld16_wait(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+        "tcgen05.wait::ld.sync.aligned;"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16x2_wait(uint32_t t0, uint32_t t1, uint32_t* v, uint32_t* w) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%32];\n"
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%33];\n"
+        "tcgen05.wait::ld.sync.aligned;"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]), "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7]),
+          "=r"(w[8]), "=r"(w[9]), "=r"(w[10]), "=r"(w[11]), "=r"(w[12]), "=r"(w[13]), "=r"(w[14]), "=r"(w[15])
+        : "r"(t0), "r"(t1) : "memory");
+}
+
 #ifdef DODE_TC_TRACE
 // bring-up instrumentation (not built by default): per-chunk SM clock stamps of one CTA
 constexpr int kTraceNk = 512;
@@ -346,6 +371,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             for (int i = 0; i < 32; ++i)
                 lo[i] = __float_as_uint(__uint_as_float(hi[i]) - __uint_as_float(hi[i] & 0xffffe000u));
             const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);
+            __syncwarp();                                       // tcgen05.st is .sync.aligned
             tmem_st16(t0, hi); tmem_st16(t0 + 16, hi + 16);
             tmem_st16(t0 + 32, lo); tmem_st16(t0 + 48, lo + 16);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
@@ -360,17 +386,17 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         for (int c0 = 16 * group; c0 < p.bn && !(p.dbg & 4); c0 += 32) {
             uint32_t v[16], w[16];
             const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
-            tmem_ld16(taddr, v);
-            if (fused_n) tmem_ld16(taddr + p.bn, w);
             float cur[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j) cur[j] = pre[j];
             const uint32_t curkeep = keep;
-            if (c0 + 32 < p.bn) {
+            if (c0 + 32 < p.bn) {                               // next chunk's operands: in flight across this chunk's stores
                 prefetch(c0 + 32);
                 if (ADA && p.mode == 0 && p.mask != nullptr) prefetch_mask(c0 + 32);
             }
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            __syncwarp();                                       // tcgen05.ld / wait::ld are .sync.aligned
+            if (fused_n) tmem_ld16x2_wait(taddr, taddr + p.bn, v, w);
+            else tmem_ld16_wait(taddr, v);
             if (m < p.M) {
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
@@ -391,6 +417,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 }
             }
         }
+        __syncwarp();
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
     __syncthreads();
