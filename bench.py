@@ -152,7 +152,7 @@ def run_reference(args, cfg, b, rank, world):
         return
     R = synth.dar_dense(cfg)
     lab = synth.labels(cfg).numpy()
-    x = synth.counts(cfg, R, synth.q_true(cfg), torch.from_numpy(lab))
+    x = synth.counts(cfg, R, synth.q_true(cfg), torch.from_numpy(lab), noise=not cfg.fig12)
     Rn = [R[c].numpy() for c in range(cfg.C)]
     etas = [np.float32(1.0 / oracle.power_iteration(Rn[c], 10)) for c in range(cfg.C)]
     q = np.ones((cfg.D, cfg.T, cfg.N), np.float32)
@@ -226,7 +226,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
         del csr
     else:
         R = synth.dar_dense(cfg, device=dev)
-        x = synth.counts(cfg, R, synth.q_true(cfg, dev), torch.from_numpy(lab))
+        x = synth.counts(cfg, R, synth.q_true(cfg, dev), torch.from_numpy(lab), noise=not cfg.fig12)   # Fig. 12: y = Bx exactly
         torch.cuda.empty_cache()
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, dense=R)
     x_cpu = x.cpu()
@@ -404,6 +404,7 @@ def main():
     ap.add_argument("--workload", default="corridor", choices=list(synth.CONFIGS))
     ap.add_argument("--b", type=int, default=None, help="minibatch days (default: the workload's)")
     ap.add_argument("--days", type=int, default=None, help="override D (bench smoke runs only)")
+    ap.add_argument("--n", type=int, default=None, help="fig12 workload: matrix dimension n (L = N = n), 100..6000 in the paper")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-visits", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -416,6 +417,10 @@ def main():
     cfg = synth.CONFIGS[args.workload]
     if args.days:
         cfg = cfg.replace(D=args.days)
+    if args.n:
+        if not cfg.fig12:
+            raise SystemExit("--n applies to --workload fig12 only")
+        cfg = cfg.replace(N=args.n, L=args.n)
     b = args.b or cfg.b
     if args.impl == "reference":
         run_reference(args, cfg, b, rank, world)

@@ -114,6 +114,7 @@ class Config:
     modulated: bool = False   # weekly + seasonal day factors (G4, cfg 2 & 4)
     label_mode: str = "uniform"  # "zero" | "uniform" | "calendar" (G6)
     sparse: bool = False      # G7 windowed lags, CSR storage
+    fig12: bool = False       # NEXT-2: the paper's efficiency experiment: random dense B, x >= 0, y = Bx
     seed: int = MASTER_SEED
 
     @property
@@ -140,6 +141,10 @@ CONFIGS = {
                            K=1000, kmin=10, kmax=40, base_mu=1.0, base_sigma=1.2,
                            modulated=True, sparse=True),
 }
+# NEXT-2: "random generate a matrix B in R^{n x n}, x in (R+)^n, compute y = Bx and solve NNLS(B, y)",
+# n from 100 to 6000.  Here: T = 1, H = 0, L = N = n, one cluster, D right-hand sides solved together (b = D).
+CONFIGS["fig12"] = Config("fig12", N=6000, L=6000, T=1, H=0, C=1, D=64, b=64, K=200, kmin=1, kmax=1,
+                          label_mode="zero", fig12=True)
 CONFIG_ORDER = ["tiny", "corridor", "multiyear", "large_dense", "large_sparse"]
 
 
@@ -177,9 +182,16 @@ def dar_dense(cfg: Config, device="cpu", s_chunk: int = 16, redraw: Optional[int
     """fp32 [C][T][H+1][L][N]; flat Dirichlet over h on covered (l, n), 0 elsewhere.
     Blocks with s+h >= T are generated too (they are simply unused, A13)."""
     C, T, H1, L, N = cfg.C, cfg.T, cfg.H + 1, cfg.L, cfg.N
-    mask = incidence_mask(cfg, device, redraw)
     if out is None:
         out = torch.empty((C, T, H1, L, N), dtype=torch.float32, device=device)
+    if cfg.fig12:                                  # a random dense matrix, entries U[0,1) (PAPER.md:571)
+        flat = out.view(-1)
+        step = 1 << 24
+        for i0 in range(0, flat.numel(), step):
+            idx = torch.arange(i0, min(flat.numel(), i0 + step), dtype=torch.int64, device=device)
+            flat[i0:i0 + idx.numel()] = uniform01(cfg.seed, S_DAR, idx)
+        return out
+    mask = incidence_mask(cfg, device, redraw)
     blk = H1 * L * N
     for c in range(C):
         for s0 in range(0, T, s_chunk):
@@ -215,6 +227,9 @@ def day_factor(cfg: Config, device="cpu") -> torch.Tensor:
 
 def q_true(cfg: Config, device="cpu", dtype=torch.float32) -> torch.Tensor:
     """[D][T][N] = base_n * profile(s) * dayfactor_d."""
+    if cfg.fig12:                                  # x in (R+)^n, one vector per right-hand side
+        idx = torch.arange(cfg.D * cfg.T * cfg.N, dtype=torch.int64, device=device)
+        return uniform01(cfg.seed, S_BASE, idx, torch.float64).view(cfg.D, cfg.T, cfg.N).to(dtype)
     n = torch.arange(cfg.N, dtype=torch.int64, device=device)
     base = torch.exp(cfg.base_mu + cfg.base_sigma * normal(cfg.seed, S_BASE, n, torch.float64))
     q = day_factor(cfg, device)[:, None, None] * profile(cfg.T, device)[None, :, None] * base[None, None, :]

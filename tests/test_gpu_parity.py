@@ -263,3 +263,34 @@ def test_r2_quality_check_matches_oracle():
         assert abs(mean - want.mean()) < 1e-5
         assert per.max() <= 1.0 + 1e-6
         g.close()
+
+
+def test_overlapped_steps_keep_day_order_and_join_orders_caller_work():
+    """Plain steps alternate on two internal streams (include/dode.h, dode_spgd_step): steps that share days must still
+    run in call order, steps on disjoint days may overlap, other library calls interleave correctly, and dode_join makes
+    the ctx stream wait for every step issued before it."""
+    cfg = synth.Config("lanes", N=70, L=90, T=20, H=3, C=1, D=64, b=16, K=1, kmin=3, kmax=9, label_mode="zero")
+    p = hz.make_problem(cfg)
+    etas = hz.oracle_etas(p)
+    A, B, Cc = list(range(0, 16)), list(range(16, 32)), list(range(8, 24))      # Cc overlaps both A and B
+    seq = [A, B, A, A, Cc, B, Cc, A, B, list(range(32, 48)), Cc, list(range(40, 56)), A]
+    sched = [(0, np.array(d, np.int32)) for d in seq]
+    g = hz.GpuSolver(p)
+    P = g.P
+    for i, (c, days) in enumerate(sched):
+        P.dode_spgd_step(g.h, days, float(etas[c]))
+        if i == 5:
+            P.dode_objective(g.h, [0, 20])             # a synchronising call in the middle of the overlapped sequence
+        if i == 8:
+            P.dode_adagrad_reset(g.h)                  # a ctx-stream call that must not disturb the lanes
+    assert "tcgen05" in P.dode_last_path(g.h)
+    # dode_join: an event recorded on the ctx stream afterwards completes only after all steps; reading q straight from
+    # a device-side copy issued on that stream must then see the final state
+    P.dode_join(g.h)
+    ev = torch.cuda.Event()
+    ev.record()
+    ev.synchronize()
+    q_gpu = g.q()
+    q_cpu = hz.oracle_run(p, sched, etas)
+    hz.assert_q_close(q_gpu, q_cpu, "lanes")
+    g.close()
