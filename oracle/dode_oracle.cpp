@@ -28,8 +28,10 @@
 // P2 KKT, P3 finite differences, P4 planted recovery, P5 closed-form linear
 // iteration, P6 Example 1, P8 adjoint, P9 descent,
 // P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR, P14 R2 closed forms,
-// P15 row-chunk Adagrad against torch.optim.Adagrad on the assembled matrix.
+// P15 row-chunk Adagrad against torch.optim.Adagrad on the assembled matrix, P16 DAR construction (O7): the paper's
+// Example 3 worked by hand, the constant-speed closed form, unit row sums, vehicle conservation through O2a.
 // No function here is "parity unpinned".
+#include <algorithm>
 #include <cmath>
 #include <cstddef>
 #include <cstdint>
@@ -281,6 +283,49 @@ double oracle_objective_day_csr(int N, int L, int T, int H, const int64_t* blk_o
             f += r * r;
         }
     return f;
+}
+
+// O7 (NEXT-4): Step 1 of the framework, the DAR matrix of one day / one pattern from link speeds (PAPER.md:187-228,
+// Eq. 17-18 and Example 3; loop order of PAPER.md:377: "iterating over departure time intervals and paths ... we iterate
+// over all the links in the path from origin to destination and compute the arrival time of each link").
+//   path of OD n: links path_links[path_ptr[n] .. path_ptr[n+1]) in travel order (one path per OD: p = 1, Eq. 41);
+//   speed[t][l]: the link's speed in interval t (length units per second), len[l] its length, dt = |H| in seconds.
+//   The vehicles departing in H_s = [s dt, (s+1) dt) are bracketed by a leading (t1 = s dt) and a trailing
+//   (t2 = (s+1) dt) trajectory; a trajectory crosses a link at the speed of the interval in which it ENTERS the link
+//   ("the speeds of links are the slopes of the trajectory"; reading A20).  At the tail of link a the
+//   flow of H_s arrives spread evenly over [a1, a2) = [tau_a(t1), tau_a(t2)) (Eq. 16), so (Eq. 18)
+//       rho(s, h2) = |[a1, a2) ∩ H_h2| / (a2 - a1)           -> R[s][h2 - s][l][n]
+//   Entries with h2 - s > H or h2 >= T are dropped (reading A6).  If a2 <= a1 (FIFO violated by a speed
+//   jump between the two entries) the whole flow is put in the interval of a1.
+// R is [T][H+1][L][N], zeroed here.  All times in double.
+void oracle_dar_build(int N, int L, int T, int H, const int32_t* path_ptr, const int32_t* path_links, const float* len,
+                      const float* speed, double dt, float* R) {
+    const size_t total = (size_t)T * (H + 1) * L * N;
+    for (size_t i = 0; i < total; ++i) R[i] = 0.f;
+    for (int s = 0; s < T; ++s)
+        for (int n = 0; n < N; ++n) {
+            double a1 = (double)s * dt, a2 = (double)(s + 1) * dt;       // arrival of the two trajectories at the next link
+            for (int j = path_ptr[n]; j < path_ptr[n + 1]; ++j) {
+                const int l = path_links[j];
+                // the share of H_s that reaches the tail of link l within each interval h2
+                const int h_first = (int)std::floor(a1 / dt);
+                if (a2 > a1) {
+                    const int h_last = (int)std::floor(a2 / dt);
+                    for (int h2 = h_first; h2 <= h_last; ++h2) {
+                        const double lo = std::max(a1, (double)h2 * dt), hi = std::min(a2, (double)(h2 + 1) * dt);
+                        if (hi <= lo) continue;
+                        const int h = h2 - s;
+                        if (h <= H && h2 < T) R[(((size_t)s * (H + 1) + h) * L + l) * N + n] = (float)((hi - lo) / (a2 - a1));
+                    }
+                } else if (h_first - s <= H && h_first < T) {
+                    R[(((size_t)s * (H + 1) + (h_first - s)) * L + l) * N + n] = 1.f;
+                }
+                // cross the link at the speed of the interval of entry
+                const int i1 = std::min(T - 1, (int)std::floor(a1 / dt)), i2 = std::min(T - 1, (int)std::floor(a2 / dt));
+                a1 += (double)len[l] / (double)speed[(size_t)i1 * L + l];
+                a2 += (double)len[l] / (double)speed[(size_t)i2 * L + l];
+            }
+        }
 }
 
 }  // extern "C"

@@ -156,3 +156,15 @@ def objective_day_csr(N: int, L: int, T: int, H: int, blk_off, row_ptr, col_idx,
     return float(lib().oracle_objective_day_csr(
         N, L, T, H, blk_off.ctypes.data_as(C.POINTER(C.c_int64)), row_ptr.ctypes.data_as(C.POINTER(C.c_int32)),
         col_idx.ctypes.data_as(C.POINTER(C.c_int32)), pv, pq, px))
+
+
+def dar_build(N: int, L: int, T: int, H: int, path_ptr, path_links, length, speed, dt: float) -> np.ndarray:
+    """O7 (NEXT-4): DAR blocks [T][H+1][L][N] of one day from link speeds (Eq. 17-18, Example 3)."""
+    path_ptr = np.ascontiguousarray(path_ptr, dtype=np.int32); path_links = np.ascontiguousarray(path_links, dtype=np.int32)
+    length = np.ascontiguousarray(length, dtype=np.float32); speed = np.ascontiguousarray(speed, dtype=np.float32)
+    assert path_ptr.shape == (N + 1,) and length.shape == (L,) and speed.shape == (T, L)
+    R = np.empty((T, H + 1, L, N), np.float32)
+    lib().oracle_dar_build(N, L, T, H, path_ptr.ctypes.data_as(C.c_void_p), path_links.ctypes.data_as(C.c_void_p),
+                           length.ctypes.data_as(C.c_void_p), speed.ctypes.data_as(C.c_void_p), C.c_double(dt),
+                           R.ctypes.data_as(C.c_void_p))
+    return R

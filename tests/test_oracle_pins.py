@@ -345,3 +345,77 @@ def test_p15_row_chunk_adagrad_against_torch(tiny12):
     qa, Ga = oracle.visit_adagrad(Rc, q, G, x[d], None, eta, eps)
     qb, Gb = oracle.visit_adagrad(Rc, q, G, x[d], np.ones((cfg.T, cfg.L), np.uint8), eta, eps)
     np.testing.assert_array_equal(qa, qb); np.testing.assert_array_equal(Ga, Gb)
+
+
+# ---- P16: DAR construction from speeds (O7, NEXT-4) -----------------------------------------------------------------
+def _example3_instance():
+    T, H, L, N, dt = 6, 4, 3, 1, 300.0
+    length = np.array([1000.0, 1500.0, 800.0], np.float32)
+    speed = np.full((T, L), 8.0, np.float32)
+    speed[0, 0], speed[0, 1] = 5.0, 10.0
+    speed[1, 0], speed[1, 1] = 4.0, 3.75
+    return T, H, L, N, dt, np.array([0, 3], np.int32), np.array([0, 1, 2], np.int32), length, speed
+
+
+def test_p16_dar_example3_worked_by_hand():
+    """Example 3 (Eq. 19-28) with numbers fixed in tests/golden/example3_three_link_dar.txt."""
+    T, H, L, N, dt, pp, pl, length, speed = _example3_instance()
+    R = oracle.dar_build(N, L, T, H, pp, pl, length, speed, dt)
+    want = np.zeros((H + 1, L))
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "example3_three_link_dar.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        l, h2, v = line.split()
+        want[int(h2), int(l)] = float(v)
+    np.testing.assert_allclose(R[0, :, :, 0], want, rtol=0, atol=1e-7)
+
+
+def test_p16_dar_constant_speed_closed_form_and_row_sums():
+    """Constant speeds: link j is reached after c_j = sum of travel times, so the flow of interval s arrives in intervals
+    s + floor(c_j/dt) and the next one with shares 1 - frac and frac (Eq. 17); every covered (s, l, n) sums to 1 over
+    h2 (Eq. 18) unless truncated at the day end / at lag H."""
+    T, H, L, N, dt = 12, 5, 7, 3, 300.0
+    rng = np.random.default_rng(4)
+    length = rng.uniform(500, 3000, L).astype(np.float32)
+    v = rng.uniform(5, 30, L).astype(np.float32)
+    speed = np.tile(v, (T, 1))
+    paths = [[0, 1, 2, 3], [2, 3, 4, 5, 6], [6]]
+    pp = np.cumsum([0] + [len(p) for p in paths]).astype(np.int32)
+    pl = np.concatenate(paths).astype(np.int32)
+    R = oracle.dar_build(N, L, T, H, pp, pl, length, speed, dt)
+    for n, path in enumerate(paths):
+        c = 0.0
+        for l in path:
+            hh, fr = int(c // dt), (c / dt) % 1.0
+            for s in range(T):
+                exp = np.zeros(H + 2)
+                if hh <= H: exp[hh] = 1.0 - fr
+                if hh + 1 <= H + 1: exp[hh + 1] = fr
+                exp = exp[:H + 1].copy()
+                exp[max(0, T - s):] = 0.0                       # arrival intervals beyond the day are dropped
+                np.testing.assert_allclose(R[s, :, l, n], exp, atol=2e-6)
+            c += float(length[l]) / float(v[l])
+        off = [l for l in range(L) if l not in path]
+        assert not R[:, :, off, n].any()
+    assert (R >= 0).all()
+
+
+def test_p16_dar_conserves_vehicles_through_the_forward_operator():
+    """Time-varying speeds, H large enough and departures early enough that nothing is truncated: each covered (s, l, n)
+    sums to 1 over the lags, so every vehicle of q is counted exactly once on every link of its path by O2a."""
+    T, H, L, N, dt = 40, 12, 9, 4, 300.0
+    rng = np.random.default_rng(9)
+    length = rng.uniform(800, 2500, L).astype(np.float32)
+    speed = rng.uniform(6, 25, (T, L)).astype(np.float32)
+    paths = [[0, 1, 2, 3, 4], [3, 4, 5], [5, 6, 7, 8], [1, 2]]
+    pp = np.cumsum([0] + [len(p) for p in paths]).astype(np.int32)
+    pl = np.concatenate(paths).astype(np.int32)
+    R = oracle.dar_build(N, L, T, H, pp, pl, length, speed, dt)
+    for n, path in enumerate(paths):
+        np.testing.assert_allclose(R[:T - H - 1, :, path, n].sum(axis=1), 1.0, atol=1e-6)
+    q = np.zeros((T, N), np.float32)
+    q[:T - H - 1] = rng.uniform(1, 50, (T - H - 1, N)).astype(np.float32)
+    x = oracle.forward_residual(R, q, np.zeros((T, L), np.float32))
+    for l in range(L):
+        users = [n for n, path in enumerate(paths) if l in path]
+        np.testing.assert_allclose(x[:, l].sum(), q[:, users].sum(), rtol=1e-5)
