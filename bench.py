@@ -395,6 +395,82 @@ def run_ours(args, cfg, b, rank, world, local_rank):
     P.dode_destroy(h)
 
 
+def run_dar_build(args, cfg, local_rank):
+    """--dar-build (NEXT-4): Step 1 of the framework, the DAR blocks of one traffic pattern from link speeds
+    (dode_dar_build; Eq. 17-18).  One step = one pattern's operator [T][H+1][L][N] built from its
+    [T][L] speeds.  The kernel's work is the output it must produce: algorithmic bytes = 4*T*(H+1)*L*N."""
+    import paper_1901_09266_b200 as P
+    P.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    DT = 300.0
+    ptr, links, length = synth.network(cfg)
+    ptr_d, links_d, len_d = ptr.to(dev), links.to(dev), length.to(dev)
+    vs = [synth.speeds(cfg, c).pin_memory() for c in range(cfg.C)]
+    vd = [v.to(dev) for v in vs]
+    nbytes = 4.0 * cfg.T * (cfg.H + 1) * cfg.L * cfg.N
+    R = torch.empty((cfg.T, cfg.H + 1, cfg.L, cfg.N), device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    sampler = ClockSampler(local_rank)
+    for i in range(max(3, args.warmup)):
+        P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, vd[i % cfg.C], DT, R)
+    torch.cuda.synchronize()
+    sampler.start()
+    ev = []
+    for i in range(args.steps):
+        flush.zero_()
+        a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, vd[i % cfg.C], DT, R)
+        z.record()
+        ev.append((a, z))
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join()
+    ms = sum(a.elapsed_time(z) for a, z in ev) / args.steps
+    nnz = int((R != 0).sum().item())
+    # end to end: speeds from pinned host memory, the operator back to the host
+    R_host = torch.empty(R.shape, dtype=torch.float32).pin_memory() if nbytes < 4e9 else None
+    e2e = None
+    if R_host is not None and args.e2e_steps > 0:
+        vtmp = torch.empty_like(vd[0])
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for i in range(args.e2e_steps):
+            vtmp.copy_(vs[i % cfg.C], non_blocking=True)
+            P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, vtmp, DT, R)
+            R_host.copy_(R, non_blocking=True)
+        torch.cuda.synchronize()
+        e2e = {"value": (time.perf_counter() - t0) * 1e3 / args.e2e_steps, "unit": "ms/pattern",
+               "h2d_bytes_per_step": int(vs[0].numel() * 4), "d2h_bytes_per_step": int(nbytes),
+               "api": "dode_dar_build (speeds uploaded from pinned host memory, operator downloaded)"}
+    hbm, _, peak_src = measured_peaks()
+    ach = nbytes / (ms * 1e-3) / 1e9
+    out = {"metric": "dar_build_time_per_pattern", "value": ms, "unit": "ms/pattern", "n_gpus": 1, "steps": args.steps,
+           "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64 times / f32 shares", "data": "synthetic",
+           "config": {"workload": f"dar_build on {cfg.name}: N={cfg.N} L={cfg.L} T={cfg.T} H={cfg.H}, one path per OD "
+                                  f"({int(ptr[-1])} path links), |H| = 300 s",
+                      "l2": "L2 flushed (256 MiB write) before every timed build"},
+           "nnz": nnz, "gpu_launches": args.steps * 2, "clocks": sampler.summary(),
+           "roofline": {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
+                        "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})", "kernel": "cudaMemsetAsync + dar_build_dense",
+                        "traffic": None},
+           "e2e": e2e}
+    if not args.no_cpu_baseline:
+        from oracle import oracle
+        Tc = cfg.T if nbytes < 1.5e9 else max(1, int(cfg.T * 1.5e9 / nbytes))      # bounded sample: the first Tc intervals
+        v0 = vs[0][:Tc].numpy()
+        t0 = time.perf_counter()
+        oracle.dar_build(cfg.N, cfg.L, Tc, cfg.H, ptr.numpy(), links.numpy(), length.numpy(), v0, DT)
+        cpu_ms = (time.perf_counter() - t0) * 1e3 * cfg.T / Tc
+        out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms/pattern", "cores": 1, "kind": "oracle",
+                               "sample": f"O7 on the first {Tc} of {cfg.T} departure intervals, extrapolated x{cfg.T / Tc:.1f}"}
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -408,6 +484,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-visits", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dar-build", action="store_true", help="NEXT-4: time dode_dar_build on the workload's network instead of SPGD")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
@@ -422,6 +499,10 @@ def main():
             raise SystemExit("--n applies to --workload fig12 only")
         cfg = cfg.replace(N=args.n, L=args.n)
     b = args.b or cfg.b
+    if args.dar_build:
+        if rank == 0:
+            run_dar_build(args, cfg, local_rank)
+        return
     if args.impl == "reference":
         run_reference(args, cfg, b, rank, world)
     else:

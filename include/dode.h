@@ -137,6 +137,22 @@ int dode_apply_t(dode_ctx* ctx, int32_t c, const float* v, float* u);
  * eta_c = 1/L_c is the step "dependent on the problem scale".  Synchronises. */
 int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out);
 
+/* NEXT-4 — Step 1 of the framework: the DAR blocks of ONE day / traffic pattern from link speeds (Eq. 17-18 and
+ * Example 3; "iterating over departure time intervals and paths").  Needs no ctx.
+ *   path_ptr    device int32 [N+1]      links of OD n's path: path_links[path_ptr[n] .. path_ptr[n+1]) in travel order
+ *   path_links  device int32 [path_ptr[N]], each in [0, L)   (one path per OD: route share p = 1 in Eq. 41)
+ *   link_len    device fp32 [L]         link lengths
+ *   speed       device fp32 [T][L]      link speed in each interval, length units per second, > 0
+ *   dt          interval length |H| in seconds (300 for the paper's 5-minute data)
+ *   R_out       device fp32 [T][H+1][L][N]  (one cluster's slab of dode_dar.dense); fully overwritten
+ * The flow departing in interval s is bracketed by the trajectories leaving at s*dt and (s+1)*dt, each crossing a link at
+ * the speed of the interval in which it enters it; at the tail of link a it arrives evenly spread over [a1, a2) and
+ *     R[s][h2-s][a][n] = |[a1,a2) ∩ H_h2| / (a2 - a1).
+ * Shares with h2-s > H or h2 >= T are dropped.  Asynchronous on `stream`; errors of this call are read
+ * with dode_last_error(NULL). */
+int dode_dar_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* path_ptr, const int32_t* path_links,
+                   const float* link_len, const float* speed, double dt, float* R_out, void* stream);
+
 /* Optional per-kernel timing for roofline reports: while enabled, every forward (kind 0) and
  * gradient+update (kind 1) launch is bracketed by CUDA events on the ctx stream.  dode_timing_read
  * synchronises, folds finished event pairs into the running totals and returns the total device

@@ -14,6 +14,7 @@
 #include "kernels_dense.cuh"
 #include "kernels_csr.cuh"
 #include "kernels_tc.cuh"
+#include "kernels_dar.cuh"
 
 #include <cstdlib>
 
@@ -956,6 +957,26 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
     }
     CU(cudaMemcpyAsync(L_out, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaGetLastError());
+    return DODE_OK;
+}
+
+int dode_dar_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* path_ptr, const int32_t* path_links,
+                   const float* link_len, const float* speed, double dt, float* R_out, void* stream) {
+    dode_ctx* ctx = nullptr;                   // no ctx: errors go to the thread-local buffer (dode_last_error(NULL))
+    if (N < 1 || L < 1 || T < 1 || H < 0 || !(dt > 0.0)) return fail(ctx, DODE_EINVAL, "dims must be positive and dt > 0");
+    if (!path_ptr || !path_links || !link_len || !speed || !R_out) return fail(ctx, DODE_EINVAL, "null argument");
+    int dev = 0, major = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return fail(ctx, DODE_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+    if (major != 10) return fail(ctx, DODE_ECUDA, "this library is built for sm_100a only (device is sm_%d0)", major);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)T * (H + 1) * L * N * sizeof(float);
+    CU(cudaMemsetAsync(R_out, 0, bytes, st));
+    const long total = (long)T * N;
+    const int blocks = (int)std::min<long>((total + 255) / 256, 148L * 16);
+    dar_build_dense<<<blocks, 256, 0, st>>>(N, L, T, H, path_ptr, path_links, link_len, speed, dt, R_out);
     CU(cudaGetLastError());
     return DODE_OK;
 }

@@ -32,6 +32,7 @@ MASTER_SEED = 20190129  # the paper's arXiv date; arbitrary
 # stream ids (one per generated array)
 S_INC_K, S_INC_START, S_DAR, S_BASE, S_DAYF, S_NOISE, S_LABEL, S_RELABEL = range(1, 9)
 S_SCHED, S_TAU, S_WIN, S_SPFRAC, S_PROBE = range(9, 14)
+S_LEN, S_VFREE, S_CONG, S_VNOISE = range(14, 18)
 
 _MASK64 = (1 << 64) - 1
 
@@ -203,6 +204,37 @@ def dar_dense(cfg: Config, device="cpu", s_chunk: int = 16, redraw: Optional[int
             tot = e.sum(dim=1, keepdim=True)
             out[c, s0:s1] = e / torch.where(tot > 0, tot, torch.ones_like(tot))
     return out
+
+
+# --------------------------------------------------------------------------
+# G9 (NEXT-4): network and speeds for the DAR construction (stand-in for the NPMRDS 5-minute probe speeds of 43 TMCs,
+# PAPER.md:484-486).  Paths are the G2 link runs in travel order; link lengths U[0.5, 3] km; speed = free-flow
+# U[24, 31] m/s reduced in the two weekday peaks (the G4 profile) by a per-link, per-pattern congestion factor
+# U[0, 0.7], times (1 + 2 % noise).
+# --------------------------------------------------------------------------
+def network(cfg: Config, device="cpu"):
+    """(path_ptr int32 [N+1], path_links int32, link_len fp32 [L]) for dode_dar_build / the oracle's O7."""
+    start, k = incidence(cfg, device)
+    ptr = torch.zeros(cfg.N + 1, dtype=torch.int64, device=device)
+    ptr[1:] = torch.cumsum(k, 0)
+    j = torch.arange(int(ptr[-1]), dtype=torch.int64, device=device)
+    owner = torch.searchsorted(ptr[1:].contiguous(), j, right=True)
+    links = start[owner] + (j - ptr[owner])
+    l = torch.arange(cfg.L, dtype=torch.int64, device=device)
+    length = 500.0 + 2500.0 * uniform01(cfg.seed, S_LEN, l)
+    return ptr.to(torch.int32), links.to(torch.int32), length.to(torch.float32)
+
+
+def speeds(cfg: Config, c: int = 0, device="cpu") -> torch.Tensor:
+    """fp32 [T][L] link speeds (m/s) of traffic pattern c."""
+    l = torch.arange(cfg.L, dtype=torch.int64, device=device)
+    vfree = 24.0 + 7.0 * uniform01(cfg.seed, S_VFREE, l, torch.float64)
+    cong = 0.7 * uniform01(cfg.seed, S_CONG, l + c * cfg.L, torch.float64)
+    peak = (profile(cfg.T, device) - 0.1).clamp(0.0, 1.0)
+    idx = torch.arange(cfg.T * cfg.L, dtype=torch.int64, device=device) + c * cfg.T * cfg.L
+    noise = 1.0 + 0.02 * normal(cfg.seed, S_VNOISE, idx, torch.float64).view(cfg.T, cfg.L)
+    v = vfree[None, :] * (1.0 - cong[None, :] * peak[:, None]) * noise
+    return v.clamp(min=1.0).to(torch.float32)
 
 
 # --------------------------------------------------------------------------

@@ -1,0 +1,80 @@
+"""NEXT-4: DAR construction from link speeds on the GPU (dode_dar_build) against the oracle's O7
+(pinned by P16), and the built operator carried through the SPGD path."""
+import numpy as np
+import pytest
+import torch
+
+import paper_1901_09266_b200 as P
+from paper_1901_09266_b200 import synth
+from tests import harness as hz
+
+pytestmark = pytest.mark.gpu
+DT = 300.0
+
+
+def _build_both(cfg, c=0):
+    from oracle import oracle
+    ptr, links, length = synth.network(cfg)
+    v = synth.speeds(cfg, c)
+    want = oracle.dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr.numpy(), links.numpy(), length.numpy(), v.numpy(), DT)
+    R = torch.full((cfg.T, cfg.H + 1, cfg.L, cfg.N), 7.0, device="cuda")          # stale contents must be overwritten
+    P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr.cuda(), links.cuda(), length.cuda(), v.cuda(), DT, R)
+    torch.cuda.synchronize()
+    return R.cpu().numpy(), want
+
+
+@pytest.mark.parametrize("shape", [(61, 37, 50, 5), (4, 6, 288, 6), (60, 120, 288, 12), (300, 90, 24, 30), (7, 5, 3, 0)])
+def test_dar_build_matches_oracle(shape):
+    N, L, T, H = shape
+    cfg = synth.Config("dar", N=N, L=L, T=T, H=H, C=2, D=4, b=2, K=1, kmin=2, kmax=min(20, L))
+    for c in range(cfg.C):
+        got, want = _build_both(cfg, c)
+        # same support (which (s, h, l, n) entries exist is an integer decision; both sides take it in double)
+        np.testing.assert_array_equal(got != 0, want != 0)
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-6)
+        assert (got >= 0).all() and got.max() <= 1.0 + 1e-6
+
+
+def test_example3_on_gpu():
+    """The hand-worked Example 3 instance (tests/golden/example3_three_link_dar.txt) through the kernel."""
+    T, H, L, N = 6, 4, 3, 1
+    length = torch.tensor([1000.0, 1500.0, 800.0])
+    speed = torch.full((T, L), 8.0)
+    speed[0, 0], speed[0, 1], speed[1, 0], speed[1, 1] = 5.0, 10.0, 4.0, 3.75
+    R = torch.empty((T, H + 1, L, N), device="cuda")
+    P.dode_dar_build(N, L, T, H, torch.tensor([0, 3], dtype=torch.int32).cuda(), torch.tensor([0, 1, 2], dtype=torch.int32).cuda(),
+                     length.cuda(), speed.cuda(), DT, R)
+    got = R.cpu().numpy()[0, :, :, 0]
+    want = np.zeros((H + 1, L))
+    want[0, 0] = 1.0
+    want[0, 1], want[1, 1] = 100 / 350, 250 / 350
+    want[1, 2], want[2, 2], want[3, 2] = 250 / 600, 300 / 600, 50 / 600
+    np.testing.assert_allclose(got, want, atol=1e-7)
+
+
+def test_built_operator_through_the_spgd_path():
+    """Step 1 -> Step 5 on the GPU: operators built by dode_dar_build for two patterns feed dode_create directly; the
+    SPGD iterates equal the oracle's on the oracle-built operators."""
+    from oracle import oracle
+    cfg = synth.Config("dar_e2e", N=40, L=30, T=36, H=6, C=2, D=24, b=8, K=10, kmin=3, kmax=8)
+    ptr, links, length = synth.network(cfg)
+    Rg = torch.empty((cfg.C, cfg.T, cfg.H + 1, cfg.L, cfg.N), device="cuda")
+    Ro = np.empty((cfg.C, cfg.T, cfg.H + 1, cfg.L, cfg.N), np.float32)
+    for c in range(cfg.C):
+        v = synth.speeds(cfg, c)
+        P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr.cuda(), links.cuda(), length.cuda(), v.cuda(), DT, Rg[c])
+        Ro[c] = oracle.dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr.numpy(), links.numpy(), length.numpy(), v.numpy(), DT)
+    lab = synth.labels(cfg)
+    x = synth.counts(cfg, torch.from_numpy(Ro), synth.q_true(cfg), lab)
+    p = hz.Problem(cfg, torch.from_numpy(Ro), lab.numpy(), x, synth.q_true(cfg))
+    sched = synth.schedule(cfg, p.labels)
+    etas = hz.oracle_etas(p)
+    h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, p.labels, x.cuda(), 1.0, dense=Rg)
+    for c, days in sched:
+        P.dode_spgd_step(h, days, float(etas[c]))
+    P.dode_sync(h)
+    out = torch.empty((cfg.D, cfg.T, cfg.N))
+    for d in range(cfg.D):
+        P.dode_get_q(h, d, out[d])
+    hz.assert_q_close(out.numpy(), hz.oracle_run(p, sched, etas), "dar_e2e")
+    P.dode_destroy(h)
