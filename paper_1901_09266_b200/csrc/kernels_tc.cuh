@@ -259,14 +259,18 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     float pre[16];
     const int erow = ((warp & 3) << 5) + lane, em = m0 + erow;
     const int egroup = warp >= 2 ? (warp - 2) >> 2 : 0;
+    // One base pointer and one day stride for both passes, rows and days clamped instead of predicated: the loads are
+    // unconditional, nothing reads their registers before the epilogue (which applies m < M, d < n), and the address
+    // is one multiply-add per element.  (Predicated per-mode loads with the full index expression were ~2400 SASS
+    // instructions ahead of the main loop — 3800 cycles before a CTA's first split in the per-chunk trace.)
+    const int emc = min(em, p.M - 1);
+    const float* ebase = p.mode == 0 ? p.x + ((size_t)tt * p.M + emc) : p.q + ((size_t)tt * p.Np + emc);
+    const size_t estride = p.mode == 0 ? (size_t)p.T * p.M : p.dayStride;
     auto prefetch = [&](int c0) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-            const int d = c0 + j;
-            pre[j] = 0.f;
-            if (em < p.M && d < dl.n)
-                pre[j] = p.mode == 0 ? __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.M + em)
-                                     : __ldcg(p.q + (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + em);
+            const int d = min(c0 + j, dl.n - 1);
+            pre[j] = __ldcg(ebase + (size_t)dl.day[d] * estride);    // through L2: q may have been written under PDL
         }
     };
     uint32_t keep = 0xffffu;                                          // bit j: row (em, day c0+j) belongs to the chunk B_o
