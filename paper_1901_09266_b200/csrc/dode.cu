@@ -25,6 +25,8 @@ struct TcBuf {
     float *Qg_full = nullptr, *Qg_lo = nullptr;   // [cap][T*Np]
     float *rp_full = nullptr, *rp_lo = nullptr;   // [cap][T*Lp]
     int cap = 0, bn = 0;
+    float* part = nullptr;                        // split-K partial sums [ksplit][T][tiles*128][bn]
+    size_t part_cap = 0;                          // floats
     CUtensorMap mapQ_f, mapQ_l, mapR_f, mapR_l;
 };
 
@@ -414,20 +416,51 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
     { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
-    auto kern = (opt.mask || opt.G) ? tc::banded_gemm_3xtf32<true> : tc::banded_gemm_3xtf32<false>;
+    const bool ada = opt.mask || opt.G;
+    auto kern = ada ? tc::banded_gemm_3xtf32<true> : tc::banded_gemm_3xtf32<false>;
+    // split-K when the time axis is too short to fill the machine (T * tiles CTAs for 148 SMs x 1-2 CTAs): e.g. the
+    // Fig. 12 workload, T = 1.  Each pass then runs ksplit CTAs per tile and a small epilogue kernel.
+    const int slots = 148 * (smem * 2 + 2048 <= 227 * 1024 ? 2 : 1);
+    auto pick_split = [&](int M, int kunit) {
+        const long ctas = (long)ceil_div(M, tc::kTileM) * d.T;
+        const int nk_max = ceil_div((long)(d.H + 1) * kunit, tc::kTileK);
+        int ks = (int)std::min<long>(slots / std::max<long>(ctas, 1), nk_max / 8);
+        if (const char* e = getenv("DODE_TC_KSPLIT")) ks = atoi(e);
+        return std::max(1, std::min(ks, 32));
+    };
+    const int ks_f = pick_split(d.L, ctx->Np), ks_g = pick_split(d.N, ctx->Lp);
+    if (ks_f > 1 || ks_g > 1) {
+        const size_t need = (size_t)std::max(ks_f * ceil_div(d.L, tc::kTileM), ks_g * ceil_div(d.N, tc::kTileM)) * tc::kTileM * d.T * bn;
+        if (tb.part_cap < need) {
+            CU(cudaStreamSynchronize(st));
+            cudaFree(tb.part); tb.part = nullptr; tb.part_cap = 0;
+            CU(cudaMalloc(&tb.part, need * sizeof(float)));
+            tb.part_cap = need;
+        }
+    }
+    p.part = tb.part;
+    auto epilogue = [&](int Mt) -> int {           // second half of a split-K pass
+        const dim3 g(ceil_div((long)Mt * (bn / 4), 256), d.T);
+        if (ada) tc::splitk_epilogue<true><<<g, 256, 0, st>>>(p, Mt, dl);
+        else tc::splitk_epilogue<false><<<g, 256, 0, st>>>(p, Mt, dl);
+        ctx->launches++;
+        return DODE_OK;
+    };
     {
         KernelTimer kt(ctx, KIND_FWD);
-        p.mode = 0; p.M = d.L; p.kunit = ctx->Np;
-        CU(launch_pdl(kern, dim3(ceil_div(d.L, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+        p.mode = 0; p.M = d.L; p.kunit = ctx->Np; p.ksplit = ks_f;
+        CU(launch_pdl(kern, dim3(ceil_div(d.L, tc::kTileM), d.T, ks_f), dim3(tc::kThreadsTC), smem,
                       st, ctx->mapA_fwd, ctx->mapA_fwd64, tb.mapQ_f, tb.mapQ_l, p, dl));
         ctx->launches++;
+        if (ks_f > 1) epilogue(ceil_div(d.L, tc::kTileM) * tc::kTileM);
     }
     {
         KernelTimer kt(ctx, KIND_GRAD);
-        p.mode = 1; p.M = d.N; p.kunit = ctx->Lp;
-        CU(launch_pdl(kern, dim3(ceil_div(d.N, tc::kTileM), d.T), dim3(tc::kThreadsTC), smem,
+        p.mode = 1; p.M = d.N; p.kunit = ctx->Lp; p.ksplit = ks_g;
+        CU(launch_pdl(kern, dim3(ceil_div(d.N, tc::kTileM), d.T, ks_g), dim3(tc::kThreadsTC), smem,
                       st, ctx->mapA_grad, ctx->mapA_grad64, tb.mapR_f, tb.mapR_l, p, dl));
         ctx->launches++;
+        if (ks_g > 1) epilogue(ceil_div(d.N, tc::kTileM) * tc::kTileM);
     }
     char buf[96];
     snprintf(buf, sizeof buf, "tcgen05_3xtf32_fwd_bn%d+tcgen05_3xtf32_grad_bn%d", bn, bn);
@@ -545,6 +578,7 @@ void dode_destroy(dode_ctx* ctx) {
     for (int i = 0; i < 2; ++i) { if (ctx->ev_step[i]) cudaEventDestroy(ctx->ev_step[i]); if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]); }
     cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
     for (TcBuf* tb : {&ctx->tcb, &ctx->lane[0].buf, &ctx->lane[1].buf}) {
+        cudaFree(tb->part);
         cudaFree(tb->Qg_full); cudaFree(tb->Qg_lo); cudaFree(tb->rp_full); cudaFree(tb->rp_lo);
     }
     for (Lane& ln : ctx->lane) {

@@ -130,6 +130,11 @@ struct TcParams {
     const uint8_t* mask; // forward: [n][T][L] bytes by position in the day list, 0 = row outside the chunk B_o (r = 0)
     float* G;            // gradient: Adagrad accumulator [D][T][Np], in place
     float eps;
+    // split-K (short time axes: T * tiles CTAs would not fill the machine): blockIdx.z takes a
+    // contiguous range of K chunks and stores its raw accumulators to part[ks][tt][m][bn]; splitk_epilogue sums the
+    // ranges in a fixed order and applies the pass's epilogue.  ksplit = 1: the fused epilogue below.
+    int ksplit;
+    float* part;
     int dbg;             // bring-up switches: 1 = no split, 2 = no MMA, 4 = no epilogue (results invalid)
 };
 
@@ -223,8 +228,11 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
 
     const int lags = (p.mode == 0 ? min(p.H, tt) : min(p.H, p.T - 1 - tt)) + 1;
-    const int nk = (lags * p.kunit + kTileK - 1) / kTileK;
-    const int w0 = p.mode == 0 ? (tt - lags + 1) * p.kunit : tt * p.kunit;     // first element of the B window
+    const int nk_all = (lags * p.kunit + kTileK - 1) / kTileK;
+    const int cps = (nk_all + p.ksplit - 1) / p.ksplit;                         // chunks per split
+    const int kbase = (int)blockIdx.z * cps;                                    // first chunk of this CTA's range
+    const int nk = max(0, min(nk_all, kbase + cps) - kbase);
+    const int w0 = (p.mode == 0 ? (tt - lags + 1) * p.kunit : tt * p.kunit) + kbase * kTileK;   // first element of the B window
 
     const bool fused_n = p.bn <= 128;
     const int acc_cols = fused_n ? 2 * p.bn : p.bn;
@@ -282,12 +290,13 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (em < p.M && d < dl.n && __ldg(p.mask + ((size_t)d * p.T + tt) * p.M + em) != 0) keep |= 1u << j;
         }
     };
-    if (p.mode == 0 && warp >= 2) prefetch(16 * egroup);             // x is a static input
+    const bool fused_epi = p.ksplit == 1;
+    if (fused_epi && p.mode == 0 && warp >= 2) prefetch(16 * egroup);             // x is a static input
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (ADA && p.mode == 0 && p.mask != nullptr && warp >= 2) prefetch_mask(16 * egroup);   // the caller's buffer: after the wait
     // q was written by the previous step's kernel, which may still have been running on this SM when this CTA was
     // launched (PDL): the launch-time L1 invalidation does not cover it, so q is read through L2 (ld.global.cg)
-    if (p.mode == 1 && warp >= 2) prefetch(16 * egroup);
+    if (fused_epi && p.mode == 1 && warp >= 2) prefetch(16 * egroup);
 
     if (warp == 0) {
         // ===== TMA producer =====
@@ -299,7 +308,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
                 mbar_expect_tx(&full[s], aBytes + 2 * bBytes);
-                tma_load_3d(st, mA, &full[s], m0, kc * kTileK, p.slab0 + tt);
+                tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
                 tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
                 tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
             }
@@ -345,7 +354,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             TC_TRACE(1, kc, 3);
             if (++s == p.stages) { s = 0; ph ^= 1; }
         }
-        if (elect_one()) { if (p.dbg & 2) mbar_arrive(accum); else umma_commit(accum); }
+        if (elect_one()) { if ((p.dbg & 2) || nk == 0) mbar_arrive(accum); else umma_commit(accum); }
         __syncwarp();
     } else {
         // ===== splitters: smem column -> registers -> TMEM (A_hi, A_lo); group g takes chunks kc = g, g+2, ... =====
@@ -394,13 +403,29 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
 #pragma unroll
             for (int j = 0; j < 16; ++j) cur[j] = pre[j];
             const uint32_t curkeep = keep;
-            if (c0 + 32 < p.bn) {                               // next chunk's operands: in flight across this chunk's stores
+            if (fused_epi && c0 + 32 < p.bn) {                  // next chunk's operands: in flight across this chunk's stores
                 prefetch(c0 + 32);
                 if (ADA && p.mode == 0 && p.mask != nullptr) prefetch_mask(c0 + 32);
             }
             __syncwarp();                                       // tcgen05.ld / wait::ld are .sync.aligned
             if (fused_n) tmem_ld16x2_wait(taddr, taddr + p.bn, v, w);
             else tmem_ld16_wait(taddr, v);
+            if (!fused_epi) {                                   // split-K: raw partial sums, 16 consecutive days per thread
+                if (m < p.M) {
+                    float4* dst = reinterpret_cast<float4*>(
+                        p.part + (((size_t)blockIdx.z * gridDim.y + tt) * ((size_t)gridDim.x * kTileM) + m) * p.bn + c0);
+#pragma unroll
+                    for (int j = 0; j < 16; j += 4) {
+                        float4 o;
+                        o.x = nk ? __uint_as_float(v[j]) + (fused_n ? __uint_as_float(w[j]) : 0.f) : 0.f;
+                        o.y = nk ? __uint_as_float(v[j + 1]) + (fused_n ? __uint_as_float(w[j + 1]) : 0.f) : 0.f;
+                        o.z = nk ? __uint_as_float(v[j + 2]) + (fused_n ? __uint_as_float(w[j + 2]) : 0.f) : 0.f;
+                        o.w = nk ? __uint_as_float(v[j + 3]) + (fused_n ? __uint_as_float(w[j + 3]) : 0.f) : 0.f;
+                        dst[j >> 2] = o;
+                    }
+                }
+                continue;
+            }
             if (m < p.M) {
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
@@ -428,6 +453,41 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(tmem_cols) : "memory");
+    }
+}
+
+// Second half of a split-K pass: out[tt][m][d] = sum_ks part[ks][tt][m][d] in a fixed order, then the pass's epilogue
+// (the same arithmetic as the fused one).  Thread = (m, 4 days); grid = (ceil(Mt*bn/4 / 256), T).
+template <bool ADA>
+__global__ void __launch_bounds__(256)
+splitk_epilogue(const __grid_constant__ TcParams p, int Mt, const __grid_constant__ DayList dl) {
+    const int tt = blockIdx.y;
+    const int q4 = p.bn >> 2;
+    const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= (long)Mt * q4) return;
+    const int m = (int)(i / q4), d0 = (int)(i - (long)m * q4) * 4;
+    if (m >= p.M) return;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int ks = 0; ks < p.ksplit; ++ks) {
+        const float4 v = __ldcg(reinterpret_cast<const float4*>(p.part + (((size_t)ks * p.T + tt) * Mt + m) * p.bn + d0));
+        acc[0] += v.x; acc[1] += v.y; acc[2] += v.z; acc[3] += v.w;
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int d = d0 + e;
+        if (d >= dl.n) break;
+        if (p.mode == 0) {
+            float r = acc[e] - __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.M + m);
+            if (ADA && p.mask != nullptr && p.mask[((size_t)d * p.T + tt) * p.M + m] == 0) r = 0.f;
+            const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
+            p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
+            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - rhi;
+        } else {
+            const size_t qi = (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
+            const float qv = __ldcg(p.q + qi);
+            if (ADA && p.G != nullptr) p.q[qi] = adagrad_update(qv, acc[e], p.G + qi, p.eta, p.eps);
+            else p.q[qi] = fmaxf(0.f, fmaf(-p.eta, acc[e], qv));
+        }
     }
 }
 

@@ -294,3 +294,20 @@ def test_overlapped_steps_keep_day_order_and_join_orders_caller_work():
     q_cpu = hz.oracle_run(p, sched, etas)
     hz.assert_q_close(q_gpu, q_cpu, "lanes")
     g.close()
+
+
+@pytest.mark.parametrize("T,H,N,L,b", [(1, 0, 600, 520, 16), (2, 1, 300, 600, 40), (3, 4, 260, 200, 8)])
+def test_short_time_axis_split_k(T, H, N, L, b):
+    """Time axes too short to fill the machine (the Fig. 12 shape, T = 1): the tensor path splits K over several CTAs
+    per tile and finishes each pass in splitk_epilogue."""
+    cfg = synth.Config("splitk", N=N, L=L, T=T, H=H, C=2, D=4 * b, b=b, K=6, kmin=5, kmax=20)
+    _run_both(cfg)          # (the last chunk of the schedule may be a ragged one below 8 days, i.e. an FFMA step)
+
+
+@pytest.mark.parametrize("ks", [2, 5])
+def test_forced_split_k_on_ragged_shapes(ks, monkeypatch):
+    """Forced split counts on ragged shapes: K ranges that are empty near the day boundary, partial tiles, pad days; the
+    Adagrad variant goes through the same epilogue kernel."""
+    monkeypatch.setenv("DODE_TC_KSPLIT", str(ks))
+    cfg = synth.Config("ragged", N=61, L=137, T=20, H=5, C=2, D=80, b=20, K=12, kmin=3, kmax=9)
+    _run_both(cfg, sample=[0, 1, 40, 79])
