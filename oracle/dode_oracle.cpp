@@ -328,4 +328,61 @@ void oracle_dar_build(int N, int L, int T, int H, const int32_t* path_ptr, const
         }
 }
 
+// O8 (NEXT-4, second half): the assignment matrix B = delta * rho * p of one pattern (Eq. 41) with
+// several paths per OD and Logit route shares (Eq. 37):
+//   paths of OD n: od_ptr[n] .. od_ptr[n+1]);  links of path k: path_links[path_ptr[k] .. path_ptr[k+1]) in travel order;
+//   c_k(s) = travel time of path k for the vehicle leaving at the start of interval s (entry-interval speeds, reading
+//            A20; one speed table per pattern = the pattern's mean speeds, reading A22);
+//   p_k(s) = exp(-theta c_k(s)) / sum_{k' in K_n} exp(-theta c_k'(s))       (Eq. 37; constant within the interval, Eq. 38);
+//   R[s][h][l][n] = sum_{k in K_n} rho_k(s, s+h; l) p_k(s)                  (Eq. 41 summed over the OD's paths, as Eq. 40 does).
+// rho_k as in O7.  R is [T][H+1][L][N], zeroed here.
+void oracle_assignment_build(int N, int L, int T, int H, const int32_t* od_ptr, const int32_t* path_ptr,
+                             const int32_t* path_links, const float* len, const float* speed, double dt, double theta,
+                             float* R) {
+    const size_t total = (size_t)T * (H + 1) * L * N;
+    std::vector<double> acc(total, 0.0);
+    for (int s = 0; s < T; ++s)
+        for (int n = 0; n < N; ++n) {
+            const int k0 = od_ptr[n], k1 = od_ptr[n + 1];
+            // route shares from the leading vehicle's path travel times
+            std::vector<double> c(k1 - k0), pk(k1 - k0);
+            double cmin = 1e300;
+            for (int k = k0; k < k1; ++k) {
+                double t = (double)s * dt;
+                for (int j = path_ptr[k]; j < path_ptr[k + 1]; ++j) {
+                    const int l = path_links[j];
+                    const int i = std::min(T - 1, (int)std::floor(t / dt));
+                    t += (double)len[l] / (double)speed[(size_t)i * L + l];
+                }
+                c[k - k0] = t - (double)s * dt;
+                cmin = std::min(cmin, c[k - k0]);
+            }
+            double z = 0.0;
+            for (int k = k0; k < k1; ++k) { pk[k - k0] = std::exp(-theta * (c[k - k0] - cmin)); z += pk[k - k0]; }
+            for (int k = k0; k < k1; ++k) {
+                const double share = pk[k - k0] / z;
+                double a1 = (double)s * dt, a2 = (double)(s + 1) * dt;
+                for (int j = path_ptr[k]; j < path_ptr[k + 1]; ++j) {
+                    const int l = path_links[j];
+                    const int h_first = (int)std::floor(a1 / dt);
+                    if (a2 > a1) {
+                        const int h_last = (int)std::floor(a2 / dt);
+                        for (int h2 = h_first; h2 <= h_last; ++h2) {
+                            const double lo = std::max(a1, (double)h2 * dt), hi = std::min(a2, (double)(h2 + 1) * dt);
+                            if (hi <= lo) continue;
+                            const int h = h2 - s;
+                            if (h <= H && h2 < T) acc[(((size_t)s * (H + 1) + h) * L + l) * N + n] += share * (hi - lo) / (a2 - a1);
+                        }
+                    } else if (h_first - s <= H && h_first < T) {
+                        acc[(((size_t)s * (H + 1) + (h_first - s)) * L + l) * N + n] += share;
+                    }
+                    const int i1 = std::min(T - 1, (int)std::floor(a1 / dt)), i2 = std::min(T - 1, (int)std::floor(a2 / dt));
+                    a1 += (double)len[l] / (double)speed[(size_t)i1 * L + l];
+                    a2 += (double)len[l] / (double)speed[(size_t)i2 * L + l];
+                }
+            }
+        }
+    for (size_t i = 0; i < total; ++i) R[i] = (float)acc[i];
+}
+
 }  // extern "C"

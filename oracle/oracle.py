@@ -168,3 +168,17 @@ def dar_build(N: int, L: int, T: int, H: int, path_ptr, path_links, length, spee
                            length.ctypes.data_as(C.c_void_p), speed.ctypes.data_as(C.c_void_p), C.c_double(dt),
                            R.ctypes.data_as(C.c_void_p))
     return R
+
+
+def assignment_build(N: int, L: int, T: int, H: int, od_ptr, path_ptr, path_links, length, speed, dt: float,
+                     theta: float) -> np.ndarray:
+    """O8 (NEXT-4): B = delta * rho * p of one pattern, several paths per OD, Logit shares (Eq. 37, 41)."""
+    od_ptr = np.ascontiguousarray(od_ptr, dtype=np.int32); path_ptr = np.ascontiguousarray(path_ptr, dtype=np.int32)
+    path_links = np.ascontiguousarray(path_links, dtype=np.int32)
+    length = np.ascontiguousarray(length, dtype=np.float32); speed = np.ascontiguousarray(speed, dtype=np.float32)
+    assert od_ptr.shape == (N + 1,) and path_ptr.shape == (od_ptr[-1] + 1,) and length.shape == (L,) and speed.shape == (T, L)
+    R = np.empty((T, H + 1, L, N), np.float32)
+    vp = lambda a: a.ctypes.data_as(C.c_void_p)
+    lib().oracle_assignment_build(N, L, T, H, vp(od_ptr), vp(path_ptr), vp(path_links), vp(length), vp(speed),
+                                  C.c_double(dt), C.c_double(theta), vp(R))
+    return R

@@ -419,3 +419,46 @@ def test_p16_dar_conserves_vehicles_through_the_forward_operator():
     for l in range(L):
         users = [n for n, path in enumerate(paths) if l in path]
         np.testing.assert_allclose(x[:, l].sum(), q[:, users].sum(), rtol=1e-5)
+
+
+# ---- P17: assignment matrix with several paths per OD and Logit shares (O8, NEXT-4) ---------------------------------
+def test_p17_single_path_reduces_to_dar_and_logit_closed_form():
+    T, H, L, N, dt = 30, 10, 8, 2, 300.0
+    rng = np.random.default_rng(12)
+    length = rng.uniform(800, 2500, L).astype(np.float32)
+    speed = rng.uniform(6, 25, (T, L)).astype(np.float32)
+    # (a) one path per OD: p = 1 and O8 == O7 (Eq. 41 with p = 1)
+    paths = [[0, 1, 2, 3], [4, 5, 6]]
+    pp = np.cumsum([0] + [len(p) for p in paths]).astype(np.int32)
+    pl = np.concatenate(paths).astype(np.int32)
+    R7 = oracle.dar_build(N, L, T, H, pp, pl, length, speed, dt)
+    R8 = oracle.assignment_build(N, L, T, H, np.array([0, 1, 2], np.int32), pp, pl, length, speed, dt, 0.01)
+    np.testing.assert_array_equal(R7, R8)
+    # (b) one OD, two link-disjoint paths: the first links carry the route shares themselves, which follow the binary
+    #     Logit closed form p_1 = 1 / (1 + exp(-theta (c_2 - c_1))) with the travel times recomputed here (Eq. 37)
+    paths = [[0, 1, 2], [4, 5, 6, 7]]
+    pp = np.cumsum([0] + [len(p) for p in paths]).astype(np.int32)
+    pl = np.concatenate(paths).astype(np.int32)
+    theta = 0.01
+    R = oracle.assignment_build(1, L, T, H, np.array([0, 2], np.int32), pp, pl, length, speed, dt, theta)
+    for s in range(T):
+        c = []
+        for path in paths:
+            t = s * dt
+            for l in path:
+                t += float(length[l]) / float(speed[min(T - 1, int(t // dt)), l])
+            c.append(t - s * dt)
+        p1 = 1.0 / (1.0 + np.exp(-theta * (c[1] - c[0])))
+        assert abs(R[s, 0, 0, 0] - p1) < 1e-6 and abs(R[s, 0, 4, 0] - (1 - p1)) < 1e-6
+    # (c) theta = 0: equal shares; a huge theta: all flow on the faster path
+    R0 = oracle.assignment_build(1, L, T, H, np.array([0, 2], np.int32), pp, pl, length, speed, dt, 0.0)
+    np.testing.assert_allclose(R0[:, 0, 0, 0], 0.5); np.testing.assert_allclose(R0[:, 0, 4, 0], 0.5)
+    Rinf = oracle.assignment_build(1, L, T, H, np.array([0, 2], np.int32), pp, pl, length, speed, dt, 50.0)
+    assert set(np.unique(np.round(Rinf[:, 0, 0, 0], 6))) <= {0.0, 1.0}
+    # (d) two paths sharing a link: the shared link's shares add up (Eq. 40 sums over k), conservation holds on it
+    paths = [[0, 1, 2], [3, 1, 5]]
+    pp = np.cumsum([0] + [len(p) for p in paths]).astype(np.int32)
+    pl = np.concatenate(paths).astype(np.int32)
+    Rs = oracle.assignment_build(1, L, T, H, np.array([0, 2], np.int32), pp, pl, length, speed, dt, theta)
+    np.testing.assert_allclose(Rs[:T - H - 1, :, 1, 0].sum(axis=1), 1.0, atol=1e-6)
+    np.testing.assert_allclose(Rs[:T - H - 1, 0, 0, 0] + Rs[:T - H - 1, 0, 3, 0], 1.0, atol=1e-6)
