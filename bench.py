@@ -406,8 +406,20 @@ def run_dar_build(args, cfg, local_rank):
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
     DT = 300.0
-    ptr, links, length = synth.network(cfg)
+    multipath = args.paths > 1
+    if multipath:       # several paths per OD, Logit route shares (Eq. 37, theta per second): dode_assignment_build
+        od, ptr, links, length = synth.network_multipath(cfg, args.paths)
+        od_d = od.to(dev)
+    else:
+        ptr, links, length = synth.network(cfg)
     ptr_d, links_d, len_d = ptr.to(dev), links.to(dev), length.to(dev)
+
+    def build(v, out):
+        if multipath:
+            P.dode_assignment_build(cfg.N, cfg.L, cfg.T, cfg.H, od_d, ptr_d, links_d, len_d, v, DT, args.theta, out)
+        else:
+            P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, v, DT, out)
+
     vs = [synth.speeds(cfg, c).pin_memory() for c in range(cfg.C)]
     vd = [v.to(dev) for v in vs]
     nbytes = 4.0 * cfg.T * (cfg.H + 1) * cfg.L * cfg.N
@@ -415,7 +427,7 @@ def run_dar_build(args, cfg, local_rank):
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
     sampler = ClockSampler(local_rank)
     for i in range(max(3, args.warmup)):
-        P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, vd[i % cfg.C], DT, R)
+        build(vd[i % cfg.C], R)
     torch.cuda.synchronize()
     sampler.start()
     ev = []
@@ -423,7 +435,7 @@ def run_dar_build(args, cfg, local_rank):
         flush.zero_()
         a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, vd[i % cfg.C], DT, R)
+        build(vd[i % cfg.C], R)
         z.record()
         ev.append((a, z))
     torch.cuda.synchronize()
@@ -440,7 +452,7 @@ def run_dar_build(args, cfg, local_rank):
         t0 = time.perf_counter()
         for i in range(args.e2e_steps):
             vtmp.copy_(vs[i % cfg.C], non_blocking=True)
-            P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr_d, links_d, len_d, vtmp, DT, R)
+            build(vtmp, R)
             R_host.copy_(R, non_blocking=True)
         torch.cuda.synchronize()
         e2e = {"value": (time.perf_counter() - t0) * 1e3 / args.e2e_steps, "unit": "ms/pattern",
@@ -451,8 +463,9 @@ def run_dar_build(args, cfg, local_rank):
     out = {"metric": "dar_build_time_per_pattern", "value": ms, "unit": "ms/pattern", "n_gpus": 1, "steps": args.steps,
            "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64 times / f32 shares", "data": "synthetic",
-           "config": {"workload": f"dar_build on {cfg.name}: N={cfg.N} L={cfg.L} T={cfg.T} H={cfg.H}, one path per OD "
-                                  f"({int(ptr[-1])} path links), |H| = 300 s",
+           "config": {"workload": f"dar_build on {cfg.name}: N={cfg.N} L={cfg.L} T={cfg.T} H={cfg.H}, "
+                                  + (f"1-{args.paths} paths per OD, Logit theta={args.theta} " if multipath else "one path per OD ")
+                                  + f"({int(ptr[-1])} path links), |H| = 300 s",
                       "l2": "L2 flushed (256 MiB write) before every timed build"},
            "nnz": nnz, "gpu_launches": args.steps * 2, "clocks": sampler.summary(),
            "roofline": {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
@@ -464,7 +477,10 @@ def run_dar_build(args, cfg, local_rank):
         Tc = cfg.T if nbytes < 1.5e9 else max(1, int(cfg.T * 1.5e9 / nbytes))      # bounded sample: the first Tc intervals
         v0 = vs[0][:Tc].numpy()
         t0 = time.perf_counter()
-        oracle.dar_build(cfg.N, cfg.L, Tc, cfg.H, ptr.numpy(), links.numpy(), length.numpy(), v0, DT)
+        if multipath:
+            oracle.assignment_build(cfg.N, cfg.L, Tc, cfg.H, od.numpy(), ptr.numpy(), links.numpy(), length.numpy(), v0, DT, args.theta)
+        else:
+            oracle.dar_build(cfg.N, cfg.L, Tc, cfg.H, ptr.numpy(), links.numpy(), length.numpy(), v0, DT)
         cpu_ms = (time.perf_counter() - t0) * 1e3 * cfg.T / Tc
         out["cpu_baseline"] = {"value": cpu_ms, "unit": "ms/pattern", "cores": 1, "kind": "oracle",
                                "sample": f"O7 on the first {Tc} of {cfg.T} departure intervals, extrapolated x{cfg.T / Tc:.1f}"}
@@ -484,6 +500,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-visits", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--paths", type=int, default=1, help="--dar-build: up to this many paths per OD with Logit route shares (Eq. 37)")
+    ap.add_argument("--theta", type=float, default=0.01, help="--dar-build --paths K: Logit dispersion factor per second (SURVEY NEXT-4)")
     ap.add_argument("--dar-build", action="store_true", help="NEXT-4: time dode_dar_build on the workload's network instead of SPGD")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

@@ -153,6 +153,18 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out);
 int dode_dar_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* path_ptr, const int32_t* path_links,
                    const float* link_len, const float* speed, double dt, float* R_out, void* stream);
 
+/* NEXT-4, with route choice: the assignment matrix B = delta * rho * p of one pattern (Eq. 41) for
+ * several paths per OD and Logit route shares p_k(s) = exp(-theta c_k(s)) / sum_k' exp(-theta c_k'(s)) (Eq. 37,
+ * PAPER.md:309-312), c_k(s) = travel time of path k for the vehicle leaving at the start of interval s, from the
+ * pattern's speeds.  R_out[s][h][l][n] = sum over the OD's paths k of rho_k(s, s+h; l) p_k(s).
+ *   od_ptr    device int32 [N+1]   paths of OD n: od_ptr[n] .. od_ptr[n+1])  (at least one each)
+ *   path_ptr  device int32 [P+1], path_links, link_len, speed, dt, R_out, stream: as dode_dar_build, P = od_ptr[N]
+ *   theta     Logit dispersion factor, >= 0 (per second of travel time)
+ * With one path per OD this is dode_dar_build. */
+int dode_assignment_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* od_ptr, const int32_t* path_ptr,
+                          const int32_t* path_links, const float* link_len, const float* speed, double dt, double theta,
+                          float* R_out, void* stream);
+
 /* Optional per-kernel timing for roofline reports: while enabled, every forward (kind 0) and
  * gradient+update (kind 1) launch is bracketed by CUDA events on the ctx stream.  dode_timing_read
  * synchronises, folds finished event pairs into the running totals and returns the total device

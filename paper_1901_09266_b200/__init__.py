@@ -19,7 +19,7 @@ SO_PATH = os.path.join(_HERE, "libdode.so")
 DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
 DODE_DENSE, DODE_CSR = 0, 1
 
-EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
+EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
            "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
@@ -58,6 +58,7 @@ def lib():
         L.dode_adagrad_reset.argtypes = [vp]
         L.dode_join.argtypes = [vp]
         L.dode_dar_build.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, C.c_double, vp, vp]
+        L.dode_assignment_build.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, C.c_double, C.c_double, vp, vp]
         L.dode_objective.argtypes = [vp, vp, i32, vp, vp]
         L.dode_get_q.argtypes = [vp, i32, vp, i32]
         L.dode_set_q.argtypes = [vp, i32, vp, i32]
@@ -150,6 +151,23 @@ def dode_dar_build(N: int, L: int, T: int, H: int, path_ptr, path_links, link_le
     rc = lib().dode_dar_build(N, L, T, H, C.c_void_p(path_ptr.data_ptr()), C.c_void_p(path_links.data_ptr()),
                               C.c_void_p(link_len.data_ptr()), C.c_void_p(speed.data_ptr()), C.c_double(dt),
                               C.c_void_p(R_out.data_ptr()), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != DODE_OK:
+        raise DodeError(rc, lib().dode_last_error(None).decode())
+
+
+def dode_assignment_build(N: int, L: int, T: int, H: int, od_ptr, path_ptr, path_links, link_len, speed, dt: float,
+                          theta: float, R_out) -> None:
+    """NEXT-4 with route choice: B = delta*rho*p [T][H+1][L][N] of one pattern, several paths per OD, Logit shares
+    (Eq. 37, 41).  All tensors on the GPU (int32 / float32); R_out is overwritten.  Asynchronous."""
+    import torch
+    for t, dt_ in ((od_ptr, torch.int32), (path_ptr, torch.int32), (path_links, torch.int32), (link_len, torch.float32),
+                   (speed, torch.float32), (R_out, torch.float32)):
+        assert t.is_cuda and t.dtype == dt_ and t.is_contiguous()
+    assert od_ptr.numel() == N + 1 and link_len.numel() == L and speed.shape == (T, L) and R_out.numel() == T * (H + 1) * L * N
+    rc = lib().dode_assignment_build(N, L, T, H, C.c_void_p(od_ptr.data_ptr()), C.c_void_p(path_ptr.data_ptr()),
+                                     C.c_void_p(path_links.data_ptr()), C.c_void_p(link_len.data_ptr()),
+                                     C.c_void_p(speed.data_ptr()), C.c_double(dt), C.c_double(theta),
+                                     C.c_void_p(R_out.data_ptr()), C.c_void_p(torch.cuda.current_stream().cuda_stream))
     if rc != DODE_OK:
         raise DodeError(rc, lib().dode_last_error(None).decode())
 

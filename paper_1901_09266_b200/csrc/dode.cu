@@ -995,11 +995,14 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
     return DODE_OK;
 }
 
-int dode_dar_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* path_ptr, const int32_t* path_links,
-                   const float* link_len, const float* speed, double dt, float* R_out, void* stream) {
+// shared by dode_dar_build (od_ptr == nullptr: one path per OD, p = 1) and dode_assignment_build
+static int build_operator(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* od_ptr, const int32_t* path_ptr,
+                          const int32_t* path_links, const float* link_len, const float* speed, double dt, double theta,
+                          float* R_out, void* stream) {
     dode_ctx* ctx = nullptr;                   // no ctx: errors go to the thread-local buffer (dode_last_error(NULL))
     if (N < 1 || L < 1 || T < 1 || H < 0 || !(dt > 0.0)) return fail(ctx, DODE_EINVAL, "dims must be positive and dt > 0");
     if (!path_ptr || !path_links || !link_len || !speed || !R_out) return fail(ctx, DODE_EINVAL, "null argument");
+    if (!(theta >= 0.0)) return fail(ctx, DODE_EINVAL, "theta must be >= 0");
     int dev = 0, major = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
@@ -1010,9 +1013,24 @@ int dode_dar_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* pa
     CU(cudaMemsetAsync(R_out, 0, bytes, st));
     const long total = (long)T * N;
     const int blocks = (int)std::min<long>((total + 255) / 256, 148L * 16);
-    dar_build_dense<<<blocks, 256, 0, st>>>(N, L, T, H, path_ptr, path_links, link_len, speed, dt, R_out);
+    if (od_ptr)
+        assignment_build_dense<<<blocks, 256, 0, st>>>(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, R_out);
+    else
+        dar_build_dense<<<blocks, 256, 0, st>>>(N, L, T, H, path_ptr, path_links, link_len, speed, dt, R_out);
     CU(cudaGetLastError());
     return DODE_OK;
+}
+
+int dode_dar_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* path_ptr, const int32_t* path_links,
+                   const float* link_len, const float* speed, double dt, float* R_out, void* stream) {
+    return build_operator(N, L, T, H, nullptr, path_ptr, path_links, link_len, speed, dt, 0.0, R_out, stream);
+}
+
+int dode_assignment_build(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* od_ptr, const int32_t* path_ptr,
+                          const int32_t* path_links, const float* link_len, const float* speed, double dt, double theta,
+                          float* R_out, void* stream) {
+    if (!od_ptr) return fail(nullptr, DODE_EINVAL, "od_ptr is null");
+    return build_operator(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, R_out, stream);
 }
 
 int dode_timing_enable(dode_ctx* ctx, int32_t on) {

@@ -45,4 +45,62 @@ dar_build_dense(int N, int L, int T, int H, const int32_t* __restrict__ path_ptr
     }
 }
 
+// Travel time of path k for the vehicle that leaves at time t0 (entry-interval speeds).
+__device__ __forceinline__ double path_travel_time(int k, double t0, int L, int T, double dt, const int32_t* __restrict__ path_ptr,
+                                                   const int32_t* __restrict__ path_links, const float* __restrict__ len,
+                                                   const float* __restrict__ speed) {
+    double t = t0;
+    const int j1 = __ldg(path_ptr + k + 1);
+    for (int j = __ldg(path_ptr + k); j < j1; ++j) {
+        const int l = __ldg(path_links + j);
+        const int i = min(T - 1, (int)floor(t / dt));
+        t += (double)__ldg(len + l) / (double)__ldg(speed + (size_t)i * L + l);
+    }
+    return t - t0;
+}
+
+// B = delta * rho * p (Eq. 41) with several paths per OD and Logit route shares (Eq. 37,
+// PAPER.md:309-312): thread (s, n) first evaluates the path travel times c_k(s) of the OD's paths for the vehicle leaving
+// at s dt (three cheap walks instead of a per-thread array: min, normaliser, share), then walks every path once more
+// as dar_build_dense does and ADDS share * rho into R[s][h][l][n] — only this thread touches column (s, n), so the
+// accumulation over paths that share a link needs no atomics and is deterministic.  R zero-filled by the caller.
+__global__ void __launch_bounds__(256)
+assignment_build_dense(int N, int L, int T, int H, const int32_t* __restrict__ od_ptr, const int32_t* __restrict__ path_ptr,
+                       const int32_t* __restrict__ path_links, const float* __restrict__ len,
+                       const float* __restrict__ speed, double dt, double theta, float* __restrict__ R) {
+    const long total = (long)T * N;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+        const int s = (int)(i / N), n = (int)(i - (long)s * N);
+        const int k0 = __ldg(od_ptr + n), k1 = __ldg(od_ptr + n + 1);
+        const double t0 = (double)s * dt;
+        double cmin = 1e300, z = 0.0;
+        for (int k = k0; k < k1; ++k) cmin = fmin(cmin, path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed));
+        for (int k = k0; k < k1; ++k) z += exp(-theta * (path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed) - cmin));
+        for (int k = k0; k < k1; ++k) {
+            const double share = exp(-theta * (path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed) - cmin)) / z;
+            double a1 = t0, a2 = (double)(s + 1) * dt;
+            const int j1 = __ldg(path_ptr + k + 1);
+            for (int j = __ldg(path_ptr + k); j < j1; ++j) {
+                const int l = __ldg(path_links + j);
+                const int h_first = (int)floor(a1 / dt);
+                if (a2 > a1) {
+                    const int h_last = (int)floor(a2 / dt);
+                    const double inv = share / (a2 - a1);
+                    for (int h2 = h_first; h2 <= h_last; ++h2) {
+                        const double lo = fmax(a1, (double)h2 * dt), hi = fmin(a2, (double)(h2 + 1) * dt);
+                        const int h = h2 - s;
+                        if (hi > lo && h <= H && h2 < T) R[(((size_t)s * (H + 1) + h) * L + l) * N + n] += (float)((hi - lo) * inv);
+                    }
+                } else if (h_first - s <= H && h_first < T) {
+                    R[(((size_t)s * (H + 1) + (h_first - s)) * L + l) * N + n] += (float)share;
+                }
+                const int i1 = min(T - 1, h_first), i2 = min(T - 1, (int)floor(a2 / dt));
+                const double ll = (double)__ldg(len + l);
+                a1 += ll / (double)__ldg(speed + (size_t)i1 * L + l);
+                a2 += ll / (double)__ldg(speed + (size_t)i2 * L + l);
+            }
+        }
+    }
+}
+
 }  // namespace dode

@@ -32,7 +32,7 @@ MASTER_SEED = 20190129  # the paper's arXiv date; arbitrary
 # stream ids (one per generated array)
 S_INC_K, S_INC_START, S_DAR, S_BASE, S_DAYF, S_NOISE, S_LABEL, S_RELABEL = range(1, 9)
 S_SCHED, S_TAU, S_WIN, S_SPFRAC, S_PROBE = range(9, 14)
-S_LEN, S_VFREE, S_CONG, S_VNOISE = range(14, 18)
+S_LEN, S_VFREE, S_CONG, S_VNOISE, S_NPATH = range(14, 19)
 
 _MASK64 = (1 << 64) - 1
 
@@ -223,6 +223,32 @@ def network(cfg: Config, device="cpu"):
     l = torch.arange(cfg.L, dtype=torch.int64, device=device)
     length = 500.0 + 2500.0 * uniform01(cfg.seed, S_LEN, l)
     return ptr.to(torch.int32), links.to(torch.int32), length.to(torch.float32)
+
+
+def network_multipath(cfg: Config, kpaths: int = 3, device="cpu"):
+    """(od_ptr int32 [N+1], path_ptr int32 [P+1], path_links int32, link_len fp32 [L]): OD n has 1..kpaths paths; path 0
+    is its G2 link run, the others are link runs drawn independently with the same rule (a stand-in for the path set
+    that "needs to be generated prior to the estimation framework", PAPER.md:422)."""
+    n = torch.arange(cfg.N, dtype=torch.int64, device=device)
+    cnt = randint(cfg.seed, S_NPATH, n, 1, kpaths)
+    od_ptr = torch.zeros(cfg.N + 1, dtype=torch.int64, device=device)
+    od_ptr[1:] = torch.cumsum(cnt, 0)
+    P = int(od_ptr[-1])
+    pid = torch.arange(P, dtype=torch.int64, device=device)
+    owner = torch.searchsorted(od_ptr[1:].contiguous(), pid, right=True)
+    alt = pid - od_ptr[owner]                                   # 0 = the OD's G2 path
+    key = owner + alt * cfg.N                                   # distinct draw per (OD, alternative); alt 0 == G2's index
+    k = randint(cfg.seed, S_INC_K, key, cfg.kmin, min(cfg.kmax, cfg.L))
+    u = _lsr(mix64(cfg.seed, S_INC_START, key), 32)
+    start = (u * (cfg.L - k + 1)) >> 32
+    path_ptr = torch.zeros(P + 1, dtype=torch.int64, device=device)
+    path_ptr[1:] = torch.cumsum(k, 0)
+    j = torch.arange(int(path_ptr[-1]), dtype=torch.int64, device=device)
+    po = torch.searchsorted(path_ptr[1:].contiguous(), j, right=True)
+    links = start[po] + (j - path_ptr[po])
+    l = torch.arange(cfg.L, dtype=torch.int64, device=device)
+    length = 500.0 + 2500.0 * uniform01(cfg.seed, S_LEN, l)
+    return od_ptr.to(torch.int32), path_ptr.to(torch.int32), links.to(torch.int32), length.to(torch.float32)
 
 
 def speeds(cfg: Config, c: int = 0, device="cpu") -> torch.Tensor:

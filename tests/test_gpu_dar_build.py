@@ -78,3 +78,29 @@ def test_built_operator_through_the_spgd_path():
         P.dode_get_q(h, d, out[d])
     hz.assert_q_close(out.numpy(), hz.oracle_run(p, sched, etas), "dar_e2e")
     P.dode_destroy(h)
+
+
+@pytest.mark.parametrize("shape,theta", [((61, 37, 50, 5), 0.01), ((60, 120, 96, 12), 0.002), ((9, 12, 20, 8), 0.0)])
+def test_assignment_build_multipath_logit_matches_oracle(shape, theta):
+    """B = delta*rho*p with 1-3 paths per OD and Logit shares (Eq. 37, 41) against the oracle's O8 (pin P17)."""
+    from oracle import oracle
+    N, L, T, H = shape
+    cfg = synth.Config("asg", N=N, L=L, T=T, H=H, C=2, D=4, b=2, K=1, kmin=2, kmax=min(12, L))
+    od, pp, pl, length = synth.network_multipath(cfg, 3)
+    assert int(od[-1]) > N                                           # some OD has more than one path
+    for c in range(cfg.C):
+        v = synth.speeds(cfg, c)
+        want = oracle.assignment_build(N, L, T, H, od.numpy(), pp.numpy(), pl.numpy(), length.numpy(), v.numpy(), DT, theta)
+        R = torch.full((T, H + 1, L, N), 3.0, device="cuda")
+        P.dode_assignment_build(N, L, T, H, od.cuda(), pp.cuda(), pl.cuda(), length.cuda(), v.cuda(), DT, theta, R)
+        got = R.cpu().numpy()
+        np.testing.assert_array_equal(got != 0, want != 0)
+        np.testing.assert_allclose(got, want, rtol=0, atol=2e-6)
+    # one path per OD through the multi-path entry point == dode_dar_build
+    ptr, links, length1 = synth.network(cfg)
+    ident = torch.arange(N + 1, dtype=torch.int32)
+    Ra = torch.empty((T, H + 1, L, N), device="cuda"); Rb = torch.empty_like(Ra)
+    v = synth.speeds(cfg, 0).cuda()
+    P.dode_assignment_build(N, L, T, H, ident.cuda(), ptr.cuda(), links.cuda(), length1.cuda(), v, DT, theta, Ra)
+    P.dode_dar_build(N, L, T, H, ptr.cuda(), links.cuda(), length1.cuda(), v, DT, Rb)
+    np.testing.assert_allclose(Ra.cpu().numpy(), Rb.cpu().numpy(), rtol=0, atol=1e-7)
