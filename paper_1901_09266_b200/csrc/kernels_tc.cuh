@@ -262,6 +262,20 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     // Programmatic dependent launch: everything above overlapped the previous kernel's tail.  The next kernel in
     // the stream may start its own prologue now; nothing produced by the previous kernel is touched before the wait.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // The operator is static: the A tiles of the first ring round are requested NOW, before the dependency wait — a CTA
+    // that gets its SM slot while the previous kernel's slower CTAs are still running streams its first `stages` chunks
+    // under that kernel's tail.  The B tiles (panels written by the previous kernel) follow after the wait; the stage's
+    // barrier expects the bytes of all three loads from the start.
+    const int npre = min(p.stages, nk);
+    if (warp == 0 && !(p.dbg & 16)) {
+        if (elect_one()) {
+            for (int kc = 0; kc < npre; ++kc) {
+                mbar_expect_tx(&full[kc], aBytes + 2 * bBytes);
+                tma_load_3d(smem + (size_t)kc * stageBytes, mA, &full[kc], m0, (kbase + kc) * kTileK, p.slab0 + tt);
+            }
+        }
+        __syncwarp();
+    }
     // Epilogue operands (x for the forward pass, the old q for the update) are fetched by the epilogue threads
     // BEFORE the main loop so that their DRAM/L2 latency is hidden behind it: 16 values per thread.
     float pre[16];
@@ -307,8 +321,10 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             TC_TRACE(0, kc, 1);
             if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
-                mbar_expect_tx(&full[s], aBytes + 2 * bBytes);
-                tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
+                if (kc >= npre || (p.dbg & 16)) {               // (the first round's A tiles were requested before the wait)
+                    mbar_expect_tx(&full[s], aBytes + 2 * bBytes);
+                    tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
+                }
                 tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
                 tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
             }
