@@ -81,6 +81,8 @@ struct dode_ctx {
     std::vector<int8_t> day_last_lane;             // [D] and its lane (-1: none)
     long rpitch = 0;
     int tc_min_b = 8;
+    // bring-up / experiment knobs, read from the environment once at dode_create (0 = off)
+    int knob_occ1 = 0, knob_stages = 0, knob_dbg = 0, knob_ksplit = 0;
     bool tc_ready = false, tc_attr = false;
     CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64;
     // streaming steps (dode_spgd_step_host): copy streams, staging buffers, ping-pong events
@@ -180,6 +182,9 @@ template <int BT, int EPI>
 static int launch_band(dode_ctx* ctx, int slot, const BandArgs& a, int nbt, const DayList& dl, int kind) {
     int cwlog2 = 0;
     while ((1 << cwlog2) < a.M4 && cwlog2 < 5) ++cwlog2;
+    // short time axes (T = 1 on the Fig. 12 shape): narrower column groups give more CTAs; 8 column threads still read
+    // whole 128-byte lines per K row
+    while (cwlog2 > 2 && (long)ceil_div(a.M4, 1 << cwlog2) * a.T * nbt < 2 * 148) --cwlog2;
     const size_t smem = (size_t)kThreads * 4 * BT * sizeof(float);
     if (smem > 48 * 1024 && !ctx->sm_opt_in[slot]) {
         CU(cudaFuncSetAttribute(band_coldot<BT, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -399,8 +404,8 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
         stages = (226 * 1024 - fixed) / stageBytes;
         nring = acc_cols + 256 <= 512 ? 4 : 2;
     }
-    if (const char* e = getenv("DODE_TC_OCC1")) if (atoi(e)) { stages = (226 * 1024 - fixed) / stageBytes; nring = acc_cols + 256 <= 512 ? 4 : 2; }
-    if (const char* e = getenv("DODE_TC_STAGES")) if (atoi(e) > 1) stages = std::min(stages, atoi(e));
+    if (ctx->knob_occ1) { stages = (226 * 1024 - fixed) / stageBytes; nring = acc_cols + 256 <= 512 ? 4 : 2; }
+    if (ctx->knob_stages > 1) stages = std::min(stages, ctx->knob_stages);
     stages = std::max(2, std::min(stages, 10));
     const size_t smem = (size_t)stages * stageBytes + fixed;
     {
@@ -415,7 +420,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = tb.rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
-    { const char* e = getenv("DODE_TC_DBG"); p.dbg = e ? atoi(e) : 0; }
+    p.dbg = ctx->knob_dbg;
     const bool ada = opt.mask || opt.G;
     auto kern = ada ? tc::banded_gemm_3xtf32<true> : tc::banded_gemm_3xtf32<false>;
     // split-K when the time axis is too short to fill the machine (T * tiles CTAs for 148 SMs x 1-2 CTAs): e.g. the
@@ -425,7 +430,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
         const long ctas = (long)ceil_div(M, tc::kTileM) * d.T;
         const int nk_max = ceil_div((long)(d.H + 1) * kunit, tc::kTileK);
         int ks = (int)std::min<long>(slots / std::max<long>(ctas, 1), nk_max / 8);
-        if (const char* e = getenv("DODE_TC_KSPLIT")) ks = atoi(e);
+        if (ctx->knob_ksplit > 0) ks = ctx->knob_ksplit;
         return std::max(1, std::min(ks, 32));
     };
     const int ks_f = pick_split(d.L, ctx->Np), ks_g = pick_split(d.N, ctx->Lp);
@@ -627,6 +632,10 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     c->day_last_id.assign(d.D, 0);
     c->day_last_lane.assign(d.D, -1);
     if (const char* e = getenv("DODE_LANES")) c->lanes_on = atoi(e) != 0;
+    if (const char* e = getenv("DODE_TC_OCC1")) c->knob_occ1 = atoi(e);
+    if (const char* e = getenv("DODE_TC_STAGES")) c->knob_stages = atoi(e);
+    if (const char* e = getenv("DODE_TC_DBG")) c->knob_dbg = atoi(e);
+    if (const char* e = getenv("DODE_TC_KSPLIT")) c->knob_ksplit = atoi(e);
     ctx = c;
 #define CUC(call)                                                                                          \
     do {                                                                                                   \
@@ -815,7 +824,6 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
     CU(sync_all(ctx));                        // pending streamed uploads of x belong to the state being evaluated
     // group positions by cluster, evaluate in sub-batches; d_obj[i] receives f of days[i]
     constexpr int kObjBatch = 64;
-    const size_t dayStride = (size_t)d.T * ctx->Np;
     const long rows = (long)d.T * ctx->Lp;
     const int rowsPerBlock = 2048, nchunks = ceil_div(rows, rowsPerBlock);
     if (ctx->part_cap < (size_t)nchunks * kObjBatch) {
