@@ -111,6 +111,16 @@ def job_day_steps_per_s(D: int, world: int, epoch_ms: float) -> float:
     return D * world / (epoch_ms * 1e-3)
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def make_epochs(cfg, lab, b, count):
     rng = synth._Counter(cfg.seed, synth.S_SCHED)
     return [synth.epoch_chunks(np.asarray(lab, np.int64), b, rng) for _ in range(count)]
@@ -323,7 +333,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
                 "frac": tfl / FP32_PEAK_TFLOPS, "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)"}
     roof.update({"kernel": kname, "launches": int(d_n), "avg_launch_ms": d_ms / max(1, d_n),
                  "traffic": traffic_from_profiles(cfg.name, dom),
-                 "other": {"hbm_GBps": gbs, "hbm_frac": gbs / hbm_peak, "fp32_TFLOPs": tfl,
+                 "other": {"hbm_GBps": gbs, "hbm_frac": gbs / hbm_peak, "hbm_frac_of_nominal_8TBps": gbs / 8000.0, "fp32_TFLOPs": tfl,
                            "fp32_frac": tfl / FP32_PEAK_TFLOPS,
                            "forward_ms_total": fwd_ms, "gradient_update_ms_total": grad_ms,
                            "step_GBps_algorithmic": (fb + gb) / (total_ms * 1e-3) / 1e9,
@@ -382,6 +392,9 @@ def run_ours(args, cfg, b, rank, world, local_rank):
                "sample": f"{visits} day-visits of the {cfg.D}-visit epoch timed single-threaded on this host "
                          f"({os.cpu_count()} cores visible), extrapolated x{cfg.D / visits:.1f}",
                "ms_per_day_visit": ms_visit}
+    if cpu is not None:
+        cpu["cpu_model"] = cpu_model()
+        cpu["nproc"] = os.cpu_count()
     out = {"metric": METRIC, "value": epoch_ms, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": epoch_ms, "higher_is_better": False, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, b),

@@ -1020,11 +1020,13 @@ static int build_operator(int32_t N, int32_t L, int32_t T, int32_t H, const int3
     const size_t bytes = (size_t)T * (H + 1) * L * N * sizeof(float);
     CU(cudaMemsetAsync(R_out, 0, bytes, st));
     const long total = (long)T * N;
-    const int blocks = (int)std::min<long>((total + 255) / 256, 148L * 16);
+    // few, long, dependent double-precision walks per thread: small blocks spread them over all SMs
+    const int threads = 64;
+    const int blocks = (int)std::min<long>((total + threads - 1) / threads, 148L * 64);
     if (od_ptr)
-        assignment_build_dense<<<blocks, 256, 0, st>>>(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, R_out);
+        assignment_build_dense<<<blocks, threads, 0, st>>>(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, R_out);
     else
-        dar_build_dense<<<blocks, 256, 0, st>>>(N, L, T, H, path_ptr, path_links, link_len, speed, dt, R_out);
+        dar_build_dense<<<blocks, threads, 0, st>>>(N, L, T, H, path_ptr, path_links, link_len, speed, dt, R_out);
     CU(cudaGetLastError());
     return DODE_OK;
 }

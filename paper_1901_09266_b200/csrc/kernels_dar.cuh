@@ -61,9 +61,11 @@ __device__ __forceinline__ double path_travel_time(int k, double t0, int L, int 
 
 // B = delta * rho * p (Eq. 41) with several paths per OD and Logit route shares (Eq. 37,
 // PAPER.md:309-312): thread (s, n) first evaluates the path travel times c_k(s) of the OD's paths for the vehicle leaving
-// at s dt (three cheap walks instead of a per-thread array: min, normaliser, share), then walks every path once more
-// as dar_build_dense does and ADDS share * rho into R[s][h][l][n] — only this thread touches column (s, n), so the
-// accumulation over paths that share a link needs no atomics and is deterministic.  R zero-filled by the caller.
+// at s dt (kept in registers for up to 8 paths, re-walked beyond that), then walks every path once more
+// as dar_build_dense does and ADDS share * rho into R[s][h][l][n].  Only this thread touches column (s, n), so the
+// accumulation over paths that share a link is deterministic; the adds are issued as fire-and-forget reductions
+// (atomicAdd with the result unused -> RED) because a plain `+=` is a dependent global load per entry and made the
+// kernel a chain of memory latencies.  R zero-filled by the caller.
 __global__ void __launch_bounds__(256)
 assignment_build_dense(int N, int L, int T, int H, const int32_t* __restrict__ od_ptr, const int32_t* __restrict__ path_ptr,
                        const int32_t* __restrict__ path_links, const float* __restrict__ len,
@@ -73,11 +75,21 @@ assignment_build_dense(int N, int L, int T, int H, const int32_t* __restrict__ o
         const int s = (int)(i / N), n = (int)(i - (long)s * N);
         const int k0 = __ldg(od_ptr + n), k1 = __ldg(od_ptr + n + 1);
         const double t0 = (double)s * dt;
+        constexpr int kCache = 8;                  // travel times of up to 8 paths stay in registers; beyond that they are re-walked
+        double cc[kCache];
+        const bool cached = k1 - k0 <= kCache;
+        auto ctime = [&](int k) {
+            return cached ? cc[k - k0] : path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed);
+        };
         double cmin = 1e300, z = 0.0;
-        for (int k = k0; k < k1; ++k) cmin = fmin(cmin, path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed));
-        for (int k = k0; k < k1; ++k) z += exp(-theta * (path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed) - cmin));
         for (int k = k0; k < k1; ++k) {
-            const double share = exp(-theta * (path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed) - cmin)) / z;
+            const double c = path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed);
+            if (cached) cc[k - k0] = c;
+            cmin = fmin(cmin, c);
+        }
+        for (int k = k0; k < k1; ++k) z += exp(-theta * (ctime(k) - cmin));
+        for (int k = k0; k < k1; ++k) {
+            const double share = exp(-theta * (ctime(k) - cmin)) / z;
             double a1 = t0, a2 = (double)(s + 1) * dt;
             const int j1 = __ldg(path_ptr + k + 1);
             for (int j = __ldg(path_ptr + k); j < j1; ++j) {
@@ -89,10 +101,11 @@ assignment_build_dense(int N, int L, int T, int H, const int32_t* __restrict__ o
                     for (int h2 = h_first; h2 <= h_last; ++h2) {
                         const double lo = fmax(a1, (double)h2 * dt), hi = fmin(a2, (double)(h2 + 1) * dt);
                         const int h = h2 - s;
-                        if (hi > lo && h <= H && h2 < T) R[(((size_t)s * (H + 1) + h) * L + l) * N + n] += (float)((hi - lo) * inv);
+                        if (hi > lo && h <= H && h2 < T)
+                            atomicAdd(R + (((size_t)s * (H + 1) + h) * L + l) * N + n, (float)((hi - lo) * inv));
                     }
                 } else if (h_first - s <= H && h_first < T) {
-                    R[(((size_t)s * (H + 1) + (h_first - s)) * L + l) * N + n] += (float)share;
+                    atomicAdd(R + (((size_t)s * (H + 1) + (h_first - s)) * L + l) * N + n, (float)share);
                 }
                 const int i1 = min(T - 1, h_first), i2 = min(T - 1, (int)floor(a2 / dt));
                 const double ll = (double)__ldg(len + l);
