@@ -135,7 +135,8 @@ struct TcParams {
     // ranges in a fixed order and applies the pass's epilogue.  ksplit = 1: the fused epilogue below.
     int ksplit;
     float* part;
-    int dbg;             // bring-up switches: 1 = no split, 2 = no MMA, 4 = no epilogue (results invalid)
+    int dbg;             // bring-up switches (results invalid): 1 = no split, 2 = no MMA, 4 = no epilogue, 8 = no B_lo load,
+                         // 128 = no B load; 16 = A tiles not requested ahead of the dependency wait (valid)
 };
 
 __device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -267,10 +268,13 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     // under that kernel's tail.  The B tiles (panels written by the previous kernel) follow after the wait; the stage's
     // barrier expects the bytes of all three loads from the start.
     const int npre = min(p.stages, nk);
+    // bring-up switches (results invalid): 8 = do not load B_lo, 128 = load no B tile at all
+    const int nB = (p.dbg & 128) ? 0 : (p.dbg & 8) ? 1 : 2;
+    const int txBytes = aBytes + nB * bBytes;
     if (warp == 0 && !(p.dbg & 16)) {
         if (elect_one()) {
             for (int kc = 0; kc < npre; ++kc) {
-                mbar_expect_tx(&full[kc], aBytes + 2 * bBytes);
+                mbar_expect_tx(&full[kc], txBytes);
                 tma_load_3d(smem + (size_t)kc * stageBytes, mA, &full[kc], m0, (kbase + kc) * kTileK, p.slab0 + tt);
             }
         }
@@ -322,11 +326,11 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
                 if (kc >= npre || (p.dbg & 16)) {               // (the first round's A tiles were requested before the wait)
-                    mbar_expect_tx(&full[s], aBytes + 2 * bBytes);
+                    mbar_expect_tx(&full[s], txBytes);
                     tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
                 }
-                tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
-                tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
+                if (nB >= 1) tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
+                if (nB >= 2) tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
             }
             __syncwarp();
             if (++s == p.stages) { s = 0; ph ^= 1; }
