@@ -311,3 +311,10 @@ def test_forced_split_k_on_ragged_shapes(ks, monkeypatch):
     monkeypatch.setenv("DODE_TC_KSPLIT", str(ks))
     cfg = synth.Config("ragged", N=61, L=137, T=20, H=5, C=2, D=80, b=20, K=12, kmin=3, kmax=9)
     _run_both(cfg, sample=[0, 1, 40, 79])
+
+
+def test_minibatch_larger_than_one_launch():
+    """A minibatch of more than 256 days is split into several launches inside one dode_spgd_step (days are independent
+    units); the sub-batches alternate on the internal streams."""
+    cfg = synth.Config("wide_b", N=30, L=40, T=12, H=3, C=1, D=640, b=300, K=5, kmin=3, kmax=9, label_mode="zero")
+    assert "tcgen05" in _run_both(cfg, sample=[0, 1, 255, 256, 299, 300, 639])
