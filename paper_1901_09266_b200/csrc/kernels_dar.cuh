@@ -76,7 +76,7 @@ assignment_build_dense(int N, int L, int T, int H, const int32_t* __restrict__ o
         const int k0 = __ldg(od_ptr + n), k1 = __ldg(od_ptr + n + 1);
         const double t0 = (double)s * dt;
         constexpr int kCache = 8;                  // travel times of up to 8 paths stay in registers; beyond that they are re-walked
-        double cc[kCache];
+        double cc[kCache] = {};
         const bool cached = k1 - k0 <= kCache;
         auto ctime = [&](int k) {
             return cached ? cc[k - k0] : path_travel_time(k, t0, L, T, dt, path_ptr, path_links, len, speed);
