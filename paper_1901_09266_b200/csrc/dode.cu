@@ -93,7 +93,6 @@ struct dode_ctx {
     int64_t host_calls = 0;
     cudaEvent_t ev_fence = nullptr;
     bool plain_since_host = true;   // non-streaming work was issued on the ctx stream since the last streaming step
-    std::vector<int32_t> prev_days;
     // optional per-kernel event timing (dode_timing_enable / dode_timing_read)
     bool timing = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -766,44 +765,46 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
         CU(sync_all(ctx));
         cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
         ctx->stage_x = ctx->stage_q = nullptr; ctx->stage_x_cap = ctx->stage_q_cap = 0;
-        CU(cudaMalloc(&ctx->stage_x, TL * n * sizeof(float)));
-        CU(cudaMalloc(&ctx->stage_q, TN * n * sizeof(float)));
+        CU(cudaMalloc(&ctx->stage_x, 2 * TL * n * sizeof(float)));      // two halves, ping-pong over calls
+        CU(cudaMalloc(&ctx->stage_q, 2 * TN * n * sizeof(float)));
         ctx->stage_x_cap = TL * n; ctx->stage_q_cap = TN * n;
     }
-    // One-deep software pipeline over calls i: upload(i+1) || step(i) || download(i-1).
-    //   upload(i)   waits for step(i-2) always and for step(i-1) if the two calls share a day (x of that day is still being read)
-    //   step(i)     waits for upload(i), for download(i-2) always and for download(i-1) if they share a day (q still being read)
+    // One-deep software pipeline over calls i: upload(i+1) || step(i) || download(i-1).  The copy streams carry ONLY the
+    // PCIe copies, so each copy engine runs them back to back; the scatter of the uploaded counts into x and the gather
+    // of the updated q into the download buffer are small kernels on the ctx stream around the step (a kernel between
+    // two copies on a copy stream left the engine idle for the kernel plus two engine hand-overs per call).  Staging
+    // buffers ping-pong over calls (half `me` = call parity).
+    //   upload(i)   waits for step(i-2): its scatter was the last reader of staging half `me`
+    //   step(i)     = scatter(i), SPGD step, gather(i) on the ctx stream; waits for upload(i) and for download(i-2),
+    //                 the last reader of the q staging half `me`
     //   download(i) waits for step(i)
-    const int me = (int)(ctx->host_calls & 1), other = me ^ 1;
-    bool shares_day = false;                       // validate_days stamped this call's days with stamp_id
-    for (int32_t pd : ctx->prev_days) shares_day |= ctx->stamp[pd] == ctx->stamp_id;
+    const int me = (int)(ctx->host_calls & 1);
+    float* sx = ctx->stage_x + (size_t)me * ctx->stage_x_cap;
+    float* sq = ctx->stage_q + (size_t)me * ctx->stage_q_cap;
     if (ctx->host_calls >= 2) CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_step[me], 0));
-    if (ctx->host_calls >= 1 && shares_day) CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_step[other], 0));
-    CU(cudaMemcpyAsync(ctx->stage_x, x_host, TL * n * sizeof(float), cudaMemcpyHostToDevice, ctx->s_h2d));
-    for (int off = 0; off < n; off += kMaxDays) {
-        DayList dl; dl.n = std::min(kMaxDays, n - off);
-        std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
-        stage_scatter_x<<<dim3(std::min<long>(64, ceil_div((long)TL, 256)), dl.n), 256, 0, ctx->s_h2d>>>(
-            ctx->stage_x + TL * off, ctx->x, (long)TL, dl);
-        ctx->launches++;
-    }
+    CU(cudaMemcpyAsync(sx, x_host, TL * n * sizeof(float), cudaMemcpyHostToDevice, ctx->s_h2d));
     CU(cudaEventRecord(ctx->ev_h2d, ctx->s_h2d));
     CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_h2d, 0));
     if (ctx->host_calls >= 2) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_d2h[me], 0));
-    if (ctx->host_calls >= 1 && shares_day) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_d2h[other], 0));
-    if ((rc = step_impl(ctx, days, n, eta, c))) return rc;
-    CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
-    CU(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_step[me], 0));
     for (int off = 0; off < n; off += kMaxDays) {
         DayList dl; dl.n = std::min(kMaxDays, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
-        stage_gather_q<<<dim3(std::min<long>(64, ceil_div((long)TN, 256)), dl.n), 256, 0, ctx->s_d2h>>>(
-            ctx->q, ctx->stage_q + TN * off, d.T, d.N, ctx->Np, dl);
+        stage_scatter_x<<<dim3(std::min<long>(64, ceil_div((long)TL, 256)), dl.n), 256, 0, ctx->stream>>>(
+            sx + TL * off, ctx->x, (long)TL, dl);
         ctx->launches++;
     }
-    CU(cudaMemcpyAsync(q_host, ctx->stage_q, TN * n * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_d2h));
+    if ((rc = step_impl(ctx, days, n, eta, c))) return rc;
+    for (int off = 0; off < n; off += kMaxDays) {
+        DayList dl; dl.n = std::min(kMaxDays, n - off);
+        std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
+        stage_gather_q<<<dim3(std::min<long>(64, ceil_div((long)TN, 256)), dl.n), 256, 0, ctx->stream>>>(
+            ctx->q, sq + TN * off, d.T, d.N, ctx->Np, dl);
+        ctx->launches++;
+    }
+    CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
+    CU(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_step[me], 0));
+    CU(cudaMemcpyAsync(q_host, sq, TN * n * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_d2h));
     CU(cudaEventRecord(ctx->ev_d2h[me], ctx->s_d2h));
-    ctx->prev_days.assign(days, days + n);
     ctx->host_calls++;
     CU(cudaGetLastError());
     return DODE_OK;
