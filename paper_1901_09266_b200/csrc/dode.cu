@@ -86,8 +86,10 @@ struct dode_ctx {
     bool tc_ready = false, tc_attr = false;
     CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64;
     // streaming steps (dode_spgd_step_host): copy streams, staging buffers, ping-pong events
-    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr, s_sc = nullptr, s_ga = nullptr;   // copies only / scatter into x / gather of q
     cudaEvent_t ev_h2d = nullptr, ev_step[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
+    cudaEvent_t ev_scat[2] = {nullptr, nullptr}, ev_gath[2] = {nullptr, nullptr};
+    std::vector<int32_t> prev_days;
     float *stage_x = nullptr, *stage_q = nullptr;
     size_t stage_x_cap = 0, stage_q_cap = 0;
     int64_t host_calls = 0;
@@ -257,6 +259,8 @@ static cudaError_t sync_all(dode_ctx* ctx) {
     cudaError_t e = cudaStreamSynchronize(ctx->stream);
     if (ctx->s_h2d) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_h2d); if (e == cudaSuccess) e = e2; }
     if (ctx->s_d2h) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_d2h); if (e == cudaSuccess) e = e2; }
+    for (cudaStream_t st : {ctx->s_sc, ctx->s_ga})
+        if (st) { cudaError_t e2 = cudaStreamSynchronize(st); if (e == cudaSuccess) e = e2; }
     for (Lane& ln : ctx->lane)
         if (ln.st) { cudaError_t e2 = cudaStreamSynchronize(ln.st); if (e == cudaSuccess) e = e2; }
     ctx->lanes_dirty = false;
@@ -577,6 +581,9 @@ void dode_destroy(dode_ctx* ctx) {
     sync_all(ctx);
     if (ctx->s_h2d) cudaStreamDestroy(ctx->s_h2d);
     if (ctx->s_d2h) cudaStreamDestroy(ctx->s_d2h);
+    if (ctx->s_sc) cudaStreamDestroy(ctx->s_sc);
+    if (ctx->s_ga) cudaStreamDestroy(ctx->s_ga);
+    for (int i = 0; i < 2; ++i) { if (ctx->ev_scat[i]) cudaEventDestroy(ctx->ev_scat[i]); if (ctx->ev_gath[i]) cudaEventDestroy(ctx->ev_gath[i]); }
     if (ctx->ev_h2d) cudaEventDestroy(ctx->ev_h2d);
     if (ctx->ev_fence) cudaEventDestroy(ctx->ev_fence);
     for (int i = 0; i < 2; ++i) { if (ctx->ev_step[i]) cudaEventDestroy(ctx->ev_step[i]); if (ctx->ev_d2h[i]) cudaEventDestroy(ctx->ev_d2h[i]); }
@@ -684,11 +691,19 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     return DODE_OK;
 }
 
+// a plain step after streaming steps: the gathers of q on s_ga (beside the ctx stream) must have read their days first
+static int fence_streaming(dode_ctx* ctx) {
+    if (!ctx->plain_since_host && ctx->s_ga)
+        for (int i = 0; i < 2; ++i) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_gath[i], 0));
+    ctx->plain_since_host = true;
+    return DODE_OK;
+}
+
 int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta) {
     if (!ctx) return DODE_EINVAL;
     int c = 0, rc;
     if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
-    ctx->plain_since_host = true;
+    if ((rc = fence_streaming(ctx))) return rc;
     return step_impl(ctx, days, n, eta, c, StepOpt(), true);
 }
 
@@ -710,7 +725,7 @@ int dode_adagrad_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, 
     }
     StepOpt opt;
     opt.mask = row_mask; opt.G = ctx->G; opt.eps = eps;
-    ctx->plain_since_host = true;
+    if ((rc = fence_streaming(ctx))) return rc;
     return step_impl(ctx, days, n, eta, c, opt);
 }
 
@@ -749,16 +764,20 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
     if (!ctx->s_h2d) {
         CU(cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
         CU(cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->s_sc, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->s_ga, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&ctx->ev_h2d, cudaEventDisableTiming));
         for (int i = 0; i < 2; ++i) {
             CU(cudaEventCreateWithFlags(&ctx->ev_step[i], cudaEventDisableTiming));
             CU(cudaEventCreateWithFlags(&ctx->ev_d2h[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_scat[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_gath[i], cudaEventDisableTiming));
         }
         CU(cudaEventCreateWithFlags(&ctx->ev_fence, cudaEventDisableTiming));
     }
     if (ctx->plain_since_host) {      // earlier steps on the ctx stream / the lanes may still read x or write q of these days
         CU(cudaEventRecord(ctx->ev_fence, ctx->stream));
-        CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_fence, 0));
+        CU(cudaStreamWaitEvent(ctx->s_sc, ctx->ev_fence, 0));
         ctx->plain_since_host = false;
     }
     if (ctx->stage_x_cap < TL * n || ctx->stage_q_cap < TN * n) {
@@ -769,42 +788,57 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
         CU(cudaMalloc(&ctx->stage_q, 2 * TN * n * sizeof(float)));
         ctx->stage_x_cap = TL * n; ctx->stage_q_cap = TN * n;
     }
-    // One-deep software pipeline over calls i: upload(i+1) || step(i) || download(i-1).  The copy streams carry ONLY the
-    // PCIe copies, so each copy engine runs them back to back; the scatter of the uploaded counts into x and the gather
-    // of the updated q into the download buffer are small kernels on the ctx stream around the step (a kernel between
-    // two copies on a copy stream left the engine idle for the kernel plus two engine hand-overs per call).  Staging
-    // buffers ping-pong over calls (half `me` = call parity).
-    //   upload(i)   waits for step(i-2): its scatter was the last reader of staging half `me`
-    //   step(i)     = scatter(i), SPGD step, gather(i) on the ctx stream; waits for upload(i) and for download(i-2),
-    //                 the last reader of the q staging half `me`
-    //   download(i) waits for step(i)
-    const int me = (int)(ctx->host_calls & 1);
+    // One-deep software pipeline over calls i: upload(i+1) || step(i) || download(i-1), on five streams:
+    //   s_h2d / s_d2h  carry ONLY the PCIe copies, so each copy engine runs them back to back (a kernel between two copies
+    //                  on a copy stream left the engine idle for the kernel plus two engine hand-overs per call)
+    //   s_sc / s_ga    scatter of the uploaded counts into x / gather of the updated q into the download buffer: small
+    //                  kernels beside the steps, off the ctx stream, which carries only the SPGD kernels
+    // Staging buffers ping-pong over calls (half `me` = call parity).  Orderings (events in stream order cover every
+    // earlier call of the same parity):
+    //   upload(i)   after scatter(i-2), the last reader of x-staging half `me`
+    //   scatter(i)  after upload(i); after step(i-2); after step(i-1) if the calls share a day (it still reads that x)
+    //   step(i)     after scatter(i); after gather(i-2); after gather(i-1) if the calls share a day (it still reads that q)
+    //   gather(i)   after step(i); after download(i-2), the last reader of q-staging half `me`
+    //   download(i) after gather(i)
+    const int me = (int)(ctx->host_calls & 1), other = me ^ 1;
+    const bool two = ctx->host_calls >= 2;
+    bool shares_day = false;                       // validate_days stamped this call's days with stamp_id
+    for (int32_t pd : ctx->prev_days) shares_day |= ctx->stamp[pd] == ctx->stamp_id;
     float* sx = ctx->stage_x + (size_t)me * ctx->stage_x_cap;
     float* sq = ctx->stage_q + (size_t)me * ctx->stage_q_cap;
-    if (ctx->host_calls >= 2) CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_step[me], 0));
+    if (two) CU(cudaStreamWaitEvent(ctx->s_h2d, ctx->ev_scat[me], 0));
     CU(cudaMemcpyAsync(sx, x_host, TL * n * sizeof(float), cudaMemcpyHostToDevice, ctx->s_h2d));
     CU(cudaEventRecord(ctx->ev_h2d, ctx->s_h2d));
-    CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_h2d, 0));
-    if (ctx->host_calls >= 2) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_d2h[me], 0));
+    CU(cudaStreamWaitEvent(ctx->s_sc, ctx->ev_h2d, 0));
+    if (two) CU(cudaStreamWaitEvent(ctx->s_sc, ctx->ev_step[me], 0));
+    if (shares_day) CU(cudaStreamWaitEvent(ctx->s_sc, ctx->ev_step[other], 0));
     for (int off = 0; off < n; off += kMaxDays) {
         DayList dl; dl.n = std::min(kMaxDays, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
-        stage_scatter_x<<<dim3(std::min<long>(64, ceil_div((long)TL, 256)), dl.n), 256, 0, ctx->stream>>>(
+        stage_scatter_x<<<dim3(std::min<long>(64, ceil_div((long)TL, 256)), dl.n), 256, 0, ctx->s_sc>>>(
             sx + TL * off, ctx->x, (long)TL, dl);
         ctx->launches++;
     }
+    CU(cudaEventRecord(ctx->ev_scat[me], ctx->s_sc));
+    CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_scat[me], 0));
+    if (two) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_gath[me], 0));
+    if (shares_day) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_gath[other], 0));
     if ((rc = step_impl(ctx, days, n, eta, c))) return rc;
+    CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
+    CU(cudaStreamWaitEvent(ctx->s_ga, ctx->ev_step[me], 0));
+    if (two) CU(cudaStreamWaitEvent(ctx->s_ga, ctx->ev_d2h[me], 0));
     for (int off = 0; off < n; off += kMaxDays) {
         DayList dl; dl.n = std::min(kMaxDays, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
-        stage_gather_q<<<dim3(std::min<long>(64, ceil_div((long)TN, 256)), dl.n), 256, 0, ctx->stream>>>(
+        stage_gather_q<<<dim3(std::min<long>(64, ceil_div((long)TN, 256)), dl.n), 256, 0, ctx->s_ga>>>(
             ctx->q, sq + TN * off, d.T, d.N, ctx->Np, dl);
         ctx->launches++;
     }
-    CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
-    CU(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_step[me], 0));
+    CU(cudaEventRecord(ctx->ev_gath[me], ctx->s_ga));
+    CU(cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_gath[me], 0));
     CU(cudaMemcpyAsync(q_host, sq, TN * n * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_d2h));
     CU(cudaEventRecord(ctx->ev_d2h[me], ctx->s_d2h));
+    ctx->prev_days.assign(days, days + n);
     ctx->host_calls++;
     CU(cudaGetLastError());
     return DODE_OK;
