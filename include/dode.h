@@ -100,7 +100,8 @@ int dode_adagrad_reset(dode_ctx* ctx);
 
 /* The same iteration for a streaming caller (bench.py's end-to-end leg): uploads the n days' counts from x_host
  * ([n][T][L], host; pinned memory makes the copies asynchronous), runs the step, and downloads the n days' updated q
- * into q_host ([n][T][N], host).  ASYNCHRONOUS and pipelined over consecutive calls on two internal copy streams:
+ * into q_host ([n][T][N], host).  ASYNCHRONOUS and pipelined over consecutive calls on two internal copy streams
+ * (PCIe copies only) and two helper streams (scatter into x, gather of q):
  * the upload of call i+1 and the download of call i-1 overlap the kernels of call i (calls that share a day are
  * ordered).  x_host must stay valid and q_host is defined only after the next synchronising call (dode_sync,
  * dode_objective, dode_get_q, dode_set_q, dode_timing_read, dode_destroy). */

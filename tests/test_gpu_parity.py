@@ -185,6 +185,37 @@ def test_get_set_q_and_host_step():
     g1.close(); g2.close()
 
 
+def test_streaming_and_plain_steps_interleaved():
+    """Streaming steps (helper streams for the scatter into x and the gather of q) interleaved with plain steps on the
+    same days, minibatches wide enough for the tensor path and its two lanes: same iterates as plain steps only, and
+    every download is its call's state."""
+    cfg = synth.Config("mix", N=24, L=20, T=16, H=4, C=1, D=24, b=12, K=3, kmin=2, kmax=6, label_mode="zero")
+    p = hz.make_problem(cfg)
+    etas = hz.oracle_etas(p)
+    g1, g2 = hz.GpuSolver(p), hz.GpuSolver(p)
+    P = g1.P
+    A, B, Cc = list(range(0, 12)), list(range(12, 24)), list(range(6, 18))
+    seq = [("host", A), ("plain", A), ("host", B), ("host", Cc), ("plain", Cc), ("plain", A), ("host", A), ("host", B),
+           ("plain", B), ("host", Cc)]
+    bufs = []
+    for rep in range(3):
+        for kind, days in seq:
+            P.dode_spgd_step(g1.h, days, float(etas[0]))
+            if kind == "plain":
+                P.dode_spgd_step(g2.h, days, float(etas[0]))
+                continue
+            want = g1.q(days).copy()
+            xh = p.x[days].contiguous().pin_memory()
+            qh = torch.empty(len(days), cfg.T, cfg.N).pin_memory()
+            P.dode_spgd_step_host(g2.h, days, float(etas[0]), xh, qh)
+            bufs.append((xh, qh, want))
+    P.dode_sync(g2.h)
+    for xh, qh, want in bufs:
+        np.testing.assert_array_equal(qh.numpy(), want)
+    np.testing.assert_array_equal(g2.q(), g1.q())
+    g1.close(); g2.close()
+
+
 def test_batch_composition_invariance_on_gpu():
     """P10 on the GPU: the same visits as b=1 steps give the same iterate to rounding."""
     cfg = synth.Config("sep", N=24, L=20, T=16, H=4, C=2, D=20, b=7, K=12, kmin=2, kmax=6)
