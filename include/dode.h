@@ -73,7 +73,8 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
 /* a1-a4: one SPGD iteration on the listed days (Alg. 1 lines 8-11):
  *   r = rho_c Q_B - X_B ;  g = rho_c^T r ;  q_d <- max(0, q_d - eta g_d)  for d in days.
  *   days  host int32 [n]; all in [0, D), distinct, same cluster — else DODE_EINVAL, state untouched.
- * Asynchronous; no host synchronisation, no device->host traffic.
+ * Asynchronous; no device->host traffic.  No host synchronisation once the minibatch panels exist: the first step of
+ * a given width allocates them (cudaMalloc + a stream synchronisation) unless dode_reserve was called before.
  * Ordering: a step starts after everything that was on the ctx stream when it was called and after every earlier
  * step that shares a day with it.  Steps on disjoint days (the chunks of one epoch) may overlap
  * each other: the library alternates them on two internal streams.  Every other library call is ordered after all
@@ -83,6 +84,27 @@ int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta);
 
 /* Makes the ctx stream wait for every step issued so far (asynchronous, no host wait). */
 int dode_join(dode_ctx* ctx);
+
+/* Pre-allocates the per-step scratch buffers of dode_spgd_step (minibatch panels of the kernel families the current
+ * options select, on the ctx stream and on the two internal step streams) for minibatches of up to max_days days, so
+ * that no later dode_spgd_step with n <= max_days allocates or synchronises.  (dode_adagrad_step's accumulator and
+ * dode_spgd_step_host's staging halves are allocated by their own first call.)  Synchronises once itself.
+ * max_days >= 1. */
+int dode_reserve(dode_ctx* ctx, int32_t max_days);
+
+/* Per-ctx kernel-selection options (no process-wide state, nothing is read from the environment).  All of them keep
+ * results valid; they exist so that tests and benchmarks can steer every kernel family over every shape.
+ *   DODE_OPT_TC_MIN_B   minibatch width from which dense steps use the tcgen05 3xTF32 kernels; 0 = never
+ *                       (FFMA kernels for every width).  Default 8.
+ *   DODE_OPT_LANES      1 = consecutive plain steps alternate on two internal streams (default), 0 = ctx stream only.
+ *   DODE_OPT_TC_KSPLIT  split-K factor of the tcgen05 kernels, 1..32; 0 = automatic (default: split only when the time
+ *                       axis is too short to fill the machine).
+ *   DODE_OPT_PDL        1 = kernels of a step are chained by programmatic dependent launch (default), 0 = plain
+ *                       stream order.
+ * Unknown option or out-of-range value: DODE_EINVAL, nothing changes.  Asynchronous (orders later steps after earlier
+ * ones where the option changes the stream they run on). */
+enum { DODE_OPT_TC_MIN_B = 0, DODE_OPT_LANES = 1, DODE_OPT_TC_KSPLIT = 2, DODE_OPT_PDL = 3 };
+int dode_set_option(dode_ctx* ctx, int32_t option, int32_t value);
 
 /* NEXT-1 — Alg. 1 as the paper prints it, on the listed days of one cluster:
  *   line 8   B_o = the rows of each day's system selected by row_mask (a chunk of the permuted row range, 398-404)
@@ -104,7 +126,8 @@ int dode_adagrad_reset(dode_ctx* ctx);
  * (PCIe copies only) and two helper streams (scatter into x, gather of q):
  * the upload of call i+1 and the download of call i-1 overlap the kernels of call i (calls that share a day are
  * ordered).  x_host must stay valid and q_host is defined only after the next synchronising call (dode_sync,
- * dode_objective, dode_get_q, dode_set_q, dode_timing_read, dode_destroy). */
+ * dode_objective, dode_r2, dode_get_q, dode_set_q, dode_lipschitz, dode_timing_read, dode_reserve, dode_destroy): each
+ * of them waits for the ctx stream AND for the library's internal step and copy streams. */
 int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta,
                         const float* x_host, float* q_host);
 
@@ -176,10 +199,13 @@ int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* lau
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 int64_t dode_launch_count(const dode_ctx* ctx);
 
-/* Which kernel family the last dode_spgd_step used, e.g. "ffma_rowdot_bt8+ffma_coldot_bt8". */
+/* Which kernel family the last step used: "<forward kernel>+<gradient kernel>", e.g.
+ * "ffma_coldot_fwd_bt4+ffma_coldot_grad_bt4", "tcgen05_3xtf32_fwd_bn64+tcgen05_3xtf32_grad_bn64",
+ * "csr_fwd_bp128+csr_grad_bp128". */
 const char* dode_last_path(const dode_ctx* ctx);
 
-/* Wait for all work issued on the ctx stream; returns a pending CUDA error if any. */
+/* Waits for all work issued on the ctx stream and on the library's internal streams; returns a pending CUDA error if
+ * any. */
 int dode_sync(dode_ctx* ctx);
 
 void dode_destroy(dode_ctx* ctx);

@@ -19,7 +19,9 @@ SO_PATH = os.path.join(_HERE, "libdode.so")
 DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
 DODE_DENSE, DODE_CSR = 0, 1
 
-EXPORTS = ["dode_create", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
+DODE_OPT_TC_MIN_B, DODE_OPT_LANES, DODE_OPT_TC_KSPLIT, DODE_OPT_PDL = 0, 1, 2, 3
+
+EXPORTS = ["dode_create", "dode_set_option", "dode_reserve", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
            "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
@@ -57,6 +59,8 @@ def lib():
         L.dode_adagrad_step.argtypes = [vp, vp, i32, f32, f32, vp]
         L.dode_adagrad_reset.argtypes = [vp]
         L.dode_join.argtypes = [vp]
+        L.dode_set_option.argtypes = [vp, i32, i32]
+        L.dode_reserve.argtypes = [vp, i32]
         L.dode_dar_build.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, C.c_double, vp, vp]
         L.dode_assignment_build.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, C.c_double, C.c_double, vp, vp]
         L.dode_objective.argtypes = [vp, vp, i32, vp, vp]
@@ -88,6 +92,35 @@ def _chk(h, rc: int):
 
 def _days(days) -> np.ndarray:
     return np.ascontiguousarray(days, dtype=np.int32)
+
+
+# Shapes of the ctx (binding-side argument validation only) and host tensors that asynchronous calls still use:
+# keyed by the handle's address; released by the next synchronising call.
+_shape = {}
+_keep = {}
+
+
+def _key(h) -> int:
+    return int(h.value) if isinstance(h, C.c_void_p) else int(h)
+
+
+def _release(h) -> None:
+    _keep.pop(_key(h), None)
+
+
+def _host(t, shape, what):
+    import torch
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+            and tuple(t.shape) == tuple(shape)):
+        raise TypeError(f"{what} must be a contiguous CPU float32 tensor of shape {tuple(shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _any(t, shape, what):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise TypeError(f"{what} must be a contiguous float32 tensor of shape {tuple(shape)}")
+    return C.c_void_p(t.data_ptr())
 
 
 def _dev(t, dtype, what):
@@ -131,7 +164,19 @@ def dode_create(N: int, L: int, T: int, H: int, Cn: int, D: int, labels, x, q0: 
                            C.c_float(q0), C.c_void_p(stream))
     if rc != 0:
         raise DodeError(rc, lib().dode_last_error(None).decode())
+    _shape[_key(h)] = (N, L, T, H, Cn, D)
     return h
+
+
+def dode_set_option(h, option: int, value: int) -> None:
+    """Kernel-selection options of this ctx (DODE_OPT_*; include/dode.h).  Results stay valid for every value."""
+    _chk(h, lib().dode_set_option(h, int(option), int(value)))
+
+
+def dode_reserve(h, max_days: int) -> None:
+    """Pre-allocates dode_spgd_step's scratch for minibatches of up to ``max_days`` days.  Synchronises."""
+    _chk(h, lib().dode_reserve(h, int(max_days)))
+    _release(h)
 
 
 def dode_spgd_step(h, days, eta: float) -> None:
@@ -183,7 +228,10 @@ def dode_adagrad_step(h, days, eta: float, eps: float = 1e-10, row_mask=None) ->
     d = _days(days)
     mp = None
     if row_mask is not None:
-        assert row_mask.is_cuda and row_mask.element_size() == 1 and row_mask.is_contiguous()
+        N, L, T = _shape[_key(h)][:3]
+        if not (row_mask.is_cuda and row_mask.element_size() == 1 and row_mask.is_contiguous()
+                and row_mask.numel() == d.size * T * L):
+            raise TypeError(f"row_mask must be a contiguous CUDA uint8 tensor with {d.size}*{T}*{L} entries")
         mp = C.c_void_p(row_mask.data_ptr())
     _chk(h, lib().dode_adagrad_step(h, d.ctypes.data, d.size, C.c_float(eta), C.c_float(eps), mp))
 
@@ -193,11 +241,17 @@ def dode_adagrad_reset(h) -> None:
 
 
 def dode_spgd_step_host(h, days, eta: float, x_host, q_host) -> None:
-    """Streaming step: uploads the days' counts from ``x_host`` ([n][T][L] CPU tensor, ideally pinned),
-    steps, downloads their q into ``q_host`` ([n][T][N] CPU tensor) and synchronises."""
+    """Streaming step: uploads the days' counts from ``x_host`` ([n][T][L] CPU float32 tensor, pinned for
+    asynchronous copies), steps, and downloads their q into ``q_host`` ([n][T][N] CPU float32 tensor).
+    ASYNCHRONOUS: the copies and kernels are only queued.  ``q_host`` is defined, and ``x_host`` may be changed, only
+    after the next synchronising call (dode_sync, dode_objective, dode_r2, dode_get_q, dode_set_q, dode_lipschitz,
+    dode_timing_read, dode_reserve, dode_destroy); this binding keeps both tensors alive until then."""
     d = _days(days)
-    _chk(h, lib().dode_spgd_step_host(h, d.ctypes.data, d.size, C.c_float(eta),
-                                      C.c_void_p(x_host.data_ptr()), C.c_void_p(q_host.data_ptr())))
+    N, L, T = _shape[_key(h)][:3]
+    xp = _host(x_host, (d.size, T, L), "x_host")
+    qp = _host(q_host, (d.size, T, N), "q_host")
+    _keep.setdefault(_key(h), []).append((x_host, q_host))
+    _chk(h, lib().dode_spgd_step_host(h, d.ctypes.data, d.size, C.c_float(eta), xp, qp))
 
 
 def dode_objective(h, days):
@@ -206,6 +260,7 @@ def dode_objective(h, days):
     per = np.empty(d.size, np.float64)
     tot = C.c_double()
     _chk(h, lib().dode_objective(h, d.ctypes.data, d.size, per.ctypes.data, C.byref(tot)))
+    _release(h)
     return per, tot.value
 
 
@@ -215,16 +270,22 @@ def dode_r2(h, days):
     per = np.empty(d.size, np.float64)
     mean = C.c_double()
     _chk(h, lib().dode_r2(h, d.ctypes.data, d.size, per.ctypes.data, C.byref(mean)))
+    _release(h)
     return per, mean.value
 
 
 def dode_get_q(h, day: int, out) -> None:
-    """Copies day's q ([T][N], Table 2 order) into ``out`` (CPU or CUDA fp32 tensor, contiguous)."""
-    _chk(h, lib().dode_get_q(h, day, C.c_void_p(out.data_ptr()), 1 if out.is_cuda else 0))
+    """Copies day's q ([T][N], Table 2 order) into ``out`` (CPU or CUDA float32 tensor [T][N], contiguous)."""
+    N, L, T = _shape[_key(h)][:3]
+    _chk(h, lib().dode_get_q(h, day, _any(out, (T, N), "out"), 1 if out.is_cuda else 0))
+    _release(h)
 
 
 def dode_set_q(h, day: int, src) -> None:
-    _chk(h, lib().dode_set_q(h, day, C.c_void_p(src.data_ptr()), 1 if src.is_cuda else 0))
+    """Overwrites day's q from ``src`` (CPU or CUDA float32 tensor [T][N], contiguous)."""
+    N, L, T = _shape[_key(h)][:3]
+    _chk(h, lib().dode_set_q(h, day, _any(src, (T, N), "src"), 1 if src.is_cuda else 0))
+    _release(h)
 
 
 def dode_apply(h, c: int, u, v) -> None:
@@ -243,6 +304,7 @@ def dode_lipschitz(h, c: int, iters: int = 50) -> float:
     """a7: L_c ~ lambda_max(rho_c^T rho_c) by power iteration through the production kernels."""
     out = C.c_double()
     _chk(h, lib().dode_lipschitz(h, c, iters, C.byref(out)))
+    _release(h)
     return out.value
 
 
@@ -254,6 +316,7 @@ def dode_timing_read(h, kind: int, reset: bool = False):
     """(total device ms, launches) of kind 0 = forward, 1 = gradient+update."""
     ms, cnt = C.c_double(), C.c_int64()
     _chk(h, lib().dode_timing_read(h, kind, C.byref(ms), C.byref(cnt), 1 if reset else 0))
+    _release(h)
     return ms.value, cnt.value
 
 
@@ -267,10 +330,13 @@ def dode_last_path(h) -> str:
 
 def dode_sync(h) -> None:
     _chk(h, lib().dode_sync(h))
+    _release(h)
 
 
 def dode_destroy(h) -> None:
     lib().dode_destroy(h)
+    _release(h)
+    _shape.pop(_key(h), None)
 
 
 def dode_last_error(h) -> str:

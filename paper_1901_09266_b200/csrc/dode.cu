@@ -16,8 +16,6 @@
 #include "kernels_tc.cuh"
 #include "kernels_dar.cuh"
 
-#include <cstdlib>
-
 using namespace dode;
 
 // Minibatch panels and their tensor maps for the tensor-core path, one set per issue stream
@@ -80,9 +78,9 @@ struct dode_ctx {
     std::vector<int64_t> day_last_id;              // [D] id of the last lane step that touched the day
     std::vector<int8_t> day_last_lane;             // [D] and its lane (-1: none)
     long rpitch = 0;
-    int tc_min_b = 8;
-    // bring-up / experiment knobs, read from the environment once at dode_create (0 = off)
-    int knob_occ1 = 0, knob_stages = 0, knob_dbg = 0, knob_ksplit = 0;
+    // kernel-selection options (dode_set_option)
+    int tc_min_b = 8, opt_ksplit = 0;
+    bool opt_pdl = true;
     bool tc_ready = false, tc_attr = false;
     CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64;
     // streaming steps (dode_spgd_step_host): copy streams, staging buffers, ping-pong events
@@ -374,28 +372,12 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn) {
     return DODE_OK;
 }
 
-// Launch with programmatic stream serialization (PDL): the kernel may start while its predecessor drains; it
-// calls griddepcontrol.wait before touching anything the predecessor wrote.  Per-kernel event timing records
-// events between launches, which serialises them again — timing mode therefore shows un-overlapped durations.
-template <typename... KArgs, typename... Args>
-static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
-    static const bool no_pdl = getenv("DODE_NO_PDL") && atoi(getenv("DODE_NO_PDL"));
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = no_pdl ? 0 : 1;
-    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
-}
+// Launch geometry of the tensor-core kernels for a minibatch of bn (multiple of 16) days
+struct TcGeom { int stages, nring; size_t smem; int ks_f, ks_g; size_t part_floats; };
 
-// one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
-static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt, TcBuf& tb, cudaStream_t st) {
+static TcGeom tc_geometry(const dode_ctx* ctx, int bn) {
     const dode_dims& d = ctx->dm;
-    const int bn = (dl.n + 15) / 16 * 16;
-    int rc = tc_ensure(ctx, tb, st, bn);
-    if (rc) return rc;
-    const size_t dayStride = (size_t)d.T * ctx->Np;
+    TcGeom g{};
     // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  Two CTAs per SM when 3 stages fit in half the
     // shared memory and 256 TMEM columns suffice.
     const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
@@ -407,13 +389,62 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
         stages = (226 * 1024 - fixed) / stageBytes;
         nring = acc_cols + 256 <= 512 ? 4 : 2;
     }
-    if (ctx->knob_occ1) { stages = (226 * 1024 - fixed) / stageBytes; nring = acc_cols + 256 <= 512 ? 4 : 2; }
-    if (ctx->knob_stages > 1) stages = std::min(stages, ctx->knob_stages);
-    stages = std::max(2, std::min(stages, 10));
-    const size_t smem = (size_t)stages * stageBytes + fixed;
+    g.stages = std::max(2, std::min(stages, 10));
+    g.nring = nring;
+    g.smem = (size_t)g.stages * stageBytes + fixed;
+    // split-K when the time axis is too short to fill the machine (T * tiles CTAs for 148 SMs x 1-2 CTAs): e.g. the
+    // Fig. 12 workload, T = 1.  Each pass then runs ksplit CTAs per tile and a small epilogue kernel.
+    const int slots = 148 * (g.smem * 2 + 2048 <= 227 * 1024 ? 2 : 1);
+    auto pick_split = [&](int M, int kunit) {
+        const long ctas = (long)ceil_div(M, tc::kTileM) * d.T;
+        const int nk_max = ceil_div((long)(d.H + 1) * kunit, tc::kTileK);
+        int ks = (int)std::min<long>(slots / std::max<long>(ctas, 1), nk_max / 8);
+        if (ctx->opt_ksplit > 0) ks = ctx->opt_ksplit;
+        return std::max(1, std::min(ks, 32));
+    };
+    g.ks_f = pick_split(d.L, ctx->Np);
+    g.ks_g = pick_split(d.N, ctx->Lp);
+    g.part_floats = (g.ks_f > 1 || g.ks_g > 1)
+        ? (size_t)std::max(g.ks_f * ceil_div(d.L, tc::kTileM), g.ks_g * ceil_div(d.N, tc::kTileM)) * tc::kTileM * d.T * bn : 0;
+    return g;
+}
+
+static int tc_ensure_part(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, size_t need) {
+    if (tb.part_cap >= need) return DODE_OK;
+    CU(cudaStreamSynchronize(st));
+    cudaFree(tb.part); tb.part = nullptr; tb.part_cap = 0;
+    CU(cudaMalloc(&tb.part, need * sizeof(float)));
+    tb.part_cap = need;
+    return DODE_OK;
+}
+
+// Launch with programmatic stream serialization (PDL): the kernel may start while its predecessor drains; it
+// calls griddepcontrol.wait before touching anything the predecessor wrote.  Per-kernel event timing records
+// events between launches, which serialises them again — timing mode therefore shows un-overlapped durations.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
+// one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
+static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt, TcBuf& tb, cudaStream_t st) {
+    const dode_dims& d = ctx->dm;
+    const int bn = (dl.n + 15) / 16 * 16;
+    int rc = tc_ensure(ctx, tb, st, bn);
+    if (rc) return rc;
+    const TcGeom geo0 = tc_geometry(ctx, bn);
+    const int stages = geo0.stages, nring = geo0.nring;
+    const size_t smem = geo0.smem;
+    const size_t dayStride = (size_t)d.T * ctx->Np;
     {
         KernelTimer kt(ctx, KIND_OTHER);
-        CU(launch_pdl(tc::gather_split, dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), dim3(256), 0,
+        CU(launch_pdl(ctx->opt_pdl, tc::gather_split, dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), dim3(256), 0,
                       st, ctx->q, dayStride, (long)dayStride / 4, tb.Qg_full, tb.Qg_lo, dl));
         ctx->launches++;
     }
@@ -423,29 +454,11 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = tb.rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
-    p.dbg = ctx->knob_dbg;
     const bool ada = opt.mask || opt.G;
     auto kern = ada ? tc::banded_gemm_3xtf32<true> : tc::banded_gemm_3xtf32<false>;
-    // split-K when the time axis is too short to fill the machine (T * tiles CTAs for 148 SMs x 1-2 CTAs): e.g. the
-    // Fig. 12 workload, T = 1.  Each pass then runs ksplit CTAs per tile and a small epilogue kernel.
-    const int slots = 148 * (smem * 2 + 2048 <= 227 * 1024 ? 2 : 1);
-    auto pick_split = [&](int M, int kunit) {
-        const long ctas = (long)ceil_div(M, tc::kTileM) * d.T;
-        const int nk_max = ceil_div((long)(d.H + 1) * kunit, tc::kTileK);
-        int ks = (int)std::min<long>(slots / std::max<long>(ctas, 1), nk_max / 8);
-        if (ctx->knob_ksplit > 0) ks = ctx->knob_ksplit;
-        return std::max(1, std::min(ks, 32));
-    };
-    const int ks_f = pick_split(d.L, ctx->Np), ks_g = pick_split(d.N, ctx->Lp);
-    if (ks_f > 1 || ks_g > 1) {
-        const size_t need = (size_t)std::max(ks_f * ceil_div(d.L, tc::kTileM), ks_g * ceil_div(d.N, tc::kTileM)) * tc::kTileM * d.T * bn;
-        if (tb.part_cap < need) {
-            CU(cudaStreamSynchronize(st));
-            cudaFree(tb.part); tb.part = nullptr; tb.part_cap = 0;
-            CU(cudaMalloc(&tb.part, need * sizeof(float)));
-            tb.part_cap = need;
-        }
-    }
+    const TcGeom& geo = geo0;
+    const int ks_f = geo.ks_f, ks_g = geo.ks_g;
+    if ((rc = tc_ensure_part(ctx, tb, st, geo.part_floats))) return rc;
     p.part = tb.part;
     auto epilogue = [&](int Mt) -> int {           // second half of a split-K pass
         const dim3 g(ceil_div((long)Mt * (bn / 4), 256), d.T);
@@ -457,7 +470,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     {
         KernelTimer kt(ctx, KIND_FWD);
         p.mode = 0; p.M = d.L; p.kunit = ctx->Np; p.ksplit = ks_f;
-        CU(launch_pdl(kern, dim3(ceil_div(d.L, tc::kTileM), d.T, ks_f), dim3(tc::kThreadsTC), smem,
+        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.L, tc::kTileM), d.T, ks_f), dim3(tc::kThreadsTC), smem,
                       st, ctx->mapA_fwd, ctx->mapA_fwd64, tb.mapQ_f, tb.mapQ_l, p, dl));
         ctx->launches++;
         if (ks_f > 1) epilogue(ceil_div(d.L, tc::kTileM) * tc::kTileM);
@@ -465,7 +478,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     {
         KernelTimer kt(ctx, KIND_GRAD);
         p.mode = 1; p.M = d.N; p.kunit = ctx->Lp; p.ksplit = ks_g;
-        CU(launch_pdl(kern, dim3(ceil_div(d.N, tc::kTileM), d.T, ks_g), dim3(tc::kThreadsTC), smem,
+        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.N, tc::kTileM), d.T, ks_g), dim3(tc::kThreadsTC), smem,
                       st, ctx->mapA_grad, ctx->mapA_grad64, tb.mapR_f, tb.mapR_l, p, dl));
         ctx->launches++;
         if (ks_g > 1) epilogue(ceil_div(d.N, tc::kTileM) * tc::kTileM);
@@ -486,17 +499,21 @@ static int join_lanes(dode_ctx* ctx) {
     return DODE_OK;
 }
 
+static int lane_init(dode_ctx* ctx, Lane& ln) {
+    if (ln.st) return DODE_OK;
+    CU(cudaStreamCreateWithFlags(&ln.st, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&ln.done, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&ln.entry, cudaEventDisableTiming));
+    return DODE_OK;
+}
+
 // picks the lane of the next step, forks it from the ctx stream and orders it after earlier steps on its days
 static int lane_begin(dode_ctx* ctx, const DayList& dl, Lane** out) {
     const int li = ctx->lane_next;
     ctx->lane_next ^= 1;
     Lane& ln = ctx->lane[li];
     Lane& ot = ctx->lane[li ^ 1];
-    if (!ln.st) {
-        CU(cudaStreamCreateWithFlags(&ln.st, cudaStreamNonBlocking));
-        CU(cudaEventCreateWithFlags(&ln.done, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&ln.entry, cudaEventDisableTiming));
-    }
+    if (int rc = lane_init(ctx, ln)) return rc;
     // fork: whatever is on the ctx stream now (the caller's work, earlier non-lane calls) precedes this step
     CU(cudaEventRecord(ln.entry, ctx->stream));
     CU(cudaStreamWaitEvent(ln.st, ln.entry, 0));
@@ -533,7 +550,7 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
         int bt, bp, rc;
         StepOpt opt = opt0;
         if (opt.mask) opt.mask += (size_t)off * d.T * d.L;
-        const bool tcp = ctx->tc_ready && dl.n >= ctx->tc_min_b;
+        const bool tcp = ctx->tc_ready && ctx->tc_min_b > 0 && dl.n >= ctx->tc_min_b;
         if (tcp && allow_lanes && ctx->lanes_on && !ctx->timing && !opt.mask && !opt.G) {
             Lane* ln = nullptr;
             if ((rc = lane_begin(ctx, dl, &ln))) return rc;
@@ -637,11 +654,6 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     c->stamp.assign(d.D, 0);
     c->day_last_id.assign(d.D, 0);
     c->day_last_lane.assign(d.D, -1);
-    if (const char* e = getenv("DODE_LANES")) c->lanes_on = atoi(e) != 0;
-    if (const char* e = getenv("DODE_TC_OCC1")) c->knob_occ1 = atoi(e);
-    if (const char* e = getenv("DODE_TC_STAGES")) c->knob_stages = atoi(e);
-    if (const char* e = getenv("DODE_TC_DBG")) c->knob_dbg = atoi(e);
-    if (const char* e = getenv("DODE_TC_KSPLIT")) c->knob_ksplit = atoi(e);
     ctx = c;
 #define CUC(call)                                                                                          \
     do {                                                                                                   \
@@ -674,12 +686,8 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
         pack_arrival_major<<<dim3((unsigned)blocks, ceil_div(c->Lp, 32), ceil_div(c->Np, 32)), 256, 0, c->stream>>>(
             R->dense, c->Af, d.T, d.H, d.L, d.N, c->Lp, c->Np);
         c->launches += 2;
-        const char* env = getenv("DODE_TC_MIN_B");      // minibatch from which the tensor-core path is used (0 = never)
-        c->tc_min_b = env ? atoi(env) : 8;
-        if (c->tc_min_b > 0) {
-            int rc = tc_setup(c);
-            if (rc) { snprintf(g_create_err, 512, "%s", c->err); dode_destroy(c); cudaGetLastError(); return rc; }
-        }
+        int rc = tc_setup(c);
+        if (rc) { snprintf(g_create_err, 512, "%s", c->err); dode_destroy(c); cudaGetLastError(); return rc; }
     } else {
         int rc = csr_build(c->csr, d, *R, c->stream, g_create_err);
         if (rc) { dode_destroy(c); cudaGetLastError(); return rc; }
@@ -710,6 +718,63 @@ int dode_spgd_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta) {
 int dode_join(dode_ctx* ctx) {
     if (!ctx) return DODE_EINVAL;
     return join_lanes(ctx);
+}
+
+int dode_set_option(dode_ctx* ctx, int32_t option, int32_t value) {
+    if (!ctx) return DODE_EINVAL;
+    switch (option) {
+        case DODE_OPT_TC_MIN_B:
+            if (value < 0) return fail(ctx, DODE_EINVAL, "DODE_OPT_TC_MIN_B must be >= 0");
+            ctx->tc_min_b = value;
+            return DODE_OK;
+        case DODE_OPT_LANES:
+            if (value != 0 && value != 1) return fail(ctx, DODE_EINVAL, "DODE_OPT_LANES must be 0 or 1");
+            ctx->lanes_on = value != 0;
+            return join_lanes(ctx);
+        case DODE_OPT_TC_KSPLIT:
+            if (value < 0 || value > 32) return fail(ctx, DODE_EINVAL, "DODE_OPT_TC_KSPLIT must be in [0, 32]");
+            ctx->opt_ksplit = value;
+            return DODE_OK;
+        case DODE_OPT_PDL:
+            if (value != 0 && value != 1) return fail(ctx, DODE_EINVAL, "DODE_OPT_PDL must be 0 or 1");
+            ctx->opt_pdl = value != 0;
+            return DODE_OK;
+        default:
+            return fail(ctx, DODE_EINVAL, "unknown option %d", option);
+    }
+}
+
+int dode_reserve(dode_ctx* ctx, int32_t max_days) {
+    if (!ctx) return DODE_EINVAL;
+    if (max_days < 1) return fail(ctx, DODE_EINVAL, "max_days must be >= 1");
+    const dode_dims& d = ctx->dm;
+    int rc;
+    if (d.storage == DODE_CSR) {
+        const int bp = csr_bp(std::min<int>(max_days, kCsrMaxDays));
+        if ((rc = ensure_buf(ctx, &ctx->r, &ctx->r_cap, (size_t)d.T * ctx->Lp * std::max(bp, 64)))) return rc;
+        if ((rc = csr_ensure(ctx->csr, d, ctx->Np, std::max(bp, 64), ctx->stream))) return fail(ctx, rc, "CSR scratch allocation failed");
+    } else {
+        const int w = round_up(std::min<int>(max_days, kMaxDays), 16);
+        const size_t dayStride = (size_t)d.T * ctx->Np;
+        // FFMA panels (b < DODE_OPT_TC_MIN_B, and dode_objective's sub-batches of 64 days)
+        if ((rc = ensure_buf(ctx, &ctx->r, &ctx->r_cap, (size_t)d.T * ctx->Lp * std::max(w, 64)))) return rc;
+        if ((rc = ensure_buf(ctx, &ctx->Qb, &ctx->qb_cap, dayStride * std::max(w, 64)))) return rc;
+        if (ctx->tc_ready && ctx->tc_min_b > 0 && max_days >= ctx->tc_min_b) {
+            for (Lane& ln : ctx->lane)
+                if ((rc = lane_init(ctx, ln))) return rc;
+            size_t part = 0;
+            for (int bn = 16; bn <= w; bn += 16) part = std::max(part, tc_geometry(ctx, bn).part_floats);
+            struct { TcBuf* tb; cudaStream_t st; } bufs[3] = {{&ctx->tcb, ctx->stream}, {&ctx->lane[0].buf, ctx->lane[0].st},
+                                                              {&ctx->lane[1].buf, ctx->lane[1].st}};
+            for (auto& b : bufs) {
+                if ((rc = tc_ensure(ctx, *b.tb, b.st, w))) return rc;
+                if ((rc = tc_ensure_part(ctx, *b.tb, b.st, part))) return rc;
+            }
+        }
+    }
+    CU(sync_all(ctx));
+    CU(cudaGetLastError());
+    return DODE_OK;
 }
 
 int dode_adagrad_step(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, float eps, const uint8_t* row_mask) {
@@ -753,6 +818,20 @@ stage_gather_q(const float* __restrict__ q, float* __restrict__ stage, int T, in
     }
 }
 
+// device staging of the streaming step: two halves each, ping-pong over calls
+static int ensure_staging(dode_ctx* ctx, int n) {
+    const dode_dims& d = ctx->dm;
+    const size_t TL = (size_t)d.T * d.L, TN = (size_t)d.T * d.N;
+    if (ctx->stage_x_cap >= TL * n && ctx->stage_q_cap >= TN * n) return DODE_OK;
+    CU(sync_all(ctx));
+    cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
+    ctx->stage_x = ctx->stage_q = nullptr; ctx->stage_x_cap = ctx->stage_q_cap = 0;
+    CU(cudaMalloc(&ctx->stage_x, 2 * TL * n * sizeof(float)));
+    CU(cudaMalloc(&ctx->stage_q, 2 * TN * n * sizeof(float)));
+    ctx->stage_x_cap = TL * n; ctx->stage_q_cap = TN * n;
+    return DODE_OK;
+}
+
 int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, const float* x_host, float* q_host) {
     if (!ctx) return DODE_EINVAL;
     int c = 0, rc;
@@ -780,14 +859,7 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
         CU(cudaStreamWaitEvent(ctx->s_sc, ctx->ev_fence, 0));
         ctx->plain_since_host = false;
     }
-    if (ctx->stage_x_cap < TL * n || ctx->stage_q_cap < TN * n) {
-        CU(sync_all(ctx));
-        cudaFree(ctx->stage_x); cudaFree(ctx->stage_q);
-        ctx->stage_x = ctx->stage_q = nullptr; ctx->stage_x_cap = ctx->stage_q_cap = 0;
-        CU(cudaMalloc(&ctx->stage_x, 2 * TL * n * sizeof(float)));      // two halves, ping-pong over calls
-        CU(cudaMalloc(&ctx->stage_q, 2 * TN * n * sizeof(float)));
-        ctx->stage_x_cap = TL * n; ctx->stage_q_cap = TN * n;
-    }
+    if ((rc = ensure_staging(ctx, n))) return rc;
     // One-deep software pipeline over calls i: upload(i+1) || step(i) || download(i-1), on five streams:
     //   s_h2d / s_d2h  carry ONLY the PCIe copies, so each copy engine runs them back to back (a kernel between two copies
     //                  on a copy stream left the engine idle for the kernel plus two engine hand-overs per call)
@@ -1033,7 +1105,7 @@ int dode_lipschitz(dode_ctx* ctx, int32_t c, int32_t iters, double* L_out) {
         if ((rc = apply_t_padded(ctx, c, ctx->pw))) return rc;
     }
     CU(cudaMemcpyAsync(L_out, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
+    CU(sync_all(ctx));
     CU(cudaGetLastError());
     return DODE_OK;
 }
@@ -1087,7 +1159,7 @@ int dode_timing_enable(dode_ctx* ctx, int32_t on) {
 int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches, int32_t reset) {
     if (!ctx) return DODE_EINVAL;
     if (kind < 0 || kind > 2) return fail(ctx, DODE_EINVAL, "kind must be 0 (forward), 1 (gradient+update) or 2");
-    CU(cudaStreamSynchronize(ctx->stream));
+    CU(sync_all(ctx));
     for (auto& p : ctx->ev_pending) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, p.a, p.b) == cudaSuccess) { ctx->t_total[p.kind] += ms; ctx->t_count[p.kind]++; }
@@ -1099,12 +1171,6 @@ int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* lau
     if (reset) { ctx->t_total[kind] = 0; ctx->t_count[kind] = 0; }
     return DODE_OK;
 }
-
-#ifdef DODE_TC_TRACE
-int dode_debug_trace(long long* host, int n) {
-    return (int)cudaMemcpyFromSymbol(host, tc::g_trace, sizeof(long long) * n);
-}
-#endif
 
 int64_t dode_launch_count(const dode_ctx* ctx) { return ctx ? ctx->launches : 0; }
 

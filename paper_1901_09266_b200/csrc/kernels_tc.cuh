@@ -135,8 +135,6 @@ struct TcParams {
     // ranges in a fixed order and applies the pass's epilogue.  ksplit = 1: the fused epilogue below.
     int ksplit;
     float* part;
-    int dbg;             // bring-up switches (results invalid): 1 = no split, 2 = no MMA, 4 = no epilogue, 8 = no B_lo load,
-                         // 128 = no B load; 16 = A tiles not requested ahead of the dependency wait (valid)
 };
 
 __device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -187,14 +185,6 @@ __device__ __forceinline__ void tmem_ld16x2_wait(uint32_t t0, uint32_t t1, uint3
         : "r"(t0), "r"(t1) : "memory");
 }
 
-#ifdef DODE_TC_TRACE
-// bring-up instrumentation (not built by default): per-chunk SM clock stamps of one CTA
-constexpr int kTraceNk = 512;
-__device__ long long g_trace[4 * kTraceNk * 4];
-#define TC_TRACE(role, kc, slot) do { if (tracing && (kc) < kTraceNk) g_trace[(((role) * kTraceNk) + (kc)) * 4 + (slot)] = clock64(); } while (0)
-#else
-#define TC_TRACE(role, kc, slot) do {} while (0)
-#endif
 
 // ADA = true compiles in the NEXT-1 epilogues (row mask on r, Adagrad accumulator).  It is a template parameter, not a
 // run-time branch, because the extra live values cost 25 registers: 117 x 320 threads no longer fits two CTAs per SM.
@@ -208,9 +198,6 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
     const int m0 = blockIdx.x * kTileM;
-#ifdef DODE_TC_TRACE
-    const bool tracing = p.mode == 0 && blockIdx.y == gridDim.y / 2 && blockIdx.x == gridDim.x / 2;
-#endif
     const int bBytes = p.bn * kTileK * 4;
     const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full | B_lo
     const int nring = p.nring;
@@ -268,10 +255,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     // under that kernel's tail.  The B tiles (panels written by the previous kernel) follow after the wait; the stage's
     // barrier expects the bytes of all three loads from the start.
     const int npre = min(p.stages, nk);
-    // bring-up switches (results invalid): 8 = do not load B_lo, 128 = load no B tile at all
-    const int nB = (p.dbg & 128) ? 0 : (p.dbg & 8) ? 1 : 2;
-    const int txBytes = aBytes + nB * bBytes;
-    if (warp == 0 && !(p.dbg & 16)) {
+    const int txBytes = aBytes + 2 * bBytes;
+    if (warp == 0) {
         if (elect_one()) {
             for (int kc = 0; kc < npre; ++kc) {
                 mbar_expect_tx(&full[kc], txBytes);
@@ -320,17 +305,15 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         // ===== TMA producer =====
         int s = 0, ph = 1;                                       // ph: parity of the previous round of slot s
         for (int kc = 0; kc < nk; ++kc) {
-            TC_TRACE(0, kc, 0);
             if (kc >= p.stages) mbar_wait(&empty[s], ph);
-            TC_TRACE(0, kc, 1);
             if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
-                if (kc >= npre || (p.dbg & 16)) {               // (the first round's A tiles were requested before the wait)
+                if (kc >= npre) {                               // (the first round's A tiles were requested before the wait)
                     mbar_expect_tx(&full[s], txBytes);
                     tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
                 }
-                if (nB >= 1) tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
-                if (nB >= 2) tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
+                tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
+                tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
             }
             __syncwarp();
             if (++s == p.stages) { s = 0; ph ^= 1; }
@@ -342,39 +325,32 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         for (int kc = 0; kc < nk; ++kc) {
             const int g = kc & 1, use = kc >> 1;
             const int jr = g * per_group + use % per_group;
-            TC_TRACE(1, kc, 0);
             mbar_wait(&full[s], ph);
-            TC_TRACE(1, kc, 1);
             mbar_wait(&split[jr], (use / per_group) & 1);
-            TC_TRACE(1, kc, 2);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes, bl0 = bf0 + bBytes;
             const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
             if (elect_one()) {
-                if (p.dbg & 2) { mbar_arrive(&empty[s]); mbar_arrive(&a_empty[jr]); }            // bring-up: no MMA
-                else {
 #pragma unroll
-                    for (int k = 0; k < kTileK / 8; ++k) {       // UMMA_K = 8 for tf32: 32 bytes along the swizzle span
-                        const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
-                        if (fused_n) {
-                            umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, (kc | k) != 0);   // [a_hi*b_full | a_hi*b_lo]
-                            umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);               //  a_lo*b_full
-                        } else {
-                            const uint64_t dbl = umma_desc_k_sw128(bl0 + k * 32);
-                            umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc1, (kc | k) != 0);
-                            umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);
-                            umma_tf32_ts(tmem_d, ahi + k * 8, dbl, idesc1, 1);
-                        }
+                for (int k = 0; k < kTileK / 8; ++k) {           // UMMA_K = 8 for tf32: 32 bytes along the swizzle span
+                    const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
+                    if (fused_n) {
+                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, (kc | k) != 0);       // [a_hi*b_full | a_hi*b_lo]
+                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);                   //  a_lo*b_full
+                    } else {
+                        const uint64_t dbl = umma_desc_k_sw128(bl0 + k * 32);
+                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc1, (kc | k) != 0);
+                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);
+                        umma_tf32_ts(tmem_d, ahi + k * 8, dbl, idesc1, 1);
                     }
-                    umma_commit(&empty[s]);
-                    umma_commit(&a_empty[jr]);
                 }
+                umma_commit(&empty[s]);
+                umma_commit(&a_empty[jr]);
             }
             __syncwarp();
-            TC_TRACE(1, kc, 3);
             if (++s == p.stages) { s = 0; ph ^= 1; }
         }
-        if (elect_one()) { if ((p.dbg & 2) || nk == 0) mbar_arrive(accum); else umma_commit(accum); }
+        if (elect_one()) { if (nk == 0) mbar_arrive(accum); else umma_commit(accum); }
         __syncwarp();
     } else {
         // ===== splitters: smem column -> registers -> TMEM (A_hi, A_lo); group g takes chunks kc = g, g+2, ... =====
@@ -387,15 +363,12 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (s == 0) ph ^= 1;
             const int use = kc >> 1;
             const int jr = group * per_group + use % per_group;
-            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 0);
             // every group observes EVERY phase of every full barrier (also for the other group's chunks): a parity
             // wait is only sound for a waiter that never falls a whole phase behind or skips one
             mbar_wait(&full[s], ph);
             if ((kc & 1) != group) continue;
-            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 1);
             if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1);
-            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 2);
-            if (lane_base >= BM || (p.dbg & 1)) { mbar_arrive(&split[jr]); continue; }    // rows never stored
+            if (lane_base >= BM) { mbar_arrive(&split[jr]); continue; }    // rows never stored
             const float* A = reinterpret_cast<const float*>(smem + (size_t)s * stageBytes) + row;
             uint32_t hi[32], lo[32];
 #pragma unroll
@@ -410,13 +383,12 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             mbar_arrive(&split[jr]);
-            if ((warp & 3) == 2 && lane == 0) TC_TRACE(2 + group, kc, 3);
         }
         // ---- epilogue ----
         mbar_wait(accum, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int m = m0 + row;
-        for (int c0 = 16 * group; c0 < p.bn && !(p.dbg & 4); c0 += 32) {
+        for (int c0 = 16 * group; c0 < p.bn; c0 += 32) {
             uint32_t v[16], w[16];
             const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
             float cur[16];

@@ -56,12 +56,7 @@ class GpuSolver:
     """Owns one dode ctx on cuda:0 for a Problem."""
 
     def __init__(self, p: Problem, csr: bool = False, q0: float = 1.0, tc_min_b: Optional[int] = None):
-        import os
         import paper_1901_09266_b200 as P
-        if tc_min_b is None:
-            os.environ.pop("DODE_TC_MIN_B", None)
-        else:
-            os.environ["DODE_TC_MIN_B"] = str(tc_min_b)      # read by dode_create
         self.P, self.p = P, p
         cfg = p.cfg
         dev = torch.device("cuda:0")
@@ -73,6 +68,8 @@ class GpuSolver:
             Rd = p.R.to(dev)
             self.h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, p.labels, xd, q0, dense=Rd)
         # the library keeps no caller pointer: dropping Rd / xd here is part of the contract under test
+        if tc_min_b is not None:
+            P.dode_set_option(self.h, P.DODE_OPT_TC_MIN_B, tc_min_b)
 
     def run(self, sched, etas):
         for c, days in sched:

@@ -50,3 +50,13 @@ def test_oracle_and_cuda_sources_share_nothing():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert not pat.search(open(os.path.join(root, f)).read()), f
+
+
+def test_library_reads_nothing_from_the_environment():
+    """include/dode.h: "no global state" — kernel selection is steered by dode_set_option only."""
+    csrc = os.path.join(ROOT, "paper_1901_09266_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+    lib = P.lib()
+    assert lib.dode_set_option(None, 0, 1) == P.DODE_EINVAL
+    assert lib.dode_reserve(None, 8) == P.DODE_EINVAL

@@ -22,11 +22,13 @@ def _objective_cpu(p, q, days):
     return np.array([o.objective_day(p.R[p.labels[d]].numpy(), q[i], p.x[d].numpy()) for i, d in enumerate(days)])
 
 
-def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False, tc_min_b=None):
+def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False, tc_min_b=None, ksplit=None):
     p = hz.make_problem_sparse(cfg) if sparse_gen else hz.make_problem(cfg)
     sched = synth.schedule(cfg, p.labels, K=K, b=b)
     etas = hz.oracle_etas(p)
     g = hz.GpuSolver(p, csr=csr, tc_min_b=tc_min_b)
+    if ksplit is not None:
+        g.P.dode_set_option(g.h, g.P.DODE_OPT_TC_KSPLIT, ksplit)
     g.run(sched, etas)
     days = list(range(cfg.D)) if sample is None else list(sample)
     q_gpu = g.q(days)
@@ -336,12 +338,11 @@ def test_short_time_axis_split_k(T, H, N, L, b):
 
 
 @pytest.mark.parametrize("ks", [2, 5])
-def test_forced_split_k_on_ragged_shapes(ks, monkeypatch):
+def test_forced_split_k_on_ragged_shapes(ks):
     """Forced split counts on ragged shapes: K ranges that are empty near the day boundary, partial tiles, pad days; the
     Adagrad variant goes through the same epilogue kernel."""
-    monkeypatch.setenv("DODE_TC_KSPLIT", str(ks))
     cfg = synth.Config("ragged", N=61, L=137, T=20, H=5, C=2, D=80, b=20, K=12, kmin=3, kmax=9)
-    _run_both(cfg, sample=[0, 1, 40, 79])
+    _run_both(cfg, sample=[0, 1, 40, 79], ksplit=ks)
 
 
 def test_minibatch_larger_than_one_launch():
@@ -349,3 +350,31 @@ def test_minibatch_larger_than_one_launch():
     units); the sub-batches alternate on the internal streams."""
     cfg = synth.Config("wide_b", N=30, L=40, T=12, H=3, C=1, D=640, b=300, K=5, kmin=3, kmax=9, label_mode="zero")
     assert "tcgen05" in _run_both(cfg, sample=[0, 1, 255, 256, 299, 300, 639])
+
+
+def test_options_and_reserve_keep_results():
+    """dode_set_option / dode_reserve (include/dode.h): every option value gives the oracle's iterates; unknown options
+    and out-of-range values are DODE_EINVAL and change nothing; after dode_reserve(b) the steps allocate nothing (the
+    launch count grows by exactly the kernels of the steps and device memory does not move)."""
+    cfg = synth.Config("opts", N=70, L=90, T=20, H=3, C=2, D=96, b=24, K=10, kmin=3, kmax=9)
+    p = hz.make_problem(cfg)
+    sched = synth.schedule(cfg, p.labels)
+    etas = hz.oracle_etas(p)
+    want = hz.oracle_run(p, sched, etas)
+    for opts in ({}, {"LANES": 0}, {"PDL": 0}, {"LANES": 0, "PDL": 0, "TC_KSPLIT": 3}, {"TC_MIN_B": 0}, {"TC_MIN_B": 100}):
+        g = hz.GpuSolver(p)
+        P = g.P
+        for k, v in opts.items():
+            P.dode_set_option(g.h, getattr(P, "DODE_OPT_" + k), v)
+        for bad in ((99, 1), (P.DODE_OPT_LANES, 2), (P.DODE_OPT_TC_KSPLIT, 33), (P.DODE_OPT_TC_MIN_B, -1), (P.DODE_OPT_PDL, -1)):
+            with pytest.raises(P.DodeError) as e:
+                P.dode_set_option(g.h, *bad)
+            assert e.value.code == P.DODE_EINVAL
+        P.dode_reserve(g.h, cfg.b)
+        free0 = torch.cuda.mem_get_info()[0]
+        g.run(sched, etas)
+        assert torch.cuda.mem_get_info()[0] == free0, "a step allocated device memory after dode_reserve"
+        path = P.dode_last_path(g.h)
+        assert ("ffma" in path) == (opts.get("TC_MIN_B") in (0, 100)), (opts, path)
+        hz.assert_q_close(g.q(), want, f"options {opts}")
+        g.close()
