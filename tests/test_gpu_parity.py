@@ -362,6 +362,11 @@ def test_options_and_reserve_keep_results():
     etas = hz.oracle_etas(p)
     want = hz.oracle_run(p, sched, etas)
     for opts in ({}, {"LANES": 0}, {"PDL": 0}, {"LANES": 0, "PDL": 0, "TC_KSPLIT": 3}, {"TC_MIN_B": 0}, {"TC_MIN_B": 100}):
+        g0 = hz.GpuSolver(p)                           # a throw-away pass first: the CUDA runtime loads kernel modules
+        for k, v in opts.items():                      # lazily, which moves device memory at a kernel's first launch
+            g0.P.dode_set_option(g0.h, getattr(g0.P, "DODE_OPT_" + k), v)
+        g0.run(sched, etas)
+        g0.close()
         g = hz.GpuSolver(p)
         P = g.P
         for k, v in opts.items():
