@@ -29,13 +29,19 @@
 // iteration, P6 Example 1, P8 adjoint, P9 descent,
 // P10 separability, P12 dense assembly by Table 2, P13 dense-vs-CSR, P14 R2 closed forms,
 // P15 row-chunk Adagrad against torch.optim.Adagrad on the assembled matrix, P16 DAR construction (O7): the paper's
-// Example 3 worked by hand, the constant-speed closed form, unit row sums, vehicle conservation through O2a.
+// Example 3 worked by hand, the constant-speed closed form, unit row sums, vehicle conservation through O2a,
+// P10b run_schedule with several clusters and a different step per iteration against per-day visit replays,
+// P18 the multi-visit day replays (oracle_replay_day / _csr: the same loops with the OUTPUT rows of a pass handed to
+// several threads, every output element accumulated in the same order) bit for bit against repeated oracle_visit.
 // No function here is "parity unpinned".
 #include <algorithm>
 #include <cmath>
 #include <cstddef>
 #include <cstdint>
+#include <chrono>
 #include <cstring>
+#include <functional>
+#include <thread>
 #include <vector>
 
 namespace {
@@ -46,9 +52,9 @@ inline size_t blk(const Dims& d, int s, int h) {            // offset of R_c[s][
     return ((size_t)s * (d.H + 1) + h) * (size_t)d.L * d.N;
 }
 
-// O2a in double (no rounding of r); x may be null (then r = rho q).
-void forward_d(const Dims& d, const float* Rc, const float* q, const float* x, double* r) {
-    for (int t = 0; t < d.T; ++t)
+// O2a in double (no rounding of r) for the output rows t0 <= t < t1; x may be null (then r = rho q).
+void forward_rows(const Dims& d, const float* Rc, const float* q, const float* x, double* r, int t0, int t1) {
+    for (int t = t0; t < t1; ++t)
         for (int l = 0; l < d.L; ++l) {
             double acc = 0.0;
             const int hmax = d.H < t ? d.H : t;
@@ -61,9 +67,13 @@ void forward_d(const Dims& d, const float* Rc, const float* q, const float* x, d
         }
 }
 
-// O2b: g = rho^T r, r given in fp32 storage.
-void gradient_f(const Dims& d, const float* Rc, const float* r, double* g) {
-    for (int s = 0; s < d.T; ++s)
+void forward_d(const Dims& d, const float* Rc, const float* q, const float* x, double* r) {
+    forward_rows(d, Rc, q, x, r, 0, d.T);
+}
+
+// O2b: g = rho^T r, r given in fp32 storage, for the output rows s0 <= s < s1.
+void gradient_rows(const Dims& d, const float* Rc, const float* r, double* g, int s0, int s1) {
+    for (int s = s0; s < s1; ++s)
         for (int n = 0; n < d.N; ++n) {
             double acc = 0.0;
             const int hmax = d.H < d.T - 1 - s ? d.H : d.T - 1 - s;
@@ -74,6 +84,24 @@ void gradient_f(const Dims& d, const float* Rc, const float* r, double* g) {
             }
             g[(size_t)s * d.N + n] = acc;
         }
+}
+
+void gradient_f(const Dims& d, const float* Rc, const float* r, double* g) {
+    gradient_rows(d, Rc, r, g, 0, d.T);
+}
+
+// fn(i0, i1) over a partition of [0, n) into `threads` contiguous ranges, one std::thread each (threads <= 1: inline).
+// Used only to hand DIFFERENT OUTPUT ROWS of one pass to different threads: no output element is shared, and the
+// order in which each element's sum is accumulated does not depend on the partition.
+void parallel_rows(int n, int threads, const std::function<void(int, int)>& fn) {
+    if (threads <= 1 || n <= 1) { fn(0, n); return; }
+    threads = std::min(threads, n);
+    std::vector<std::thread> pool;
+    for (int k = 0; k < threads; ++k) {
+        const int i0 = (int)((long)n * k / threads), i1 = (int)((long)n * (k + 1) / threads);
+        pool.emplace_back(fn, i0, i1);
+    }
+    for (auto& th : pool) th.join();
 }
 
 void visit(const Dims& d, const float* Rc, float* q, const float* x, float eta,
@@ -233,12 +261,11 @@ double oracle_power_iteration(int N, int L, int T, int H, const float* Rc, int i
 // sparse representation"; Table 2 "Sparse").
 // blk_off[(s*(H+1)+h)] = first nnz of block (s,h) (int64, T*(H+1)+1 entries, for this cluster);
 // row_ptr[(s*(H+1)+h)*(L+1) + l] = offset of row l relative to the block start; col = OD index n.
-void oracle_visit_csr(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
-                      const int32_t* col_idx, const float* val, float* q, const float* x, float eta) {
-    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
-    std::vector<float> rf(TL);
-    std::vector<double> g(TN, 0.0);
-    for (int t = 0; t < T; ++t)
+static void csr_forward_rows(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
+                             const int32_t* col_idx, const float* val, const float* q, const float* x, float* rf,
+                             int t0, int t1) {
+    (void)T;
+    for (int t = t0; t < t1; ++t)
         for (int l = 0; l < L; ++l) {
             double acc = 0.0;
             const int hmax = H < t ? H : t;
@@ -250,7 +277,12 @@ void oracle_visit_csr(int N, int L, int T, int H, const int64_t* blk_off, const 
             }
             rf[(size_t)t * L + l] = (float)(acc - (double)x[(size_t)t * L + l]);
         }
-    for (int s = 0; s < T; ++s) {
+}
+
+// g rows s0 <= s < s1 (g zeroed by the caller); every entry of block (s,h) adds into row s only
+static void csr_gradient_rows(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
+                              const int32_t* col_idx, const float* val, const float* rf, double* g, int s0, int s1) {
+    for (int s = s0; s < s1; ++s) {
         const int hmax = H < T - 1 - s ? H : T - 1 - s;
         for (int h = 0; h <= hmax; ++h) {
             const size_t b = (size_t)s * (H + 1) + h;
@@ -260,10 +292,73 @@ void oracle_visit_csr(int N, int L, int T, int H, const int64_t* blk_off, const 
                     g[(size_t)s * N + col_idx[k]] += (double)val[k] * (double)rf[(size_t)(s + h) * L + l];
         }
     }
+}
+
+void oracle_visit_csr(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
+                      const int32_t* col_idx, const float* val, float* q, const float* x, float eta) {
+    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<float> rf(TL);
+    std::vector<double> g(TN, 0.0);
+    csr_forward_rows(N, L, T, H, blk_off, row_ptr, col_idx, val, q, x, rf.data(), 0, T);
+    csr_gradient_rows(N, L, T, H, blk_off, row_ptr, col_idx, val, rf.data(), g.data(), 0, T);
     for (size_t i = 0; i < TN; ++i) {
         const double v = (double)q[i] - (double)eta * g[i];
         q[i] = (float)(v > 0.0 ? v : 0.0);
     }
+}
+
+// Multi-visit replay of ONE day for the full-K parity tests ("the oracle replays the full K-iteration
+// schedule for a seeded sample of days"; days are independent units).  `visits` consecutive visits with
+// the same operator and step — O2a, O2b, O2c exactly as oracle_visit / oracle_visit_csr compute them (the same row
+// functions; r complete before any q changes) — with the output rows of each pass split over `threads` threads.
+// After visit number ckpt[j] (1-based, ascending) q is copied to out[j].  The replay stops early once `budget_s`
+// seconds have passed (checked between visits; <= 0: no limit); the number of visits done is returned.
+int oracle_replay_day(int N, int L, int T, int H, const float* Rc, float* q, const float* x, float eta, int visits,
+                      const int32_t* ckpt, int nckpt, float* out, int threads, double budget_s) {
+    Dims d{N, L, T, H};
+    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<double> rd(TL), g(TN);
+    std::vector<float> rf(TL);
+    const auto t_start = std::chrono::steady_clock::now();
+    int j = 0, v = 0;
+    for (; v < visits; ++v) {
+        if (budget_s > 0 && v > 0 &&
+            std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count() > budget_s) break;
+        parallel_rows(T, threads, [&](int t0, int t1) { forward_rows(d, Rc, q, x, rd.data(), t0, t1); });
+        for (size_t i = 0; i < TL; ++i) rf[i] = (float)rd[i];                 // r stored fp32 (O2a)
+        parallel_rows(T, threads, [&](int s0, int s1) { gradient_rows(d, Rc, rf.data(), g.data(), s0, s1); });
+        for (size_t i = 0; i < TN; ++i) {                                     // O2c
+            const double w = (double)q[i] - (double)eta * g[i];
+            q[i] = (float)(w > 0.0 ? w : 0.0);
+        }
+        while (j < nckpt && ckpt[j] == v + 1) { std::memcpy(out + (size_t)j * TN, q, TN * sizeof(float)); ++j; }
+    }
+    return v;
+}
+
+int oracle_replay_day_csr(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,
+                          const int32_t* col_idx, const float* val, float* q, const float* x, float eta, int visits,
+                          const int32_t* ckpt, int nckpt, float* out, int threads, double budget_s) {
+    const size_t TL = (size_t)T * L, TN = (size_t)T * N;
+    std::vector<float> rf(TL);
+    std::vector<double> g(TN);
+    const auto t_start = std::chrono::steady_clock::now();
+    int j = 0, v = 0;
+    for (; v < visits; ++v) {
+        if (budget_s > 0 && v > 0 &&
+            std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count() > budget_s) break;
+        std::fill(g.begin(), g.end(), 0.0);
+        parallel_rows(T, threads, [&](int t0, int t1) {
+            csr_forward_rows(N, L, T, H, blk_off, row_ptr, col_idx, val, q, x, rf.data(), t0, t1); });
+        parallel_rows(T, threads, [&](int s0, int s1) {
+            csr_gradient_rows(N, L, T, H, blk_off, row_ptr, col_idx, val, rf.data(), g.data(), s0, s1); });
+        for (size_t i = 0; i < TN; ++i) {
+            const double w = (double)q[i] - (double)eta * g[i];
+            q[i] = (float)(w > 0.0 ? w : 0.0);
+        }
+        while (j < nckpt && ckpt[j] == v + 1) { std::memcpy(out + (size_t)j * TN, q, TN * sizeof(float)); ++j; }
+    }
+    return v;
 }
 
 double oracle_objective_day_csr(int N, int L, int T, int H, const int64_t* blk_off, const int32_t* row_ptr,

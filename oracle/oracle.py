@@ -22,7 +22,7 @@ _lib = None
 
 def build_oracle(force: bool = False) -> str:
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-o", _SO, _SRC])
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", _SO, _SRC])
     return _SO
 
 
@@ -148,6 +148,34 @@ def visit_csr(N: int, L: int, T: int, H: int, blk_off, row_ptr, col_idx, val, q,
                            col_idx.ctypes.data_as(C.POINTER(C.c_int32)), pv,
                            q.ctypes.data_as(C.POINTER(C.c_float)), px, C.c_float(eta))
     return q
+
+
+def replay_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray, eta: float, visits: int, checkpoints: Sequence[int],
+               threads: int = 1, budget_s: float = 0.0, csr=None):
+    """``visits`` consecutive visits of one day (exactly ``visit`` / ``visit_csr`` repeated; pin P18), the output rows of
+    each pass split over ``threads`` threads.  Returns (q after each checkpoint visit count reached, visits done): the
+    replay stops early once ``budget_s`` seconds have passed.  ``csr`` = (N, L, T, H, blk_off, row_ptr, col_idx, val)
+    replays through the CSR loops instead (then ``Rc`` is ignored)."""
+    ck = np.ascontiguousarray(sorted(int(c) for c in checkpoints), dtype=np.int32)
+    assert ck.size == 0 or (ck[0] >= 1 and ck[-1] <= visits)
+    x, px = _f(x)
+    q = np.array(q, dtype=np.float32, order="C", copy=True)
+    out = np.empty((ck.size,) + q.shape, np.float32)
+    pq, po, pc = q.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p), ck.ctypes.data_as(C.c_void_p)
+    if csr is None:
+        N, L, T, H = _dims(Rc)
+        Rc, pR = _f(Rc)
+        done = lib().oracle_replay_day(N, L, T, H, pR, pq, px, C.c_float(eta), int(visits), pc, int(ck.size), po,
+                                       int(threads), C.c_double(budget_s))
+    else:
+        N, L, T, H, blk_off, row_ptr, col_idx, val = csr
+        blk_off = np.ascontiguousarray(blk_off, np.int64); row_ptr = np.ascontiguousarray(row_ptr, np.int32)
+        col_idx = np.ascontiguousarray(col_idx, np.int32); val, pv = _f(val)
+        done = lib().oracle_replay_day_csr(N, L, T, H, blk_off.ctypes.data_as(C.c_void_p), row_ptr.ctypes.data_as(C.c_void_p),
+                                           col_idx.ctypes.data_as(C.c_void_p), pv, pq, px, C.c_float(eta), int(visits),
+                                           pc, int(ck.size), po, int(threads), C.c_double(budget_s))
+    reached = [int(c) for c in ck if c <= done]
+    return {c: out[i] for i, c in enumerate(reached)}, int(done)
 
 
 def objective_day_csr(N: int, L: int, T: int, H: int, blk_off, row_ptr, col_idx, val, q, x) -> float:

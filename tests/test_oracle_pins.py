@@ -248,6 +248,68 @@ def test_p10_separability_and_schedule(tiny12):
     np.testing.assert_array_equal(q5, qa[5])
 
 
+def test_p10b_schedule_with_several_clusters_and_a_step_per_iteration():
+    """oracle_run_schedule picks the operator by the DAY's label and the step by the ITERATION (dode_oracle.cpp: `R +
+    Rc_sz * labels[day]`, `sched_eta[k]`).  Pinned against replays that use nothing but oracle.visit with R[labels[d]]
+    and eta[k], bit for bit, on C = 3 clusters whose operators differ and with a different step in every iteration: a
+    wrong cluster stride, an operator picked by the chunk's position, or a step indexed by day fail it."""
+    cfg = synth.Config("p10b", N=5, L=7, T=9, H=3, C=3, D=17, b=3, K=40, kmin=2, kmax=4)
+    R = synth.dar_dense(cfg).numpy()
+    lab = synth.labels(cfg).numpy()
+    assert len(set(lab.tolist())) == 3 and not np.array_equal(R[0], R[1]) and not np.array_equal(R[1], R[2])
+    x = synth.counts(cfg, torch.from_numpy(R), synth.q_true(cfg), torch.from_numpy(lab)).numpy()
+    sched = synth.schedule(cfg, lab)
+    base = [_eta(R[c]) for c in range(cfg.C)]
+    etas = [np.float32(base[c] * (0.35 + 0.6 * ((7 * k) % 11) / 11.0)) for k, (c, _) in enumerate(sched)]
+    assert len(set(float(e) for e in etas)) > 20
+    q0 = (1.0 + np.random.default_rng(3).random((cfg.D, cfg.T, cfg.N))).astype(np.float32)
+    got = oracle.run_schedule(R, lab, x, q0, sched, etas)
+    want = q0.copy()
+    for k, (c, days) in enumerate(sched):
+        for d in days:
+            assert lab[d] == c
+            want[d] = oracle.visit(R[lab[d]], want[d], x[d], float(etas[k]))
+    np.testing.assert_array_equal(got, want)
+    assert not np.array_equal(got, q0)
+    # and the mistakes it is meant to catch do change the result on this instance
+    wrong = q0.copy()
+    for k, (c, days) in enumerate(sched):
+        for d in days:
+            wrong[d] = oracle.visit(R[(lab[d] + 1) % cfg.C], wrong[d], x[d], float(etas[k]))
+    assert np.abs(wrong - want).max() > 1e-3
+
+
+@pytest.mark.parametrize("threads", [1, 3, 8])
+def test_p18_day_replay_equals_repeated_visits(tiny12, threads):
+    """oracle_replay_day / oracle_replay_day_csr (the full-K replays of the GPU parity tests): the output rows of each
+    pass go to several threads, every output element is accumulated in the same order — so any thread count, dense or
+    CSR, must reproduce repeated oracle_visit / oracle_visit_csr BIT FOR BIT at every checkpoint."""
+    cfg, R, lab, qt, x, _ = tiny12
+    eta = _eta(R[0])
+    q0 = (1.0 + np.random.default_rng(8).random((cfg.T, cfg.N))).astype(np.float32)
+    ck = [1, 2, 5, 11, 12]
+    got, done = oracle.replay_day(R[0], q0, x[6], eta, 12, ck, threads=threads)
+    assert done == 12 and sorted(got) == ck
+    q = q0
+    for v in range(1, 13):
+        q = oracle.visit(R[0], q, x[6], eta)
+        if v in got:
+            np.testing.assert_array_equal(got[v], q)
+    assert (q == 0).any() and (q > 0).any()          # the projection is active on this instance
+    csr = synth.dense_to_csr(torch.from_numpy(R))
+    arrs = (cfg.N, cfg.L, cfg.T, cfg.H, csr.blk_off.numpy(), csr.row_ptr.numpy(), csr.col_idx.numpy(), csr.val.numpy())
+    got, done = oracle.replay_day(None, q0, x[6], eta, 7, [3, 7], threads=threads, csr=arrs)
+    q = q0
+    for v in range(1, 8):
+        q = oracle.visit_csr(*arrs, q, x[6], eta)
+        if v in got:
+            np.testing.assert_array_equal(got[v], q)
+    assert done == 7 and sorted(got) == [3, 7]
+    # a spent time budget stops the replay between visits and reports how far it got
+    got, done = oracle.replay_day(R[0], q0, x[6], eta, 100000, [1, 100000], threads=threads, budget_s=0.05)
+    assert 1 <= done < 100000 and sorted(got) == [1]
+
+
 def test_schedule_epoch_structure():
     """A8: per epoch every day appears exactly once; chunks are same-cluster, <= b, ragged tails kept."""
     cfg = synth.CONFIGS["corridor"]
