@@ -4,7 +4,9 @@ dominant kernel and the CPU oracle timed beside it.
 
 A *step* is one SPGD epoch of the workload: every day receives exactly one projected-gradient step, i.e.
 sum_c ceil(D_c / b) calls of dode_spgd_step (a1-a4 of SURVEY.md §8(a)) in the seeded A8 schedule order.
-Default workload: BASELINE.json configs[1] ("corridor": N=60 L=120 T=288 H=12 C=4 D=365, minibatch 32).
+Default workload: BASELINE.json configs[3] ("large_dense": N=1000 L=800 T=288 H=12 C=2 D=1096), the largest dense
+single-GPU workload and the one north_star's roofline targets are defined on: the G8 minibatch sweep b in {1, 8, 64, 256},
+each width from a fresh q0; the line's `value`, `roofline`, `e2e` are those of b = 256 and `sweep` carries all four.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--b B] [--impl reference]
 
@@ -30,9 +32,12 @@ from paper_1901_09266_b200 import synth
 
 METRIC = "spgd_epoch_time_over_all_days"
 UNIT = "ms/epoch"
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 flop x clocks.max.sm
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # NOMINAL: SMs x FP32 lanes x 2 flop x clocks.max.sm; the rooflines
+                                                    # divide by the MEASURED rate (dode_probe_fp32_peak), both are printed
 
 
+DEFAULT_WORKLOAD = "large_dense"          # BASELINE.json configs[3]: the largest dense single-GPU workload, where
+LARGE_DENSE_SWEEP = (1, 8, 64, 256)       # north_star defines its >= 0.70 HBM / >= 0.50 FP32 targets (G8 sweep)
 TF32_OVER_BF16 = 1.1 / 2.25      # nominal dense tensor ratio (B200_PROFILING.md): tf32 1.1 PF vs bf16 2.25 PF
 
 
@@ -152,38 +157,60 @@ def cpu_oracle_sample(cfg, Rc, c0, lab, x, eta, visits):
 
 
 def run_reference(args, cfg, b, rank, world):
-    """--impl reference: the CPU oracle (oracle/), as it stands, on this host; one step = a bounded sample of an
-    epoch (args.ref_visits day-visits), extrapolated to the epoch (x D / visits)."""
+    """--impl reference: the CPU oracle (oracle/), as it stands, on this host's cores.  One step = a bounded sample of an
+    epoch — args.ref_visits day-visits of one cluster's days through oracle.replay_day (the loops of oracle_visit with
+    the output rows over all host threads; pin P18) — and `value` extrapolates it to the epoch (x D / visits).
+    `ms_per_step` is the measured time of a step's sample.  The operator of ONE cluster and the counts of a few of its
+    days are generated here (on the GPU if one is visible — input synthesis only — else on the host)."""
     if rank != 0:
         return
     from oracle import oracle
-    if cfg.N * cfg.L * cfg.T * (cfg.H + 1) * cfg.C * 4 > 8e9:
-        print(json.dumps({"impl": "reference", "unavailable": "workload too large to generate on the host"}))
-        return
-    R = synth.dar_dense(cfg)
-    lab = synth.labels(cfg).numpy()
-    x = synth.counts(cfg, R, synth.q_true(cfg), torch.from_numpy(lab), noise=not cfg.fig12)
-    Rn = [R[c].numpy() for c in range(cfg.C)]
-    etas = [np.float32(1.0 / oracle.power_iteration(Rn[c], 10)) for c in range(cfg.C)]
-    q = np.ones((cfg.D, cfg.T, cfg.N), np.float32)
+    oracle.build_oracle()
+    threads = os.cpu_count() or 1
+    gen_dev = "cuda" if torch.cuda.is_available() else "cpu"
+    cfg1 = cfg.replace(C=1, D=min(cfg.D, 8), label_mode="zero")
+    lab1 = synth.labels(cfg1)
+    if cfg.sparse:
+        csr, x = synth.sparse_problem(cfg1, gen_dev)
+        arrs = (cfg.N, cfg.L, cfg.T, cfg.H, csr.blk_off.cpu().numpy(), csr.row_ptr.cpu().numpy(),
+                csr.col_idx.cpu().numpy(), csr.val.cpu().numpy())
+        Rn = None
+        x = x.cpu().numpy()
+        del csr
+        eta = np.float32(1e-3)                       # any step: one visit costs the same
+    else:
+        R = synth.dar_dense(cfg1, device=gen_dev)
+        x = synth.counts(cfg1, R, synth.q_true(cfg1, gen_dev), lab1, noise=not cfg.fig12).cpu().numpy()
+        Rn = R[0].cpu().numpy()
+        del R
+        arrs = None
+        eta = np.float32(1e-3)
+    if gen_dev == "cuda":
+        torch.cuda.empty_cache()
     v = args.ref_visits
-    times = []
-    day = 0
+    if v is None:                                    # about 1-10 s per step
+        work = (cfg.nb * cfg.L * cfg.N if not cfg.sparse else 4.3e8) * 4 / 3e9 / max(1, threads // 2)
+        v = int(max(1, min(cfg.D, 2.0 / max(work, 1e-4))))
+    q = [np.ones((cfg.T, cfg.N), np.float32) for _ in range(cfg1.D)]
+    times, day = [], 0
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         for _ in range(v):
-            c = int(lab[day])
-            q[day] = oracle.visit(Rn[c], q[day], x[day].numpy(), float(etas[c]))
-            day = (day + 1) % cfg.D
+            got, _ = oracle.replay_day(Rn, q[day], x[day], float(eta), 1, [1], threads=threads, csr=arrs)
+            q[day] = got[1]
+            day = (day + 1) % cfg1.D
         if it >= args.warmup:
             times.append((time.perf_counter() - t0) * 1e3)
-    epoch_ms = float(np.mean(times)) * cfg.D / v
+    step_ms = float(np.mean(times))
+    epoch_ms = step_ms * cfg.D / v
     out = {"impl": "reference", "metric": METRIC, "value": epoch_ms, "unit": UNIT, "n_gpus": args.gpus,
-           "steps": args.steps, "warmup": args.warmup, "ms_per_step": epoch_ms, "higher_is_better": False,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": False,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 storage", "data": "synthetic",
            "config": workload_config(cfg, b),
-           "cpu_baseline": {"value": epoch_ms, "unit": UNIT, "cores": 1, "kind": "oracle",
-                            "sample": f"{v} day-visits per step of the {cfg.D}-visit epoch, extrapolated x{cfg.D / v:.1f}"},
+           "cpu_baseline": {"value": epoch_ms, "unit": UNIT, "cores": threads, "kind": "oracle",
+                            "sample": f"{v} day-visit(s) per step (ms_per_step is that sample's time) of the {cfg.D}-visit epoch, "
+                                      f"oracle_replay_day on {threads} threads, extrapolated x{cfg.D / v:.1f}; inputs generated on {gen_dev}",
+                            "cpu_model": cpu_model()},
            "e2e": {"value": epoch_ms, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out))
 
@@ -196,18 +223,177 @@ def workload_config(cfg, b):
                   "except on the tiny workload"}
 
 
-def traffic_from_profiles(workload, kernel_kind):
-    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` summary, or None."""
+def traffic_from_profiles(workload, b, kernel_kind):
+    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` summaries (profiles/traffic.json,
+    keyed "<workload>_b<minibatch>", else "<workload>"), or None."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if not os.path.exists(p):
         return None
     try:
-        return json.load(open(p)).get(workload, {}).get(kernel_kind)
+        t = json.load(open(p))
+        return (t.get(f"{workload}_b{b}") or t.get(workload) or {}).get(kernel_kind)
     except Exception:
         return None
 
 
-def run_ours(args, cfg, b, rank, world, local_rank):
+def reset_state(P, h, cfg, ones_dev):
+    """q <- q0 = 1 on every day (G8: every minibatch width of the sweep starts from a fresh q0)."""
+    for d in range(cfg.D):
+        P.dode_set_q(h, d, ones_dev)
+
+
+def measure_b(P, h, cfg, lab, etas, b, steps, warmup, timing_epochs, flush, world, dev, nnz_c=None):
+    """Times `steps` SPGD epochs at minibatch b (after `warmup` untimed ones) with CUDA events, L2 flushed before every
+    epoch, then `timing_epochs` more with an event pair around every launch for the roofline of the dominant kernel."""
+    import torch.distributed as dist
+    epochs = make_epochs(cfg, lab, b, warmup + steps)
+    P.dode_reserve(h, min(b, 256))
+
+    def run_epoch(ep):
+        for c, days in ep:
+            P.dode_spgd_step(h, days, float(etas[c]))
+
+    for ep in epochs[:warmup]:
+        run_epoch(ep)
+    P.dode_sync(h)
+    launches0 = P.dode_launch_count(h)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = []
+    wall0 = time.perf_counter()
+    for ep in epochs[warmup:]:
+        flush.zero_()                                    # L2 flush, outside the event pair
+        a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        run_epoch(ep)
+        P.dode_join(h)                                   # the end event must follow the steps on the library's lanes
+        z.record()
+        ev.append((a, z))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    wall = time.perf_counter() - wall0
+    total_ms = max_over_ranks(sum(a.elapsed_time(z) for a, z in ev), dev)
+    epoch_ms = total_ms / steps
+    launches = P.dode_launch_count(h) - launches0
+    # per-kernel durations for the roofline: epochs again with a CUDA-event pair around every launch on the library's
+    # stream (dode_timing_*).  Event records between launches serialise them, so this pass is kept out of the region
+    # `value` is measured on (where consecutive kernels overlap by programmatic dependent launch).
+    P.dode_timing_enable(h, True)
+    P.dode_timing_read(h, 0, True); P.dode_timing_read(h, 1, True)
+    widest, path = 0, P.dode_last_path(h)
+    t_epochs = epochs[warmup:][:timing_epochs]
+    for ep in t_epochs:
+        flush.zero_()
+        for c, days in ep:
+            P.dode_spgd_step(h, days, float(etas[c]))
+            if len(days) > widest:                       # name the kernels of a full-width minibatch, not of a
+                widest, path = len(days), P.dode_last_path(h)   # cluster's ragged tail (host-side string, no sync)
+    fwd_ms, fwd_n = P.dode_timing_read(h, 0)
+    grad_ms, grad_n = P.dode_timing_read(h, 1)
+    P.dode_timing_enable(h, False)
+    fb = gb = fl = 0.0                                   # algorithmic work summed over the event-timed launches
+    for ep in t_epochs:
+        for c, days in ep:
+            if cfg.sparse:
+                f_b = 8.0 * nnz_c + 4.0 * len(days) * cfg.T * (cfg.N + cfg.L)
+                g_b = 8.0 * nnz_c + 4.0 * len(days) * cfg.T * cfg.N
+                f_l = 2.0 * nnz_c * len(days)
+            else:
+                f_b, g_b, f_l = algorithmic(cfg, len(days))
+            fb += f_b; gb += g_b; fl += f_l
+    step_b = step_f = 0.0                                # and over the epochs `value` was timed on
+    for ep in epochs[warmup:]:
+        for c, days in ep:
+            if cfg.sparse:
+                step_b += 16.0 * nnz_c + 4.0 * len(days) * cfg.T * (2 * cfg.N + cfg.L)
+                step_f += 4.0 * nnz_c * len(days)
+            else:
+                f_b, g_b, f_l = algorithmic(cfg, len(days))
+                step_b += f_b + g_b; step_f += 2 * f_l
+    return {"b": b, "epoch_ms": epoch_ms, "total_ms": total_ms, "wall_s": wall, "launches": int(launches), "path": path,
+            "iters_per_epoch": len(epochs[0]), "steps": steps, "warmup": warmup,
+            "fwd_ms": fwd_ms, "fwd_n": fwd_n, "grad_ms": grad_ms, "grad_n": grad_n, "fb": fb, "gb": gb, "fl": fl,
+            "step_GBps": step_b / (total_ms * 1e-3) / 1e9, "step_TFLOPs": step_f / (total_ms * 1e-3) / 1e12}
+
+
+def roofline_of(cfg, m, peaks):
+    """The `roofline` object of one measurement (DESIGN.md §7/§11): the dominant kernel's algorithmic bytes or flops per
+    launch / its average event-timed launch duration, against the measured peak of the unit that bounds it."""
+    hbm_peak, bf16_peak, peak_src, fp32_peak, fp32_src = peaks
+    tensor_path = m["path"].startswith("tcgen05")
+    tc_peak = bf16_peak * TF32_OVER_BF16 / 3.0          # 3xTF32: three tf32 MMAs per fp32 product
+    dom = "forward" if m["fwd_ms"] >= m["grad_ms"] else "gradient_update"
+    d_ms, d_n, d_bytes = (m["fwd_ms"], m["fwd_n"], m["fb"]) if dom == "forward" else (m["grad_ms"], m["grad_n"], m["gb"])
+    gbs = d_bytes / (d_ms * 1e-3) / 1e9 if d_ms > 0 else 0.0
+    tfl = m["fl"] / (d_ms * 1e-3) / 1e12 if d_ms > 0 else 0.0
+    t_hbm = d_bytes / (hbm_peak * 1e9)
+    t_alu = m["fl"] / ((tc_peak if tensor_path else fp32_peak) * 1e12)
+    path = m["path"]
+    kname = path.split("+")[0 if dom == "forward" else 1] if "+" in path else path
+    if t_hbm >= t_alu:
+        roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"}
+    elif tensor_path:
+        roof = {"bound": "tensor", "achieved": tfl, "peak": tc_peak, "unit": "TFLOP/s", "frac": tfl / tc_peak,
+                "peak_source": f"MEASURED_PEAKS.json bf16_tflops ({peak_src}) x 1.1/2.25 (tf32) / 3 (3xTF32 MMAs per product)"}
+    else:
+        roof = {"bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s", "frac": tfl / fp32_peak,
+                "peak_source": fp32_src}
+    roof.update({"kernel": kname, "launches": int(d_n), "avg_launch_ms": d_ms / max(1, d_n),
+                 "traffic": traffic_from_profiles(cfg.name, m["b"], dom),
+                 "other": {"hbm_GBps": gbs, "hbm_frac": gbs / hbm_peak, "hbm_frac_of_nominal_8TBps": gbs / 8000.0,
+                           "fp32_TFLOPs": tfl, "fp32_frac_of_measured_ffma_peak": tfl / fp32_peak,
+                           "fp32_frac_of_nominal_ffma_peak": tfl / FP32_PEAK_TFLOPS, "ffma_peak_measured_TFLOPs": fp32_peak,
+                           "ffma_peak_nominal_TFLOPs": FP32_PEAK_TFLOPS,
+                           "forward_ms_total": m["fwd_ms"], "gradient_update_ms_total": m["grad_ms"],
+                           "step_GBps_algorithmic": m["step_GBps"], "step_TFLOPs_algorithmic": m["step_TFLOPs"]}})
+    return roof
+
+
+def measure_e2e(P, h, cfg, lab, etas, b, x_cpu, e2e_steps, world, dev):
+    """The same epochs through dode_spgd_step_host (H2D of the minibatch counts, D2H of its q), wall clock including the
+    final dode_sync; then the same pinned buffers copied back to back with no kernels at all = the PCIe floor."""
+    import torch.distributed as dist
+    # pinned host copies of the minibatches' counts and result buffers: distinct schedules for as many epochs as fit
+    # in 8 GB of pinned memory (at least one), cycled over the timed epochs; x of a day is the same in every epoch
+    per_epoch = cfg.D * cfg.T * (cfg.L + cfg.N) * 4
+    n_stage = int(max(1, min(e2e_steps, (8 << 30) // per_epoch)))
+    e_epochs = make_epochs(cfg, lab, b, n_stage)
+    stage = [[(c, days, x_cpu[torch.from_numpy(days.astype(np.int64))].contiguous().pin_memory(),
+               torch.empty((len(days), cfg.T, cfg.N), dtype=torch.float32).pin_memory()) for c, days in ep]
+             for ep in e_epochs]
+    for c, days, xh, qh in stage[-1]:                # untimed warm-up epoch (staging buffers, copy streams)
+        P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
+    P.dode_sync(h)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for k in range(e2e_steps):
+        for c, days, xh, qh in stage[k % n_stage]:
+            P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
+    P.dode_sync(h)                               # every upload, step and download of the timed epochs has finished
+    torch.cuda.synchronize()
+    e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / e2e_steps, dev)
+    # PCIe floor: the same uploads and downloads on two streams, no kernels
+    s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+    xd = torch.empty((min(b, cfg.D), cfg.T, cfg.L), device=dev)
+    qd = torch.empty((min(b, cfg.D), cfg.T, cfg.N), device=dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for c, days, xh, qh in stage[0]:
+        with torch.cuda.stream(s_up):
+            xd[:len(days)].copy_(xh, non_blocking=True)
+        with torch.cuda.stream(s_dn):
+            qh.copy_(qd[:len(days)], non_blocking=True)
+    torch.cuda.synchronize()
+    floor_ms = (time.perf_counter() - t0) * 1e3
+    return e_ms, floor_ms
+
+
+def run_ours(args, cfg, sweep, rank, world, local_rank):
     import paper_1901_09266_b200 as P
     P.lib()                                   # fail loudly if the CUDA library is missing
     if not torch.cuda.is_available():
@@ -217,16 +403,27 @@ def run_ours(args, cfg, b, rank, world, local_rank):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
+    try:
+        _run_ours(P, args, cfg, sweep, rank, world, local_rank, dev)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+def _run_ours(P, args, cfg, sweep, rank, world, local_rank, dev):
     cfg = rank_config(cfg, rank, world)
+    b_head = sweep[-1]                        # the line's `value` is the last (widest) minibatch of the sweep
 
     # ---- inputs, generated once on the device (synth: no solver arithmetic) ----
     lab = synth.labels(cfg).numpy()
+    nnz_c = None
+    csr_host = None
     if cfg.sparse:
         csr, x = synth.sparse_problem(cfg, dev)
         torch.cuda.empty_cache()              # the library allocates with cudaMalloc: give torch's cached blocks back first
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, csr=csr)
         nnz_c = csr.nnz / cfg.C
-        csr_host = None
         if rank == 0 and not args.no_cpu_baseline:          # one cluster's CSR blocks for the oracle's timing leg
             c0, nbk = int(lab[0]), cfg.T * (cfg.H + 1)
             bo = csr.blk_off[c0 * nbk:(c0 + 1) * nbk + 1].cpu().numpy()
@@ -249,136 +446,48 @@ def run_ours(args, cfg, b, rank, world, local_rank):
     torch.cuda.empty_cache()
 
     etas = np.array([np.float32(1.0 / P.dode_lipschitz(h, c, 30)) for c in range(cfg.C)], np.float32)   # a7
-    epochs = make_epochs(cfg, lab, b, args.warmup + args.steps)
-    iters_per_epoch = len(epochs[0])
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
-
-    def run_epoch(ep):
-        for c, days in ep:
-            P.dode_spgd_step(h, days, float(etas[c]))
-
-    for ep in epochs[:args.warmup]:
-        run_epoch(ep)
-    P.dode_sync(h)
-    launches0 = P.dode_launch_count(h)
+    ones_dev = torch.ones((cfg.T, cfg.N), dtype=torch.float32, device=dev)
+    hbm_peak, bf16_peak, peak_src = measured_peaks()
+    fp32_peak = P.dode_probe_fp32_peak(5)             # hand-written FFMA loop, measured on this GPU now
+    peaks = (hbm_peak, bf16_peak, peak_src, fp32_peak,
+             f"dode_probe_fp32_peak on this GPU ({fp32_peak:.1f} TFLOP/s; nominal 148 SMs x 128 lanes x 2 x 1.965 GHz = {FP32_PEAK_TFLOPS:.2f})")
 
     sampler = ClockSampler(local_rank)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
     sampler.start()
-    ev = []
-    wall0 = time.perf_counter()
-    for ep in epochs[args.warmup:]:
-        flush.zero_()                                    # L2 flush, outside the event pair
-        a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        run_epoch(ep)
-        P.dode_join(h)                                   # the end event must follow the steps on the library's lanes
-        z.record()
-        ev.append((a, z))
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    wall = time.perf_counter() - wall0
+    results = {}
+    for b in sweep:
+        head = b == b_head
+        if len(sweep) > 1:
+            reset_state(P, h, cfg, ones_dev)
+        steps = args.steps if head else max(1, min(args.steps, args.sweep_steps))
+        warm = args.warmup if head else min(args.warmup, 3)
+        results[b] = measure_b(P, h, cfg, lab, etas, b, steps, warm, steps if head else min(steps, 2), flush, world, dev, nnz_c)
     sampler.stop_flag = True
     sampler.join()
-    total_ms = sum(a.elapsed_time(z) for a, z in ev)
-    total_ms = max_over_ranks(total_ms, dev)
-    epoch_ms = total_ms / args.steps
-    launches = P.dode_launch_count(h) - launches0
-    path = P.dode_last_path(h)
-    # per-kernel durations for the roofline: the same epochs again with a CUDA-event pair around every launch on the
-    # library's stream (dode_timing_*).  Event records between launches serialise them, so this pass is kept out of
-    # the region `value` is measured on (where consecutive kernels overlap by programmatic dependent launch).
-    P.dode_timing_enable(h, True)
-    P.dode_timing_read(h, 0, True); P.dode_timing_read(h, 1, True)
-    widest = 0
-    for ep in epochs[args.warmup:]:
-        flush.zero_()
-        for c, days in ep:
-            P.dode_spgd_step(h, days, float(etas[c]))
-            if len(days) > widest:                       # name the kernels of a full-width minibatch, not of a
-                widest, path = len(days), P.dode_last_path(h)   # cluster's ragged tail (host-side string, no sync)
-    fwd_ms, fwd_n = P.dode_timing_read(h, 0)
-    grad_ms, grad_n = P.dode_timing_read(h, 1)
-    P.dode_timing_enable(h, False)
+    m = results[b_head]
+    epoch_ms = m["epoch_ms"]
+    roof = roofline_of(cfg, m, peaks)
 
-    # ---- roofline of the dominant kernel (algorithmic work summed over the timed launches) ----
-    fb = gb = fl = 0.0
-    for ep in epochs[args.warmup:]:
-        for c, days in ep:
-            if cfg.sparse:
-                f_b = 8.0 * nnz_c + 4.0 * len(days) * cfg.T * (cfg.N + cfg.L)
-                g_b = 8.0 * nnz_c + 4.0 * len(days) * cfg.T * cfg.N
-                f_l = 2.0 * nnz_c * len(days)
-            else:
-                f_b, g_b, f_l = algorithmic(cfg, len(days))
-            fb += f_b; gb += g_b; fl += f_l
-    hbm_peak, bf16_peak, peak_src = measured_peaks()
-    tensor_path = path.startswith("tcgen05")
-    # 3xTF32: three tf32 MMAs per fp32 product, so the fp32-equivalent tensor peak is tf32 peak / 3
-    tc_peak = bf16_peak * TF32_OVER_BF16 / 3.0
-    dom = "forward" if fwd_ms >= grad_ms else "gradient_update"
-    d_ms, d_n, d_bytes = (fwd_ms, fwd_n, fb) if dom == "forward" else (grad_ms, grad_n, gb)
-    gbs = d_bytes / (d_ms * 1e-3) / 1e9 if d_ms > 0 else 0.0
-    tfl = fl / (d_ms * 1e-3) / 1e12 if d_ms > 0 else 0.0
-    t_hbm = d_bytes / (hbm_peak * 1e9)
-    t_alu = fl / ((tc_peak if tensor_path else FP32_PEAK_TFLOPS) * 1e12)
-    kname = path.split("+")[0 if dom == "forward" else 1] if "+" in path else path
-    if t_hbm >= t_alu:
-        roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
-                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"}
-    elif tensor_path:
-        roof = {"bound": "tensor", "achieved": tfl, "peak": tc_peak, "unit": "TFLOP/s", "frac": tfl / tc_peak,
-                "peak_source": f"MEASURED_PEAKS.json bf16_tflops ({peak_src}) x 1.1/2.25 (tf32) / 3 (3xTF32 MMAs per product)"}
-    else:
-        roof = {"bound": "alu", "achieved": tfl, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": tfl / FP32_PEAK_TFLOPS, "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)"}
-    roof.update({"kernel": kname, "launches": int(d_n), "avg_launch_ms": d_ms / max(1, d_n),
-                 "traffic": traffic_from_profiles(cfg.name, dom),
-                 "other": {"hbm_GBps": gbs, "hbm_frac": gbs / hbm_peak, "hbm_frac_of_nominal_8TBps": gbs / 8000.0, "fp32_TFLOPs": tfl,
-                           "fp32_frac": tfl / FP32_PEAK_TFLOPS,
-                           "forward_ms_total": fwd_ms, "gradient_update_ms_total": grad_ms,
-                           "step_GBps_algorithmic": (fb + gb) / (total_ms * 1e-3) / 1e9,
-                           "step_TFLOPs_algorithmic": 2 * fl / (total_ms * 1e-3) / 1e12}})
-
-    # ---- e2e: the same epochs through dode_spgd_step_host (H2D of the minibatch counts, D2H of its q) ----
+    # ---- e2e at the headline minibatch ----
     e2e = None
     if args.e2e_steps is None:                 # enough epochs for ~2 s of streaming, so that pipeline fill and the final
         args.e2e_steps = int(min(20, max(3, 2000.0 / max(epoch_ms, 1e-3))))     # sync are amortised (3..20 epochs)
     if args.e2e_steps > 0:
-        # pinned host copies of the minibatches' counts and result buffers: distinct schedules for as many epochs as fit
-        # in 8 GB of pinned memory (at least one), cycled over the timed epochs; x of a day is the same in every epoch
-        per_epoch = cfg.D * cfg.T * (cfg.L + cfg.N) * 4
-        n_stage = int(max(1, min(args.e2e_steps, (8 << 30) // per_epoch)))
-        e_epochs = make_epochs(cfg, lab, b, n_stage)
-        stage = [[(c, days, x_cpu[torch.from_numpy(days.astype(np.int64))].contiguous().pin_memory(),
-                   torch.empty((len(days), cfg.T, cfg.N), dtype=torch.float32).pin_memory()) for c, days in ep]
-                 for ep in e_epochs]
-        for c, days, xh, qh in stage[-1]:                # untimed warm-up epoch (staging buffers, copy streams)
-            P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
-        P.dode_sync(h)
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for k in range(args.e2e_steps):
-            for c, days, xh, qh in stage[k % n_stage]:
-                P.dode_spgd_step_host(h, days, float(etas[c]), xh, qh)
-        P.dode_sync(h)                               # every upload, step and download of the timed epochs has finished
-        torch.cuda.synchronize()
-        e_ms = (time.perf_counter() - t0) * 1e3 / args.e2e_steps
-        e_ms = max_over_ranks(e_ms, dev)
+        e_ms, floor_ms = measure_e2e(P, h, cfg, lab, etas, b_head, x_cpu, args.e2e_steps, world, dev)
         e2e = {"value": e_ms, "unit": UNIT, "h2d_bytes_per_step": int(cfg.D * cfg.T * cfg.L * 4),
-               "d2h_bytes_per_step": int(cfg.D * cfg.T * cfg.N * 4), "epochs": args.e2e_steps, "api": "dode_spgd_step_host (pinned host buffers; uploads/downloads pipelined against the kernels on copy streams, dode_sync inside the timed region)"}
+               "d2h_bytes_per_step": int(cfg.D * cfg.T * cfg.N * 4), "epochs": args.e2e_steps,
+               "pcie_floor_ms_per_epoch": floor_ms, "device_ms_per_epoch": epoch_ms,
+               "bound": "pcie" if floor_ms > epoch_ms else "device",
+               "api": "dode_spgd_step_host (pinned host buffers; uploads/downloads pipelined against the kernels on copy "
+                      "streams, dode_sync inside the timed region); pcie_floor = the same buffers copied with no kernels"}
 
     if rank != 0:
         P.dode_destroy(h)
         return
     # Step 6 quality check on the state the run ends with — a sanity figure, outside every timed region
     _, r2_mean = P.dode_r2(h, list(range(cfg.D)))
-    # ---- CPU oracle beside it (bounded sample, rank 0 only) ----
+    # ---- CPU oracle beside it (bounded sample, rank 0 only, single thread) ----
     cpu = None
     if cfg.sparse and csr_host is not None:
         from oracle import oracle
@@ -395,7 +504,7 @@ def run_ours(args, cfg, b, rank, world, local_rank):
                "ms_per_day_visit": ms_visit}
     if R_cpu is not None:
         per_visit = cfg.nb * cfg.L * cfg.N * 4 / 3e9            # rough s per visit at ~3 GFLOP/s scalar double
-        visits = int(max(3, min(2 * cfg.D, 15.0 / max(per_visit, 1e-4))))
+        visits = int(max(1 if per_visit > 5 else 3, min(2 * cfg.D, 15.0 / max(per_visit, 1e-4))))
         c0 = int(lab[0])
         ms_visit, visits = cpu_oracle_sample(cfg, R_cpu, c0, lab, x_cpu, etas[c0], visits)
         cpu = {"value": ms_visit * cfg.D, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -407,13 +516,20 @@ def run_ours(args, cfg, b, rank, world, local_rank):
         cpu["nproc"] = os.cpu_count()
     out = {"metric": METRIC, "value": epoch_ms, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": epoch_ms, "higher_is_better": False, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, b),
-           "day_steps_per_s": job_day_steps_per_s(cfg.D, world, epoch_ms), "spgd_iterations_per_epoch": iters_per_epoch,
-           "ms_per_spgd_iteration": epoch_ms / iters_per_epoch, "kernel_path": path,
-           "gpu_launches": int(launches), "wall_s_timed_region": wall, "clocks": sampler.summary(),
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, b_head),
+           "day_steps_per_s": job_day_steps_per_s(cfg.D, world, epoch_ms), "spgd_iterations_per_epoch": m["iters_per_epoch"],
+           "ms_per_spgd_iteration": epoch_ms / m["iters_per_epoch"], "kernel_path": m["path"],
+           "gpu_launches": m["launches"], "wall_s_timed_region": m["wall_s"], "clocks": sampler.summary(),
            "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,
-           "fit": {"r2_mean_over_days": r2_mean, "after_epochs": 2 * (args.warmup + args.steps) + (args.e2e_steps + 1 if args.e2e_steps > 0 else 0),
-                   "note": "Step 6 quality check of the final state (paper reports 0.87 on its real data, PAPER.md:553)"}}
+           "fit": {"r2_mean_over_days": r2_mean,
+                   "note": "Step 6 quality check of the state the run ends with (paper reports 0.87 on its real data, PAPER.md:553)"}}
+    if len(sweep) > 1:
+        # G8 (BASELINE.json configs[3]): the memory-bound to compute-bound crossover, every width from a fresh q0.
+        # north_star's targets: >= 0.70 of HBM at small minibatch, >= 0.50 of FP32 peak at large minibatch.
+        out["sweep"] = {str(b): {"ms_per_epoch": r["epoch_ms"], "ms_per_spgd_iteration": r["epoch_ms"] / r["iters_per_epoch"],
+                                 "steps": r["steps"], "warmup": r["warmup"], "kernel_path": r["path"],
+                                 "gpu_launches": r["launches"], "roofline": roofline_of(cfg, r, peaks)}
+                        for b, r in results.items()}
     print(json.dumps(out))
     P.dode_destroy(h)
 
@@ -518,19 +634,22 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="corridor", choices=list(synth.CONFIGS))
-    ap.add_argument("--b", type=int, default=None, help="minibatch days (default: the workload's)")
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(synth.CONFIGS))
+    ap.add_argument("--b", type=int, default=None, help="minibatch days (default: the workload's; large_dense: the G8 sweep "
+                                                        "1, 8, 64, 256 with the line's value at 256)")
+    ap.add_argument("--sweep-steps", type=int, default=5, help="timed epochs of the sweep's non-headline widths (<= --steps)")
     ap.add_argument("--days", type=int, default=None, help="override D (bench smoke runs only)")
     ap.add_argument("--n", type=int, default=None, help="fig12 workload: matrix dimension n (L = N = n), 100..6000 in the paper")
+    ap.add_argument("--sweep", action="store_true", help="fig12 workload: the whole Fig. 12 curve n = 100 ... 6000 in one JSON line")
     ap.add_argument("--e2e-steps", type=int, default=None, help="timed end-to-end epochs (default: 3..20, about 2 s of streaming)")
-    ap.add_argument("--ref-visits", type=int, default=8)
+    ap.add_argument("--ref-visits", type=int, default=None, help="--impl reference: day-visits per step (default: about 1-10 s of work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--paths", type=int, default=1, help="--dar-build: up to this many paths per OD with Logit route shares (Eq. 37)")
     ap.add_argument("--theta", type=float, default=0.01, help="--dar-build --paths K: Logit dispersion factor per second (SURVEY NEXT-4)")
     ap.add_argument("--dar-build", action="store_true", help="NEXT-4: time dode_dar_build on the workload's network instead of SPGD")
     args = ap.parse_args()
-    if args.warmup < 3 and args.impl == "ours":
-        args.warmup = max(args.warmup, 1)
+    if args.impl == "ours":
+        args.warmup = max(args.warmup, 3)              # timing rule: W >= 3
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -541,15 +660,16 @@ def main():
         if not cfg.fig12:
             raise SystemExit("--n applies to --workload fig12 only")
         cfg = cfg.replace(N=args.n, L=args.n)
-    b = args.b or cfg.b
+    # BASELINE.json configs[3] is a minibatch sweep (G8); north_star's two roofline targets are defined on it
+    sweep = [args.b] if args.b else (list(LARGE_DENSE_SWEEP) if cfg.name == "large_dense" else [cfg.b])
     if args.dar_build:
         if rank == 0:
             run_dar_build(args, cfg, local_rank)
         return
     if args.impl == "reference":
-        run_reference(args, cfg, b, rank, world)
+        run_reference(args, cfg, sweep[-1], rank, world)
     else:
-        run_ours(args, cfg, b, rank, world, local_rank)
+        run_ours(args, cfg, sweep, rank, world, local_rank)
 
 
 if __name__ == "__main__":

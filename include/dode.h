@@ -196,6 +196,12 @@ int dode_assignment_build(int32_t N, int32_t L, int32_t T, int32_t H, const int3
 int dode_timing_enable(dode_ctx* ctx, int32_t on);
 int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches, int32_t reset);
 
+/* Measurement helper (needs no ctx, not on the SPGD path): the device's FP32 FFMA rate from a register-only kernel of
+ * independent fused multiply-add chains (2 CTAs x 1024 threads per SM, 8 chains per thread), best of `reps` timed
+ * launches after one warm-up, in TFLOP/s (2 flops per FFMA).  bench.py uses it as the denominator of every "alu"
+ * roofline instead of the nominal SMs x 128 lanes x 2 x clock.  Synchronises `stream`.  Errors: dode_last_error(NULL). */
+int dode_probe_fp32_peak(int32_t reps, double* tflops, void* stream);
+
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 int64_t dode_launch_count(const dode_ctx* ctx);
 

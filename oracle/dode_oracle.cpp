@@ -153,6 +153,17 @@ double oracle_objective_day(int N, int L, int T, int H, const float* Rc, const f
     return f;
 }
 
+// O3 with the rows of the forward pass split over `threads` threads; the squares are summed in index order afterwards,
+// so the value equals oracle_objective_day bit for bit (pin P18).
+double oracle_objective_day_mt(int N, int L, int T, int H, const float* Rc, const float* q, const float* x, int threads) {
+    Dims d{N, L, T, H};
+    std::vector<double> rd((size_t)T * L);
+    parallel_rows(T, threads, [&](int t0, int t1) { forward_rows(d, Rc, q, x, rd.data(), t0, t1); });
+    double f = 0.0;
+    for (double v : rd) f += v * v;
+    return f;
+}
+
 // O5 (Step 6 "quality check"; "R-square between the observed link flow and estimated link flow",
 // PAPER.md:553): coefficient of determination of one day's fitted counts, observed counts as the reference
 // (reading A17):  R2 = 1 - sum (x - rho q)^2 / sum (x - mean(x))^2  over the day's T*L entries, all in double.

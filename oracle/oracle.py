@@ -36,6 +36,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(build_oracle())
         _lib.oracle_objective_day.restype = C.c_double
+        _lib.oracle_objective_day_mt.restype = C.c_double
         _lib.oracle_r2_day.restype = C.c_double
         _lib.oracle_objective_day_csr.restype = C.c_double
         _lib.oracle_power_iteration.restype = C.c_double
@@ -76,10 +77,13 @@ def visit(Rc: np.ndarray, q: np.ndarray, x: np.ndarray, eta: float) -> np.ndarra
     return q
 
 
-def objective_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray) -> float:
-    """O3 for one day: sum of squared residuals, no 1/2 (Eq. 42)."""
+def objective_day(Rc: np.ndarray, q: np.ndarray, x: np.ndarray, threads: int = 1) -> float:
+    """O3 for one day: sum of squared residuals, no 1/2 (Eq. 42).  threads > 1: the forward rows are
+    computed by several threads and summed in the same order (same value, pin P18)."""
     N, L, T, H = _dims(Rc)
     Rc, pR = _f(Rc); q, pq = _f(q); x, px = _f(x)
+    if threads > 1:
+        return float(lib().oracle_objective_day_mt(N, L, T, H, pR, pq, px, int(threads)))
     return float(lib().oracle_objective_day(N, L, T, H, pR, pq, px))
 
 

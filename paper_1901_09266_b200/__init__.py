@@ -22,7 +22,7 @@ DODE_DENSE, DODE_CSR = 0, 1
 DODE_OPT_TC_MIN_B, DODE_OPT_LANES, DODE_OPT_TC_KSPLIT, DODE_OPT_PDL = 0, 1, 2, 3
 
 EXPORTS = ["dode_create", "dode_set_option", "dode_reserve", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
-           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_launch_count", "dode_last_path", "dode_sync",
+           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_probe_fp32_peak", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
 
@@ -72,6 +72,7 @@ def lib():
         L.dode_lipschitz.argtypes = [vp, i32, i32, vp]
         L.dode_timing_enable.argtypes = [vp, i32]
         L.dode_timing_read.argtypes = [vp, i32, vp, vp, i32]
+        L.dode_probe_fp32_peak.argtypes = [i32, vp, vp]
         L.dode_launch_count.argtypes = [vp]
         L.dode_launch_count.restype = C.c_int64
         L.dode_last_path.argtypes = [vp]
@@ -318,6 +319,16 @@ def dode_timing_read(h, kind: int, reset: bool = False):
     _chk(h, lib().dode_timing_read(h, kind, C.byref(ms), C.byref(cnt), 1 if reset else 0))
     _release(h)
     return ms.value, cnt.value
+
+
+def dode_probe_fp32_peak(reps: int = 5) -> float:
+    """Measured FP32 FFMA rate of the current device in TFLOP/s (a measurement helper, not on the SPGD path)."""
+    import torch
+    out = C.c_double()
+    rc = lib().dode_probe_fp32_peak(int(reps), C.byref(out), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != DODE_OK:
+        raise DodeError(rc, lib().dode_last_error(None).decode())
+    return out.value
 
 
 def dode_launch_count(h) -> int:

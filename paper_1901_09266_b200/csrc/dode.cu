@@ -15,6 +15,7 @@
 #include "kernels_csr.cuh"
 #include "kernels_tc.cuh"
 #include "kernels_dar.cuh"
+#include "kernels_probe.cuh"
 
 using namespace dode;
 
@@ -1148,6 +1149,40 @@ int dode_assignment_build(int32_t N, int32_t L, int32_t T, int32_t H, const int3
                           float* R_out, void* stream) {
     if (!od_ptr) return fail(nullptr, DODE_EINVAL, "od_ptr is null");
     return build_operator(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, R_out, stream);
+}
+
+int dode_probe_fp32_peak(int32_t reps, double* tflops, void* stream) {
+    dode_ctx* ctx = nullptr;
+    if (reps < 1 || !tflops) return fail(ctx, DODE_EINVAL, "reps < 1 or null output");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* buf = nullptr;
+    CU(cudaMalloc(&buf, 4096));
+    const float init[3] = {0.999f, 0.001f, 1.0f};
+    cudaError_t e = cudaMemcpyAsync(buf, init, sizeof init, cudaMemcpyHostToDevice, st);
+    cudaEvent_t a = nullptr, b = nullptr;
+    if (e == cudaSuccess) e = cudaEventCreate(&a);
+    if (e == cudaSuccess) e = cudaEventCreate(&b);
+    const int outer = 2048, blocks = sms * 2, threads = 1024;
+    double best = 0.0;
+    for (int r = 0; r <= reps && e == cudaSuccess; ++r) {                 // launch 0 is the warm-up
+        cudaEventRecord(a, st);
+        ffma_peak_probe<<<blocks, threads, 0, st>>>(buf, buf + 8, outer);
+        cudaEventRecord(b, st);
+        e = cudaEventSynchronize(b);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+        const double fl = 2.0 * kProbeChains * kProbeInner * (double)outer * threads * blocks;
+        if (r > 0 && ms > 0.f) best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    }
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaFree(buf);
+    if (e != cudaSuccess) return fail(ctx, DODE_ECUDA, "ffma_peak_probe: %s", cudaGetErrorString(e));
+    *tflops = best;
+    return DODE_OK;
 }
 
 int dode_timing_enable(dode_ctx* ctx, int32_t on) {

@@ -296,6 +296,7 @@ def test_p18_day_replay_equals_repeated_visits(tiny12, threads):
         if v in got:
             np.testing.assert_array_equal(got[v], q)
     assert (q == 0).any() and (q > 0).any()          # the projection is active on this instance
+    assert oracle.objective_day(R[0], q, x[6], threads=threads) == oracle.objective_day(R[0], q, x[6])
     csr = synth.dense_to_csr(torch.from_numpy(R))
     arrs = (cfg.N, cfg.L, cfg.T, cfg.H, csr.blk_off.numpy(), csr.row_ptr.numpy(), csr.col_idx.numpy(), csr.val.numpy())
     got, done = oracle.replay_day(None, q0, x[6], eta, 7, [3, 7], threads=threads, csr=arrs)
