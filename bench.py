@@ -534,6 +534,80 @@ def _run_ours(P, args, cfg, sweep, rank, world, local_rank, dev):
     P.dode_destroy(h)
 
 
+def run_fig12_sweep(args, local_rank):
+    """--workload fig12 --sweep (NEXT-2): the paper's efficiency experiment (Fig. 12) as ONE line:
+    random dense B (n x n), x >= 0, y = Bx, n = 100 ... 6000, solved for 64 right-hand sides at once (T = 1, H = 0, b = 64).
+    Per n: GPU time of one SPGD iteration (CUDA events, L2 flushed between iterations), the oracle's time for the same
+    iteration (timed on a bounded number of right-hand sides, extrapolated to the 64), and the forward kernel's
+    fraction of the HBM roofline.  The paper's third arm (active-set NNLS) is a comparison system and is not timed."""
+    import paper_1901_09266_b200 as P
+    from oracle import oracle
+    P.lib()
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    hbm_peak, _, peak_src = measured_peaks()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    curve = []
+    base = synth.CONFIGS["fig12"]
+    for n in (100, 300, 1000, 3000, 6000):
+        cfg = base.replace(N=n, L=n)
+        lab = synth.labels(cfg).numpy()
+        R = synth.dar_dense(cfg, device=dev)
+        x = synth.counts(cfg, R, synth.q_true(cfg, dev), torch.from_numpy(lab), noise=False)
+        h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, dense=R)
+        eta = float(np.float32(1.0 / P.dode_lipschitz(h, 0, 30)))
+        days = np.arange(cfg.D, dtype=np.int32)
+        P.dode_reserve(h, cfg.D)
+        for _ in range(max(3, args.warmup)):
+            P.dode_spgd_step(h, days, eta)
+        P.dode_sync(h)
+        ev = []
+        for _ in range(args.steps):
+            flush.zero_()
+            a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            P.dode_spgd_step(h, days, eta)
+            P.dode_join(h)
+            z.record()
+            ev.append((a, z))
+        torch.cuda.synchronize()
+        gpu_ms = sum(a.elapsed_time(z) for a, z in ev) / args.steps
+        path = P.dode_last_path(h)
+        P.dode_destroy(h)
+        alg_bytes = 2 * 4.0 * n * n + 4.0 * cfg.D * (3 * n)            # B once per pass + q read/write + y read
+        Rn, xn = R[0].cpu().numpy(), x.cpu().numpy()
+        rhs = int(max(1, min(cfg.D, 4e8 / (4.0 * n * n))))              # bounded sample: ~0.2-2 s of oracle work
+        q = np.ones((cfg.T, cfg.N), np.float32)
+        t0 = time.perf_counter()
+        for d in range(rhs):
+            oracle.visit(Rn, q, xn[d], eta)
+        cpu_ms = (time.perf_counter() - t0) * 1e3 * cfg.D / rhs
+        curve.append({"n": n, "gpu_ms": gpu_ms, "oracle_ms": cpu_ms, "oracle_rhs_timed": rhs,
+                      "frac": alg_bytes / (gpu_ms * 1e-3) / 1e9 / hbm_peak, "kernel_path": path})
+        del R, x
+        torch.cuda.empty_cache()
+    sampler.stop_flag = True
+    sampler.join()
+    last = curve[-1]
+    out = {"metric": "fig12_spgd_iteration_time", "value": last["gpu_ms"], "unit": "ms/iteration", "n_gpus": 1,
+           "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": last["gpu_ms"], "higher_is_better": False,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": "fig12 sweep (PAPER.md:569-583): random dense B n x n, x >= 0, y = Bx, 64 right-hand sides "
+                                  "(T=1, H=0, b=64), n = 100, 300, 1000, 3000, 6000; value = n 6000",
+                      "l2": "L2 flushed (256 MiB write) before every timed iteration"},
+           "curve": curve, "clocks": sampler.summary(), "gpu_launches": None,
+           "roofline": {"bound": "hbm", "achieved": last["frac"] * hbm_peak, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": last["frac"], "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
+                        "kernel": last["kernel_path"], "traffic": None,
+                        "note": "whole iteration (both passes) on algorithmic bytes 2*4n^2 + state, n = 6000"},
+           "cpu_baseline": {"value": last["oracle_ms"], "unit": "ms/iteration", "cores": 1, "kind": "oracle",
+                            "sample": f"{last['oracle_rhs_timed']} of 64 right-hand sides timed, extrapolated"},
+           "e2e": None}
+    print(json.dumps(out))
+
+
 def run_dar_build(args, cfg, local_rank):
     """--dar-build (NEXT-4): Step 1 of the framework, the DAR blocks of one traffic pattern from link speeds
     (dode_dar_build; Eq. 17-18).  One step = one pattern's operator [T][H+1][L][N] built from its
@@ -665,6 +739,12 @@ def main():
     if args.dar_build:
         if rank == 0:
             run_dar_build(args, cfg, local_rank)
+        return
+    if args.sweep:
+        if not cfg.fig12:
+            raise SystemExit("--sweep applies to --workload fig12 only")
+        if rank == 0:
+            run_fig12_sweep(args, local_rank)
         return
     if args.impl == "reference":
         run_reference(args, cfg, sweep[-1], rank, world)

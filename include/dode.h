@@ -189,6 +189,22 @@ int dode_assignment_build(int32_t N, int32_t L, int32_t T, int32_t H, const int3
                           const int32_t* path_links, const float* link_len, const float* speed, double dt, double theta,
                           float* R_out, void* stream);
 
+/* NEXT-4 for large networks: the same operator as dode_assignment_build (od_ptr == NULL: dode_dar_build, one path per OD),
+ * emitted directly in the boundary CSR format of dode_dar for ONE cluster / pattern ("coordinate format sparse
+ * representation"; Table 2 "Sparse") — the dense slab of a config-4-sized network would be
+ * terabytes.  Blocks in [s][h] order, rows = links, columns = OD pairs ascending; several paths of one OD through the same
+ * link and lag are merged (their shares add up, Eq. 41); shares with h > H or s+h >= T are dropped.
+ *   blk_off_out  device int64 [T*(H+1) + 1];  row_ptr_out  device int32 [T*(H+1)][L+1]
+ *   col_idx_out  device int32 [cap];          val_out      device fp32 [cap]
+ *   cap          entries the two arrays can hold;  nnz_out  host int64
+ * If cap is smaller than the number of shares the walk emits (before merging), nothing is written, *nnz_out receives that
+ * number and DODE_ENOMEM is returned: call once with cap = 0 to size the arrays.  On success *nnz_out = entries written.
+ * Uses temporary device memory of about 24 bytes per share.  Synchronises `stream`.  Errors: dode_last_error(NULL). */
+int dode_assignment_build_csr(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* od_ptr, const int32_t* path_ptr,
+                              const int32_t* path_links, const float* link_len, const float* speed, double dt, double theta,
+                              int64_t* blk_off_out, int32_t* row_ptr_out, int32_t* col_idx_out, float* val_out,
+                              int64_t cap, int64_t* nnz_out, void* stream);
+
 /* Optional per-kernel timing for roofline reports: while enabled, every forward (kind 0) and
  * gradient+update (kind 1) launch is bracketed by CUDA events on the ctx stream.  dode_timing_read
  * synchronises, folds finished event pairs into the running totals and returns the total device

@@ -21,7 +21,7 @@ DODE_DENSE, DODE_CSR = 0, 1
 
 DODE_OPT_TC_MIN_B, DODE_OPT_LANES, DODE_OPT_TC_KSPLIT, DODE_OPT_PDL = 0, 1, 2, 3
 
-EXPORTS = ["dode_create", "dode_set_option", "dode_reserve", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
+EXPORTS = ["dode_create", "dode_set_option", "dode_reserve", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_assignment_build_csr", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
            "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_probe_fp32_peak", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
@@ -63,6 +63,8 @@ def lib():
         L.dode_reserve.argtypes = [vp, i32]
         L.dode_dar_build.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, C.c_double, vp, vp]
         L.dode_assignment_build.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, C.c_double, C.c_double, vp, vp]
+        L.dode_assignment_build_csr.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, C.c_double, C.c_double,
+                                                vp, vp, vp, vp, C.c_int64, vp, vp]
         L.dode_objective.argtypes = [vp, vp, i32, vp, vp]
         L.dode_get_q.argtypes = [vp, i32, vp, i32]
         L.dode_set_q.argtypes = [vp, i32, vp, i32]
@@ -216,6 +218,47 @@ def dode_assignment_build(N: int, L: int, T: int, H: int, od_ptr, path_ptr, path
                                      C.c_void_p(R_out.data_ptr()), C.c_void_p(torch.cuda.current_stream().cuda_stream))
     if rc != DODE_OK:
         raise DodeError(rc, lib().dode_last_error(None).decode())
+
+
+def dode_assignment_build_csr(N: int, L: int, T: int, H: int, od_ptr, path_ptr, path_links, link_len, speed, dt: float,
+                              theta: float = 0.0):
+    """NEXT-4 for large networks: the operator of one pattern in the boundary CSR format.  ``od_ptr`` None = one path per
+    OD (dode_dar_build's operator).  All inputs on the GPU (int32 / float32).  Returns an object with CUDA tensors
+    blk_off (int64 [T*(H+1)+1]), row_ptr (int32 [T*(H+1)][L+1]), col_idx (int32 [nnz]), val (float32 [nnz]) — what
+    dode_create(csr=...) takes for a one-cluster problem.  Synchronises."""
+    import torch
+    from types import SimpleNamespace
+    for t, dt_ in ((path_ptr, torch.int32), (path_links, torch.int32), (link_len, torch.float32), (speed, torch.float32)):
+        assert t.is_cuda and t.dtype == dt_ and t.is_contiguous()
+    assert link_len.numel() == L and speed.shape == (T, L)
+    odp = None
+    if od_ptr is not None:
+        assert od_ptr.is_cuda and od_ptr.dtype == torch.int32 and od_ptr.numel() == N + 1
+        odp = C.c_void_p(od_ptr.data_ptr())
+    dev = speed.device
+    blk_off = torch.empty(T * (H + 1) + 1, dtype=torch.int64, device=dev)
+    row_ptr = torch.empty((T * (H + 1), L + 1), dtype=torch.int32, device=dev)
+    stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    nnz = C.c_int64()
+
+    def call(col, val, cap):
+        return lib().dode_assignment_build_csr(
+            N, L, T, H, odp, C.c_void_p(path_ptr.data_ptr()), C.c_void_p(path_links.data_ptr()),
+            C.c_void_p(link_len.data_ptr()), C.c_void_p(speed.data_ptr()), C.c_double(dt), C.c_double(theta),
+            C.c_void_p(blk_off.data_ptr()), C.c_void_p(row_ptr.data_ptr()),
+            None if col is None else C.c_void_p(col.data_ptr()), None if val is None else C.c_void_p(val.data_ptr()),
+            C.c_int64(cap), C.byref(nnz), stream)
+
+    rc = call(None, None, 0)                       # sizing call
+    if rc not in (DODE_OK, DODE_ENOMEM):
+        raise DodeError(rc, lib().dode_last_error(None).decode())
+    cap = max(1, nnz.value)
+    col = torch.empty(cap, dtype=torch.int32, device=dev)
+    val = torch.empty(cap, dtype=torch.float32, device=dev)
+    rc = call(col, val, cap)
+    if rc != DODE_OK:
+        raise DodeError(rc, lib().dode_last_error(None).decode())
+    return SimpleNamespace(blk_off=blk_off, row_ptr=row_ptr, col_idx=col[:nnz.value], val=val[:nnz.value], nnz=nnz.value)
 
 
 def dode_join(h) -> None:

@@ -13,6 +13,7 @@
 
 #include "kernels_dense.cuh"
 #include "kernels_csr.cuh"
+#include <cub/device/device_reduce.cuh>
 #include "kernels_tc.cuh"
 #include "kernels_dar.cuh"
 #include "kernels_probe.cuh"
@@ -75,6 +76,7 @@ struct dode_ctx {
     Lane lane[2];
     bool lanes_on = true, lanes_dirty = false;     // dirty: lane work not yet joined into the ctx stream
     int lane_next = 0;
+    unsigned lanes_used = 0;                       // lanes the latest step_impl call issued work on (bit per lane)
     int64_t lane_step_id = 0;
     std::vector<int64_t> day_last_id;              // [D] id of the last lane step that touched the day
     std::vector<int8_t> day_last_lane;             // [D] and its lane (-1: none)
@@ -336,20 +338,22 @@ static int tc_setup(dode_ctx* ctx) {
     return DODE_OK;
 }
 
-static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn) {
+// panels for `rows` minibatch days (>= dsplit * bn) and B tensor maps with boxes of bn days
+static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows) {
     const dode_dims& d = ctx->dm;
     const size_t qlen = (size_t)d.T * ctx->Np;
-    if (tb.cap < bn) {
+    if (tb.cap < rows) {
+        const int bn_alloc = rows;
         CU(cudaStreamSynchronize(st));
         cudaFree(tb.Qg_full); cudaFree(tb.Qg_lo); cudaFree(tb.rp_full); cudaFree(tb.rp_lo);
         tb.Qg_full = tb.Qg_lo = tb.rp_full = tb.rp_lo = nullptr;
         tb.cap = 0; tb.bn = 0;
-        CU(cudaMalloc(&tb.Qg_full, bn * qlen * 4)); CU(cudaMalloc(&tb.Qg_lo, bn * qlen * 4));
-        CU(cudaMalloc(&tb.rp_full, (size_t)bn * ctx->rpitch * 4)); CU(cudaMalloc(&tb.rp_lo, (size_t)bn * ctx->rpitch * 4));
-        CU(cudaMemsetAsync(tb.Qg_full, 0, bn * qlen * 4, st)); CU(cudaMemsetAsync(tb.Qg_lo, 0, bn * qlen * 4, st));
-        CU(cudaMemsetAsync(tb.rp_full, 0, (size_t)bn * ctx->rpitch * 4, st));
-        CU(cudaMemsetAsync(tb.rp_lo, 0, (size_t)bn * ctx->rpitch * 4, st));
-        tb.cap = bn;
+        CU(cudaMalloc(&tb.Qg_full, bn_alloc * qlen * 4)); CU(cudaMalloc(&tb.Qg_lo, bn_alloc * qlen * 4));
+        CU(cudaMalloc(&tb.rp_full, (size_t)bn_alloc * ctx->rpitch * 4)); CU(cudaMalloc(&tb.rp_lo, (size_t)bn_alloc * ctx->rpitch * 4));
+        CU(cudaMemsetAsync(tb.Qg_full, 0, bn_alloc * qlen * 4, st)); CU(cudaMemsetAsync(tb.Qg_lo, 0, bn_alloc * qlen * 4, st));
+        CU(cudaMemsetAsync(tb.rp_full, 0, (size_t)bn_alloc * ctx->rpitch * 4, st));
+        CU(cudaMemsetAsync(tb.rp_lo, 0, (size_t)bn_alloc * ctx->rpitch * 4, st));
+        tb.cap = bn_alloc;
     }
     if (tb.bn != bn) {
         // B operands: K-major windows of the per-day vectors, SWIZZLE_128B tiles of {32 floats, bn days}
@@ -366,8 +370,12 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn) {
         tb.bn = bn;
     }
     if (!ctx->tc_attr) {
-        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<false, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<false, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->tc_attr = true;
     }
     return DODE_OK;
@@ -376,14 +384,20 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn) {
 // Launch geometry of the tensor-core kernels for a minibatch of bn (multiple of 16) days
 struct TcGeom { int stages, nring; size_t smem; int ks_f, ks_g; size_t part_floats; };
 
-static TcGeom tc_geometry(const dode_ctx* ctx, int bn) {
+// minibatch of n days -> day groups per tile (1, or 2 above 128 days) and days per group (MMA N, multiple of 16)
+static void tc_day_groups(int n, int* dsplit, int* bn) {
+    *dsplit = n > 128 ? 2 : 1;
+    *bn = round_up(ceil_div(n, *dsplit), 16);
+}
+
+static TcGeom tc_geometry(const dode_ctx* ctx, int bn, int dsplit) {
     const dode_dims& d = ctx->dm;
     TcGeom g{};
     // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  Two CTAs per SM when 3 stages fit in half the
     // shared memory and 256 TMEM columns suffice.
     const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
     const int fixed = 1024 + 256;
-    const int acc_cols = bn <= 128 ? 2 * bn : bn;
+    const int acc_cols = 2 * bn;
     int stages = (112 * 1024 - fixed) / stageBytes;
     int nring = 2;
     if (stages < 3 || acc_cols + 128 > 256) {          // one CTA per SM
@@ -397,7 +411,7 @@ static TcGeom tc_geometry(const dode_ctx* ctx, int bn) {
     // Fig. 12 workload, T = 1.  Each pass then runs ksplit CTAs per tile and a small epilogue kernel.
     const int slots = 148 * (g.smem * 2 + 2048 <= 227 * 1024 ? 2 : 1);
     auto pick_split = [&](int M, int kunit) {
-        const long ctas = (long)ceil_div(M, tc::kTileM) * d.T;
+        const long ctas = (long)ceil_div(M, tc::kTileM) * d.T * dsplit;
         const int nk_max = ceil_div((long)(d.H + 1) * kunit, tc::kTileK);
         int ks = (int)std::min<long>(slots / std::max<long>(ctas, 1), nk_max / 8);
         if (ctx->opt_ksplit > 0) ks = ctx->opt_ksplit;
@@ -406,7 +420,7 @@ static TcGeom tc_geometry(const dode_ctx* ctx, int bn) {
     g.ks_f = pick_split(d.L, ctx->Np);
     g.ks_g = pick_split(d.N, ctx->Lp);
     g.part_floats = (g.ks_f > 1 || g.ks_g > 1)
-        ? (size_t)std::max(g.ks_f * ceil_div(d.L, tc::kTileM), g.ks_g * ceil_div(d.N, tc::kTileM)) * tc::kTileM * d.T * bn : 0;
+        ? (size_t)std::max(g.ks_f * ceil_div(d.L, tc::kTileM), g.ks_g * ceil_div(d.N, tc::kTileM)) * tc::kTileM * d.T * bn * dsplit : 0;
     return g;
 }
 
@@ -436,10 +450,11 @@ static cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 
 // one SPGD iteration of a sub-batch (8 <= n <= 256 days) on the tensor cores
 static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt, TcBuf& tb, cudaStream_t st) {
     const dode_dims& d = ctx->dm;
-    const int bn = (dl.n + 15) / 16 * 16;
-    int rc = tc_ensure(ctx, tb, st, bn);
+    int dsplit, bn;
+    tc_day_groups(dl.n, &dsplit, &bn);
+    int rc = tc_ensure(ctx, tb, st, bn, dsplit * bn);
     if (rc) return rc;
-    const TcGeom geo0 = tc_geometry(ctx, bn);
+    const TcGeom geo0 = tc_geometry(ctx, bn, dsplit);
     const int stages = geo0.stages, nring = geo0.nring;
     const size_t smem = geo0.smem;
     const size_t dayStride = (size_t)d.T * ctx->Np;
@@ -450,19 +465,22 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
         ctx->launches++;
     }
     tc::TcParams p{};
-    p.T = d.T; p.H = d.H; p.Lp = ctx->Lp; p.Np = ctx->Np; p.bn = bn; p.stages = stages; p.nring = nring;
+    p.T = d.T; p.H = d.H; p.Lp = ctx->Lp; p.Np = ctx->Np; p.bn = bn; p.dsplit = dsplit; p.bnt = dsplit * bn;
+    p.stages = stages; p.nring = nring;
     p.slab0 = c * d.T;
     p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = tb.rp_lo; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
     const bool ada = opt.mask || opt.G;
-    auto kern = ada ? tc::banded_gemm_3xtf32<true> : tc::banded_gemm_3xtf32<false>;
+    auto kern = bn <= 32 ? (ada ? tc::banded_gemm_3xtf32<true, 16> : tc::banded_gemm_3xtf32<false, 16>)
+              : bn <= 64 ? (ada ? tc::banded_gemm_3xtf32<true, 32> : tc::banded_gemm_3xtf32<false, 32>)
+                         : (ada ? tc::banded_gemm_3xtf32<true, 64> : tc::banded_gemm_3xtf32<false, 64>);
     const TcGeom& geo = geo0;
     const int ks_f = geo.ks_f, ks_g = geo.ks_g;
     if ((rc = tc_ensure_part(ctx, tb, st, geo.part_floats))) return rc;
     p.part = tb.part;
     auto epilogue = [&](int Mt) -> int {           // second half of a split-K pass
-        const dim3 g(ceil_div((long)Mt * (bn / 4), 256), d.T);
+        const dim3 g(ceil_div((long)Mt * (p.bnt / 4), 256), d.T);
         if (ada) tc::splitk_epilogue<true><<<g, 256, 0, st>>>(p, Mt, dl);
         else tc::splitk_epilogue<false><<<g, 256, 0, st>>>(p, Mt, dl);
         ctx->launches++;
@@ -471,7 +489,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     {
         KernelTimer kt(ctx, KIND_FWD);
         p.mode = 0; p.M = d.L; p.kunit = ctx->Np; p.ksplit = ks_f;
-        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.L, tc::kTileM), d.T, ks_f), dim3(tc::kThreadsTC), smem,
+        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.L, tc::kTileM) * dsplit, d.T, ks_f), dim3(tc::kThreadsTC), smem,
                       st, ctx->mapA_fwd, ctx->mapA_fwd64, tb.mapQ_f, tb.mapQ_l, p, dl));
         ctx->launches++;
         if (ks_f > 1) epilogue(ceil_div(d.L, tc::kTileM) * tc::kTileM);
@@ -479,13 +497,14 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     {
         KernelTimer kt(ctx, KIND_GRAD);
         p.mode = 1; p.M = d.N; p.kunit = ctx->Lp; p.ksplit = ks_g;
-        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.N, tc::kTileM), d.T, ks_g), dim3(tc::kThreadsTC), smem,
+        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.N, tc::kTileM) * dsplit, d.T, ks_g), dim3(tc::kThreadsTC), smem,
                       st, ctx->mapA_grad, ctx->mapA_grad64, tb.mapR_f, tb.mapR_l, p, dl));
         ctx->launches++;
         if (ks_g > 1) epilogue(ceil_div(d.N, tc::kTileM) * tc::kTileM);
     }
     char buf[96];
-    snprintf(buf, sizeof buf, "tcgen05_3xtf32_fwd_bn%d+tcgen05_3xtf32_grad_bn%d", bn, bn);
+    snprintf(buf, sizeof buf, dsplit > 1 ? "tcgen05_3xtf32_fwd_bn%dx2+tcgen05_3xtf32_grad_bn%dx2"
+                                         : "tcgen05_3xtf32_fwd_bn%d+tcgen05_3xtf32_grad_bn%d", bn, bn);
     ctx->path = buf;
     return DODE_OK;
 }
@@ -544,6 +563,7 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
     const dode_dims& d = ctx->dm;
     const size_t dayStride = (size_t)d.T * ctx->Np;
     const int chunk = d.storage == DODE_CSR ? kCsrMaxDays : kMaxDays;
+    ctx->lanes_used = 0;
     for (int off = 0; off < n; off += chunk) {          // days are independent units
         DayList dl;
         dl.n = std::min(chunk, n - off);
@@ -557,6 +577,7 @@ static int step_impl(dode_ctx* ctx, const int32_t* days, int32_t n, float eta, i
             if ((rc = lane_begin(ctx, dl, &ln))) return rc;
             if ((rc = tc_step(ctx, c, dl, eta, opt, ln->buf, ln->st))) return rc;
             if ((rc = lane_end(ctx, ln))) return rc;
+            ctx->lanes_used |= 1u << (ln - ctx->lane);
             continue;
         }
         if ((rc = join_lanes(ctx))) return rc;
@@ -635,6 +656,8 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     if (d.storage != DODE_DENSE && d.storage != DODE_CSR) return fail(ctx, DODE_EINVAL, "unknown storage %d", d.storage);
     if (d.T > 65535) return fail(ctx, DODE_EINVAL, "T=%d exceeds 65535 (the time index rides on grid.y)", d.T);
     if (d.storage == DODE_DENSE && !R->dense) return fail(ctx, DODE_EINVAL, "R->dense is null");
+    if (d.storage == DODE_CSR && (d.L >= (1 << kPayLinkBits) || d.H + kRB >= (1 << (31 - kPayLinkBits))))
+        return fail(ctx, DODE_EINVAL, "CSR storage supports L < 2^20 and H < 2^11 - 4 (L=%d H=%d)", d.L, d.H);
     if (d.storage == DODE_CSR && (!R->blk_off || !R->row_ptr || (R->nnz > 0 && (!R->col_idx || !R->val)) || R->nnz < 0))
         return fail(ctx, DODE_EINVAL, "CSR arrays are null or nnz < 0");
     for (int i = 0; i < d.D; ++i)
@@ -764,11 +787,18 @@ int dode_reserve(dode_ctx* ctx, int32_t max_days) {
             for (Lane& ln : ctx->lane)
                 if ((rc = lane_init(ctx, ln))) return rc;
             size_t part = 0;
-            for (int bn = 16; bn <= w; bn += 16) part = std::max(part, tc_geometry(ctx, bn).part_floats);
+            int rows = 0, bn_max = 16;
+            for (int n = 1; n <= std::min<int>(max_days, kMaxDays); ++n) {
+                int ds, bn;
+                tc_day_groups(n, &ds, &bn);
+                part = std::max(part, tc_geometry(ctx, bn, ds).part_floats);
+                rows = std::max(rows, ds * bn);
+                bn_max = std::max(bn_max, bn);
+            }
             struct { TcBuf* tb; cudaStream_t st; } bufs[3] = {{&ctx->tcb, ctx->stream}, {&ctx->lane[0].buf, ctx->lane[0].st},
                                                               {&ctx->lane[1].buf, ctx->lane[1].st}};
             for (auto& b : bufs) {
-                if ((rc = tc_ensure(ctx, *b.tb, b.st, w))) return rc;
+                if ((rc = tc_ensure(ctx, *b.tb, b.st, bn_max, rows))) return rc;
                 if ((rc = tc_ensure_part(ctx, *b.tb, b.st, part))) return rc;
             }
         }
@@ -838,7 +868,9 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
     int c = 0, rc;
     if ((rc = validate_days(ctx, days, n, true, &c))) return rc;
     if (!x_host || !q_host) return fail(ctx, DODE_EINVAL, "x_host or q_host is null");
-    if ((rc = join_lanes(ctx))) return rc;
+    // (consecutive streaming steps keep alternating on the internal step streams like plain ones; the lanes are joined
+    // into the ctx stream only at the transition from plain calls, for the fence below)
+    if (ctx->plain_since_host && (rc = join_lanes(ctx))) return rc;
     const dode_dims& d = ctx->dm;
     const size_t TL = (size_t)d.T * d.L, TN = (size_t)d.T * d.N;
     if (!ctx->s_h2d) {
@@ -896,9 +928,15 @@ int dode_spgd_step_host(dode_ctx* ctx, const int32_t* days, int32_t n, float eta
     CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_scat[me], 0));
     if (two) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_gath[me], 0));
     if (shares_day) CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_gath[other], 0));
-    if ((rc = step_impl(ctx, days, n, eta, c))) return rc;
-    CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
-    CU(cudaStreamWaitEvent(ctx->s_ga, ctx->ev_step[me], 0));
+    if ((rc = step_impl(ctx, days, n, eta, c, StepOpt(), true))) return rc;
+    if (ctx->lanes_used) {                        // the step ran on internal step streams: the gather follows those
+        for (int li = 0; li < 2; ++li)
+            if (ctx->lanes_used & (1u << li)) CU(cudaStreamWaitEvent(ctx->s_ga, ctx->lane[li].done, 0));
+        CU(cudaEventRecord(ctx->ev_step[me], ctx->s_ga));
+    } else {
+        CU(cudaEventRecord(ctx->ev_step[me], ctx->stream));
+        CU(cudaStreamWaitEvent(ctx->s_ga, ctx->ev_step[me], 0));
+    }
     if (two) CU(cudaStreamWaitEvent(ctx->s_ga, ctx->ev_d2h[me], 0));
     for (int off = 0; off < n; off += kMaxDays) {
         DayList dl; dl.n = std::min(kMaxDays, n - off);
@@ -1151,6 +1189,91 @@ int dode_assignment_build(int32_t N, int32_t L, int32_t T, int32_t H, const int3
     return build_operator(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, R_out, stream);
 }
 
+int dode_assignment_build_csr(int32_t N, int32_t L, int32_t T, int32_t H, const int32_t* od_ptr, const int32_t* path_ptr,
+                              const int32_t* path_links, const float* link_len, const float* speed, double dt, double theta,
+                              int64_t* blk_off_out, int32_t* row_ptr_out, int32_t* col_idx_out, float* val_out,
+                              int64_t cap, int64_t* nnz_out, void* stream) {
+    dode_ctx* ctx = nullptr;
+    if (N < 1 || L < 1 || T < 1 || H < 0 || !(dt > 0.0)) return fail(ctx, DODE_EINVAL, "dims must be positive and dt > 0");
+    if (!path_ptr || !path_links || !link_len || !speed || !nnz_out) return fail(ctx, DODE_EINVAL, "null argument");
+    if (!(theta >= 0.0)) return fail(ctx, DODE_EINVAL, "theta must be >= 0");
+    if (cap > 0 && (!blk_off_out || !row_ptr_out || !col_idx_out || !val_out)) return fail(ctx, DODE_EINVAL, "null output");
+    int dev = 0, major = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return fail(ctx, DODE_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+    if (major != 10) return fail(ctx, DODE_ECUDA, "this library is built for sm_100a only (device is sm_%d0)", major);
+    cudaStream_t st = (cudaStream_t)stream;
+    const long total = (long)T * N, blocks_sh = (long)T * (H + 1);
+    const int threads = 64;
+    const int grid = (int)std::min<long>((total + threads - 1) / threads, 148L * 64);
+    int32_t* cnt = nullptr; int64_t* offs = nullptr; void* tmp = nullptr; int64_t* d_nu = nullptr;
+    unsigned long long *k0 = nullptr, *k1 = nullptr; float *v0 = nullptr, *v1 = nullptr;
+    int rc = DODE_OK;
+    int64_t nt = 0, nu = 0;
+    auto cleanup = [&]() { cudaFree(cnt); cudaFree(offs); cudaFree(tmp); cudaFree(d_nu); cudaFree(k0); cudaFree(k1); cudaFree(v0); cudaFree(v1); };
+#define BCU(call)                                                                                                     \
+    do {                                                                                                              \
+        cudaError_t e_ = (call);                                                                                      \
+        if (e_ != cudaSuccess) {                                                                                      \
+            rc = fail(ctx, e_ == cudaErrorMemoryAllocation ? DODE_ENOMEM : DODE_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+            cleanup(); cudaGetLastError();                                                                            \
+            return rc;                                                                                                \
+        }                                                                                                             \
+    } while (0)
+    BCU(cudaMalloc(&cnt, (size_t)total * 4));
+    BCU(cudaMalloc(&offs, (size_t)(total + 1) * 8));
+    BCU(cudaMalloc(&d_nu, 8));
+    assignment_tuples<<<grid, threads, 0, st>>>(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, cnt,
+                                                nullptr, nullptr, nullptr);
+    size_t tb_scan = 0;
+    cub::DeviceScan::ExclusiveSum(nullptr, tb_scan, cnt, offs, (int)total, st);
+    BCU(cudaMalloc(&tmp, tb_scan));
+    BCU(cub::DeviceScan::ExclusiveSum(tmp, tb_scan, cnt, offs, (int)total, st));
+    int64_t last_off = 0; int32_t last_cnt = 0;
+    BCU(cudaMemcpyAsync(&last_off, offs + total - 1, 8, cudaMemcpyDeviceToHost, st));
+    BCU(cudaMemcpyAsync(&last_cnt, cnt + total - 1, 4, cudaMemcpyDeviceToHost, st));
+    BCU(cudaStreamSynchronize(st));
+    nt = last_off + last_cnt;
+    if (cap < nt) {                               // the caller sizes its arrays from this
+        *nnz_out = nt;
+        cleanup();
+        return fail(ctx, DODE_ENOMEM, "output capacity %lld is below the %lld shares to emit", (long long)cap, (long long)nt);
+    }
+    cudaFree(tmp); tmp = nullptr;
+    if (!blk_off_out || !row_ptr_out) {           // sizing call on an operator without a single share
+        *nnz_out = 0;
+        cleanup();
+        return DODE_OK;
+    }
+    if (nt > 0) {
+        BCU(cudaMalloc(&k0, (size_t)nt * 8)); BCU(cudaMalloc(&k1, (size_t)nt * 8));
+        BCU(cudaMalloc(&v0, (size_t)nt * 4)); BCU(cudaMalloc(&v1, (size_t)nt * 4));
+        assignment_tuples<<<grid, threads, 0, st>>>(N, L, T, H, od_ptr, path_ptr, path_links, link_len, speed, dt, theta, cnt,
+                                                    offs, k0, v0);
+        int bits = 1;
+        while (bits < 64 && ((unsigned long long)1 << bits) < (unsigned long long)blocks_sh * L * N) ++bits;
+        size_t tb_sort = 0, tb_red = 0;
+        cub::DeviceRadixSort::SortPairs(nullptr, tb_sort, k0, k1, v0, v1, nt, 0, bits, st);
+        cub::DeviceReduce::ReduceByKey(nullptr, tb_red, k1, k0, v1, val_out, d_nu, cub::Sum(), nt, st);
+        BCU(cudaMalloc(&tmp, std::max(tb_sort, tb_red)));
+        BCU(cub::DeviceRadixSort::SortPairs(tmp, tb_sort, k0, k1, v0, v1, nt, 0, bits, st));
+        // equal keys = several paths of one OD over one link in one lag: their shares add up (Eq. 41 summed over the OD's paths)
+        BCU(cub::DeviceReduce::ReduceByKey(tmp, tb_red, k1, k0, v1, val_out, d_nu, cub::Sum(), nt, st));
+        BCU(cudaMemcpyAsync(&nu, d_nu, 8, cudaMemcpyDeviceToHost, st));
+        BCU(cudaStreamSynchronize(st));
+        csr_cols_from_keys<<<1184, 256, 0, st>>>(k0, nu, N, col_idx_out);
+    }
+    const long nb = blocks_sh * (L + 1);
+    csr_bounds_from_keys<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(k0, nu, blocks_sh, L, N, blk_off_out, row_ptr_out);
+    BCU(cudaStreamSynchronize(st));
+    BCU(cudaGetLastError());
+#undef BCU
+    cleanup();
+    *nnz_out = nu;
+    return DODE_OK;
+}
+
 int dode_probe_fp32_peak(int32_t reps, double* tflops, void* stream) {
     dode_ctx* ctx = nullptr;
     if (reps < 1 || !tflops) return fail(ctx, DODE_EINVAL, "reps < 1 or null output");
@@ -1206,6 +1329,16 @@ int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* lau
     if (reset) { ctx->t_total[kind] = 0; ctx->t_count[kind] = 0; }
     return DODE_OK;
 }
+
+#ifdef DODE_BRINGUP
+// bring-up only: the record of waits that gave up (kernels_tc.cuh); not declared in include/dode.h
+int dode_bringup_wait_record(int* host64) {
+    int z = 0;
+    cudaError_t e = cudaMemcpyFromSymbol(host64, tc::g_wait_rec, sizeof(int) * 64);
+    cudaMemcpyToSymbol(tc::g_wait_abort, &z, sizeof(int));
+    return (int)e;
+}
+#endif
 
 int64_t dode_launch_count(const dode_ctx* ctx) { return ctx ? ctx->launches : 0; }
 

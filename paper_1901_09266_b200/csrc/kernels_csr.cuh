@@ -4,19 +4,24 @@
 // re-packed, on the device, into two lag-merged ROW-BLOCKED sparse matrices so that both passes stream their
 // non-zeros contiguously and deterministically (no atomics on the hot path) and so that one gathered panel row
 // feeds up to kRB output rows:
-//   F (forward):  row block (t, l/4) holds one entry per distinct (h,n) of the blocks (t-h,h), h<=min(H,t), that
-//                 touches any of its 4 links: payload off = n - h*Np, values val[4] (0 where a link has no entry)
-//                 -> operand Qb[(t*Np + off)*bp + d].  Paths are contiguous link runs with slowly growing lag
-//                 (PAPER.md:195-228), so adjacent links share most (h,n): ~2.5x fewer gathers than plain CSR.
+//   F (forward):  row block (t/2, l/4) — 4 links x 2 arrival intervals = 8 output rows — holds one entry per distinct
+//                 state row (s,n) that feeds any of them: payload (s - (2*(t/2) - H))*Np + n, values val[8] by
+//                 (t%2)*4 + l%4 (0 where an output has no entry) -> operand Qb[(s*Np + n)*bp + d].  Paths are
+//                 contiguous link runs with slowly growing lag and 2-4 adjacent lags per link, so
+//                 adjacent links AND adjacent arrival intervals share most (s,n): 3.7 products per gathered row
+//                 against 1 for plain CSR and 2.3 for 4 links x 1 interval (the gathers, not the FMAs, bound the pass).
 //   G (gradient): row block (s/4, n) holds one entry per distinct residual row (t,l), t = s+h, reached from any of
-//                 its 4 departure intervals: payload kl = (t - 4*(s/4))*L + l, values val[4] by s%4
-//                 -> operand r[((4*(s/4))*L + kl)*bp + d].  The lag window of a (link, OD) pair spans 2-4 adjacent
+//                 its 4 departure intervals: payload ((t - 4*(s/4)) << 20) | l, values val[4] by s%4, entries sorted
+//                 by (t, l) -> operand r[(t*L + l)*bp + d].  The lag window of a (link, OD) pair spans 2-4 adjacent
 //                 lags, so consecutive departure intervals share most residual rows: ~2x fewer gathers.
+//                 ODs are processed in PATH ORDER (permG: sorted by the first link of their path) in groups of
+//                 kGradWarps; each group knows the link range [lo, lo+span) its paths cover, so that a CTA can stage
+//                 the residual rows r[t][lo..lo+span) of one arrival interval with ONE bulk copy (csr_grad_staged).
 // Entries with s+h >= T are dropped.  The re-pack is a radix sort of 64-bit keys, a head-flag scan
 // and a scatter (CUB, create-time only).
 //
-// Hot path: the minibatch state is gathered once per step into day-fastest panels Qb[T*Np][bp] and
-// Xb[T*L][bp] (coalesced transposes), so that one entry pulls bp contiguous floats; a warp owns one
+// Hot path: the minibatch state is gathered once per step into the day-fastest panel Qb[T*Np][bp]
+// (a coalesced transpose), so that one entry pulls bp contiguous floats; a warp owns one
 // row block and its lanes run along the days.  The update q <- max(0, q - eta g) is applied to Qb in the
 // gradient kernel's epilogue and scattered back to q[d][s][n].
 #pragma once
@@ -29,20 +34,27 @@
 
 #include "../../include/dode.h"
 #include "kernels_dense.cuh"
+#include "kernels_tc.cuh"      // mbarrier / elect helpers
 
 namespace dode {
 
 constexpr int kCsrMaxDays = 128;
-constexpr int kRB = 4;            // output rows per row block
+constexpr int kRB = 4;            // links (forward) / departure intervals (gradient) per row block
+constexpr int kFT = 2;            // arrival intervals per forward row block
+constexpr int kFS = kRB * kFT;    // output rows (value slots) of a forward entry
+constexpr int kGradWarps = 16;    // ODs (consumer warps) per CTA of csr_grad_staged
+constexpr int kPayLinkBits = 20;  // gradient payload: (t_rel << 20) | l
 
 struct CsrCluster {
-    int64_t* rowptrF = nullptr;   // [T*ceil(L/4) + 1]
-    int32_t* payF = nullptr;      // [nuF]  n - h*Np
-    float4* valF = nullptr;       // [nuF]  by l%4
+    int64_t* rowptrF = nullptr;   // [ceil(T/2)*ceil(L/4) + 1]
+    int32_t* payF = nullptr;      // [nuF]  (s - (2*(t/2) - H))*Np + n
+    float4* valF = nullptr;       // [2*nuF] eight values per entry, slot (t%2)*4 + l%4
     int64_t* rowptrG = nullptr;   // [ceil(T/4)*Np + 1]
     int32_t* payG = nullptr;      // [nuG]  (t - 4*(s/4))*L + l
     float4* valG = nullptr;       // [nuG]  by s%4
     int32_t* permG = nullptr;     // [Np]   OD indices ordered by the first link of their path (processing order of a3)
+    int32_t* grpLo = nullptr;     // [ceil(Np/kGradWarps)] first link covered by the ODs permG[g*kGradWarps ...]
+    int span = 0;                 // max over groups of (last link - first link + 1); 0 = no entries
     int64_t nnz = 0;              // valid entries (s+h < T)
     int64_t nuF = 0, nuG = 0;     // distinct (row block, payload) entries
 };
@@ -52,16 +64,16 @@ struct CsrStore {
     int C = 0;
     CsrCluster* cl = nullptr;     // host array [C]
     float* Qb = nullptr;          // [T*Np][bp]
-    float* Xb = nullptr;          // [T*L][bp]
     int cap_bp = 0;
     // NEXT-1 (row-chunk + Adagrad), allocated on first use
     float* Mb = nullptr;          // [T*L][bp]  row mask as 0/1 floats
     float* Gb = nullptr;          // [T*Np][bp] Adagrad accumulator panel
     int cap_bp_ada = 0;
+    bool staged_attr[5] = {false, false, false, false, false};   // csr_grad_staged<DV> shared-memory opt-in done
 };
 
 // ---- create-time re-pack ---------------------------------------------------------------------------
-// one warp per input CSR row (s,h,l) of cluster c; key = ((row block * K + payload) << 2) | row in block
+// one warp per input CSR row (s,h,l) of cluster c; key = ((row block * K + payload) << slot bits) | slot
 __global__ void csr_expand_keys(const int64_t* __restrict__ blk_off, const int32_t* __restrict__ row_ptr,
                                 const int32_t* __restrict__ col_idx, int c, int N, int Np, int L, int T, int H,
                                 int64_t base, unsigned long long* __restrict__ keyF,
@@ -76,40 +88,42 @@ __global__ void csr_expand_keys(const int64_t* __restrict__ blk_off, const int32
     const long b = (long)c * T * (H + 1) + sh;
     const int32_t* rp = row_ptr + b * (L + 1);
     const int64_t k0 = blk_off[b] + rp[l], k1 = blk_off[b] + rp[l + 1];
-    const unsigned long long KF = (unsigned long long)(H + 1) * Np, KG = (unsigned long long)(H + kRB) * L;
+    const unsigned long long KF = (unsigned long long)(H + kFT) * Np, KG = (unsigned long long)(H + kRB) * L;
     const unsigned long long LB = (unsigned long long)(L + kRB - 1) / kRB;
     const bool valid = s + h < T;
-    const int t = s + h, sb = s / kRB;
+    const int t = s + h, sb = s / kRB, tb = t / kFT;
     for (int64_t k = k0 + lane; k < k1; k += 32) {
         const int n = col_idx[k];
-        const unsigned long long rbF = (unsigned long long)t * LB + l / kRB, payF = (unsigned long long)h * Np + n;
+        const unsigned long long rbF = (unsigned long long)tb * LB + l / kRB;
+        const unsigned long long payF = (unsigned long long)(s - (tb * kFT - H)) * Np + n;       // s >= t - H >= tb*kFT - H
         const unsigned long long rbG = (unsigned long long)sb * Np + n, payG = (unsigned long long)(t - sb * kRB) * L + l;
-        keyF[k - base] = valid ? ((rbF * KF + payF) << 2) | (unsigned)(l % kRB) : ~0ull;
+        keyF[k - base] = valid ? ((rbF * KF + payF) << 3) | (unsigned)((t % kFT) * kRB + l % kRB) : ~0ull;
         keyG[k - base] = valid ? ((rbG * KG + payG) << 2) | (unsigned)(s % kRB) : ~0ull;
     }
 }
 
 // head[i] = 1 where a new (row block, payload) starts in the sorted key array
-__global__ void csr_heads(const unsigned long long* __restrict__ keys, int64_t n, int32_t* __restrict__ head) {
+__global__ void csr_heads(const unsigned long long* __restrict__ keys, int64_t n, int shift, int32_t* __restrict__ head) {
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        head[i] = (i == 0 || (keys[i] >> 2) != (keys[i - 1] >> 2)) ? 1 : 0;
+        head[i] = (i == 0 || (keys[i] >> shift) != (keys[i - 1] >> shift)) ? 1 : 0;
 }
 
-// uidx = inclusive scan of head; entry u = uidx[i]-1 receives val[i] in slot key&3; heads also write payload and key
+// uidx = inclusive scan of head; entry u = uidx[i]-1 receives val[i] in slot key & (2^shift - 1); heads also write
+// payload and key
 __global__ void csr_scatter_unique(const unsigned long long* __restrict__ keys, const float* __restrict__ val,
-                                   const int32_t* __restrict__ uidx, int64_t n, unsigned long long K, int Np, int forward,
+                                   const int32_t* __restrict__ uidx, int64_t n, unsigned long long K, int L, int shift,
                                    float* __restrict__ val4, int32_t* __restrict__ pay, unsigned long long* __restrict__ ukey) {
+    const bool forward = shift == 3;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const unsigned long long key = keys[i], kk = key >> 2;
+        const unsigned long long key = keys[i], kk = key >> shift;
         const int64_t u = (int64_t)uidx[i] - 1;
-        val4[u * 4 + (int)(key & 3)] = val[i];
-        if (i == 0 || kk != (keys[i - 1] >> 2)) {
+        val4[(u << shift) + (int)(key & ((1u << shift) - 1))] = val[i];
+        if (i == 0 || kk != (keys[i - 1] >> shift)) {
             const unsigned long long rem = kk % K;
             if (forward) {
-                const int h = (int)(rem / Np), nn = (int)(rem - (unsigned long long)h * Np);
-                pay[u] = nn - h * Np;
+                pay[u] = (int32_t)rem;                                             // s_rel * Np + n
             } else {
-                pay[u] = (int32_t)rem;
+                pay[u] = (int32_t)(((rem / L) << kPayLinkBits) | (rem % L));      // (t - 4*(s/4), l)
             }
             ukey[u] = kk;
         }
@@ -138,10 +152,29 @@ __global__ void csr_first_link(const int64_t* __restrict__ rowptrG, const int32_
     int best = L;
     for (long sb = 0; sb < SB && best == L; ++sb) {
         const int64_t k0 = rowptrG[sb * Np + n], k1 = rowptrG[sb * Np + n + 1];
-        for (int64_t k = k0; k < k1; ++k) best = min(best, payG[k] % L);
+        for (int64_t k = k0; k < k1; ++k) best = min(best, payG[k] & ((1 << kPayLinkBits) - 1));
     }
     first[n] = best;
     ident[n] = n;
+}
+
+// lowest / highest link of every OD's entries: one warp per gradient row block
+__global__ void csr_od_span(const int64_t* __restrict__ rowptrG, const int32_t* __restrict__ payG, int Np, long rblocks,
+                            int32_t* __restrict__ odmin, int32_t* __restrict__ odmax) {
+    const long w = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (w >= rblocks) return;
+    const int n = (int)(w % Np);
+    int lo = INT32_MAX, hi = -1;
+    for (int64_t k = rowptrG[w] + lane; k < rowptrG[w + 1]; k += 32) {
+        const int l = payG[k] & ((1 << kPayLinkBits) - 1);
+        lo = min(lo, l); hi = max(hi, l);
+    }
+    for (int o = 16; o; o >>= 1) {
+        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if (lane == 0 && hi >= 0) { atomicMin(odmin + n, lo); atomicMax(odmax + n, hi); }
 }
 
 __global__ void count_invalid(const unsigned long long* __restrict__ keys, int64_t n, unsigned long long* cnt) {
@@ -157,12 +190,13 @@ inline void csr_free(CsrStore& st) {
         for (int c = 0; c < st.C; ++c) {
             cudaFree(st.cl[c].rowptrF); cudaFree(st.cl[c].payF); cudaFree(st.cl[c].valF);
             cudaFree(st.cl[c].rowptrG); cudaFree(st.cl[c].payG); cudaFree(st.cl[c].valG); cudaFree(st.cl[c].permG);
+            cudaFree(st.cl[c].grpLo);
         }
         delete[] st.cl;
         st.cl = nullptr;
     }
-    cudaFree(st.Qb); cudaFree(st.Xb); cudaFree(st.Mb); cudaFree(st.Gb);
-    st.Qb = st.Xb = st.Mb = st.Gb = nullptr;
+    cudaFree(st.Qb); cudaFree(st.Mb); cudaFree(st.Gb);
+    st.Qb = st.Mb = st.Gb = nullptr;
     st.ready = false;
 }
 
@@ -201,8 +235,8 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
     cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, head, head, (int)maxn, stream);
     const size_t tmp_bytes = std::max(tmp_sort, tmp_scan);
     CSR_CU(cudaMalloc(&tmp, tmp_bytes));
-    const unsigned long long KF = (unsigned long long)(d.H + 1) * Np, KG = (unsigned long long)(d.H + kRB) * d.L;
-    const long LB = (d.L + kRB - 1) / kRB, SB = (d.T + kRB - 1) / kRB;
+    const unsigned long long KF = (unsigned long long)(d.H + kFT) * Np, KG = (unsigned long long)(d.H + kRB) * d.L;
+    const long LB = (d.L + kRB - 1) / kRB, SB = (d.T + kRB - 1) / kRB, TB = (d.T + kFT - 1) / kFT;
     for (int c = 0; c < d.C; ++c) {
         CsrCluster& cl = st.cl[c];
         const int64_t n = off[c + 1] - off[c];
@@ -221,12 +255,13 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
         for (int pass = 0; pass < 2; ++pass) {
             unsigned long long* kin = pass == 0 ? kF : kG;
             const unsigned long long K = pass == 0 ? KF : KG;
-            const long rows = pass == 0 ? (long)d.T * LB : SB * Np;          // row blocks
+            const long rows = pass == 0 ? TB * LB : SB * Np;                 // row blocks
+            const int shift = pass == 0 ? 3 : 2;                             // log2(value slots per entry)
             int64_t nu = 0;
             if (nv > 0) {
                 // invalid keys are all-ones: sort on all 64 bits so they land at the end
                 CSR_CU(cub::DeviceRadixSort::SortPairs(tmp, tmp_sort, kin, kS, R.val + off[c], vS, n, 0, 64, stream));
-                csr_heads<<<1184, 256, 0, stream>>>(kS, nv, head);
+                csr_heads<<<1184, 256, 0, stream>>>(kS, nv, shift, head);
                 CSR_CU(cub::DeviceScan::InclusiveSum(tmp, tmp_scan, head, head, (int)nv, stream));
                 int32_t last = 0;
                 CSR_CU(cudaMemcpyAsync(&last, head + nv - 1, 4, cudaMemcpyDeviceToHost, stream));
@@ -238,11 +273,11 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
             int64_t** rowptr = pass == 0 ? &cl.rowptrF : &cl.rowptrG;
             (pass == 0 ? cl.nuF : cl.nuG) = nu;
             CSR_CU(cudaMalloc(pay, std::max<int64_t>(nu, 1) * 4));
-            CSR_CU(cudaMalloc(val4, std::max<int64_t>(nu, 1) * 16));
+            CSR_CU(cudaMalloc(val4, (std::max<int64_t>(nu, 1) * 4) << shift));
             CSR_CU(cudaMalloc(rowptr, (rows + 1) * 8));
             if (nu > 0) {
-                CSR_CU(cudaMemsetAsync(*val4, 0, nu * 16, stream));
-                csr_scatter_unique<<<1184, 256, 0, stream>>>(kS, vS, head, nv, K, Np, pass == 0,
+                CSR_CU(cudaMemsetAsync(*val4, 0, (nu * 4) << shift, stream));
+                csr_scatter_unique<<<1184, 256, 0, stream>>>(kS, vS, head, nv, K, d.L, shift,
                                                              reinterpret_cast<float*>(*val4), *pay, ukey);
             }
             csr_rowptr<<<(unsigned)((rows + 1 + 255) / 256), 256, 0, stream>>>(ukey, nu, rows, K, *rowptr);
@@ -261,6 +296,35 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
             if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(stream);
             cudaFree(t2); cudaFree(sc);
             CSR_CU(e2);
+        }
+        // link range of every group of kGradWarps path-adjacent ODs (csr_grad_staged stages r[t][lo..lo+span) per CTA)
+        {
+            int32_t* mm = nullptr;                       // [Np] min | [Np] max
+            CSR_CU(cudaMalloc(&mm, (size_t)2 * Np * 4));
+            CSR_CU(cudaMemsetAsync(mm, 0x7f, (size_t)Np * 4, stream));
+            CSR_CU(cudaMemsetAsync(mm + Np, 0xff, (size_t)Np * 4, stream));
+            const long rbl = SB * Np;
+            csr_od_span<<<(unsigned)((rbl * 32 + 255) / 256), 256, 0, stream>>>(cl.rowptrG, cl.payG, Np, rbl, mm, mm + Np);
+            std::vector<int32_t> hmm((size_t)2 * Np), hperm(Np);
+            cudaError_t e3 = cudaMemcpyAsync(hmm.data(), mm, (size_t)2 * Np * 4, cudaMemcpyDeviceToHost, stream);
+            if (e3 == cudaSuccess) e3 = cudaMemcpyAsync(hperm.data(), cl.permG, (size_t)Np * 4, cudaMemcpyDeviceToHost, stream);
+            if (e3 == cudaSuccess) e3 = cudaStreamSynchronize(stream);
+            cudaFree(mm);
+            CSR_CU(e3);
+            const int groups = (Np + kGradWarps - 1) / kGradWarps;
+            std::vector<int32_t> glo(groups, 0);
+            cl.span = 0;
+            for (int g = 0; g < groups; ++g) {
+                int lo = INT32_MAX, hi = -1;
+                for (int i = g * kGradWarps; i < std::min(Np, (g + 1) * kGradWarps); ++i) {
+                    const int n = hperm[i];
+                    if (hmm[(size_t)Np + n] >= 0) { lo = std::min(lo, hmm[n]); hi = std::max(hi, hmm[(size_t)Np + n]); }
+                }
+                if (hi >= 0) { glo[g] = lo; cl.span = std::max(cl.span, hi - lo + 1); }
+            }
+            CSR_CU(cudaMalloc(&cl.grpLo, (size_t)groups * 4));
+            CSR_CU(cudaMemcpyAsync(cl.grpLo, glo.data(), (size_t)groups * 4, cudaMemcpyHostToDevice, stream));
+            CSR_CU(cudaStreamSynchronize(stream));
         }
         CSR_CU(cudaStreamSynchronize(stream));
     }
@@ -314,83 +378,97 @@ scatter_days(const float* __restrict__ src, int bp, long rowLen, float* __restri
     }
 }
 
+// residual row (relative to the row block's first arrival interval) of a gradient payload
+__device__ __forceinline__ long pay_row(int pay, int L) {
+    return (long)(pay >> kPayLinkBits) * L + (pay & ((1 << kPayLinkBits) - 1));
+}
+
 template <int DV> struct DVec;
 template <> struct DVec<1> { using type = float; };
 template <> struct DVec<2> { using type = float2; };
 template <> struct DVec<4> { using type = float4; };
 
-// a2 (CSR): one warp per row block (t, l/4) of F; lanes along days (DV days per lane, bp = 32*DV).
-// r[(t*L+l)*rbp + d] = sum_k val_k[l%4] * Qb[(t*Np + off_k)*bp + d] - Xb[(t*L+l)*bp + d]   for d < rbp
+// a2 (CSR): one warp per row block (t/2, l/4) of F = 8 output rows; lanes along days (DV days per lane, bp = 32*DV).
+//   r[(t*L+l)*rbp + d] = sum_k val_k[(t%2)*4 + l%4] * Qb[(base + pay_k)*bp + d] - x[day_d][t][l]    for d < rbp,
+//   base = (2*(t/2) - H)*Np.  The counts are read straight from x[D][T][L] (one scalar per output and day).
+// A chunk of 32 entries is fetched by the whole warp with coalesced loads; the eight values of an entry are then
+// broadcast from shared memory (two LDS.128 at a warp-uniform address) and its payload by one shuffle — nine shuffles
+// per entry would cost more LSU slots than the 512-byte gather they accompany.
 template <int DV>
-__global__ void __launch_bounds__(256, 4)
-csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ off, const float4* __restrict__ val,
-        const float* __restrict__ Qb, const float* __restrict__ Xb, const float* __restrict__ Mb, float* __restrict__ r,
-        long rblocks, int L, int LB, int Np, int rbp) {
+__global__ void __launch_bounds__(256, 3)
+csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, const float4* __restrict__ val,
+        const float* __restrict__ Qb, const float* __restrict__ x, const float* __restrict__ Mb, float* __restrict__ r,
+        long rblocks, int T, int H, int L, int LB, int Np, int rbp, const __grid_constant__ DayList dl) {
     constexpr int bp = 32 * DV;
     using vec = typename DVec<DV>::type;
+    __shared__ float4 sval[8][64];                   // per warp: 32 entries x 2 float4
     // Warps walk the row blocks LINK-BLOCK-major, time-minor: the warps in flight then cover a few dozen neighbouring
     // link blocks over all t, whose OD sets overlap (paths are link runs), so the panel rows they gather (~100 MB) stay
     // in L2; time-major order would sweep the whole 25-lag window of every OD (256 MB) for every t.
     const long w = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     if (w >= rblocks) return;
-    const int T = (int)(rblocks / LB);
-    const long lb = w / T, t = w - lb * T;
-    const long rb = t * LB + lb;
+    const int TB = (int)(rblocks / LB);
+    const long lb = w / TB, tb = w - lb * TB;
+    const long rb = tb * LB + lb;
     const int l0 = (int)lb * kRB;
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
-    const float* qrow = Qb + (size_t)t * Np * bp + lane * DV;
-    float acc[kRB][DV];
+    const float* qrow = Qb + ((long)tb * kFT - H) * Np * bp + lane * DV;      // entries only reach rows >= 0
+    float acc[kFS][DV];
 #pragma unroll
-    for (int i = 0; i < kRB; ++i)
+    for (int i = 0; i < kFS; ++i)
 #pragma unroll
         for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
     for (int64_t kb = k0; kb < k1; kb += 32) {
-        const int64_t k = kb + lane;
-        const int o = k < k1 ? __ldg(off + k) : 0;
-        const float4 v = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
         const int cnt = (int)min((int64_t)32, k1 - kb);
+        const int o = lane < cnt ? __ldg(pay + kb + lane) : 0;
+        __syncwarp();                                // the previous chunk's values have been read
+        if (lane < 2 * cnt) sval[wib][lane] = __ldg(val + 2 * kb + lane);
+        if (lane + 32 < 2 * cnt) sval[wib][lane + 32] = __ldg(val + 2 * kb + lane + 32);
+        __syncwarp();
         int j = 0;
         for (; j + 2 <= cnt; j += 2) {
-            vec qv[2]; float vv[2][kRB];
+            vec qv[2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const int oo = __shfl_sync(0xffffffffu, o, j + u);
-                vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
-                vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
                 qv[u] = *reinterpret_cast<const vec*>(qrow + (long)oo * bp);
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
+                const float4 va = sval[wib][2 * (j + u)], vb = sval[wib][2 * (j + u) + 1];
+                const float vv[kFS] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
                 const float* qf = reinterpret_cast<const float*>(&qv[u]);
 #pragma unroll
-                for (int i = 0; i < kRB; ++i)
+                for (int i = 0; i < kFS; ++i)
 #pragma unroll
-                    for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[u][i], qf[e], acc[i][e]);
+                    for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[i], qf[e], acc[i][e]);
             }
         }
-        for (; j < cnt; ++j) {
+        if (j < cnt) {
             const int oo = __shfl_sync(0xffffffffu, o, j);
-            const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
-                                   __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
             const vec qv = *reinterpret_cast<const vec*>(qrow + (long)oo * bp);
+            const float4 va = sval[wib][2 * j], vb = sval[wib][2 * j + 1];
+            const float vv[kFS] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
             const float* qf = reinterpret_cast<const float*>(&qv);
 #pragma unroll
-            for (int i = 0; i < kRB; ++i)
+            for (int i = 0; i < kFS; ++i)
 #pragma unroll
-                for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(v4[i], qf[e], acc[i][e]);
+                for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[i], qf[e], acc[i][e]);
         }
     }
 #pragma unroll
-    for (int i = 0; i < kRB; ++i) {
-        const int l = l0 + i;
-        if (l >= L) break;
+    for (int i = 0; i < kFS; ++i) {
+        const int l = l0 + (i & (kRB - 1));
+        const long t = tb * kFT + (i >> 2);
+        if (l >= L || t >= T) continue;
         const size_t row = (size_t)t * L + l;
-        if (Xb != nullptr) {
-            const vec xv = *reinterpret_cast<const vec*>(Xb + row * bp + lane * DV);
-            const float* xf = reinterpret_cast<const float*>(&xv);
+        if (x != nullptr) {
 #pragma unroll
-            for (int e = 0; e < DV; ++e) acc[i][e] -= xf[e];
+            for (int e = 0; e < DV; ++e) {
+                const int d = lane * DV + e;
+                acc[i][e] = d < dl.n ? acc[i][e] - __ldg(x + ((size_t)dl.day[d] * T + t) * L + l) : 0.f;   // pad days: r = 0
+            }
         }
         if (Mb != nullptr) {                      // rows outside the chunk B_o contribute no residual
             const vec mv = *reinterpret_cast<const vec*>(Mb + row * bp + lane * DV);
@@ -454,7 +532,7 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
                     const int oo = __shfl_sync(0xffffffffu, o, j + u);
                     vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
                     vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
-                    rv[u] = *reinterpret_cast<const vec*>(rrow + (long)oo * bp);
+                    rv[u] = *reinterpret_cast<const vec*>(rrow + pay_row(oo, L) * bp);
                 }
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
@@ -473,7 +551,7 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
 #pragma unroll
             for (int e = 0; e < DV; ++e)
                 if (full || lane * DV + e < rbp) {
-                    const float rv = rrow[(long)oo * rbp + e];
+                    const float rv = rrow[pay_row(oo, L) * rbp + e];
 #pragma unroll
                     for (int i = 0; i < kRB; ++i) acc[i][e] = fmaf(v4[i], rv, acc[i][e]);
                 }
@@ -499,20 +577,133 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
     }
 }
 
+// a3+a4 (CSR) with the residual rows staged in shared memory.  CTA = one group of kGradWarps path-adjacent ODs (one
+// consumer warp each) x one block of 4 departure intervals + one producer warp.  The entries of a row block are sorted by
+// arrival interval t, and all the residual rows the group can touch at one t are the contiguous run
+// r[t][lo .. lo+span) of the panel, so the producer streams t = 4*sb, 4*sb+1, ... through a ring of stages with ONE bulk
+// copy (cp.async.bulk -> mbarrier) each, and every consumer works through its entries of stage t from shared memory
+// (LDS.128: 4 wavefronts per 512-byte row instead of ~8 cycles through L1, and no LSU request per gathered row at all on
+// the global side).  Every consumer passes through every stage (with or without entries) so that the ring's barriers
+// stay in step.  grid = (groups, ceil(T/4)): consecutive CTAs are neighbouring groups at the same time block, whose
+// rows overlap — the bulk copies hit L2.
+template <int DV>
+__global__ void __launch_bounds__((kGradWarps + 1) * 32)
+csr_grad_staged(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, const float4* __restrict__ val,
+                const int32_t* __restrict__ perm, const int32_t* __restrict__ grp_lo, const float* __restrict__ r,
+                float* __restrict__ Qb, float eta, float* __restrict__ Gb, float eps,
+                int T, int H, int L, int N, int Np, int span, int nst) {
+    constexpr int bp = 32 * DV;
+    using vec = typename DVec<DV>::type;
+    extern __shared__ __align__(128) uint8_t csr_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = blockIdx.x, sb = blockIdx.y;
+    const int lo = grp_lo[g];
+    const int rows = min(span, L - lo);                         // the run must not leave the panel
+    const size_t stageBytes = (size_t)span * bp * sizeof(float);
+    uint64_t* full = reinterpret_cast<uint64_t*>(csr_smem + (size_t)nst * stageBytes);
+    uint64_t* empty = full + nst;
+    const int nq = min(H + kRB, T - sb * kRB);                  // arrival intervals 4*sb .. 4*sb+nq-1 can be referenced
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < nst; ++i) { tc::mbar_init(&full[i], 1); tc::mbar_init(&empty[i], kGradWarps); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == kGradWarps) {
+        // ===== producer =====
+        const uint32_t bytes = (uint32_t)((size_t)rows * bp * sizeof(float));
+        int slot = 0, ph = 1;
+        for (int q = 0; q < nq; ++q) {
+            if (q >= nst) tc::mbar_wait(&empty[slot], ph);
+            if (tc::elect_one()) {
+                tc::mbar_expect_tx(&full[slot], bytes);
+                const float* src = r + ((size_t)(sb * kRB + q) * L + lo) * bp;
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             ::"r"(tc::smem_u32(csr_smem + (size_t)slot * stageBytes)), "l"(src), "r"(bytes),
+                               "r"(tc::smem_u32(&full[slot])) : "memory");
+            }
+            __syncwarp();
+            if (++slot == nst) { slot = 0; ph ^= 1; }
+        }
+        return;
+    }
+    // ===== consumers: warp = one OD of the group, 4 departure intervals =====
+    const int oi = g * kGradWarps + warp;
+    const int n = oi < Np ? __ldg(perm + oi) : N;
+    const bool valid = n < N;
+    int64_t kb = 0, k1 = 0;
+    if (valid) { kb = rowptr[(long)sb * Np + n]; k1 = rowptr[(long)sb * Np + n + 1]; }
+    float acc[kRB][DV];
+#pragma unroll
+    for (int i = 0; i < kRB; ++i)
+#pragma unroll
+        for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
+    // current chunk of 32 entries: lane j holds entry kb + j
+    int o = 0, cnt = 0, j = 0;
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    auto load_chunk = [&]() {
+        const int64_t k = kb + lane;
+        o = k < k1 ? __ldg(pay + k) : 0;
+        v = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
+        cnt = (int)min((int64_t)32, k1 - kb);
+        j = 0;
+    };
+    if (kb < k1) load_chunk();
+    int slot = 0, ph = 0;
+    for (int q = 0; q < nq; ++q) {
+        tc::mbar_wait(&full[slot], ph);
+        const float* stage = reinterpret_cast<const float*>(csr_smem + (size_t)slot * stageBytes) + lane * DV;
+        while (cnt > 0) {
+            if (j == cnt) {                                     // chunk used up: next one, if any
+                kb += 32;
+                if (kb >= k1) { cnt = 0; break; }
+                load_chunk();
+            }
+            const int oo = __shfl_sync(0xffffffffu, o, j);
+            if ((oo >> kPayLinkBits) != q) break;               // belongs to a later arrival interval
+            const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
+                                   __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
+            const vec rv = *reinterpret_cast<const vec*>(stage + (size_t)((oo & ((1 << kPayLinkBits) - 1)) - lo) * bp);
+            const float* rf = reinterpret_cast<const float*>(&rv);
+#pragma unroll
+            for (int i = 0; i < kRB; ++i)
+#pragma unroll
+                for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(v4[i], rf[e], acc[i][e]);
+            ++j;
+        }
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(&empty[slot]);
+        if (++slot == nst) { slot = 0; ph ^= 1; }
+    }
+    if (!valid) return;
+#pragma unroll
+    for (int i = 0; i < kRB; ++i) {
+        const long s = (long)sb * kRB + i;
+        if (s >= T) break;
+        vec* qp = reinterpret_cast<vec*>(Qb + ((size_t)s * Np + n) * bp + lane * DV);
+        vec qv = *qp;
+        float* qf = reinterpret_cast<float*>(&qv);
+#pragma unroll
+        for (int e = 0; e < DV; ++e) {
+            if (Gb != nullptr) qf[e] = adagrad_update(qf[e], acc[i][e], Gb + ((size_t)s * Np + n) * bp + lane * DV + e, eta, eps);
+            else qf[e] = fmaxf(0.f, fmaf(-eta, acc[i][e], qf[e]));
+        }
+        *qp = qv;
+    }
+}
+
 inline int csr_bp(int n) { return n <= 32 ? 32 : n <= 64 ? 64 : 128; }
 
 inline int csr_ensure(CsrStore& st, const dode_dims& d, int Np, int bp, cudaStream_t stream) {
     if (st.cap_bp >= bp) return DODE_OK;
     cudaStreamSynchronize(stream);
-    cudaFree(st.Qb); cudaFree(st.Xb);
-    st.Qb = st.Xb = nullptr; st.cap_bp = 0;
+    cudaFree(st.Qb);
+    st.Qb = nullptr; st.cap_bp = 0;
     if (cudaMalloc(&st.Qb, (size_t)d.T * Np * bp * 4) != cudaSuccess) return DODE_ENOMEM;
-    if (cudaMalloc(&st.Xb, (size_t)d.T * d.L * bp * 4) != cudaSuccess) return DODE_ENOMEM;
     st.cap_bp = bp;
     return DODE_OK;
 }
 
-// gathers + forward.  rbp: stride of r (== bp for steps/objective, 1 for dode_apply).
+// state gather + forward.  rbp: stride of r (== bp for steps/objective, 1 for dode_apply).
 inline int csr_ensure_ada(CsrStore& st, const dode_dims& d, int Np, int bp, cudaStream_t stream) {
     if (st.cap_bp_ada >= bp) return DODE_OK;
     cudaStreamSynchronize(stream);
@@ -534,23 +725,20 @@ inline int csr_forward(CsrStore& st, int c, const float* qbase, size_t dayStride
     const CsrCluster& cl = st.cl[c];
     const long qlen = (long)d.T * Np, xlen = (long)d.T * d.L;
     gather_days<float, false><<<dim3((unsigned)((qlen + 31) / 32), bp / 32), 256, 0, stream>>>(qbase, dayStride, qlen, st.Qb, bp, dl);
-    if (xbase)
-        gather_days<float, false><<<dim3((unsigned)((xlen + 31) / 32), bp / 32), 256, 0, stream>>>(xbase, (size_t)d.T * d.L, xlen, st.Xb, bp, dl);
     if (mask) {
         gather_days<uint8_t, true><<<dim3((unsigned)((xlen + 31) / 32), bp / 32), 256, 0, stream>>>(mask, (size_t)d.T * d.L, xlen, st.Mb, bp, dl);
         *launches += 1;
     }
     const float* Mb = mask ? st.Mb : nullptr;
     const int LB = (d.L + kRB - 1) / kRB;
-    const long rblocks = (long)d.T * LB;
+    const long rblocks = (long)((d.T + kFT - 1) / kFT) * LB;
     const unsigned grid = (unsigned)((rblocks * 32 + 255) / 256);
-    const float* Xb = xbase ? st.Xb : nullptr;
     switch (bp) {
-        case 32: csr_fwd<1><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, Mb, r, rblocks, d.L, LB, Np, rbp); break;
-        case 64: csr_fwd<2><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, Mb, r, rblocks, d.L, LB, Np, rbp); break;
-        default: csr_fwd<4><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, Xb, Mb, r, rblocks, d.L, LB, Np, rbp); break;
+        case 32: csr_fwd<1><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, xbase, Mb, r, rblocks, d.T, d.H, d.L, LB, Np, rbp, dl); break;
+        case 64: csr_fwd<2><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, xbase, Mb, r, rblocks, d.T, d.H, d.L, LB, Np, rbp, dl); break;
+        default: csr_fwd<4><<<grid, 256, 0, stream>>>(cl.rowptrF, cl.payF, cl.valF, st.Qb, xbase, Mb, r, rblocks, d.T, d.H, d.L, LB, Np, rbp, dl); break;
     }
-    *launches += xbase ? 3 : 2;
+    *launches += 2;
     return DODE_OK;
 }
 
@@ -576,10 +764,34 @@ inline int csr_gradient(CsrStore& st, int c, const float* r, float* qbase, size_
         Gb = st.Gb;
         *launches += 1;
     }
-    switch (bp) {
-        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+    // staged kernel when the ring (>= 2 stages of span rows) fits in half an SM's shared memory; else the gather kernel
+    const size_t stageBytes = (size_t)cl.span * bp * sizeof(float);
+    const int nst = stageBytes ? (int)std::min<size_t>(6, (100 * 1024) / stageBytes) : 0;
+    if (rbp == bp && nst >= 2) {
+        const dim3 sg((Np + kGradWarps - 1) / kGradWarps, (d.T + kRB - 1) / kRB);
+        const size_t smem = (size_t)nst * stageBytes + 2 * nst * sizeof(uint64_t);
+        const int threads = (kGradWarps + 1) * 32;
+#define DODE_STAGED(DVV)                                                                                                   \
+        do {                                                                                                                \
+            if (!st.staged_attr[DVV]) {                                                                                     \
+                cudaFuncSetAttribute(csr_grad_staged<DVV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);        \
+                st.staged_attr[DVV] = true;                                                                                 \
+            }                                                                                                               \
+            csr_grad_staged<DVV><<<sg, threads, smem, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, cl.grpLo, r, st.Qb, \
+                                                                eta, Gb, eps, d.T, d.H, d.L, d.N, Np, cl.span, nst);        \
+        } while (0)
+        switch (bp) {
+            case 32: DODE_STAGED(1); break;
+            case 64: DODE_STAGED(2); break;
+            default: DODE_STAGED(4); break;
+        }
+#undef DODE_STAGED
+    } else {
+        switch (bp) {
+            case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+            case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+            default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        }
     }
     scatter_days<<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(st.Qb, bp, rows, qbase, dayStride, dl);
     if (Gbase) {

@@ -17,11 +17,18 @@
 // 3xTF32 (north_star: "3xTF32 tensor-core emulation ... where the tolerance still holds"):
 //   a = a_hi + a_lo with a_hi = a truncated to TF32 (what the tensor core reads from an fp32 container),
 //   a_lo = a - a_hi (exact in fp32);   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo   (error ~2^-20 relative).
-//   B_lo panels are produced where B is produced (gather kernel / forward epilogue).  For bn <= 128 the
-//   B_full and B_lo tiles, adjacent in smem, are fed as ONE N = 2*bn operand: D[:, 0:bn] += A_hi*B_full
-//   (+ A_lo*B_full by a second MMA), D[:, bn:2bn] += A_hi*B_lo, and the epilogue adds the two halves
-//   -> 2 MMAs per K-step instead of 3.
-// TMEM columns: [0, acc_cols) accumulators, then nring x (32 cols A_hi | 32 cols A_lo).
+//   B_lo panels are produced where B is produced (gather kernel / forward epilogue).  The B_full and B_lo tiles,
+//   adjacent in smem, are fed as ONE N = 2*bn operand (bn <= 128 days per CTA; wider minibatches are split into two
+//   day groups, blockIdx.x & 1): D[:, 0:bn] += A_hi*B_full (the MAIN sum), D[:, bn:2bn] += A_hi*B_lo, and a second MMA
+//   adds A_lo*B_full into the same CORRECTION half -> 2 MMAs per K-step; the epilogue adds the two halves.
+// Accumulation accuracy (measured): tcgen05 adds into its FP32 accumulator with round-toward-zero, so
+//   every accumulating instruction loses ~half an ulp of the running sum, always in the same direction: a relative bias
+//   of about -n * 2^-24 after n instructions on same-signed data (-1.5e-5 at K = 2048, -2e-4 at K = 13312 with every
+//   MMA landing in one accumulator).  Two measures bound it independently of K: (1) the small correction products never
+//   touch the main accumulator (above), (2) every kFlushChunks K chunks the accumulators are DRAINED by the splitter
+//   threads into fp32 registers (round-to-nearest adds) and restarted, so that no accumulator ever takes more than
+//   4 * kFlushChunks additions (bias <= ~4e-6 relative, whatever K).
+// TMEM columns: [0, 2*bn) accumulators, then nring x (32 cols A_hi | 32 cols A_lo).
 //
 // Warp roles (320 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 and 6-9 = two
 // groups of splitters that take alternate K chunks, then the epilogue (TMEM -> registers -> global, fused
@@ -40,6 +47,7 @@ constexpr int kThreadsTC = 320;
 constexpr int kTileM = 128;
 constexpr int kTileK = 32;                       // 32 fp32 = 128 B = one SWIZZLE_128B span
 constexpr int kABytes = kTileM * kTileK * 4;     // 16 KB
+constexpr int kFlushChunks = 16;                 // K chunks between two drains of the TMEM accumulators (see above)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -52,8 +60,17 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+#ifdef DODE_BRINGUP
+// bring-up only (never in the default build): a wait that gives up after ~1e7 polls, records who waited for what, and
+// raises a flag that makes every other wait give up too, so that a deadlocked kernel ends and the record can be read
+__device__ int g_wait_abort = 0;
+__device__ int g_wait_rec[64];
+#endif
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0, int aux = 0) {
     uint32_t done;
+#ifdef DODE_BRINGUP
+    long spins = 0;
+#endif
     do {
         asm volatile(
             "{\n"
@@ -61,6 +78,26 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
             "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
             "selp.b32 %0, 1, 0, p;\n"
             "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+#ifdef DODE_BRINGUP
+        if (!done && ((++spins & 0xffff) == 0)) {
+            const bool aborted = *(volatile int*)&g_wait_abort != 0;
+            if (aborted || spins > (1L << 24)) {
+                if (!aborted && atomicAdd(&g_wait_abort, 1) == 0) {          // first to give up names the block to report
+                    g_wait_rec[60] = blockIdx.x; g_wait_rec[61] = blockIdx.y; g_wait_rec[62] = blockIdx.z;
+                    __threadfence();
+                }
+                __threadfence();
+                if ((threadIdx.x & 31) == 0 && (int)blockIdx.x == *(volatile int*)&g_wait_rec[60] &&
+                    (int)blockIdx.y == *(volatile int*)&g_wait_rec[61] && (int)blockIdx.z == *(volatile int*)&g_wait_rec[62]) {
+                    const int k = atomicAdd(&g_wait_rec[59], 1);
+                    if (k < 14) { int* r = g_wait_rec + 4 * k; r[0] = tag; r[1] = aux; r[2] = threadIdx.x >> 5; r[3] = (int)parity; }
+                }
+                return;
+            }
+        }
+#else
+        (void)tag; (void)aux;
+#endif
     } while (!done);
 }
 
@@ -115,7 +152,9 @@ struct TcParams {
     int kunit;           // K rows per lag (Np forward, Lp gradient)
     int slab0;           // c*T: first (cluster, time) slab of the A tensor map
     int Lp, Np;
-    int bn;              // MMA N (days rounded up to 16)
+    int bn;              // days per CTA (MMA N of the main product), a multiple of 16, <= 128
+    int dsplit;          // day groups per output tile (1, or 2 for minibatches wider than 128 days): blockIdx.x % dsplit
+    int bnt;             // dsplit * bn: padded minibatch width (row stride of the split-K partial sums)
     int stages;
     int nring;           // TMEM A buffers (2 or 4), half per splitter group
     // epilogue
@@ -188,8 +227,10 @@ __device__ __forceinline__ void tmem_ld16x2_wait(uint32_t t0, uint32_t t1, uint3
 
 // ADA = true compiles in the NEXT-1 epilogues (row mask on r, Adagrad accumulator).  It is a template parameter, not a
 // run-time branch, because the extra live values cost 25 registers: 117 x 320 threads no longer fits two CTAs per SM.
-template <bool ADA>
-__global__ void __launch_bounds__(kThreadsTC, 2)
+// PART = fp32 partial sums a splitter thread carries across drains = its share of the bn day columns (bn <= 2 * PART):
+// 16 / 32 for the two-CTAs-per-SM shapes (bn <= 32 / 64), 64 for bn <= 128 (one CTA per SM).
+template <bool ADA, int PART>
+__global__ void __launch_bounds__(kThreadsTC, PART <= 32 ? 2 : 1)
 banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA64,
                    const __grid_constant__ CUtensorMap mapBf, const __grid_constant__ CUtensorMap mapBl,
                    const __grid_constant__ TcParams p, const __grid_constant__ DayList dl) {
@@ -197,7 +238,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
-    const int m0 = blockIdx.x * kTileM;
+    const int m0 = ((int)blockIdx.x / p.dsplit) * kTileM;
+    const int d0 = ((int)blockIdx.x % p.dsplit) * p.bn;       // first day (position in the list) of this CTA's group
     const int bBytes = p.bn * kTileK * 4;
     const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full | B_lo
     const int nring = p.nring;
@@ -212,8 +254,9 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     uint64_t* empty = bars + p.stages;            // [stages] MMAs of the stage retired
     uint64_t* split = bars + 2 * p.stages;        // [nring] A_hi/A_lo in TMEM
     uint64_t* a_empty = split + 4;                // [nring] MMAs that read this TMEM buffer retired
-    uint64_t* accum = a_empty + 4;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
+    uint64_t* accum = a_empty + 4;                // all MMAs issued so far retired (every drain and the end)
+    uint64_t* drained = accum + 1;                // the splitter threads have read the accumulators of a drain
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(drained + 1);
 
     const int lags = (p.mode == 0 ? min(p.H, tt) : min(p.H, p.T - 1 - tt)) + 1;
     const int nk_all = (lags * p.kunit + kTileK - 1) / kTileK;
@@ -222,15 +265,16 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int nk = max(0, min(nk_all, kbase + cps) - kbase);
     const int w0 = (p.mode == 0 ? (tt - lags + 1) * p.kunit : tt * p.kunit) + kbase * kTileK;   // first element of the B window
 
-    const bool fused_n = p.bn <= 128;
-    const int acc_cols = fused_n ? 2 * p.bn : p.bn;
+    const int acc_cols = 2 * p.bn;
     uint32_t tmem_cols = 32;
     while ((int)tmem_cols < acc_cols + 64 * nring) tmem_cols <<= 1;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        // empty[s]: the MMAs of the stage retired (1 commit) AND every splitter warp has seen the stage land (8 arrivals)
+        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1 + 8); }
         for (int j = 0; j < nring; ++j) { mbar_init(&split[j], 128); mbar_init(&a_empty[j], 1); }
         mbar_init(accum, 1);
+        mbar_init(drained, 256);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(mA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapBf) : "memory");
@@ -280,7 +324,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     auto prefetch = [&](int c0) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-            const int d = min(c0 + j, dl.n - 1);
+            const int d = min(d0 + c0 + j, dl.n - 1);
             pre[j] = __ldcg(ebase + (size_t)dl.day[d] * estride);    // through L2: q may have been written under PDL
         }
     };
@@ -289,7 +333,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         keep = 0;
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-            const int d = c0 + j;
+            const int d = d0 + c0 + j;
             if (em < p.M && d < dl.n && __ldg(p.mask + ((size_t)d * p.T + tt) * p.M + em) != 0) keep |= 1u << j;
         }
     };
@@ -305,15 +349,15 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         // ===== TMA producer =====
         int s = 0, ph = 1;                                       // ph: parity of the previous round of slot s
         for (int kc = 0; kc < nk; ++kc) {
-            if (kc >= p.stages) mbar_wait(&empty[s], ph);
+            if (kc >= p.stages) mbar_wait(&empty[s], ph, 1, kc);
             if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
                 if (kc >= npre) {                               // (the first round's A tiles were requested before the wait)
                     mbar_expect_tx(&full[s], txBytes);
                     tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
                 }
-                tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, 0);
-                tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, 0);
+                tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, d0);
+                tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, d0);
             }
             __syncwarp();
             if (++s == p.stages) { s = 0; ph ^= 1; }
@@ -325,24 +369,24 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         for (int kc = 0; kc < nk; ++kc) {
             const int g = kc & 1, use = kc >> 1;
             const int jr = g * per_group + use % per_group;
-            mbar_wait(&full[s], ph);
-            mbar_wait(&split[jr], (use / per_group) & 1);
+            const bool restart = kc % kFlushChunks == 0;        // first chunk of a segment: the accumulators start over
+            if (restart && kc > 0) {                            // drain: the splitter threads read the sums so far
+                if (elect_one()) umma_commit(accum);
+                __syncwarp();
+                mbar_wait(drained, (kc / kFlushChunks - 1) & 1, 2, kc);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            }
+            mbar_wait(&full[s], ph, 3, kc);
+            mbar_wait(&split[jr], (use / per_group) & 1, 4, kc);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes, bl0 = bf0 + bBytes;
+            const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes;
             const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
             if (elect_one()) {
 #pragma unroll
                 for (int k = 0; k < kTileK / 8; ++k) {           // UMMA_K = 8 for tf32: 32 bytes along the swizzle span
                     const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
-                    if (fused_n) {
-                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, (kc | k) != 0);       // [a_hi*b_full | a_hi*b_lo]
-                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);                   //  a_lo*b_full
-                    } else {
-                        const uint64_t dbl = umma_desc_k_sw128(bl0 + k * 32);
-                        umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc1, (kc | k) != 0);
-                        umma_tf32_ts(tmem_d, alo + k * 8, dbf, idesc1, 1);
-                        umma_tf32_ts(tmem_d, ahi + k * 8, dbl, idesc1, 1);
-                    }
+                    umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, !(restart && k == 0));   // [a_hi*b_full | a_hi*b_lo]
+                    umma_tf32_ts(tmem_d + (uint32_t)p.bn, alo + k * 8, dbf, idesc1, 1);     // correction half += a_lo*b_full
                 }
                 umma_commit(&empty[s]);
                 umma_commit(&a_empty[jr]);
@@ -357,40 +401,74 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         const int group = (warp - 2) >> 2;
         const int lane_base = (warp & 3) * 32;                  // TMEM lanes this warp may touch
         const int row = lane_base + lane;                       // output row within the tile == TMEM lane
+        const uint32_t tacc = tmem_d + ((uint32_t)lane_base << 16);
+        // partial sums of this thread's day columns (chunks c0 = 16*group + 32*i), filled by the drains
+        float part[PART];
+#pragma unroll
+        for (int j = 0; j < PART; ++j) part[j] = 0.f;
         int s = -1, ph = 1;
         for (int kc = 0; kc < nk; ++kc) {
+            if (kc > 0 && kc % kFlushChunks == 0) {
+                // ---- drain (both groups, every thread its own columns): main + correction halves into registers ----
+                mbar_wait(accum, (kc / kFlushChunks - 1) & 1, 5, kc);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < PART / 16; ++i) {
+                    const int c0 = 16 * group + 32 * i;
+                    if (c0 < p.bn) {                            // warp-uniform
+                        uint32_t v[16], w[16];
+                        tmem_ld16x2_wait(tacc + (uint32_t)c0, tacc + (uint32_t)(c0 + p.bn), v, w);
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) part[i * 16 + j] += __uint_as_float(v[j]) + __uint_as_float(w[j]);
+                    }
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                mbar_arrive(drained);
+            }
             if (++s == p.stages) s = 0;
             if (s == 0) ph ^= 1;
             const int use = kc >> 1;
             const int jr = group * per_group + use % per_group;
-            // every group observes EVERY phase of every full barrier (also for the other group's chunks): a parity
-            // wait is only sound for a waiter that never falls a whole phase behind or skips one
-            mbar_wait(&full[s], ph);
+            // Every splitter warp observes EVERY phase of every full barrier (also for the other group's chunks) and
+            // acknowledges it on empty[s]: a parity wait is only sound for a waiter that never falls a whole phase
+            // behind, and the stage is not refilled before all eight warps have seen it.  (Without the acknowledgement a
+            // warp that is slow to start can still be waiting for chunk 0 when chunk `stages` lands in the same slot —
+            // refilling needs only the OTHER group's MMAs — and then waits for ever: seen once in ~300 steps on the
+            // multiyear shape.)
+            mbar_wait(&full[s], ph, 6, kc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
             if ((kc & 1) != group) continue;
-            if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1);
+            if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1, 7, kc);
             if (lane_base >= BM) { mbar_arrive(&split[jr]); continue; }    // rows never stored
             const float* A = reinterpret_cast<const float*>(smem + (size_t)s * stageBytes) + row;
-            uint32_t hi[32], lo[32];
-#pragma unroll
-            for (int k = 0; k < 32; ++k) hi[k] = __float_as_uint(A[k * BM]);
-#pragma unroll
-            for (int i = 0; i < 32; ++i)
-                lo[i] = __float_as_uint(__uint_as_float(hi[i]) - __uint_as_float(hi[i] & 0xffffe000u));
             const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);
-            __syncwarp();                                       // tcgen05.st is .sync.aligned
-            tmem_st16(t0, hi); tmem_st16(t0 + 16, hi + 16);
-            tmem_st16(t0 + 32, lo); tmem_st16(t0 + 48, lo + 16);
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {                    // two halves of the 32 K rows: 32 live registers, not 64
+                uint32_t hi[16], lo[16];
+#pragma unroll
+                for (int k = 0; k < 16; ++k) hi[k] = __float_as_uint(A[(hf * 16 + k) * BM]);
+#pragma unroll
+                for (int i = 0; i < 16; ++i)
+                    lo[i] = __float_as_uint(__uint_as_float(hi[i]) - __uint_as_float(hi[i] & 0xffffe000u));
+                __syncwarp();                                   // tcgen05.st is .sync.aligned
+                tmem_st16(t0 + hf * 16, hi);
+                tmem_st16(t0 + 32 + hf * 16, lo);
+            }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             mbar_arrive(&split[jr]);
         }
         // ---- epilogue ----
-        mbar_wait(accum, 0);
+        mbar_wait(accum, (nk > 0 ? (nk - 1) / kFlushChunks : 0) & 1, 8, nk);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int m = m0 + row;
-        for (int c0 = 16 * group; c0 < p.bn; c0 += 32) {
+#pragma unroll
+        for (int i = 0; i < PART / 16; ++i) {
+            const int c0 = 16 * group + 32 * i;
+            if (c0 >= p.bn) break;
             uint32_t v[16], w[16];
-            const uint32_t taddr = tmem_d + ((uint32_t)lane_base << 16) + (uint32_t)c0;
             float cur[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j) cur[j] = pre[j];
@@ -400,30 +478,26 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 if (ADA && p.mode == 0 && p.mask != nullptr) prefetch_mask(c0 + 32);
             }
             __syncwarp();                                       // tcgen05.ld / wait::ld are .sync.aligned
-            if (fused_n) tmem_ld16x2_wait(taddr, taddr + p.bn, v, w);
-            else tmem_ld16_wait(taddr, v);
+            tmem_ld16x2_wait(tacc + (uint32_t)c0, tacc + (uint32_t)(c0 + p.bn), v, w);
+            float sum[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+                sum[j] = nk ? part[i * 16 + j] + (__uint_as_float(v[j]) + __uint_as_float(w[j])) : 0.f;
             if (!fused_epi) {                                   // split-K: raw partial sums, 16 consecutive days per thread
                 if (m < p.M) {
                     float4* dst = reinterpret_cast<float4*>(
-                        p.part + (((size_t)blockIdx.z * gridDim.y + tt) * ((size_t)gridDim.x * kTileM) + m) * p.bn + c0);
+                        p.part + (((size_t)blockIdx.z * gridDim.y + tt) * ((size_t)(gridDim.x / p.dsplit) * kTileM) + m) * p.bnt + d0 + c0);
 #pragma unroll
-                    for (int j = 0; j < 16; j += 4) {
-                        float4 o;
-                        o.x = nk ? __uint_as_float(v[j]) + (fused_n ? __uint_as_float(w[j]) : 0.f) : 0.f;
-                        o.y = nk ? __uint_as_float(v[j + 1]) + (fused_n ? __uint_as_float(w[j + 1]) : 0.f) : 0.f;
-                        o.z = nk ? __uint_as_float(v[j + 2]) + (fused_n ? __uint_as_float(w[j + 2]) : 0.f) : 0.f;
-                        o.w = nk ? __uint_as_float(v[j + 3]) + (fused_n ? __uint_as_float(w[j + 3]) : 0.f) : 0.f;
-                        dst[j >> 2] = o;
-                    }
+                    for (int j = 0; j < 16; j += 4) dst[j >> 2] = make_float4(sum[j], sum[j + 1], sum[j + 2], sum[j + 3]);
                 }
                 continue;
             }
             if (m < p.M) {
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
-                    const int d = c0 + j;
+                    const int d = d0 + c0 + j;
                     if (d < dl.n) {
-                        const float acc = __uint_as_float(v[j]) + (fused_n ? __uint_as_float(w[j]) : 0.f);
+                        const float acc = sum[j];
                         if (p.mode == 0) {
                             const float r = (!ADA || ((curkeep >> j) & 1u)) ? acc - cur[j] : 0.f;
                             const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
@@ -454,14 +528,14 @@ template <bool ADA>
 __global__ void __launch_bounds__(256)
 splitk_epilogue(const __grid_constant__ TcParams p, int Mt, const __grid_constant__ DayList dl) {
     const int tt = blockIdx.y;
-    const int q4 = p.bn >> 2;
+    const int q4 = p.bnt >> 2;
     const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (i >= (long)Mt * q4) return;
     const int m = (int)(i / q4), d0 = (int)(i - (long)m * q4) * 4;
     if (m >= p.M) return;
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
     for (int ks = 0; ks < p.ksplit; ++ks) {
-        const float4 v = __ldcg(reinterpret_cast<const float4*>(p.part + (((size_t)ks * p.T + tt) * Mt + m) * p.bn + d0));
+        const float4 v = __ldcg(reinterpret_cast<const float4*>(p.part + (((size_t)ks * p.T + tt) * Mt + m) * p.bnt + d0));
         acc[0] += v.x; acc[1] += v.y; acc[2] += v.z; acc[3] += v.w;
     }
 #pragma unroll

@@ -104,3 +104,79 @@ def test_assignment_build_multipath_logit_matches_oracle(shape, theta):
     P.dode_assignment_build(N, L, T, H, ident.cuda(), ptr.cuda(), links.cuda(), length1.cuda(), v, DT, theta, Ra)
     P.dode_dar_build(N, L, T, H, ptr.cuda(), links.cuda(), length1.cuda(), v, DT, Rb)
     np.testing.assert_allclose(Ra.cpu().numpy(), Rb.cpu().numpy(), rtol=0, atol=1e-7)
+
+
+def _csr_equal(got, want_dense, atol):
+    """got: CSR namespace from dode_assignment_build_csr (one cluster); want_dense: [T][H+1][L][N] numpy."""
+    want = synth.dense_to_csr(torch.from_numpy(want_dense[None]))
+    np.testing.assert_array_equal(got.blk_off.cpu().numpy(), want.blk_off.numpy())
+    np.testing.assert_array_equal(got.row_ptr.cpu().numpy(), want.row_ptr.numpy())
+    np.testing.assert_array_equal(got.col_idx.cpu().numpy(), want.col_idx.numpy())      # identical support, ascending columns
+    np.testing.assert_allclose(got.val.cpu().numpy(), want.val.numpy(), rtol=0, atol=atol)
+
+
+@pytest.mark.parametrize("shape,paths,theta", [((61, 37, 50, 5), 1, 0.0), ((61, 37, 50, 5), 3, 0.01), ((60, 120, 96, 12), 3, 0.002),
+                                               ((7, 5, 3, 0), 1, 0.0), ((300, 90, 24, 30), 2, 0.01)])
+def test_assignment_build_csr_matches_oracle(shape, paths, theta):
+    """CSR output: the oracle's dense O7 / O8 operator converted to the boundary CSR format must
+    equal the kernel's arrays — offsets, row pointers and column indices exactly, values to 2e-6 (merged multi-path shares
+    are summed in another order).  An operator built this way feeds dode_create(csr=...) directly."""
+    from oracle import oracle
+    N, L, T, H = shape
+    cfg = synth.Config("asg_csr", N=N, L=L, T=T, H=H, C=1, D=6, b=3, K=6, kmin=2, kmax=min(12, L), label_mode="zero")
+    v = synth.speeds(cfg, 0)
+    if paths == 1:
+        ptr, links, length = synth.network(cfg)
+        want = oracle.dar_build(N, L, T, H, ptr.numpy(), links.numpy(), length.numpy(), v.numpy(), DT)
+        got = P.dode_assignment_build_csr(N, L, T, H, None, ptr.cuda(), links.cuda(), length.cuda(), v.cuda(), DT)
+    else:
+        od, ptr, links, length = synth.network_multipath(cfg, paths)
+        want = oracle.assignment_build(N, L, T, H, od.numpy(), ptr.numpy(), links.numpy(), length.numpy(), v.numpy(), DT, theta)
+        got = P.dode_assignment_build_csr(N, L, T, H, od.cuda(), ptr.cuda(), links.cuda(), length.cuda(), v.cuda(), DT, theta)
+    assert got.nnz == int((want != 0).sum())
+    _csr_equal(got, want, 2e-6)
+    # Step 1 -> Step 5 without ever forming the dense slab on the GPU
+    lab = synth.labels(cfg)
+    Ro = torch.from_numpy(want[None])
+    x = synth.counts(cfg, Ro, synth.q_true(cfg), lab)
+    p = hz.Problem(cfg, Ro, lab.numpy(), x, synth.q_true(cfg))
+    sched = synth.schedule(cfg, p.labels)
+    etas = hz.oracle_etas(p)
+    h = P.dode_create(N, L, T, H, 1, cfg.D, p.labels, x.cuda(), 1.0, csr=got)
+    for c, days in sched:
+        P.dode_spgd_step(h, days, float(etas[c]))
+    out = torch.empty((cfg.D, T, N))
+    for d in range(cfg.D):
+        P.dode_get_q(h, d, out[d])
+    hz.assert_q_close(out.numpy(), hz.oracle_run(p, sched, etas), "csr-built operator")
+    P.dode_destroy(h)
+
+
+def test_per_day_operators_undo_reading_d3():
+    """the paper builds the DAR matrix PER DAY from that day's speeds; north_star
+    shares one operator per cluster.  The per-day flow is the same library with C = D: one operator per day built from
+    its own speed table, every day its own cluster, minibatches of one day — iterates equal the oracle's."""
+    from oracle import oracle
+    cfg = synth.Config("per_day", N=30, L=24, T=36, H=6, C=10, D=10, b=1, K=40, kmin=3, kmax=8)
+    ptr, links, length = synth.network(cfg)
+    Rg = torch.empty((cfg.D, cfg.T, cfg.H + 1, cfg.L, cfg.N), device="cuda")
+    Ro = np.empty((cfg.D, cfg.T, cfg.H + 1, cfg.L, cfg.N), np.float32)
+    for d in range(cfg.D):
+        v = synth.speeds(cfg, d)                                   # a speed table of its own for every day
+        P.dode_dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr.cuda(), links.cuda(), length.cuda(), v.cuda(), DT, Rg[d])
+        Ro[d] = oracle.dar_build(cfg.N, cfg.L, cfg.T, cfg.H, ptr.numpy(), links.numpy(), length.numpy(), v.numpy(), DT)
+    assert np.abs(Ro[0] - Ro[1]).max() > 1e-3                      # the days' operators do differ
+    lab = torch.arange(cfg.D, dtype=torch.int32)
+    x = synth.counts(cfg, torch.from_numpy(Ro), synth.q_true(cfg), lab)
+    p = hz.Problem(cfg, torch.from_numpy(Ro), lab.numpy(), x, synth.q_true(cfg))
+    sched = synth.schedule(cfg, p.labels)
+    assert all(len(days) == 1 for _, days in sched)
+    etas = hz.oracle_etas(p)
+    h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.D, cfg.D, p.labels, x.cuda(), 1.0, dense=Rg)
+    for c, days in sched:
+        P.dode_spgd_step(h, days, float(etas[c]))
+    out = torch.empty((cfg.D, cfg.T, cfg.N))
+    for d in range(cfg.D):
+        P.dode_get_q(h, d, out[d])
+    hz.assert_q_close(out.numpy(), hz.oracle_run(p, sched, etas), "per-day operators")
+    P.dode_destroy(h)
