@@ -396,7 +396,7 @@ static TcGeom tc_geometry(const dode_ctx* ctx, int bn, int dsplit) {
     // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  Two CTAs per SM when 3 stages fit in half the
     // shared memory and 256 TMEM columns suffice.
     const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
-    const int fixed = 1024 + 256;
+    const int fixed = 1024 + 512;                  // alignment slack + barriers (3*stages + 10 of them) + the TMEM slot
     const int acc_cols = 2 * bn;
     int stages = (112 * 1024 - fixed) / stageBytes;
     int nring = 2;

@@ -250,9 +250,14 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int aBytes = BM * kTileK * 4;
     const CUtensorMap* mA = half ? &mapA64 : &mapA;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stageBytes);
-    uint64_t* full = bars;                        // [stages] TMA landed
-    uint64_t* empty = bars + p.stages;            // [stages] MMAs of the stage retired
-    uint64_t* split = bars + 2 * p.stages;        // [nring] A_hi/A_lo in TMEM
+    // full: TMA landed.  One barrier per (splitter group, stage): chunk kc completes full[(kc & 1) * stages + kc % stages],
+    // so every waiter of a barrier (that group's splitters and the MMA warp) sees EVERY one of its phases in turn.  With
+    // one barrier per stage a group would have to watch the other group's chunks go by just to keep count, and a warp
+    // that is slow to start could fall two phases behind (a stage is refilled as soon as the OTHER group's MMAs retire)
+    // and wait for ever — seen once in ~300 steps on the multiyear shape.
+    uint64_t* full = bars;                        // [2][stages]
+    uint64_t* empty = bars + 2 * p.stages;        // [stages] MMAs of the stage retired
+    uint64_t* split = bars + 3 * p.stages;        // [nring] A_hi/A_lo in TMEM
     uint64_t* a_empty = split + 4;                // [nring] MMAs that read this TMEM buffer retired
     uint64_t* accum = a_empty + 4;                // all MMAs issued so far retired (every drain and the end)
     uint64_t* drained = accum + 1;                // the splitter threads have read the accumulators of a drain
@@ -270,8 +275,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     while ((int)tmem_cols < acc_cols + 64 * nring) tmem_cols <<= 1;
 
     if (threadIdx.x == 0) {
-        // empty[s]: the MMAs of the stage retired (1 commit) AND every splitter warp has seen the stage land (8 arrivals)
-        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1 + 8); }
+        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&full[p.stages + s], 1); mbar_init(&empty[s], 1); }
         for (int j = 0; j < nring; ++j) { mbar_init(&split[j], 128); mbar_init(&a_empty[j], 1); }
         mbar_init(accum, 1);
         mbar_init(drained, 256);
@@ -302,9 +306,10 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int txBytes = aBytes + 2 * bBytes;
     if (warp == 0) {
         if (elect_one()) {
-            for (int kc = 0; kc < npre; ++kc) {
-                mbar_expect_tx(&full[kc], txBytes);
-                tma_load_3d(smem + (size_t)kc * stageBytes, mA, &full[kc], m0, (kbase + kc) * kTileK, p.slab0 + tt);
+            for (int kc = 0; kc < npre; ++kc) {                  // (kc < stages: the stage index is kc)
+                uint64_t* fb = &full[(kc & 1) * p.stages + kc];
+                mbar_expect_tx(fb, txBytes);
+                tma_load_3d(smem + (size_t)kc * stageBytes, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
             }
         }
         __syncwarp();
@@ -352,12 +357,13 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (kc >= p.stages) mbar_wait(&empty[s], ph, 1, kc);
             if (elect_one()) {
                 uint8_t* st = smem + (size_t)s * stageBytes;
+                uint64_t* fb = &full[(kc & 1) * p.stages + s];
                 if (kc >= npre) {                               // (the first round's A tiles were requested before the wait)
-                    mbar_expect_tx(&full[s], txBytes);
-                    tma_load_3d(st, mA, &full[s], m0, (kbase + kc) * kTileK, p.slab0 + tt);
+                    mbar_expect_tx(fb, txBytes);
+                    tma_load_3d(st, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
                 }
-                tma_load_2d(st + kABytes, &mapBf, &full[s], w0 + kc * kTileK, d0);
-                tma_load_2d(st + kABytes + bBytes, &mapBl, &full[s], w0 + kc * kTileK, d0);
+                tma_load_2d(st + kABytes, &mapBf, fb, w0 + kc * kTileK, d0);
+                tma_load_2d(st + kABytes + bBytes, &mapBl, fb, w0 + kc * kTileK, d0);
             }
             __syncwarp();
             if (++s == p.stages) { s = 0; ph ^= 1; }
@@ -365,7 +371,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp walks the loop, one elected lane issues =====
         const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc2 = umma_idesc_tf32(2 * p.bn);
-        int s = 0, ph = 0;
+        int s = 0;
+        uint32_t fph[2] = {0u, 0u};                             // parity of the next phase of full[g][s], bit s
         for (int kc = 0; kc < nk; ++kc) {
             const int g = kc & 1, use = kc >> 1;
             const int jr = g * per_group + use % per_group;
@@ -376,7 +383,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 mbar_wait(drained, (kc / kFlushChunks - 1) & 1, 2, kc);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             }
-            mbar_wait(&full[s], ph, 3, kc);
+            mbar_wait(&full[g * p.stages + s], (fph[g] >> s) & 1u, 3, kc);
+            fph[g] ^= 1u << s;
             mbar_wait(&split[jr], (use / per_group) & 1, 4, kc);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes;
@@ -392,7 +400,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 umma_commit(&a_empty[jr]);
             }
             __syncwarp();
-            if (++s == p.stages) { s = 0; ph ^= 1; }
+            if (++s == p.stages) s = 0;
         }
         if (elect_one()) { if (nk == 0) mbar_arrive(accum); else umma_commit(accum); }
         __syncwarp();
@@ -406,7 +414,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         float part[PART];
 #pragma unroll
         for (int j = 0; j < PART; ++j) part[j] = 0.f;
-        int s = -1, ph = 1;
+        int s = -1;
+        uint32_t fph = 0u;                                      // parity of the next phase of this group's full[s], bit s
         for (int kc = 0; kc < nk; ++kc) {
             if (kc > 0 && kc % kFlushChunks == 0) {
                 // ---- drain (both groups, every thread its own columns): main + correction halves into registers ----
@@ -427,26 +436,18 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 mbar_arrive(drained);
             }
             if (++s == p.stages) s = 0;
-            if (s == 0) ph ^= 1;
+            if ((kc & 1) != group) continue;
             const int use = kc >> 1;
             const int jr = group * per_group + use % per_group;
-            // Every splitter warp observes EVERY phase of every full barrier (also for the other group's chunks) and
-            // acknowledges it on empty[s]: a parity wait is only sound for a waiter that never falls a whole phase
-            // behind, and the stage is not refilled before all eight warps have seen it.  (Without the acknowledgement a
-            // warp that is slow to start can still be waiting for chunk 0 when chunk `stages` lands in the same slot —
-            // refilling needs only the OTHER group's MMAs — and then waits for ever: seen once in ~300 steps on the
-            // multiyear shape.)
-            mbar_wait(&full[s], ph, 6, kc);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
-            if ((kc & 1) != group) continue;
+            mbar_wait(&full[group * p.stages + s], (fph >> s) & 1u, 6, kc);
+            fph ^= 1u << s;
             if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1, 7, kc);
             if (lane_base >= BM) { mbar_arrive(&split[jr]); continue; }    // rows never stored
             const float* A = reinterpret_cast<const float*>(smem + (size_t)s * stageBytes) + row;
             const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {                    // two halves of the 32 K rows: 32 live registers, not 64
-                uint32_t hi[16], lo[16];
+                uint32_t hi[16], lo[16];                        // (one 32-wide pass spills beside the partial sums: measured slower)
 #pragma unroll
                 for (int k = 0; k < 16; ++k) hi[k] = __float_as_uint(A[(hf * 16 + k) * BM]);
 #pragma unroll
