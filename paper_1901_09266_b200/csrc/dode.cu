@@ -656,8 +656,6 @@ int dode_create(dode_ctx** out, const dode_dims* dims, const dode_dar* R, const 
     if (d.storage != DODE_DENSE && d.storage != DODE_CSR) return fail(ctx, DODE_EINVAL, "unknown storage %d", d.storage);
     if (d.T > 65535) return fail(ctx, DODE_EINVAL, "T=%d exceeds 65535 (the time index rides on grid.y)", d.T);
     if (d.storage == DODE_DENSE && !R->dense) return fail(ctx, DODE_EINVAL, "R->dense is null");
-    if (d.storage == DODE_CSR && (d.L >= (1 << kPayLinkBits) || d.H + kRB >= (1 << (31 - kPayLinkBits))))
-        return fail(ctx, DODE_EINVAL, "CSR storage supports L < 2^20 and H < 2^11 - 4 (L=%d H=%d)", d.L, d.H);
     if (d.storage == DODE_CSR && (!R->blk_off || !R->row_ptr || (R->nnz > 0 && (!R->col_idx || !R->val)) || R->nnz < 0))
         return fail(ctx, DODE_EINVAL, "CSR arrays are null or nnz < 0");
     for (int i = 0; i < d.D; ++i)

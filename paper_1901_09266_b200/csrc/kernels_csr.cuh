@@ -11,12 +11,9 @@
 //                 adjacent links AND adjacent arrival intervals share most (s,n): 3.7 products per gathered row
 //                 against 1 for plain CSR and 2.3 for 4 links x 1 interval (the gathers, not the FMAs, bound the pass).
 //   G (gradient): row block (s/4, n) holds one entry per distinct residual row (t,l), t = s+h, reached from any of
-//                 its 4 departure intervals: payload ((t - 4*(s/4)) << 20) | l, values val[4] by s%4, entries sorted
-//                 by (t, l) -> operand r[(t*L + l)*bp + d].  The lag window of a (link, OD) pair spans 2-4 adjacent
+//                 its 4 departure intervals: payload kl = (t - 4*(s/4))*L + l, values val[4] by s%4
+//                 -> operand r[((4*(s/4))*L + kl)*bp + d].  The lag window of a (link, OD) pair spans 2-4 adjacent
 //                 lags, so consecutive departure intervals share most residual rows: ~2x fewer gathers.
-//                 ODs are processed in PATH ORDER (permG: sorted by the first link of their path) in groups of
-//                 kGradWarps; each group knows the link range [lo, lo+span) its paths cover, so that a CTA can stage
-//                 the residual rows r[t][lo..lo+span) of one arrival interval with ONE bulk copy (csr_grad_staged).
 // Entries with s+h >= T are dropped.  The re-pack is a radix sort of 64-bit keys, a head-flag scan
 // and a scatter (CUB, create-time only).
 //
@@ -34,7 +31,6 @@
 
 #include "../../include/dode.h"
 #include "kernels_dense.cuh"
-#include "kernels_tc.cuh"      // mbarrier / elect helpers
 
 namespace dode {
 
@@ -42,8 +38,6 @@ constexpr int kCsrMaxDays = 128;
 constexpr int kRB = 4;            // links (forward) / departure intervals (gradient) per row block
 constexpr int kFT = 2;            // arrival intervals per forward row block
 constexpr int kFS = kRB * kFT;    // output rows (value slots) of a forward entry
-constexpr int kGradWarps = 16;    // ODs (consumer warps) per CTA of csr_grad_staged
-constexpr int kPayLinkBits = 20;  // gradient payload: (t_rel << 20) | l
 
 struct CsrCluster {
     int64_t* rowptrF = nullptr;   // [ceil(T/2)*ceil(L/4) + 1]
@@ -53,8 +47,6 @@ struct CsrCluster {
     int32_t* payG = nullptr;      // [nuG]  (t - 4*(s/4))*L + l
     float4* valG = nullptr;       // [nuG]  by s%4
     int32_t* permG = nullptr;     // [Np]   OD indices ordered by the first link of their path (processing order of a3)
-    int32_t* grpLo = nullptr;     // [ceil(Np/kGradWarps)] first link covered by the ODs permG[g*kGradWarps ...]
-    int span = 0;                 // max over groups of (last link - first link + 1); 0 = no entries
     int64_t nnz = 0;              // valid entries (s+h < T)
     int64_t nuF = 0, nuG = 0;     // distinct (row block, payload) entries
 };
@@ -69,7 +61,6 @@ struct CsrStore {
     float* Mb = nullptr;          // [T*L][bp]  row mask as 0/1 floats
     float* Gb = nullptr;          // [T*Np][bp] Adagrad accumulator panel
     int cap_bp_ada = 0;
-    bool staged_attr[5] = {false, false, false, false, false};   // csr_grad_staged<DV> shared-memory opt-in done
 };
 
 // ---- create-time re-pack ---------------------------------------------------------------------------
@@ -123,7 +114,7 @@ __global__ void csr_scatter_unique(const unsigned long long* __restrict__ keys, 
             if (forward) {
                 pay[u] = (int32_t)rem;                                             // s_rel * Np + n
             } else {
-                pay[u] = (int32_t)(((rem / L) << kPayLinkBits) | (rem % L));      // (t - 4*(s/4), l)
+                pay[u] = (int32_t)rem;
             }
             ukey[u] = kk;
         }
@@ -152,29 +143,10 @@ __global__ void csr_first_link(const int64_t* __restrict__ rowptrG, const int32_
     int best = L;
     for (long sb = 0; sb < SB && best == L; ++sb) {
         const int64_t k0 = rowptrG[sb * Np + n], k1 = rowptrG[sb * Np + n + 1];
-        for (int64_t k = k0; k < k1; ++k) best = min(best, payG[k] & ((1 << kPayLinkBits) - 1));
+        for (int64_t k = k0; k < k1; ++k) best = min(best, payG[k] % L);
     }
     first[n] = best;
     ident[n] = n;
-}
-
-// lowest / highest link of every OD's entries: one warp per gradient row block
-__global__ void csr_od_span(const int64_t* __restrict__ rowptrG, const int32_t* __restrict__ payG, int Np, long rblocks,
-                            int32_t* __restrict__ odmin, int32_t* __restrict__ odmax) {
-    const long w = (blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    if (w >= rblocks) return;
-    const int n = (int)(w % Np);
-    int lo = INT32_MAX, hi = -1;
-    for (int64_t k = rowptrG[w] + lane; k < rowptrG[w + 1]; k += 32) {
-        const int l = payG[k] & ((1 << kPayLinkBits) - 1);
-        lo = min(lo, l); hi = max(hi, l);
-    }
-    for (int o = 16; o; o >>= 1) {
-        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-    }
-    if (lane == 0 && hi >= 0) { atomicMin(odmin + n, lo); atomicMax(odmax + n, hi); }
 }
 
 __global__ void count_invalid(const unsigned long long* __restrict__ keys, int64_t n, unsigned long long* cnt) {
@@ -190,7 +162,6 @@ inline void csr_free(CsrStore& st) {
         for (int c = 0; c < st.C; ++c) {
             cudaFree(st.cl[c].rowptrF); cudaFree(st.cl[c].payF); cudaFree(st.cl[c].valF);
             cudaFree(st.cl[c].rowptrG); cudaFree(st.cl[c].payG); cudaFree(st.cl[c].valG); cudaFree(st.cl[c].permG);
-            cudaFree(st.cl[c].grpLo);
         }
         delete[] st.cl;
         st.cl = nullptr;
@@ -297,35 +268,6 @@ inline int csr_build(CsrStore& st, const dode_dims& d, const dode_dar& R, cudaSt
             cudaFree(t2); cudaFree(sc);
             CSR_CU(e2);
         }
-        // link range of every group of kGradWarps path-adjacent ODs (csr_grad_staged stages r[t][lo..lo+span) per CTA)
-        {
-            int32_t* mm = nullptr;                       // [Np] min | [Np] max
-            CSR_CU(cudaMalloc(&mm, (size_t)2 * Np * 4));
-            CSR_CU(cudaMemsetAsync(mm, 0x7f, (size_t)Np * 4, stream));
-            CSR_CU(cudaMemsetAsync(mm + Np, 0xff, (size_t)Np * 4, stream));
-            const long rbl = SB * Np;
-            csr_od_span<<<(unsigned)((rbl * 32 + 255) / 256), 256, 0, stream>>>(cl.rowptrG, cl.payG, Np, rbl, mm, mm + Np);
-            std::vector<int32_t> hmm((size_t)2 * Np), hperm(Np);
-            cudaError_t e3 = cudaMemcpyAsync(hmm.data(), mm, (size_t)2 * Np * 4, cudaMemcpyDeviceToHost, stream);
-            if (e3 == cudaSuccess) e3 = cudaMemcpyAsync(hperm.data(), cl.permG, (size_t)Np * 4, cudaMemcpyDeviceToHost, stream);
-            if (e3 == cudaSuccess) e3 = cudaStreamSynchronize(stream);
-            cudaFree(mm);
-            CSR_CU(e3);
-            const int groups = (Np + kGradWarps - 1) / kGradWarps;
-            std::vector<int32_t> glo(groups, 0);
-            cl.span = 0;
-            for (int g = 0; g < groups; ++g) {
-                int lo = INT32_MAX, hi = -1;
-                for (int i = g * kGradWarps; i < std::min(Np, (g + 1) * kGradWarps); ++i) {
-                    const int n = hperm[i];
-                    if (hmm[(size_t)Np + n] >= 0) { lo = std::min(lo, hmm[n]); hi = std::max(hi, hmm[(size_t)Np + n]); }
-                }
-                if (hi >= 0) { glo[g] = lo; cl.span = std::max(cl.span, hi - lo + 1); }
-            }
-            CSR_CU(cudaMalloc(&cl.grpLo, (size_t)groups * 4));
-            CSR_CU(cudaMemcpyAsync(cl.grpLo, glo.data(), (size_t)groups * 4, cudaMemcpyHostToDevice, stream));
-            CSR_CU(cudaStreamSynchronize(stream));
-        }
         CSR_CU(cudaStreamSynchronize(stream));
     }
     CSR_CU(cudaGetLastError());
@@ -376,11 +318,6 @@ scatter_days(const float* __restrict__ src, int bp, long rowLen, float* __restri
         const long i = i0 + tx;
         if (d < dl.n && i < rowLen) dst[(size_t)dl.day[d] * dayStride + i] = tile[tx][dd];
     }
-}
-
-// residual row (relative to the row block's first arrival interval) of a gradient payload
-__device__ __forceinline__ long pay_row(int pay, int L) {
-    return (long)(pay >> kPayLinkBits) * L + (pay & ((1 << kPayLinkBits) - 1));
 }
 
 template <int DV> struct DVec;
@@ -532,7 +469,7 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
                     const int oo = __shfl_sync(0xffffffffu, o, j + u);
                     vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
                     vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
-                    rv[u] = *reinterpret_cast<const vec*>(rrow + pay_row(oo, L) * bp);
+                    rv[u] = *reinterpret_cast<const vec*>(rrow + (long)oo * bp);
                 }
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
@@ -551,7 +488,7 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
 #pragma unroll
             for (int e = 0; e < DV; ++e)
                 if (full || lane * DV + e < rbp) {
-                    const float rv = rrow[pay_row(oo, L) * rbp + e];
+                    const float rv = rrow[(long)oo * rbp + e];
 #pragma unroll
                     for (int i = 0; i < kRB; ++i) acc[i][e] = fmaf(v4[i], rv, acc[i][e]);
                 }
@@ -574,120 +511,6 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
         } else if (lane == 0) {
             gout[(size_t)s * N + n] = acc[i][0];
         }
-    }
-}
-
-// a3+a4 (CSR) with the residual rows staged in shared memory.  CTA = one group of kGradWarps path-adjacent ODs (one
-// consumer warp each) x one block of 4 departure intervals + one producer warp.  The entries of a row block are sorted by
-// arrival interval t, and all the residual rows the group can touch at one t are the contiguous run
-// r[t][lo .. lo+span) of the panel, so the producer streams t = 4*sb, 4*sb+1, ... through a ring of stages with ONE bulk
-// copy (cp.async.bulk -> mbarrier) each, and every consumer works through its entries of stage t from shared memory
-// (LDS.128: 4 wavefronts per 512-byte row instead of ~8 cycles through L1, and no LSU request per gathered row at all on
-// the global side).  Every consumer passes through every stage (with or without entries) so that the ring's barriers
-// stay in step.  grid = (groups, ceil(T/4)): consecutive CTAs are neighbouring groups at the same time block, whose
-// rows overlap — the bulk copies hit L2.
-template <int DV>
-__global__ void __launch_bounds__((kGradWarps + 1) * 32)
-csr_grad_staged(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, const float4* __restrict__ val,
-                const int32_t* __restrict__ perm, const int32_t* __restrict__ grp_lo, const float* __restrict__ r,
-                float* __restrict__ Qb, float eta, float* __restrict__ Gb, float eps,
-                int T, int H, int L, int N, int Np, int span, int nst) {
-    constexpr int bp = 32 * DV;
-    using vec = typename DVec<DV>::type;
-    extern __shared__ __align__(128) uint8_t csr_smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int g = blockIdx.x, sb = blockIdx.y;
-    const int lo = grp_lo[g];
-    const int rows = min(span, L - lo);                         // the run must not leave the panel
-    const size_t stageBytes = (size_t)span * bp * sizeof(float);
-    uint64_t* full = reinterpret_cast<uint64_t*>(csr_smem + (size_t)nst * stageBytes);
-    uint64_t* empty = full + nst;
-    const int nq = min(H + kRB, T - sb * kRB);                  // arrival intervals 4*sb .. 4*sb+nq-1 can be referenced
-    if (threadIdx.x == 0) {
-        for (int i = 0; i < nst; ++i) { tc::mbar_init(&full[i], 1); tc::mbar_init(&empty[i], kGradWarps); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (warp == kGradWarps) {
-        // ===== producer =====
-        const uint32_t bytes = (uint32_t)((size_t)rows * bp * sizeof(float));
-        int slot = 0, ph = 1;
-        for (int q = 0; q < nq; ++q) {
-            if (q >= nst) tc::mbar_wait(&empty[slot], ph);
-            if (tc::elect_one()) {
-                tc::mbar_expect_tx(&full[slot], bytes);
-                const float* src = r + ((size_t)(sb * kRB + q) * L + lo) * bp;
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                             ::"r"(tc::smem_u32(csr_smem + (size_t)slot * stageBytes)), "l"(src), "r"(bytes),
-                               "r"(tc::smem_u32(&full[slot])) : "memory");
-            }
-            __syncwarp();
-            if (++slot == nst) { slot = 0; ph ^= 1; }
-        }
-        return;
-    }
-    // ===== consumers: warp = one OD of the group, 4 departure intervals =====
-    const int oi = g * kGradWarps + warp;
-    const int n = oi < Np ? __ldg(perm + oi) : N;
-    const bool valid = n < N;
-    int64_t kb = 0, k1 = 0;
-    if (valid) { kb = rowptr[(long)sb * Np + n]; k1 = rowptr[(long)sb * Np + n + 1]; }
-    float acc[kRB][DV];
-#pragma unroll
-    for (int i = 0; i < kRB; ++i)
-#pragma unroll
-        for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
-    // current chunk of 32 entries: lane j holds entry kb + j
-    int o = 0, cnt = 0, j = 0;
-    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-    auto load_chunk = [&]() {
-        const int64_t k = kb + lane;
-        o = k < k1 ? __ldg(pay + k) : 0;
-        v = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
-        cnt = (int)min((int64_t)32, k1 - kb);
-        j = 0;
-    };
-    if (kb < k1) load_chunk();
-    int slot = 0, ph = 0;
-    for (int q = 0; q < nq; ++q) {
-        tc::mbar_wait(&full[slot], ph);
-        const float* stage = reinterpret_cast<const float*>(csr_smem + (size_t)slot * stageBytes) + lane * DV;
-        while (cnt > 0) {
-            if (j == cnt) {                                     // chunk used up: next one, if any
-                kb += 32;
-                if (kb >= k1) { cnt = 0; break; }
-                load_chunk();
-            }
-            const int oo = __shfl_sync(0xffffffffu, o, j);
-            if ((oo >> kPayLinkBits) != q) break;               // belongs to a later arrival interval
-            const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
-                                   __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
-            const vec rv = *reinterpret_cast<const vec*>(stage + (size_t)((oo & ((1 << kPayLinkBits) - 1)) - lo) * bp);
-            const float* rf = reinterpret_cast<const float*>(&rv);
-#pragma unroll
-            for (int i = 0; i < kRB; ++i)
-#pragma unroll
-                for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(v4[i], rf[e], acc[i][e]);
-            ++j;
-        }
-        __syncwarp();
-        if (lane == 0) tc::mbar_arrive(&empty[slot]);
-        if (++slot == nst) { slot = 0; ph ^= 1; }
-    }
-    if (!valid) return;
-#pragma unroll
-    for (int i = 0; i < kRB; ++i) {
-        const long s = (long)sb * kRB + i;
-        if (s >= T) break;
-        vec* qp = reinterpret_cast<vec*>(Qb + ((size_t)s * Np + n) * bp + lane * DV);
-        vec qv = *qp;
-        float* qf = reinterpret_cast<float*>(&qv);
-#pragma unroll
-        for (int e = 0; e < DV; ++e) {
-            if (Gb != nullptr) qf[e] = adagrad_update(qf[e], acc[i][e], Gb + ((size_t)s * Np + n) * bp + lane * DV + e, eta, eps);
-            else qf[e] = fmaxf(0.f, fmaf(-eta, acc[i][e], qf[e]));
-        }
-        *qp = qv;
     }
 }
 
@@ -764,34 +587,10 @@ inline int csr_gradient(CsrStore& st, int c, const float* r, float* qbase, size_
         Gb = st.Gb;
         *launches += 1;
     }
-    // staged kernel when the ring (>= 2 stages of span rows) fits in half an SM's shared memory; else the gather kernel
-    const size_t stageBytes = (size_t)cl.span * bp * sizeof(float);
-    const int nst = stageBytes ? (int)std::min<size_t>(6, (100 * 1024) / stageBytes) : 0;
-    if (rbp == bp && nst >= 2) {
-        const dim3 sg((Np + kGradWarps - 1) / kGradWarps, (d.T + kRB - 1) / kRB);
-        const size_t smem = (size_t)nst * stageBytes + 2 * nst * sizeof(uint64_t);
-        const int threads = (kGradWarps + 1) * 32;
-#define DODE_STAGED(DVV)                                                                                                   \
-        do {                                                                                                                \
-            if (!st.staged_attr[DVV]) {                                                                                     \
-                cudaFuncSetAttribute(csr_grad_staged<DVV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);        \
-                st.staged_attr[DVV] = true;                                                                                 \
-            }                                                                                                               \
-            csr_grad_staged<DVV><<<sg, threads, smem, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, cl.grpLo, r, st.Qb, \
-                                                                eta, Gb, eps, d.T, d.H, d.L, d.N, Np, cl.span, nst);        \
-        } while (0)
-        switch (bp) {
-            case 32: DODE_STAGED(1); break;
-            case 64: DODE_STAGED(2); break;
-            default: DODE_STAGED(4); break;
-        }
-#undef DODE_STAGED
-    } else {
-        switch (bp) {
-            case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
-            case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
-            default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
-        }
+    switch (bp) {
+        case 32: csr_grad<1, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        case 64: csr_grad<2, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
+        default: csr_grad<4, true><<<grid, 256, 0, stream>>>(cl.rowptrG, cl.payG, cl.valG, cl.permG, r, st.Qb, nullptr, eta, Gb, eps, rblocks, d.T, d.L, d.N, Np, rbp); break;
     }
     scatter_days<<<dim3((unsigned)((rows + 31) / 32), bp / 32), 256, 0, stream>>>(st.Qb, bp, rows, qbase, dayStride, dl);
     if (Gbase) {
