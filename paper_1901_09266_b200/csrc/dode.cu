@@ -14,6 +14,7 @@
 #include "kernels_dense.cuh"
 #include "kernels_csr.cuh"
 #include <cub/device/device_reduce.cuh>
+#include <cuda/std/functional>
 #include "kernels_tc.cuh"
 #include "kernels_dar.cuh"
 #include "kernels_probe.cuh"
@@ -1253,11 +1254,11 @@ int dode_assignment_build_csr(int32_t N, int32_t L, int32_t T, int32_t H, const 
         while (bits < 64 && ((unsigned long long)1 << bits) < (unsigned long long)blocks_sh * L * N) ++bits;
         size_t tb_sort = 0, tb_red = 0;
         cub::DeviceRadixSort::SortPairs(nullptr, tb_sort, k0, k1, v0, v1, nt, 0, bits, st);
-        cub::DeviceReduce::ReduceByKey(nullptr, tb_red, k1, k0, v1, val_out, d_nu, cub::Sum(), nt, st);
+        cub::DeviceReduce::ReduceByKey(nullptr, tb_red, k1, k0, v1, val_out, d_nu, cuda::std::plus<>{}, nt, st);
         BCU(cudaMalloc(&tmp, std::max(tb_sort, tb_red)));
         BCU(cub::DeviceRadixSort::SortPairs(tmp, tb_sort, k0, k1, v0, v1, nt, 0, bits, st));
         // equal keys = several paths of one OD over one link in one lag: their shares add up (Eq. 41 summed over the OD's paths)
-        BCU(cub::DeviceReduce::ReduceByKey(tmp, tb_red, k1, k0, v1, val_out, d_nu, cub::Sum(), nt, st));
+        BCU(cub::DeviceReduce::ReduceByKey(tmp, tb_red, k1, k0, v1, val_out, d_nu, cuda::std::plus<>{}, nt, st));
         BCU(cudaMemcpyAsync(&nu, d_nu, 8, cudaMemcpyDeviceToHost, st));
         BCU(cudaStreamSynchronize(st));
         csr_cols_from_keys<<<1184, 256, 0, st>>>(k0, nu, N, col_idx_out);

@@ -320,10 +320,25 @@ scatter_days(const float* __restrict__ src, int bp, long rowLen, float* __restri
     }
 }
 
+// A lane owns DV consecutive days of a panel row (day = lane*DV + e): one 16-byte vector access per lane and row.  (The
+// other mapping, day = lane + 32*e with one 128-byte line per load instruction, was measured 8 % slower on configs[4].)
 template <int DV> struct DVec;
 template <> struct DVec<1> { using type = float; };
 template <> struct DVec<2> { using type = float2; };
 template <> struct DVec<4> { using type = float4; };
+template <int DV> __device__ __forceinline__ int day_of(int lane, int e) { return lane * DV + e; }
+template <int DV> __device__ __forceinline__ void ld_days(const float* __restrict__ row, int lane, float* v) {
+    const typename DVec<DV>::type t = *reinterpret_cast<const typename DVec<DV>::type*>(row + lane * DV);
+#pragma unroll
+    for (int e = 0; e < DV; ++e) v[e] = reinterpret_cast<const float*>(&t)[e];
+}
+template <int DV> __device__ __forceinline__ void st_days(float* __restrict__ row, int lane, const float* v) {
+    typename DVec<DV>::type t;
+#pragma unroll
+    for (int e = 0; e < DV; ++e) reinterpret_cast<float*>(&t)[e] = v[e];
+    *reinterpret_cast<typename DVec<DV>::type*>(row + lane * DV) = t;
+}
+
 
 // a2 (CSR): one warp per row block (t/2, l/4) of F = 8 output rows; lanes along days (DV days per lane, bp = 32*DV).
 //   r[(t*L+l)*rbp + d] = sum_k val_k[(t%2)*4 + l%4] * Qb[(base + pay_k)*bp + d] - x[day_d][t][l]    for d < rbp,
@@ -337,7 +352,6 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
         const float* __restrict__ Qb, const float* __restrict__ x, const float* __restrict__ Mb, float* __restrict__ r,
         long rblocks, int T, int H, int L, int LB, int Np, int rbp, const __grid_constant__ DayList dl) {
     constexpr int bp = 32 * DV;
-    using vec = typename DVec<DV>::type;
     __shared__ float4 sval[8][64];                   // per warp: 32 entries x 2 float4
     // Warps walk the row blocks LINK-BLOCK-major, time-minor: the warps in flight then cover a few dozen neighbouring
     // link blocks over all t, whose OD sets overlap (paths are link runs), so the panel rows they gather (~100 MB) stay
@@ -350,7 +364,7 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
     const long rb = tb * LB + lb;
     const int l0 = (int)lb * kRB;
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
-    const float* qrow = Qb + ((long)tb * kFT - H) * Np * bp + lane * DV;      // entries only reach rows >= 0
+    const float* qrow = Qb + ((long)tb * kFT - H) * Np * bp;                  // entries only reach rows >= 0
     float acc[kFS][DV];
 #pragma unroll
     for (int i = 0; i < kFS; ++i)
@@ -365,17 +379,17 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
         __syncwarp();
         int j = 0;
         for (; j + 2 <= cnt; j += 2) {
-            vec qv[2];
+            float qv[2][DV];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const int oo = __shfl_sync(0xffffffffu, o, j + u);
-                qv[u] = *reinterpret_cast<const vec*>(qrow + (long)oo * bp);
+                ld_days<DV>(qrow + (long)oo * bp, lane, qv[u]);
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const float4 va = sval[wib][2 * (j + u)], vb = sval[wib][2 * (j + u) + 1];
                 const float vv[kFS] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
-                const float* qf = reinterpret_cast<const float*>(&qv[u]);
+                const float* qf = qv[u];
 #pragma unroll
                 for (int i = 0; i < kFS; ++i)
 #pragma unroll
@@ -384,10 +398,10 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
         }
         if (j < cnt) {
             const int oo = __shfl_sync(0xffffffffu, o, j);
-            const vec qv = *reinterpret_cast<const vec*>(qrow + (long)oo * bp);
+            float qf[DV];
+            ld_days<DV>(qrow + (long)oo * bp, lane, qf);
             const float4 va = sval[wib][2 * j], vb = sval[wib][2 * j + 1];
             const float vv[kFS] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
-            const float* qf = reinterpret_cast<const float*>(&qv);
 #pragma unroll
             for (int i = 0; i < kFS; ++i)
 #pragma unroll
@@ -403,26 +417,22 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
         if (x != nullptr) {
 #pragma unroll
             for (int e = 0; e < DV; ++e) {
-                const int d = lane * DV + e;
+                const int d = day_of<DV>(lane, e);
                 acc[i][e] = d < dl.n ? acc[i][e] - __ldg(x + ((size_t)dl.day[d] * T + t) * L + l) : 0.f;   // pad days: r = 0
             }
         }
         if (Mb != nullptr) {                      // rows outside the chunk B_o contribute no residual
-            const vec mv = *reinterpret_cast<const vec*>(Mb + row * bp + lane * DV);
-            const float* mf = reinterpret_cast<const float*>(&mv);
+            float mf[DV];
+            ld_days<DV>(Mb + row * bp, lane, mf);
 #pragma unroll
             for (int e = 0; e < DV; ++e) acc[i][e] = mf[e] != 0.f ? acc[i][e] : 0.f;
         }
         if (rbp == bp) {
-            vec out;
-            float* of = reinterpret_cast<float*>(&out);
-#pragma unroll
-            for (int e = 0; e < DV; ++e) of[e] = acc[i][e];
-            *reinterpret_cast<vec*>(r + row * bp + lane * DV) = out;
+            st_days<DV>(r + row * bp, lane, acc[i]);
         } else {
 #pragma unroll
             for (int e = 0; e < DV; ++e)
-                if (lane * DV + e < rbp) r[row * rbp + lane * DV + e] = acc[i][e];
+                if (day_of<DV>(lane, e) < rbp) r[row * rbp + day_of<DV>(lane, e)] = acc[i][e];
         }
     }
 }
@@ -435,7 +445,6 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
          const int32_t* __restrict__ perm, const float* __restrict__ r, float* __restrict__ Qb, float* __restrict__ gout, float eta,
          float* __restrict__ Gb, float eps, long rblocks, int T, int L, int N, int Np, int rbp) {
     constexpr int bp = 32 * DV;
-    using vec = typename DVec<DV>::type;
     // Warps walk the row blocks OD-major in path order (perm: ODs sorted by the first link of their path), time-minor:
     // the warps in flight then gather residual rows of a few dozen neighbouring links over all t (~10 MB, L2-resident)
     // instead of the 28-interval window of every link (72 MB, which thrashes a 63 MB L2 partition).
@@ -449,7 +458,7 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
     const long rb = sb * Np + n;
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const bool full = rbp == bp;
-    const float* rrow = r + (size_t)sb * kRB * L * rbp + lane * DV;
+    const float* rrow = r + (size_t)sb * kRB * L * rbp;
     float acc[kRB][DV];
 #pragma unroll
     for (int i = 0; i < kRB; ++i)
@@ -463,17 +472,17 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
         int j = 0;
         if (full) {
             for (; j + 2 <= cnt; j += 2) {
-                vec rv[2]; float vv[2][kRB];
+                float rv[2][DV]; float vv[2][kRB];
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const int oo = __shfl_sync(0xffffffffu, o, j + u);
                     vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
                     vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
-                    rv[u] = *reinterpret_cast<const vec*>(rrow + (long)oo * bp);
+                    ld_days<DV>(rrow + (long)oo * bp, lane, rv[u]);
                 }
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
-                    const float* rf = reinterpret_cast<const float*>(&rv[u]);
+                    const float* rf = rv[u];
 #pragma unroll
                     for (int i = 0; i < kRB; ++i)
 #pragma unroll
@@ -487,8 +496,8 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
                                    __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
 #pragma unroll
             for (int e = 0; e < DV; ++e)
-                if (full || lane * DV + e < rbp) {
-                    const float rv = rrow[(long)oo * rbp + e];
+                if (full || day_of<DV>(lane, e) < rbp) {
+                    const float rv = rrow[(long)oo * rbp + day_of<DV>(lane, e)];
 #pragma unroll
                     for (int i = 0; i < kRB; ++i) acc[i][e] = fmaf(v4[i], rv, acc[i][e]);
                 }
@@ -499,15 +508,15 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
         const long s = sb * kRB + i;
         if (s >= T) break;
         if (UPDATE) {
-            vec* qp = reinterpret_cast<vec*>(Qb + ((size_t)s * Np + n) * bp + lane * DV);
-            vec qv = *qp;
-            float* qf = reinterpret_cast<float*>(&qv);
+            float* qp = Qb + ((size_t)s * Np + n) * bp;
+            float qf[DV];
+            ld_days<DV>(qp, lane, qf);
 #pragma unroll
             for (int e = 0; e < DV; ++e) {
-                if (Gb != nullptr) qf[e] = adagrad_update(qf[e], acc[i][e], Gb + ((size_t)s * Np + n) * bp + lane * DV + e, eta, eps);
+                if (Gb != nullptr) qf[e] = adagrad_update(qf[e], acc[i][e], Gb + ((size_t)s * Np + n) * bp + day_of<DV>(lane, e), eta, eps);
                 else qf[e] = fmaxf(0.f, fmaf(-eta, acc[i][e], qf[e]));
             }
-            *qp = qv;
+            st_days<DV>(qp, lane, qf);
         } else if (lane == 0) {
             gout[(size_t)s * N + n] = acc[i][0];
         }
