@@ -154,15 +154,13 @@ static int fail(dode_ctx* c, int code, const char* fmt, ...) {
 static inline int ceil_div(long a, long b) { return (int)((a + b - 1) / b); }
 static inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
-// Padded extent of an operator dimension: whole 128-byte lines per row when that costs at most 3 % more bytes,
-// else whole 32-byte sectors under the same limit, else the 16 bytes float4 / TMA need.  (Measured on config 1: padding
-// 60 -> 64 and 120 -> 128 moved 14 % more bytes and was 6 % slower than 16-byte alignment.)
+// Padded extent of an operator dimension: whole 128-byte lines per row when that costs at most 3 % more bytes, else
+// whole 32-byte sectors (8 floats).  8 is also what the tensor path needs: the K windows of the bf16 correction panels
+// start at multiples of the padded dimension, and a TMA box must start on a 16-byte boundary (8 bf16).
 static int pad_dim(int n) {
-    for (int a : {32, 8}) {
-        const int p = round_up(n, a);
-        if ((long)p * 100 <= (long)n * 103) return p;
-    }
-    return round_up(n, 4);
+    const int p = round_up(n, 32);
+    if ((long)p * 100 <= (long)n * 103) return p;
+    return round_up(n, 8);
 }
 
 static int ensure_buf(dode_ctx* ctx, float** buf, size_t* cap, size_t floats) {
@@ -305,15 +303,15 @@ static PFN_encodeTiled get_encode() {
 
 // fp32 tensor, innermost dim first; out-of-bounds elements read as zero
 static int make_map(dode_ctx* ctx, CUtensorMap* m, const void* base, int rank, const uint64_t* dims,
-                    const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128, bool atom32 = false) {
+                    const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128, bool bf16_sw64 = false) {
     PFN_encodeTiled enc = get_encode();
     if (!enc) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled is unavailable");
     cuuint64_t gd[3]; cuuint64_t gs[2]; cuuint32_t bx[3]; cuuint32_t es[3] = {1, 1, 1};
     for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; }
     for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_bytes[i];
-    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     atom32 ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+    CUresult r = enc(m, bf16_sw64 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank,
+                     const_cast<void*>(base), gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     bf16_sw64 ? CU_TENSOR_MAP_SWIZZLE_64B : swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(ctx, DODE_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
     return DODE_OK;
@@ -363,11 +361,16 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows
         const uint32_t bb[2] = {(uint32_t)tc::kTileK, (uint32_t)bn};
         int rc;
         if ((rc = make_map(ctx, &tb.mapQ_f, tb.Qg_full, 2, qd, qs, bb, true))) return rc;
-        if ((rc = make_map(ctx, &tb.mapQ_l, tb.Qg_lo, 2, qd, qs, bb, true))) return rc;
+        // the correction operands: two bf16 planes (bf16(v) | bf16(v - tf32(v))) of tb.cap rows each in the same allocation
+        const uint64_t qd16[2] = {(uint64_t)qlen, (uint64_t)2 * tb.cap};
+        const uint64_t qs16[1] = {(uint64_t)qlen * 2};
+        if ((rc = make_map(ctx, &tb.mapQ_l, tb.Qg_lo, 2, qd16, qs16, bb, false, true))) return rc;
         const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)tb.cap};
         const uint64_t rs[1] = {(uint64_t)ctx->rpitch * 4};
         if ((rc = make_map(ctx, &tb.mapR_f, tb.rp_full, 2, rd, rs, bb, true))) return rc;
-        if ((rc = make_map(ctx, &tb.mapR_l, tb.rp_lo, 2, rd, rs, bb, true))) return rc;
+        const uint64_t rd16[2] = {(uint64_t)ctx->rpitch, (uint64_t)2 * tb.cap};
+        const uint64_t rs16[1] = {(uint64_t)ctx->rpitch * 2};
+        if ((rc = make_map(ctx, &tb.mapR_l, tb.rp_lo, 2, rd16, rs16, bb, false, true))) return rc;
         tb.bn = bn;
     }
     if (!ctx->tc_attr) {
@@ -462,14 +465,14 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     {
         KernelTimer kt(ctx, KIND_OTHER);
         CU(launch_pdl(ctx->opt_pdl, tc::gather_split, dim3(std::min<long>(64, ceil_div((long)dayStride / 4, 256)), dl.n), dim3(256), 0,
-                      st, ctx->q, dayStride, (long)dayStride / 4, tb.Qg_full, tb.Qg_lo, dl));
+                      st, ctx->q, dayStride, (long)dayStride / 4, tb.Qg_full, reinterpret_cast<__nv_bfloat16*>(tb.Qg_lo), tb.cap, dl));
         ctx->launches++;
     }
     tc::TcParams p{};
     p.T = d.T; p.H = d.H; p.Lp = ctx->Lp; p.Np = ctx->Np; p.bn = bn; p.dsplit = dsplit; p.bnt = dsplit * bn;
     p.stages = stages; p.nring = nring;
     p.slab0 = c * d.T;
-    p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = tb.rp_lo; p.rpitch = ctx->rpitch;
+    p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = reinterpret_cast<__nv_bfloat16*>(tb.rp_lo); p.pcap = tb.cap; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
     p.mask = opt.mask; p.G = opt.G; p.eps = opt.eps;
     const bool ada = opt.mask || opt.G;

@@ -35,6 +35,7 @@
 // -x / projected update), column chunks interleaved between the groups.
 #pragma once
 #include <cuda.h>
+#include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -136,6 +137,22 @@ __device__ __forceinline__ uint64_t umma_desc_k_sw128(uint32_t saddr) {
     return d;
 }
 
+// K-major SWIZZLE_64B descriptor for the bf16 tiles (rows of 32 bf16 = 64 B, 8-row groups 512 B apart).
+__device__ __forceinline__ uint64_t umma_desc_k_sw64(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(512 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)4 << 61;                            // layout type SWIZZLE_64B
+    return d;
+}
+
+// kind::f16 instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = bn.
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int bn) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+}
+
 // kind::tf32 instruction descriptor: D = F32, A = B = TF32, both K-major, M = 128, N = bn.
 __host__ __device__ constexpr uint32_t umma_idesc_tf32(int bn) {
     return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
@@ -160,7 +177,8 @@ struct TcParams {
     // epilogue
     const float* x;      // [D][T][L]        (forward)
     float* rp_full;      // [bcap][rpitch]   (forward output / gradient B operand)
-    float* rp_lo;
+    __nv_bfloat16* rp_lo;   // [2][pcap][rpitch] bf16: bf16(r) then bf16(r - tf32(r))
+    int pcap;               // rows of the minibatch panels (second bf16 plane starts at row pcap)
     long rpitch;
     float* q;            // [D][T][Np]       (gradient, in place)
     size_t dayStride;
@@ -184,6 +202,28 @@ __device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, u
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n"
         "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+
+__device__ __forceinline__ void umma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
+}
+// two fp32 -> one word of two bf16 (round to nearest even): `lo` in bits 0-15 (the lower K index), `hi` in bits 16-31
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    uint32_t d;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    return d;
+}
+__device__ __forceinline__ float tf32_lo(float v) { return v - __uint_as_float(__float_as_uint(v) & 0xffffe000u); }
 
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
     asm volatile(
@@ -241,7 +281,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int m0 = ((int)blockIdx.x / p.dsplit) * kTileM;
     const int d0 = ((int)blockIdx.x % p.dsplit) * p.bn;       // first day (position in the list) of this CTA's group
     const int bBytes = p.bn * kTileK * 4;
-    const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full | B_lo
+    const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full (fp32) | bf16(B) | bf16(B_lo)   (half a B tile each)
     const int nring = p.nring;
     // a tile with <= 64 valid outputs (small networks, ragged last tile) fetches and splits a 64-wide A box; the
     // MMA still runs M = 128 and the upper accumulator rows are never stored
@@ -363,14 +403,15 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                     tma_load_3d(st, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
                 }
                 tma_load_2d(st + kABytes, &mapBf, fb, w0 + kc * kTileK, d0);
-                tma_load_2d(st + kABytes + bBytes, &mapBl, fb, w0 + kc * kTileK, d0);
+                tma_load_2d(st + kABytes + bBytes, &mapBl, fb, w0 + kc * kTileK, d0);                       // bf16(B)
+                tma_load_2d(st + kABytes + bBytes + bBytes / 2, &mapBl, fb, w0 + kc * kTileK, p.pcap + d0);   // bf16(B_lo)
             }
             __syncwarp();
             if (++s == p.stages) { s = 0; ph ^= 1; }
         }
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp walks the loop, one elected lane issues =====
-        const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc2 = umma_idesc_tf32(2 * p.bn);
+        const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc16 = umma_idesc_bf16(p.bn);
         int s = 0;
         uint32_t fph[2] = {0u, 0u};                             // parity of the next phase of full[g][s], bit s
         for (int kc = 0; kc < nk; ++kc) {
@@ -388,13 +429,16 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             mbar_wait(&split[jr], (use / per_group) & 1, 4, kc);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes;
-            const uint32_t ahi = tmem_ring + (uint32_t)jr * 64, alo = ahi + 32;
+            const uint32_t afull = tmem_ring + (uint32_t)jr * 64, a16 = afull + 32, alo16 = afull + 48;
+            const uint32_t bh0 = bf0 + bBytes, bl0 = bh0 + bBytes / 2;
             if (elect_one()) {
 #pragma unroll
-                for (int k = 0; k < kTileK / 8; ++k) {           // UMMA_K = 8 for tf32: 32 bytes along the swizzle span
-                    const uint64_t dbf = umma_desc_k_sw128(bf0 + k * 32);
-                    umma_tf32_ts(tmem_d, ahi + k * 8, dbf, idesc2, !(restart && k == 0));   // [a_hi*b_full | a_hi*b_lo]
-                    umma_tf32_ts(tmem_d + (uint32_t)p.bn, alo + k * 8, dbf, idesc1, 1);     // correction half += a_lo*b_full
+                for (int k = 0; k < kTileK / 8; ++k)             // main product, UMMA_K = 8 for tf32 (32 bytes of the 128-byte rows)
+                    umma_tf32_ts(tmem_d, afull + k * 8, umma_desc_k_sw128(bf0 + k * 32), idesc1, !(restart && k == 0));
+#pragma unroll
+                for (int k = 0; k < kTileK / 16; ++k) {          // corrections in bf16, UMMA_K = 16 (32 bytes of the 64-byte rows)
+                    umma_bf16_ts(tmem_d + (uint32_t)p.bn, alo16 + k * 8, umma_desc_k_sw64(bh0 + k * 32), idesc16, !(restart && k == 0));  // a_lo * b
+                    umma_bf16_ts(tmem_d + (uint32_t)p.bn, a16 + k * 8, umma_desc_k_sw64(bl0 + k * 32), idesc16, 1);                       // a * b_lo
                 }
                 umma_commit(&empty[s]);
                 umma_commit(&a_empty[jr]);
@@ -447,15 +491,19 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {                    // two halves of the 32 K rows: 32 live registers, not 64
-                uint32_t hi[16], lo[16];                        // (one 32-wide pass spills beside the partial sums: measured slower)
+                uint32_t hi[16], h16[8], l16[8];                // (one 32-wide pass spills beside the partial sums: measured slower)
 #pragma unroll
                 for (int k = 0; k < 16; ++k) hi[k] = __float_as_uint(A[(hf * 16 + k) * BM]);
 #pragma unroll
-                for (int i = 0; i < 16; ++i)
-                    lo[i] = __float_as_uint(__uint_as_float(hi[i]) - __uint_as_float(hi[i] & 0xffffe000u));
+                for (int i = 0; i < 8; ++i) {
+                    const float a0 = __uint_as_float(hi[2 * i]), a1 = __uint_as_float(hi[2 * i + 1]);
+                    h16[i] = pack_bf16(a0, a1);
+                    l16[i] = pack_bf16(tf32_lo(a0), tf32_lo(a1));
+                }
                 __syncwarp();                                   // tcgen05.st is .sync.aligned
-                tmem_st16(t0 + hf * 16, hi);
-                tmem_st16(t0 + 32 + hf * 16, lo);
+                tmem_st16(t0 + hf * 16, hi);                    // fp32 as it is: the tensor core reads its TF32 part
+                tmem_st8(t0 + 32 + hf * 8, h16);
+                tmem_st8(t0 + 48 + hf * 8, l16);
             }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -501,9 +549,9 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                         const float acc = sum[j];
                         if (p.mode == 0) {
                             const float r = (!ADA || ((curkeep >> j) & 1u)) ? acc - cur[j] : 0.f;
-                            const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
                             p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
-                            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - rhi;
+                            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = __float2bfloat16_rn(r);
+                            p.rp_lo[(size_t)(p.pcap + d) * p.rpitch + (size_t)tt * p.Lp + m] = __float2bfloat16_rn(tf32_lo(r));
                         } else {
                             const size_t qi = (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
                             if (ADA && p.G != nullptr) p.q[qi] = adagrad_update(cur[j], acc, p.G + qi, p.eta, p.eps);
@@ -546,9 +594,9 @@ splitk_epilogue(const __grid_constant__ TcParams p, int Mt, const __grid_constan
         if (p.mode == 0) {
             float r = acc[e] - __ldg(p.x + ((size_t)dl.day[d] * p.T + tt) * p.M + m);
             if (ADA && p.mask != nullptr && p.mask[((size_t)d * p.T + tt) * p.M + m] == 0) r = 0.f;
-            const float rhi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);
             p.rp_full[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r;
-            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = r - rhi;
+            p.rp_lo[(size_t)d * p.rpitch + (size_t)tt * p.Lp + m] = __float2bfloat16_rn(r);
+            p.rp_lo[(size_t)(p.pcap + d) * p.rpitch + (size_t)tt * p.Lp + m] = __float2bfloat16_rn(tf32_lo(r));
         } else {
             const size_t qi = (size_t)dl.day[d] * p.dayStride + (size_t)tt * p.Np + m;
             const float qv = __ldcg(p.q + qi);
@@ -558,25 +606,23 @@ splitk_epilogue(const __grid_constant__ TcParams p, int Mt, const __grid_constan
     }
 }
 
-// a1 for the tensor path: Qg_full[d][i] = q[day_d][i], Qg_lo[d][i] = q - trunc_tf32(q), i over T*Np (float4 wide)
+// a1 for the tensor path: Qg_full[d][i] = q[day_d][i] (fp32) and the two bf16 planes of the correction operands,
+// g16[d][i] = bf16(q), g16[pcap + d][i] = bf16(q - trunc_tf32(q)), i over T*Np (float4 wide)
 __global__ void __launch_bounds__(256)
-gather_split(const float* __restrict__ q, size_t dayStride, long len4, float* __restrict__ gfull, float* __restrict__ glo,
-             const __grid_constant__ DayList dl) {
+gather_split(const float* __restrict__ q, size_t dayStride, long len4, float* __restrict__ gfull, __nv_bfloat16* __restrict__ g16,
+             int pcap, const __grid_constant__ DayList dl) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");          // q is written by the previous step's update
     const int d = blockIdx.y;
     const float4* src = reinterpret_cast<const float4*>(q + (size_t)dl.day[d] * dayStride);
     float4* f = reinterpret_cast<float4*>(gfull + (size_t)d * dayStride);
-    float4* l = reinterpret_cast<float4*>(glo + (size_t)d * dayStride);
+    uint2* h = reinterpret_cast<uint2*>(g16 + (size_t)d * dayStride);
+    uint2* l = reinterpret_cast<uint2*>(g16 + (size_t)(pcap + d) * dayStride);
     for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < len4; i += (long)gridDim.x * blockDim.x) {
         const float4 v = __ldcg(src + i);          // through L2: see the note on PDL and L1 in banded_gemm_3xtf32
-        float4 lo;
-        lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
-        lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
-        lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
-        lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
         f[i] = v;
-        l[i] = lo;
+        h[i] = make_uint2(pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
+        l[i] = make_uint2(pack_bf16(tf32_lo(v.x), tf32_lo(v.y)), pack_bf16(tf32_lo(v.z), tf32_lo(v.w)));
     }
 }
 
