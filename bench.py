@@ -38,6 +38,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # NOMINAL: SMs x FP32 lanes 
 
 DEFAULT_WORKLOAD = "large_dense"          # BASELINE.json configs[3]: the largest dense single-GPU workload, where
 LARGE_DENSE_SWEEP = (1, 8, 64, 256)       # north_star defines its >= 0.70 HBM / >= 0.50 FP32 targets (G8 sweep)
+TC_TF32_EQUIV_PER_PRODUCT = 2.0  # tensor work of the 3xTF32 kernel per fp32 product, in TF32 MMA units (see roofline_of)
 TF32_OVER_BF16 = 1.1 / 2.25      # nominal dense tensor ratio (B200_PROFILING.md): tf32 1.1 PF vs bf16 2.25 PF
 
 
@@ -323,7 +324,9 @@ def roofline_of(cfg, m, peaks):
     launch / its average event-timed launch duration, against the measured peak of the unit that bounds it."""
     hbm_peak, bf16_peak, peak_src, fp32_peak, fp32_src = peaks
     tensor_path = m["path"].startswith("tcgen05")
-    tc_peak = bf16_peak * TF32_OVER_BF16 / 3.0          # 3xTF32: three tf32 MMAs per fp32 product
+    # 3xTF32 with bf16 corrections: per fp32 product one TF32 MMA (a*b, both truncated to TF32) and two bf16 MMAs
+    # (a_lo*b, a*b_lo) at half the TF32 cost each = 2 TF32 MMA-equivalents, so fp32-equivalent peak = tf32 peak / 2
+    tc_peak = bf16_peak * TF32_OVER_BF16 / TC_TF32_EQUIV_PER_PRODUCT
     dom = "forward" if m["fwd_ms"] >= m["grad_ms"] else "gradient_update"
     d_ms, d_n, d_bytes = (m["fwd_ms"], m["fwd_n"], m["fb"]) if dom == "forward" else (m["grad_ms"], m["grad_n"], m["gb"])
     gbs = d_bytes / (d_ms * 1e-3) / 1e9 if d_ms > 0 else 0.0
@@ -337,7 +340,8 @@ def roofline_of(cfg, m, peaks):
                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"}
     elif tensor_path:
         roof = {"bound": "tensor", "achieved": tfl, "peak": tc_peak, "unit": "TFLOP/s", "frac": tfl / tc_peak,
-                "peak_source": f"MEASURED_PEAKS.json bf16_tflops ({peak_src}) x 1.1/2.25 (tf32) / 3 (3xTF32 MMAs per product)"}
+                "peak_source": f"MEASURED_PEAKS.json bf16_tflops ({peak_src}) x 1.1/2.25 (nominal tf32:bf16) / 2 (one TF32 MMA + two "
+                               "bf16 MMAs at half its cost per fp32 product)"}
     else:
         roof = {"bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s", "frac": tfl / fp32_peak,
                 "peak_source": fp32_src}

@@ -1,5 +1,5 @@
 // Tensor-core path of a2-a4 for minibatch b >= 8: banded block GEMMs on tcgen05 (5th-gen tensor
-// cores, FP32 accumulators in TMEM) with 3xTF32 split arithmetic, TMA-staged operands.
+// cores, FP32 accumulators in TMEM) with 3xTF32 split arithmetic (bf16 correction terms), TMA-staged operands.
 //
 // Per output tile (time index tt, 128 outputs m0..m0+127) the pass is one GEMM
 //        D[128 x BN] = sum_k A[k][m] * B[k][d]             (BN = b rounded up to 16 days)
@@ -10,17 +10,23 @@
 // A never feeds the tensor core from shared memory: 3xTF32 has to split A = A_hi + A_lo anyway, so splitter
 // threads (thread = output row = TMEM lane) read their COLUMN of the landed tile (consecutive lanes ->
 // consecutive words, conflict-free), and write A_hi / A_lo into tensor memory with tcgen05.st; tcgen05.mma
-// then takes A from TMEM (TS form) and B from shared memory (SWIZZLE_128B K-major descriptors).
+// then takes A from TMEM (TS form) and B from shared memory (K-major descriptors: SWIZZLE_128B fp32, SWIZZLE_64B bf16).
 // Truncation at the day boundary falls out of zero rows packed at create time and of TMA's
 // zero fill beyond the end of the per-day vector / of the K rows of a slab.
 //
 // 3xTF32 (north_star: "3xTF32 tensor-core emulation ... where the tolerance still holds"):
 //   a = a_hi + a_lo with a_hi = a truncated to TF32 (what the tensor core reads from an fp32 container),
-//   a_lo = a - a_hi (exact in fp32);   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo   (error ~2^-20 relative).
-//   B_lo panels are produced where B is produced (gather kernel / forward epilogue).  The B_full and B_lo tiles,
-//   adjacent in smem, are fed as ONE N = 2*bn operand (bn <= 128 days per CTA; wider minibatches are split into two
-//   day groups, blockIdx.x & 1): D[:, 0:bn] += A_hi*B_full (the MAIN sum), D[:, bn:2bn] += A_hi*B_lo, and a second MMA
-//   adds A_lo*B_full into the same CORRECTION half -> 2 MMAs per K-step; the epilogue adds the two halves.
+//   a_lo = a - a_hi (exact in fp32);   a*b ~= a_hi*b_hi + a_lo*b + a*b_lo   (a_lo*b_lo ~ 2^-22 dropped).
+//   The MAIN product a_hi*b_hi runs as kind::tf32 on the fp32 data itself (K = 8 per instruction) into D[:, 0:bn].
+//   The two CORRECTION products are 2^-11 of it, so their factors need only bf16 precision (rounding a 2^-11-sized
+//   factor to 8 bits costs 2^-19 of the product, unbiased): they run as kind::f16 on bf16 operands (K = 16 per
+//   instruction, i.e. half the tensor time of a TF32 instruction per K) into their own accumulator D[:, bn:2bn]:
+//       D_corr += bf16(a_lo) * bf16(b)  +  bf16(a) * bf16(b_lo).
+//   Per 32-row K chunk: 4 TF32 + 4 bf16 instructions = the tensor time of 2 TF32 products per fp32 product, not 3.
+//   B operands per minibatch: one fp32 plane and two bf16 planes (bf16(v), bf16(v - tf32(v))), produced where B is
+//   produced (gather kernel / forward epilogue) — the same bytes as fp32 v and v_lo.  A: the splitters store the fp32
+//   values (32 TMEM columns) and the two bf16 planes packed two per column (16 + 16 columns).  bn <= 128 days per CTA;
+//   wider minibatches are split into two day groups (blockIdx.x & 1).  The epilogue adds main and correction halves.
 // Accumulation accuracy (measured): tcgen05 adds into its FP32 accumulator with round-toward-zero, so
 //   every accumulating instruction loses ~half an ulp of the running sum, always in the same direction: a relative bias
 //   of about -n * 2^-24 after n instructions on same-signed data (-1.5e-5 at K = 2048, -2e-4 at K = 13312 with every
@@ -28,7 +34,7 @@
 //   touch the main accumulator (above), (2) every kFlushChunks K chunks the accumulators are DRAINED by the splitter
 //   threads into fp32 registers (round-to-nearest adds) and restarted, so that no accumulator ever takes more than
 //   4 * kFlushChunks additions (bias <= ~4e-6 relative, whatever K).
-// TMEM columns: [0, 2*bn) accumulators, then nring x (32 cols A_hi | 32 cols A_lo).
+// TMEM columns: [0, 2*bn) accumulators, then nring x (32 cols A fp32 | 16 cols bf16(A) | 16 cols bf16(A_lo)).
 //
 // Warp roles (320 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2-5 and 6-9 = two
 // groups of splitters that take alternate K chunks, then the epilogue (TMEM -> registers -> global, fused
