@@ -241,6 +241,15 @@ def test_csr_path_on_dense_blocks(b):
     assert path.startswith("csr_")
 
 
+@pytest.mark.parametrize("b", [20, 100])
+def test_csr_wide_link_ranges_and_ragged_time_axis(b):
+    """Paths that cover hundreds of links (every gradient row block gathers from a 390-link range) at two panel widths;
+    T = 37 leaves a ragged last block of departure intervals and a ragged forward time pair."""
+    cfg = synth.Config("csr_wide", N=24, L=400, T=37, H=3, C=1, D=2 * b, b=b, K=4, kmin=340, kmax=390, label_mode="zero")
+    path = _run_both(cfg, csr=True, sample=[0, 1, b, 2 * b - 1])
+    assert path.startswith("csr_")
+
+
 def test_csr_path_on_generated_sparse_instance():
     """configs[4]'s structure at small size (G7 windowed lags, heavy-tailed demand, calendar factors)."""
     cfg = synth.Config("sparse_small", N=400, L=90, T=40, H=10, C=3, D=60, b=24, K=10, kmin=6, kmax=20,
