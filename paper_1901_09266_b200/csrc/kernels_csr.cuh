@@ -38,6 +38,10 @@ constexpr int kCsrMaxDays = 128;
 constexpr int kRB = 4;            // links (forward) / departure intervals (gradient) per row block
 constexpr int kFT = 2;            // arrival intervals per forward row block
 constexpr int kFS = kRB * kFT;    // output rows (value slots) of a forward entry
+// Gathered panel rows a warp keeps in flight: both passes stall on the latency of the gathers (ncu: long-scoreboard stalls
+// dominate), so more loads in flight pay until the registers run out (measured on configs[4]: forward 7.92 / 7.48 / 7.43 /
+// 7.08 ms at 2 / 4 / 6 / 8; gradient, which runs 4 CTAs of 64 registers per SM, 9.77 / 9.46 / 13.3 / 16.9 ms).
+constexpr int kInFlightF = 8, kInFlightG = 4;     // (gradient with 3 CTAs per SM and 6 / 8 in flight: 10.8 / 12.3 ms)
 
 struct CsrCluster {
     int64_t* rowptrF = nullptr;   // [ceil(T/2)*ceil(L/4) + 1]
@@ -327,6 +331,44 @@ template <> struct DVec<1> { using type = float; };
 template <> struct DVec<2> { using type = float2; };
 template <> struct DVec<4> { using type = float4; };
 template <int DV> __device__ __forceinline__ int day_of(int lane, int e) { return lane * DV + e; }
+
+// Accumulator of one output row over a lane's DV days.  Both CSR passes are bound by instruction issue (about 28 per
+// gathered row at an IPC near 2), so the multiply-adds are issued as packed pairs: fma.rn.f32x2 (sm_100) does two fp32 FMAs
+// per instruction, and ptxas takes the duplicated scalar factor as a broadcast operand (SASS: FFMA2 Rd, Ra.F32,
+// Rb.F32x2.HI_LO, Rc.F32x2.HI_LO) — half the FMA instructions, same arithmetic (each half is an ordinary fp32 fma.rn).
+__device__ __forceinline__ unsigned long long pack2(float a, float b) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+template <int DV> struct DayAcc;
+template <> struct DayAcc<1> {
+    float a = 0.f;
+    __device__ __forceinline__ void fma(float v, const float* q) { a = fmaf(v, q[0], a); }
+    __device__ __forceinline__ void get(float* o) const { o[0] = a; }
+};
+template <> struct DayAcc<2> {
+    unsigned long long p = 0ull;
+    __device__ __forceinline__ void fma(float v, const float* q) { p = ffma2(pack2(v, v), pack2(q[0], q[1]), p); }
+    __device__ __forceinline__ void get(float* o) const { asm("mov.b64 {%0, %1}, %2;" : "=f"(o[0]), "=f"(o[1]) : "l"(p)); }
+};
+template <> struct DayAcc<4> {
+    unsigned long long p0 = 0ull, p1 = 0ull;
+    __device__ __forceinline__ void fma(float v, const float* q) {
+        const unsigned long long vv = pack2(v, v);
+        p0 = ffma2(vv, pack2(q[0], q[1]), p0);
+        p1 = ffma2(vv, pack2(q[2], q[3]), p1);
+    }
+    __device__ __forceinline__ void get(float* o) const {
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(o[0]), "=f"(o[1]) : "l"(p0));
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(o[2]), "=f"(o[3]) : "l"(p1));
+    }
+};
 template <int DV> __device__ __forceinline__ void ld_days(const float* __restrict__ row, int lane, float* v) {
     const typename DVec<DV>::type t = *reinterpret_cast<const typename DVec<DV>::type*>(row + lane * DV);
 #pragma unroll
@@ -365,11 +407,7 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
     const int l0 = (int)lb * kRB;
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const float* qrow = Qb + ((long)tb * kFT - H) * Np * bp;                  // entries only reach rows >= 0
-    float acc[kFS][DV];
-#pragma unroll
-    for (int i = 0; i < kFS; ++i)
-#pragma unroll
-        for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
+    DayAcc<DV> accp[kFS];
     for (int64_t kb = k0; kb < k1; kb += 32) {
         const int cnt = (int)min((int64_t)32, k1 - kb);
         const int o = lane < cnt ? __ldg(pay + kb + lane) : 0;
@@ -378,36 +416,34 @@ csr_fwd(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ pay, con
         if (lane + 32 < 2 * cnt) sval[wib][lane + 32] = __ldg(val + 2 * kb + lane + 32);
         __syncwarp();
         int j = 0;
-        for (; j + 2 <= cnt; j += 2) {
-            float qv[2][DV];
+        for (; j + kInFlightF <= cnt; j += kInFlightF) {
+            float qv[kInFlightF][DV];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < kInFlightF; ++u) {
                 const int oo = __shfl_sync(0xffffffffu, o, j + u);
                 ld_days<DV>(qrow + (long)oo * bp, lane, qv[u]);
             }
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
+            for (int u = 0; u < kInFlightF; ++u) {
                 const float4 va = sval[wib][2 * (j + u)], vb = sval[wib][2 * (j + u) + 1];
                 const float vv[kFS] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
-                const float* qf = qv[u];
 #pragma unroll
-                for (int i = 0; i < kFS; ++i)
-#pragma unroll
-                    for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[i], qf[e], acc[i][e]);
+                for (int i = 0; i < kFS; ++i) accp[i].fma(vv[i], qv[u]);
             }
         }
-        if (j < cnt) {
+        for (; j < cnt; ++j) {
             const int oo = __shfl_sync(0xffffffffu, o, j);
             float qf[DV];
             ld_days<DV>(qrow + (long)oo * bp, lane, qf);
             const float4 va = sval[wib][2 * j], vb = sval[wib][2 * j + 1];
             const float vv[kFS] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
 #pragma unroll
-            for (int i = 0; i < kFS; ++i)
-#pragma unroll
-                for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[i], qf[e], acc[i][e]);
+            for (int i = 0; i < kFS; ++i) accp[i].fma(vv[i], qf);
         }
     }
+    float acc[kFS][DV];
+#pragma unroll
+    for (int i = 0; i < kFS; ++i) accp[i].get(acc[i]);
 #pragma unroll
     for (int i = 0; i < kFS; ++i) {
         const int l = l0 + (i & (kRB - 1));
@@ -459,11 +495,7 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const bool full = rbp == bp;
     const float* rrow = r + (size_t)sb * kRB * L * rbp;
-    float acc[kRB][DV];
-#pragma unroll
-    for (int i = 0; i < kRB; ++i)
-#pragma unroll
-        for (int e = 0; e < DV; ++e) acc[i][e] = 0.f;
+    DayAcc<DV> accp[kRB];
     for (int64_t kb = k0; kb < k1; kb += 32) {
         const int64_t k = kb + lane;
         const int o = k < k1 ? __ldg(kl + k) : 0;
@@ -471,38 +503,40 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
         const int cnt = (int)min((int64_t)32, k1 - kb);
         int j = 0;
         if (full) {
-            for (; j + 2 <= cnt; j += 2) {
-                float rv[2][DV]; float vv[2][kRB];
+            for (; j + kInFlightG <= cnt; j += kInFlightG) {
+                float rv[kInFlightG][DV]; float vv[kInFlightG][kRB];
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
+                for (int u = 0; u < kInFlightG; ++u) {
                     const int oo = __shfl_sync(0xffffffffu, o, j + u);
                     vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
                     vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
                     ld_days<DV>(rrow + (long)oo * bp, lane, rv[u]);
                 }
 #pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const float* rf = rv[u];
+                for (int u = 0; u < kInFlightG; ++u)
 #pragma unroll
-                    for (int i = 0; i < kRB; ++i)
-#pragma unroll
-                        for (int e = 0; e < DV; ++e) acc[i][e] = fmaf(vv[u][i], rf[e], acc[i][e]);
-                }
+                    for (int i = 0; i < kRB; ++i) accp[i].fma(vv[u][i], rv[u]);
             }
         }
         for (; j < cnt; ++j) {
             const int oo = __shfl_sync(0xffffffffu, o, j);
             const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
                                    __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
+            float rf[DV];
+            if (full) {
+                ld_days<DV>(rrow + (long)oo * bp, lane, rf);
+            } else {
 #pragma unroll
-            for (int e = 0; e < DV; ++e)
-                if (full || day_of<DV>(lane, e) < rbp) {
-                    const float rv = rrow[(long)oo * rbp + day_of<DV>(lane, e)];
+                for (int e = 0; e < DV; ++e)
+                    rf[e] = day_of<DV>(lane, e) < rbp ? rrow[(long)oo * rbp + day_of<DV>(lane, e)] : 0.f;
+            }
 #pragma unroll
-                    for (int i = 0; i < kRB; ++i) acc[i][e] = fmaf(v4[i], rv, acc[i][e]);
-                }
+            for (int i = 0; i < kRB; ++i) accp[i].fma(v4[i], rf);
         }
     }
+    float acc[kRB][DV];
+#pragma unroll
+    for (int i = 0; i < kRB; ++i) accp[i].get(acc[i]);
 #pragma unroll
     for (int i = 0; i < kRB; ++i) {
         const long s = sb * kRB + i;
