@@ -64,6 +64,7 @@ struct dode_ctx {
     double* d_part = nullptr;    // objective partials
     size_t part_cap = 0;
     double* d_obj = nullptr;     // [D] per-day objective + 2 scalars
+    double* d_mom = nullptr;     // [2*D] per-day sum and sum of squares of x (dode_r2), allocated by its first call
     float *pu = nullptr, *pv = nullptr, *pw = nullptr;   // apply / power-iteration scratch: [T][Np], [T][Lp], [T][N]
     std::vector<int32_t> labels;
     std::vector<int32_t> stamp;  // distinctness check
@@ -643,7 +644,7 @@ void dode_destroy(dode_ctx* ctx) {
     cudaFree(ctx->Ag); cudaFree(ctx->Af); cudaFree(ctx->G); cudaFree(ctx->q); cudaFree(ctx->x); cudaFree(ctx->r); cudaFree(ctx->Qb);
     for (auto& p : ctx->ev_pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
-    cudaFree(ctx->d_part); cudaFree(ctx->d_obj); cudaFree(ctx->pu); cudaFree(ctx->pv); cudaFree(ctx->pw);
+    cudaFree(ctx->d_part); cudaFree(ctx->d_obj); cudaFree(ctx->d_mom); cudaFree(ctx->pu); cudaFree(ctx->pv); cudaFree(ctx->pw);
     csr_free(ctx->csr);
     delete ctx;
 }
@@ -980,8 +981,9 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
         CU(cudaMalloc(&ctx->d_part, (size_t)nchunks * kObjBatch * sizeof(double)));
         ctx->part_cap = (size_t)nchunks * kObjBatch;
     }
-    std::vector<double> host(n);
-    std::vector<int> pos;
+    std::vector<double> host(n), tmp(n);
+    std::vector<int> pos, order;                 // order[k] = position in `days` of the k-th result on the device
+    order.reserve(n);
     for (int c = 0; c < d.C; ++c) {
         pos.clear();
         for (int i = 0; i < n; ++i)
@@ -994,14 +996,15 @@ int dode_objective(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_da
             if ((rc = forward_batch(ctx, c, dl, &bt, &bp))) return rc;
             sumsq_partial<<<dim3(nchunks, ceil_div(dl.n, 32)), kThreads, 0, ctx->stream>>>(ctx->r, ctx->d_part, rows, bp,
                                                                                          dl.n, rowsPerBlock);
-            sumsq_final<<<ceil_div(dl.n, 64), 64, 0, ctx->stream>>>(ctx->d_part, ctx->d_obj, nchunks, dl.n);
+            sumsq_final<<<ceil_div(dl.n, 64), 64, 0, ctx->stream>>>(ctx->d_part, ctx->d_obj + order.size(), nchunks, dl.n);
             ctx->launches += 2;
-            std::vector<double> tmp(dl.n);
-            CU(cudaMemcpyAsync(tmp.data(), ctx->d_obj, dl.n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-            CU(cudaStreamSynchronize(ctx->stream));
-            for (int j = 0; j < dl.n; ++j) host[pos[off + j]] = tmp[j];
+            for (int j = 0; j < dl.n; ++j) order.push_back(pos[off + j]);
         }
     }
+    // one download and one host synchronisation for the whole list (d_obj holds D + 8 doubles, n <= D)
+    CU(cudaMemcpyAsync(tmp.data(), ctx->d_obj, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int k = 0; k < n; ++k) host[order[k]] = tmp[k];
     CU(cudaGetLastError());
     double tot = 0.0;
     for (int i = 0; i < n; ++i) tot += host[i];
@@ -1021,25 +1024,25 @@ int dode_r2(dode_ctx* ctx, const int32_t* days, int32_t n, double* per_day, doub
         n = d.D;
     }
     if (n <= 0) return fail(ctx, DODE_EINVAL, "n <= 0");
-    std::vector<double> f(n), mom(2 * (size_t)kMaxDays);
-    int rc = dode_objective(ctx, days, n, f.data(), nullptr);            // validates the list, SS_res per day
+    std::vector<double> f(n), mom(2 * (size_t)n);
+    int rc = dode_objective(ctx, days, n, f.data(), nullptr);            // validates the list (distinct: n <= D), SS_res per day
     if (rc) return rc;
+    if (!ctx->d_mom) CU(cudaMalloc(&ctx->d_mom, 2 * (size_t)d.D * sizeof(double)));
     const long TL = (long)d.T * d.L;
-    double acc = 0.0;
-    constexpr int kChunk = 32;                 // 2*kChunk doubles fit the objective's partial buffer (>= 64 doubles)
-    for (int off = 0; off < n; off += kChunk) {
-        DayList dl; dl.n = std::min(kChunk, n - off);
+    for (int off = 0; off < n; off += kMaxDays) {
+        DayList dl; dl.n = std::min(kMaxDays, n - off);
         std::memcpy(dl.day, days + off, sizeof(int) * dl.n);
-        x_moments<<<dl.n, kThreads, 0, ctx->stream>>>(ctx->x, TL, ctx->d_part, dl);
+        x_moments<<<dl.n, kThreads, 0, ctx->stream>>>(ctx->x, TL, ctx->d_mom + 2 * (size_t)off, dl);
         ctx->launches++;
-        CU(cudaMemcpyAsync(mom.data(), ctx->d_part, sizeof(double) * 2 * dl.n, cudaMemcpyDeviceToHost, ctx->stream));
-        CU(cudaStreamSynchronize(ctx->stream));
-        for (int i = 0; i < dl.n; ++i) {
-            const double ss_tot = mom[2 * i + 1] - mom[2 * i] * mom[2 * i] / (double)TL;
-            const double r2 = 1.0 - f[off + i] / ss_tot;
-            if (per_day) per_day[off + i] = r2;
-            acc += r2;
-        }
+    }
+    CU(cudaMemcpyAsync(mom.data(), ctx->d_mom, sizeof(double) * 2 * n, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));              // one host round trip for the whole list
+    double acc = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const double ss_tot = mom[2 * i + 1] - mom[2 * i] * mom[2 * i] / (double)TL;
+        const double r2 = 1.0 - f[i] / ss_tot;
+        if (per_day) per_day[i] = r2;
+        acc += r2;
     }
     CU(cudaGetLastError());
     if (mean) *mean = acc / n;
