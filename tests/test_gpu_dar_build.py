@@ -52,6 +52,20 @@ def test_example3_on_gpu():
     np.testing.assert_allclose(got, want, atol=1e-7)
 
 
+def test_fifo_violation_on_gpu():
+    """The hand-worked FIFO-violation instance (tests/golden/fifo_violation_two_link.txt; reading A20) through the dense
+    kernel and the CSR builder."""
+    from tests.test_oracle_pins import _fifo_violation_instance
+    T, H, L, N, dt, pp, pl, length, speed, want = _fifo_violation_instance()
+    tp, tl, tn, ts = (torch.from_numpy(a).cuda() for a in (pp, pl, length, speed))
+    R = torch.empty((T, H + 1, L, N), device="cuda")
+    P.dode_dar_build(N, L, T, H, tp, tl, tn, ts, dt, R)
+    np.testing.assert_allclose(R.cpu().numpy()[:2, :, :, 0], want[:2], atol=1e-7)
+    from oracle import oracle
+    _csr_equal(P.dode_assignment_build_csr(N, L, T, H, None, tp, tl, tn, ts, dt),
+               oracle.dar_build(N, L, T, H, pp, pl, length, speed, dt), 1e-7)
+
+
 def test_built_operator_through_the_spgd_path():
     """Step 1 -> Step 5 on the GPU: operators built by dode_dar_build for two patterns feed dode_create directly; the
     SPGD iterates equal the oracle's on the oracle-built operators."""

@@ -433,6 +433,33 @@ def test_p16_dar_example3_worked_by_hand():
     np.testing.assert_allclose(R[0, :, :, 0], want, rtol=0, atol=1e-7)
 
 
+def _fifo_violation_instance():
+    T, H, L, N, dt = 4, 3, 2, 1, 300.0
+    length = np.array([3000.0, 600.0], np.float32)
+    speed = np.full((T, L), 10.0, np.float32)
+    speed[0, 0] = 5.0
+    speed[1:, 0] = 30.0
+    want = np.zeros((T, H + 1, L))
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "fifo_violation_two_link.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        s_, l, h2, v = line.split()
+        want[int(s_), int(h2) - int(s_), int(l)] = float(v)
+    return T, H, L, N, dt, np.array([0, 2], np.int32), np.array([0, 1], np.int32), length, speed, want
+
+
+def test_p16_dar_fifo_violation_worked_by_hand():
+    """The `a2 <= a1` branch of O7 (reading A20): when a speed jump lets the trailing trajectory overtake the leading one,
+    the whole flow goes to the interval of the LEADING arrival (tests/golden/fifo_violation_two_link.txt, worked by hand),
+    and the next departure interval is an ordinary window again."""
+    T, H, L, N, dt, pp, pl, length, speed, want = _fifo_violation_instance()
+    R = oracle.dar_build(N, L, T, H, pp, pl, length, speed, dt)
+    np.testing.assert_allclose(R[:2, :, :, 0], want[:2], rtol=0, atol=1e-7)
+    # the multi-path builder with one path takes the same branch
+    R8 = oracle.assignment_build(N, L, T, H, np.array([0, 1], np.int32), pp, pl, length, speed, dt, 0.01)
+    np.testing.assert_array_equal(R8, R)
+
+
 def test_p16_dar_constant_speed_closed_form_and_row_sums():
     """Constant speeds: link j is reached after c_j = sum of travel times, so the flow of interval s arrives in intervals
     s + floor(c_j/dt) and the next one with shares 1 - frac and frac (Eq. 17); every covered (s, l, n) sums to 1 over
