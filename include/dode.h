@@ -12,7 +12,8 @@
  * s = h1-1, h = h2-h1).  Blocks with s+h >= T may be present; they are ignored.
  *
  * Conventions: plain C types; every function returns DODE_OK (0) or a negative dode_status;
- * nothing is written to stdout/stderr; no global state; no CPU fallback — every call fails with
+ * nothing is written to stdout/stderr; no global state (one stated exception: the static scratch array of
+ * dode_visit_static); no CPU fallback — every call fails with
  * DODE_ECUDA if no usable sm_100 device/context exists.  "device" pointers are CUDA device
  * pointers valid in the current context (e.g. torch-allocated); "host" pointers are ordinary
  * host memory.  All work is issued on the stream given to dode_create or ordered with it as dode_spgd_step states.  A sticky CUDA error is
@@ -217,6 +218,28 @@ int dode_timing_read(dode_ctx* ctx, int32_t kind, double* total_ms, int64_t* lau
  * launches after one warm-up, in TFLOP/s (2 flops per FFMA).  bench.py uses it as the denominator of every "alu"
  * roofline instead of the nominal SMs x 128 lanes x 2 x clock.  Synchronises `stream`.  Errors: dode_last_error(NULL). */
 int dode_probe_fp32_peak(int32_t reps, double* tflops, void* stream);
+
+/* One visit of ONE day (Alg. 1 lines 9-11 on a single-day minibatch; the same r = rho q - x,
+ * g = rho^T r, q <- max(0, q - eta g) as dode_spgd_step with n = 1) for callers that may not allocate: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Needs no ctx and calls no cudaMalloc, cudaFree
+ * or allocating library routine: the day's residual r [T][L] — the only scratch of a visit — lives in a file-scope
+ * device array of DODE_STATIC_SCRATCH_FLOATS floats (1 MiB) that every GPU loading the library holds until exit.
+ *   R    device fp32 [T][H+1][L][N], the boundary order of dode_dar.dense for one cluster (n fastest), read only
+ *   q    device fp32 [T][N], updated in place;   x  device fp32 [T][L], read only;   eta > 0
+ *   stream  the cudaStream_t (as void*) both kernels are launched on; asynchronous, nothing is synchronised
+ * Limits: T*L <= DODE_STATIC_SCRATCH_FLOATS and T <= 65535, else DODE_EINVAL with the sizes in dode_last_error(NULL)
+ * and nothing launched (use dode_create + dode_spgd_step for larger days: they allocate at create / first use).
+ * Every call on a device shares that device's array.  The forward kernel writes every element the gradient kernel reads,
+ * so nothing has to start at zero and no call sees the previous call's contents; but two calls that OVERLAP on one GPU
+ * (different streams, or several host threads each on its own stream) race on r: keep calls on a device in one stream
+ * or order them with events.  The first call on each device looks up the array's device address
+ * (cudaGetSymbolAddress with that device current, once per device, under a mutex); later calls only launch.
+ * Plain FP32 FFMA kernels (one warp per residual element; 32 OD columns x 8 row slices per gradient CTA) on the
+ * unpadded boundary layout — a convenience path, not the tuned one; results agree with dode_spgd_step within the
+ * tolerance of DESIGN.md §4 (different FP32 summation order). */
+#define DODE_STATIC_SCRATCH_FLOATS (1 << 18)
+int dode_visit_static(int32_t N, int32_t L, int32_t T, int32_t H, const float* R, float* q, const float* x, float eta,
+                      void* stream);
 
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 int64_t dode_launch_count(const dode_ctx* ctx);

@@ -22,7 +22,7 @@ DODE_DENSE, DODE_CSR = 0, 1
 DODE_OPT_TC_MIN_B, DODE_OPT_LANES, DODE_OPT_TC_KSPLIT, DODE_OPT_PDL = 0, 1, 2, 3
 
 EXPORTS = ["dode_create", "dode_set_option", "dode_reserve", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_assignment_build_csr", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
-           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_probe_fp32_peak", "dode_launch_count", "dode_last_path", "dode_sync",
+           "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_probe_fp32_peak", "dode_visit_static", "dode_launch_count", "dode_last_path", "dode_sync",
            "dode_destroy", "dode_last_error"]
 
 
@@ -75,6 +75,7 @@ def lib():
         L.dode_timing_enable.argtypes = [vp, i32]
         L.dode_timing_read.argtypes = [vp, i32, vp, vp, i32]
         L.dode_probe_fp32_peak.argtypes = [i32, vp, vp]
+        L.dode_visit_static.argtypes = [i32, i32, i32, i32, vp, vp, vp, f32, vp]
         L.dode_launch_count.argtypes = [vp]
         L.dode_launch_count.restype = C.c_int64
         L.dode_last_path.argtypes = [vp]
@@ -199,6 +200,24 @@ def dode_dar_build(N: int, L: int, T: int, H: int, path_ptr, path_links, link_le
     rc = lib().dode_dar_build(N, L, T, H, C.c_void_p(path_ptr.data_ptr()), C.c_void_p(path_links.data_ptr()),
                               C.c_void_p(link_len.data_ptr()), C.c_void_p(speed.data_ptr()), C.c_double(dt),
                               C.c_void_p(R_out.data_ptr()), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != DODE_OK:
+        raise DodeError(rc, lib().dode_last_error(None).decode())
+
+
+STATIC_SCRATCH_FLOATS = 1 << 18          # include/dode.h: DODE_STATIC_SCRATCH_FLOATS
+
+
+def dode_visit_static(R, q, x, eta: float) -> None:
+    """One visit of one day with NO allocation (include/dode.h: dode_visit_static): R [T][H+1][L][N], q [T][N] (updated in
+    place), x [T][L], float32 CUDA tensors; the residual lives in the library's static device array, so T*L must not
+    exceed STATIC_SCRATCH_FLOATS (DodeError otherwise).  Runs on torch's current stream; asynchronous."""
+    import torch
+    for t in (R, q, x):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+    T, H1, L, N = R.shape
+    assert q.shape == (T, N) and x.shape == (T, L)
+    rc = lib().dode_visit_static(N, L, T, H1 - 1, C.c_void_p(R.data_ptr()), C.c_void_p(q.data_ptr()),
+                                 C.c_void_p(x.data_ptr()), C.c_float(eta), C.c_void_p(torch.cuda.current_stream().cuda_stream))
     if rc != DODE_OK:
         raise DodeError(rc, lib().dode_last_error(None).decode())
 

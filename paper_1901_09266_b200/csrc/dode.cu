@@ -7,6 +7,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1310,6 +1311,119 @@ int dode_probe_fp32_peak(int32_t reps, double* tflops, void* stream) {
     cudaFree(buf);
     if (e != cudaSuccess) return fail(ctx, DODE_ECUDA, "ffma_peak_probe: %s", cudaGetErrorString(e));
     *tflops = best;
+    return DODE_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// dode_visit_static (include/dode.h): one visit of one day without any allocation.  The residual r [T][L] is the
+// visit's only scratch; it lives in g_static_scratch below — one copy per GPU that loads this library, held until the
+// process exits.  In HOST code the name g_static_scratch is a host-side stand-in, not a device address: the address a
+// kernel can use comes from cudaGetSymbolAddress, looked up once per device with that device current.
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) float g_static_scratch[DODE_STATIC_SCRATCH_FLOATS];
+
+// Alg. 1 line 9, inner part: r[t][l] = sum_{h <= min(H,t)} sum_n R[t-h][h][l][n] q[t-h][n] - x[t][l].
+// One warp per (t, l): lanes stride the N columns of each of the (<= H+1) operator rows, then a shuffle reduction.
+__global__ void __launch_bounds__(256)
+visit_static_residual(int N, int L, int T, int H, const float* __restrict__ R, const float* __restrict__ q,
+                      const float* __restrict__ x, float* __restrict__ r) {
+    const long w = (long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (w >= (long)T * L) return;
+    const int t = (int)(w / L), l = (int)(w % L);
+    const int hmax = min(H, t);
+    float acc0 = 0.f, acc1 = 0.f;
+    for (int h = 0; h <= hmax; ++h) {
+        const float* row = R + (((size_t)(t - h) * (H + 1) + h) * L + l) * (size_t)N;
+        const float* qs = q + (size_t)(t - h) * N;
+        int n = lane;
+        for (; n + 32 < N; n += 64) {
+            acc0 = fmaf(__ldg(row + n), qs[n], acc0);
+            acc1 = fmaf(__ldg(row + n + 32), qs[n + 32], acc1);
+        }
+        if (n < N) acc0 = fmaf(__ldg(row + n), qs[n], acc0);
+    }
+    float acc = acc0 + acc1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) r[w] = acc - x[w];
+}
+
+// Alg. 1 lines 9-11: g[s][n] = sum_{h <= min(H,T-1-s)} sum_l R[s][h][l][n] r[s+h][l];
+// q[s][n] <- max(0, q[s][n] - eta g[s][n]).  The rows (h, l) of departure s are one contiguous slab of R and meet the
+// contiguous window r[s*L ..]: row k = h*L + l <-> r[s*L + k].  CTA = 32 columns x 8 row slices, grid (ceil(N/32), T).
+__global__ void __launch_bounds__(256)
+visit_static_update(int N, int L, int T, int H, const float* __restrict__ R, const float* __restrict__ r,
+                    float* __restrict__ q, float eta) {
+    __shared__ float part[8][33];
+    const int col = threadIdx.x & 31, ks = threadIdx.x >> 5;
+    const int s = blockIdx.y, n = blockIdx.x * 32 + col;
+    const int K = (min(H, T - 1 - s) + 1) * L;
+    const float* Rs = R + (size_t)s * (H + 1) * L * (size_t)N + n;
+    const float* rs = r + (size_t)s * L;
+    float acc0 = 0.f, acc1 = 0.f;
+    if (n < N) {
+        int k = ks;
+        for (; k + 8 < K; k += 16) {
+            acc0 = fmaf(__ldg(Rs + (size_t)k * N), rs[k], acc0);
+            acc1 = fmaf(__ldg(Rs + (size_t)(k + 8) * N), rs[k + 8], acc1);
+        }
+        if (k < K) acc0 = fmaf(__ldg(Rs + (size_t)k * N), rs[k], acc0);
+    }
+    part[ks][col] = acc0 + acc1;
+    __syncthreads();
+    if (ks == 0 && n < N) {
+        float g = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) g += part[j][col];
+        float* qp = q + (size_t)s * N + n;
+        *qp = fmaxf(0.f, *qp - eta * g);
+    }
+}
+
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_static_mu;
+static float* g_static_ptr[kStaticMaxDevices] = {nullptr};
+
+// Device address of the current device's copy of g_static_scratch (looked up once per device).
+static int static_scratch(float** out) {
+    dode_ctx* ctx = nullptr;
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(ctx, DODE_EINVAL, "device ordinal %d outside [0, %d)", dev, kStaticMaxDevices);
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return fail(ctx, DODE_ECUDA, "cudaGetSymbolAddress returned a null address on device %d", dev);
+        g_static_ptr[dev] = static_cast<float*>(p);
+    }
+    *out = g_static_ptr[dev];
+    return DODE_OK;
+}
+
+extern "C" {
+
+int dode_visit_static(int32_t N, int32_t L, int32_t T, int32_t H, const float* R, float* q, const float* x, float eta,
+                      void* stream) {
+    dode_ctx* ctx = nullptr;
+    if (N < 1 || L < 1 || T < 1 || H < 0) return fail(ctx, DODE_EINVAL, "N, L, T must be positive and H >= 0");
+    if (!R || !q || !x) return fail(ctx, DODE_EINVAL, "null R, q or x");
+    if (!(eta > 0.f)) return fail(ctx, DODE_EINVAL, "eta must be > 0");
+    if ((long)T * L > (long)DODE_STATIC_SCRATCH_FLOATS || T > 65535)
+        return fail(ctx, DODE_EINVAL,
+                    "dode_visit_static: T*L = %ld residual floats (T = %d) exceed the static scratch of %d floats / the "
+                    "limit T <= 65535; this entry point allocates nothing — use dode_create + dode_spgd_step",
+                    (long)T * L, (int)T, (int)DODE_STATIC_SCRATCH_FLOATS);
+    float* r = nullptr;
+    const int rc = static_scratch(&r);
+    if (rc != DODE_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    visit_static_residual<<<ceil_div((long)T * L, 8), 256, 0, st>>>(N, L, T, H, R, q, x, r);
+    visit_static_update<<<dim3(ceil_div(N, 32), T), 256, 0, st>>>(N, L, T, H, R, r, q, eta);
+    CU(cudaGetLastError());
     return DODE_OK;
 }
 
