@@ -102,9 +102,11 @@ int dode_reserve(dode_ctx* ctx, int32_t max_days);
  *                       axis is too short to fill the machine).
  *   DODE_OPT_PDL        1 = kernels of a step are chained by programmatic dependent launch (default), 0 = plain
  *                       stream order.
+ *   DODE_OPT_TC_BSTAGES stages of the tcgen05 kernels' minibatch-panel (B) ring, 2..8; 0 = automatic (default).  The
+ *                       operator (A) ring takes the rest of the shared memory.
  * Unknown option or out-of-range value: DODE_EINVAL, nothing changes.  Asynchronous (orders later steps after earlier
  * ones where the option changes the stream they run on). */
-enum { DODE_OPT_TC_MIN_B = 0, DODE_OPT_LANES = 1, DODE_OPT_TC_KSPLIT = 2, DODE_OPT_PDL = 3 };
+enum { DODE_OPT_TC_MIN_B = 0, DODE_OPT_LANES = 1, DODE_OPT_TC_KSPLIT = 2, DODE_OPT_PDL = 3, DODE_OPT_TC_BSTAGES = 4 };
 int dode_set_option(dode_ctx* ctx, int32_t option, int32_t value);
 
 /* NEXT-1 — Alg. 1 as the paper prints it, on the listed days of one cluster:

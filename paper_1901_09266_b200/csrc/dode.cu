@@ -85,7 +85,7 @@ struct dode_ctx {
     std::vector<int8_t> day_last_lane;             // [D] and its lane (-1: none)
     long rpitch = 0;
     // kernel-selection options (dode_set_option)
-    int tc_min_b = 8, opt_ksplit = 0;
+    int tc_min_b = 8, opt_ksplit = 0, opt_bstages = 0;
     bool opt_pdl = true;
     bool tc_ready = false, tc_attr = false;
     CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64;
@@ -388,7 +388,7 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows
 }
 
 // Launch geometry of the tensor-core kernels for a minibatch of bn (multiple of 16) days
-struct TcGeom { int stages, nring; size_t smem; int ks_f, ks_g; size_t part_floats; };
+struct TcGeom { int stages, bstages, nring; size_t smem; int ks_f, ks_g; size_t part_floats; };
 
 // minibatch of n days -> day groups per tile (1, or 2 above 128 days) and days per group (MMA N, multiple of 16)
 static void tc_day_groups(int n, int* dsplit, int* bn) {
@@ -399,20 +399,23 @@ static void tc_day_groups(int n, int* dsplit, int* bn) {
 static TcGeom tc_geometry(const dode_ctx* ctx, int bn, int dsplit) {
     const dode_dims& d = ctx->dm;
     TcGeom g{};
-    // TMA ring: stage = A tile (16 KB) + B_full + B_lo tiles.  Two CTAs per SM when 3 stages fit in half the
-    // shared memory and 256 TMEM columns suffice.
-    const int stageBytes = tc::kABytes + 2 * bn * tc::kTileK * 4;
-    const int fixed = 1024 + 512;                  // alignment slack + barriers (3*stages + 10 of them) + the TMEM slot
+    // Two TMA rings (kernels_tc.cuh): B stages of B_full + bf16(B) + bf16(B_lo) tiles — the panels sit in L2, a shallow
+    // ring covers them — and A stages of one 16 KB tile each, as many as the rest of the shared memory holds (the A
+    // bytes in flight per SM are what hides the HBM latency).  Two CTAs per SM when 256 TMEM columns suffice.
+    // An SM has 228 KB of shared memory, 1 KB of it reserved per resident CTA; a CTA may use up to 227 KB.
+    const int bStage = 2 * bn * tc::kTileK * 4;
+    const int fixed = 512;                         // barriers (2*SA + SB + 10 of them) + the TMEM slot
     const int acc_cols = 2 * bn;
-    int stages = (112 * 1024 - fixed) / stageBytes;
-    int nring = 2;
-    if (stages < 3 || acc_cols + 128 > 256) {          // one CTA per SM
-        stages = (226 * 1024 - fixed) / stageBytes;
-        nring = acc_cols + 256 <= 512 ? 4 : 2;
-    }
-    g.stages = std::max(2, std::min(stages, 10));
-    g.nring = nring;
-    g.smem = (size_t)g.stages * stageBytes + fixed;
+    const bool two = acc_cols + 128 <= 256;
+    const int budget = (two ? 228 * 1024 / 2 - 1024 : 227 * 1024) - fixed;
+    int sb = ctx->opt_bstages > 0 ? ctx->opt_bstages : 3;      // measured: 2 starves the MMA warp at every width, 4 = 3
+    int sa = (budget - sb * bStage) / tc::kABytes;
+    sa = std::max(2, std::min(sa, 16));
+    sb = std::max(2, std::min(sb, sa));
+    g.stages = sa;
+    g.bstages = sb;
+    g.nring = two ? 2 : (acc_cols + 256 <= 512 ? 4 : 2);
+    g.smem = (size_t)sa * tc::kABytes + (size_t)sb * bStage + fixed;
     // split-K when the time axis is too short to fill the machine (T * tiles CTAs for 148 SMs x 1-2 CTAs): e.g. the
     // Fig. 12 workload, T = 1.  Each pass then runs ksplit CTAs per tile and a small epilogue kernel.
     const int slots = 148 * (g.smem * 2 + 2048 <= 227 * 1024 ? 2 : 1);
@@ -472,7 +475,7 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     }
     tc::TcParams p{};
     p.T = d.T; p.H = d.H; p.Lp = ctx->Lp; p.Np = ctx->Np; p.bn = bn; p.dsplit = dsplit; p.bnt = dsplit * bn;
-    p.stages = stages; p.nring = nring;
+    p.stages = stages; p.bstages = geo0.bstages; p.nring = nring;
     p.slab0 = c * d.T;
     p.x = ctx->x; p.rp_full = tb.rp_full; p.rp_lo = reinterpret_cast<__nv_bfloat16*>(tb.rp_lo); p.pcap = tb.cap; p.rpitch = ctx->rpitch;
     p.q = ctx->q; p.dayStride = dayStride; p.eta = eta;
@@ -762,6 +765,10 @@ int dode_set_option(dode_ctx* ctx, int32_t option, int32_t value) {
         case DODE_OPT_TC_KSPLIT:
             if (value < 0 || value > 32) return fail(ctx, DODE_EINVAL, "DODE_OPT_TC_KSPLIT must be in [0, 32]");
             ctx->opt_ksplit = value;
+            return DODE_OK;
+        case DODE_OPT_TC_BSTAGES:
+            if (value != 0 && (value < 2 || value > 8)) return fail(ctx, DODE_EINVAL, "DODE_OPT_TC_BSTAGES must be 0 or in [2, 8]");
+            ctx->opt_bstages = value;
             return DODE_OK;
         case DODE_OPT_PDL:
             if (value != 0 && value != 1) return fail(ctx, DODE_EINVAL, "DODE_OPT_PDL must be 0 or 1");

@@ -178,7 +178,8 @@ struct TcParams {
     int bn;              // days per CTA (MMA N of the main product), a multiple of 16, <= 128
     int dsplit;          // day groups per output tile (1, or 2 for minibatches wider than 128 days): blockIdx.x % dsplit
     int bnt;             // dsplit * bn: padded minibatch width (row stride of the split-K partial sums)
-    int stages;
+    int stages;          // A ring: stages of one 16 KB A tile each (HBM latency: as deep as shared memory allows)
+    int bstages;         // B ring: stages of B_full | bf16(B) | bf16(B_lo) (panels live in L2: 2-3 suffice), <= stages
     int nring;           // TMEM A buffers (2 or 4), half per splitter group
     // epilogue
     const float* x;      // [D][T][L]        (forward)
@@ -280,14 +281,21 @@ __global__ void __launch_bounds__(kThreadsTC, PART <= 32 ? 2 : 1)
 banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapA64,
                    const __grid_constant__ CUtensorMap mapBf, const __grid_constant__ CUtensorMap mapBl,
                    const __grid_constant__ TcParams p, const __grid_constant__ DayList dl) {
-    extern __shared__ __align__(1024) uint8_t smem_raw[];
-    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    // SWIZZLE_128B tiles need 1024-byte alignment: the declared alignment places the dynamic shared memory (the kernel
+    // has no static shared memory) on such a boundary of the CTA's window; no slack is allocated for a manual round-up.
+    extern __shared__ __align__(1024) uint8_t smem[];
+    if ((smem_u32(smem) & 1023u) != 0u) __trap();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
     const int m0 = ((int)blockIdx.x / p.dsplit) * kTileM;
     const int d0 = ((int)blockIdx.x % p.dsplit) * p.bn;       // first day (position in the list) of this CTA's group
     const int bBytes = p.bn * kTileK * 4;
-    const int stageBytes = kABytes + 2 * bBytes;                 // A | B_full (fp32) | bf16(B) | bf16(B_lo)   (half a B tile each)
+    // Two rings, because the two operands have different latencies to hide: A streams from HBM (deep ring), the B
+    // panels sit in L2 (shallow ring).  Chunk kc uses A stage kc % SA and B stage kc % SB; MMAs retire in order, so
+    // "chunk kc - SB retired" frees B stage kc % SB for chunk kc AND the A stage of chunk kc - SB for chunk kc - SB + SA.
+    const int SA = p.stages, SB = p.bstages;
+    const int bStage = 2 * bBytes;                               // B_full (fp32) | bf16(B) | bf16(B_lo)   (half a B tile each)
+    uint8_t* ringB = smem + (size_t)SA * kABytes;
     const int nring = p.nring;
     // a tile with <= 64 valid outputs (small networks, ragged last tile) fetches and splits a 64-wide A box; the
     // MMA still runs M = 128 and the upper accumulator rows are never stored
@@ -295,15 +303,16 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int BM = half ? kTileM / 2 : kTileM;                   // A tile in smem: [kTileK rows][BM floats], no swizzle
     const int aBytes = BM * kTileK * 4;
     const CUtensorMap* mA = half ? &mapA64 : &mapA;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * stageBytes);
-    // full: TMA landed.  One barrier per (splitter group, stage): chunk kc completes full[(kc & 1) * stages + kc % stages],
+    uint64_t* bars = reinterpret_cast<uint64_t*>(ringB + (size_t)SB * bStage);
+    // full: TMA landed (A and B of one chunk; armed when the A tile is requested, the B tiles join later).
+    // One barrier per (splitter group, A stage): chunk kc completes full[(kc & 1) * SA + kc % SA],
     // so every waiter of a barrier (that group's splitters and the MMA warp) sees EVERY one of its phases in turn.  With
     // one barrier per stage a group would have to watch the other group's chunks go by just to keep count, and a warp
     // that is slow to start could fall two phases behind (a stage is refilled as soon as the OTHER group's MMAs retire)
     // and wait for ever — seen once in ~300 steps on the multiyear shape.
-    uint64_t* full = bars;                        // [2][stages]
-    uint64_t* empty = bars + 2 * p.stages;        // [stages] MMAs of the stage retired
-    uint64_t* split = bars + 3 * p.stages;        // [nring] A_hi/A_lo in TMEM
+    uint64_t* full = bars;                        // [2][SA]
+    uint64_t* empty = bars + 2 * SA;              // [SB] MMAs of the chunk in this B stage retired
+    uint64_t* split = empty + SB;                 // [nring] A_hi/A_lo in TMEM
     uint64_t* a_empty = split + 4;                // [nring] MMAs that read this TMEM buffer retired
     uint64_t* accum = a_empty + 4;                // all MMAs issued so far retired (every drain and the end)
     uint64_t* drained = accum + 1;                // the splitter threads have read the accumulators of a drain
@@ -321,7 +330,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     while ((int)tmem_cols < acc_cols + 64 * nring) tmem_cols <<= 1;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&full[p.stages + s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < SA; ++s) { mbar_init(&full[s], 1); mbar_init(&full[SA + s], 1); }
+        for (int s = 0; s < SB; ++s) mbar_init(&empty[s], 1);
         for (int j = 0; j < nring; ++j) { mbar_init(&split[j], 128); mbar_init(&a_empty[j], 1); }
         mbar_init(accum, 1);
         mbar_init(drained, 256);
@@ -345,17 +355,17 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     // the stream may start its own prologue now; nothing produced by the previous kernel is touched before the wait.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // The operator is static: the A tiles of the first ring round are requested NOW, before the dependency wait — a CTA
-    // that gets its SM slot while the previous kernel's slower CTAs are still running streams its first `stages` chunks
+    // that gets its SM slot while the previous kernel's slower CTAs are still running streams its first SA chunks
     // under that kernel's tail.  The B tiles (panels written by the previous kernel) follow after the wait; the stage's
     // barrier expects the bytes of all three loads from the start.
-    const int npre = min(p.stages, nk);
+    const int npre = min(SA, nk);
     const int txBytes = aBytes + 2 * bBytes;
     if (warp == 0) {
         if (elect_one()) {
-            for (int kc = 0; kc < npre; ++kc) {                  // (kc < stages: the stage index is kc)
-                uint64_t* fb = &full[(kc & 1) * p.stages + kc];
+            for (int kc = 0; kc < npre; ++kc) {                  // (kc < SA: the stage index is kc)
+                uint64_t* fb = &full[(kc & 1) * SA + kc];
                 mbar_expect_tx(fb, txBytes);
-                tma_load_3d(smem + (size_t)kc * stageBytes, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
+                tma_load_3d(smem + (size_t)kc * kABytes, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
             }
         }
         __syncwarp();
@@ -398,27 +408,32 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
 
     if (warp == 0) {
         // ===== TMA producer =====
-        int s = 0, ph = 1;                                       // ph: parity of the previous round of slot s
+        int sb = 0, ph = 1;                                      // ph: parity of the previous round of B slot sb
+        int sa = 0;                                              // A stage of chunk kc (== that of chunk kc - SB + SA ... + SB)
         for (int kc = 0; kc < nk; ++kc) {
-            if (kc >= p.stages) mbar_wait(&empty[s], ph, 1, kc);
+            if (kc >= SB) mbar_wait(&empty[sb], ph, 1, kc);      // chunk kc - SB retired
             if (elect_one()) {
-                uint8_t* st = smem + (size_t)s * stageBytes;
-                uint64_t* fb = &full[(kc & 1) * p.stages + s];
-                if (kc >= npre) {                               // (the first round's A tiles were requested before the wait)
-                    mbar_expect_tx(fb, txBytes);
-                    tma_load_3d(st, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
+                const int ka = kc - SB + SA;                     // the A stage that chunk kc - SB leaves takes chunk ka
+                if (kc >= SB && ka < nk) {                       // (ka >= SA >= npre: the first round was requested before the wait)
+                    int sk = sa - SB; if (sk < 0) sk += SA;      // ka % SA == (kc - SB) % SA
+                    uint64_t* fa = &full[(ka & 1) * SA + sk];
+                    mbar_expect_tx(fa, txBytes);
+                    tma_load_3d(smem + (size_t)sk * kABytes, mA, fa, m0, (kbase + ka) * kTileK, p.slab0 + tt);
                 }
-                tma_load_2d(st + kABytes, &mapBf, fb, w0 + kc * kTileK, d0);
-                tma_load_2d(st + kABytes + bBytes, &mapBl, fb, w0 + kc * kTileK, d0);                       // bf16(B)
-                tma_load_2d(st + kABytes + bBytes + bBytes / 2, &mapBl, fb, w0 + kc * kTileK, p.pcap + d0);   // bf16(B_lo)
+                uint8_t* st = ringB + (size_t)sb * bStage;
+                uint64_t* fb = &full[(kc & 1) * SA + sa];
+                tma_load_2d(st, &mapBf, fb, w0 + kc * kTileK, d0);
+                tma_load_2d(st + bBytes, &mapBl, fb, w0 + kc * kTileK, d0);                       // bf16(B)
+                tma_load_2d(st + bBytes + bBytes / 2, &mapBl, fb, w0 + kc * kTileK, p.pcap + d0);   // bf16(B_lo)
             }
             __syncwarp();
-            if (++s == p.stages) { s = 0; ph ^= 1; }
+            if (++sb == SB) { sb = 0; ph ^= 1; }
+            if (++sa == SA) sa = 0;
         }
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp walks the loop, one elected lane issues =====
         const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc16 = umma_idesc_bf16(p.bn);
-        int s = 0;
+        int s = 0, sb = 0;                                      // A stage (names the chunk's full barrier), B stage
         uint32_t fph[2] = {0u, 0u};                             // parity of the next phase of full[g][s], bit s
         for (int kc = 0; kc < nk; ++kc) {
             const int g = kc & 1, use = kc >> 1;
@@ -430,11 +445,11 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 mbar_wait(drained, (kc / kFlushChunks - 1) & 1, 2, kc);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             }
-            mbar_wait(&full[g * p.stages + s], (fph[g] >> s) & 1u, 3, kc);
+            mbar_wait(&full[g * SA + s], (fph[g] >> s) & 1u, 3, kc);
             fph[g] ^= 1u << s;
             mbar_wait(&split[jr], (use / per_group) & 1, 4, kc);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t bf0 = smem_u32(smem + (size_t)s * stageBytes) + kABytes;
+            const uint32_t bf0 = smem_u32(ringB + (size_t)sb * bStage);
             const uint32_t afull = tmem_ring + (uint32_t)jr * 64, a16 = afull + 32, alo16 = afull + 48;
             const uint32_t bh0 = bf0 + bBytes, bl0 = bh0 + bBytes / 2;
             if (elect_one()) {
@@ -446,11 +461,12 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                     umma_bf16_ts(tmem_d + (uint32_t)p.bn, alo16 + k * 8, umma_desc_k_sw64(bh0 + k * 32), idesc16, !(restart && k == 0));  // a_lo * b
                     umma_bf16_ts(tmem_d + (uint32_t)p.bn, a16 + k * 8, umma_desc_k_sw64(bl0 + k * 32), idesc16, 1);                       // a * b_lo
                 }
-                umma_commit(&empty[s]);
+                umma_commit(&empty[sb]);
                 umma_commit(&a_empty[jr]);
             }
             __syncwarp();
-            if (++s == p.stages) s = 0;
+            if (++s == SA) s = 0;
+            if (++sb == SB) sb = 0;
         }
         if (elect_one()) { if (nk == 0) mbar_arrive(accum); else umma_commit(accum); }
         __syncwarp();
@@ -485,15 +501,15 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 mbar_arrive(drained);
             }
-            if (++s == p.stages) s = 0;
+            if (++s == SA) s = 0;
             if ((kc & 1) != group) continue;
             const int use = kc >> 1;
             const int jr = group * per_group + use % per_group;
-            mbar_wait(&full[group * p.stages + s], (fph >> s) & 1u, 6, kc);
+            mbar_wait(&full[group * SA + s], (fph >> s) & 1u, 6, kc);
             fph ^= 1u << s;
             if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1, 7, kc);
             if (lane_base >= BM) { mbar_arrive(&split[jr]); continue; }    // rows never stored
-            const float* A = reinterpret_cast<const float*>(smem + (size_t)s * stageBytes) + row;
+            const float* A = reinterpret_cast<const float*>(smem + (size_t)s * kABytes) + row;
             const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {                    // two halves of the 32 K rows: 32 live registers, not 64

@@ -370,7 +370,8 @@ def test_options_and_reserve_keep_results():
     sched = synth.schedule(cfg, p.labels)
     etas = hz.oracle_etas(p)
     want = hz.oracle_run(p, sched, etas)
-    for opts in ({}, {"LANES": 0}, {"PDL": 0}, {"LANES": 0, "PDL": 0, "TC_KSPLIT": 3}, {"TC_MIN_B": 0}, {"TC_MIN_B": 100}):
+    for opts in ({}, {"LANES": 0}, {"PDL": 0}, {"LANES": 0, "PDL": 0, "TC_KSPLIT": 3}, {"TC_MIN_B": 0}, {"TC_MIN_B": 100},
+                 {"TC_BSTAGES": 2}, {"TC_BSTAGES": 5, "TC_KSPLIT": 2}, {"TC_BSTAGES": 8}):
         g0 = hz.GpuSolver(p)                           # a throw-away pass first: the CUDA runtime loads kernel modules
         for k, v in opts.items():                      # lazily, which moves device memory at a kernel's first launch
             g0.P.dode_set_option(g0.h, getattr(g0.P, "DODE_OPT_" + k), v)
@@ -380,7 +381,8 @@ def test_options_and_reserve_keep_results():
         P = g.P
         for k, v in opts.items():
             P.dode_set_option(g.h, getattr(P, "DODE_OPT_" + k), v)
-        for bad in ((99, 1), (P.DODE_OPT_LANES, 2), (P.DODE_OPT_TC_KSPLIT, 33), (P.DODE_OPT_TC_MIN_B, -1), (P.DODE_OPT_PDL, -1)):
+        for bad in ((99, 1), (P.DODE_OPT_LANES, 2), (P.DODE_OPT_TC_KSPLIT, 33), (P.DODE_OPT_TC_MIN_B, -1), (P.DODE_OPT_PDL, -1),
+                    (P.DODE_OPT_TC_BSTAGES, 1), (P.DODE_OPT_TC_BSTAGES, 9)):
             with pytest.raises(P.DodeError) as e:
                 P.dode_set_option(g.h, *bad)
             assert e.value.code == P.DODE_EINVAL
