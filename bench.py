@@ -442,6 +442,8 @@ def _run_ours(P, args, cfg, sweep, rank, world, local_rank, dev):
         h = P.dode_create(cfg.N, cfg.L, cfg.T, cfg.H, cfg.C, cfg.D, lab, x, 1.0, dense=R)
     if args.tc_bstages:
         P.dode_set_option(h, P.DODE_OPT_TC_BSTAGES, args.tc_bstages)
+    if args.tc_pair is not None:
+        P.dode_set_option(h, P.DODE_OPT_TC_PAIR, args.tc_pair)
     x_cpu = x.cpu()
     R_cpu = None
     if rank == 0 and not args.no_cpu_baseline and not cfg.sparse:
@@ -768,6 +770,7 @@ def main():
     ap.add_argument("--ref-visits", type=int, default=None, help="--impl reference: day-visits per step (default: about 1-10 s of work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tc-bstages", type=int, default=0, help="DODE_OPT_TC_BSTAGES: stages of the tcgen05 kernels' B ring (0 = automatic)")
+    ap.add_argument("--tc-pair", type=int, default=None, help="DODE_OPT_TC_PAIR: 0 = single-CTA tcgen05 kernels only, 1 = CTA pairs (default), 2 = pairs only")
     ap.add_argument("--paths", type=int, default=1, help="--dar-build: up to this many paths per OD with Logit route shares (Eq. 37)")
     ap.add_argument("--theta", type=float, default=0.01, help="--dar-build --paths K: Logit dispersion factor per second (SURVEY NEXT-4)")
     ap.add_argument("--dar-build", action="store_true", help="NEXT-4: time dode_dar_build on the workload's network instead of SPGD")

@@ -104,9 +104,14 @@ int dode_reserve(dode_ctx* ctx, int32_t max_days);
  *                       stream order.
  *   DODE_OPT_TC_BSTAGES stages of the tcgen05 kernels' minibatch-panel (B) ring, 2..8; 0 = automatic (default).  The
  *                       operator (A) ring takes the rest of the shared memory.
+ *   DODE_OPT_TC_PAIR    tcgen05 kernels for minibatches wider than 64 days: 1 = pairs of CTAs on the two SMs of a TPC
+ *                       (tcgen05.mma.cta_group::2 on 256-output tiles, each CTA staging half of the minibatch panel
+ *                       tile), an odd last 128-output tile on the single-CTA kernel (default); 2 = pairs only (an odd
+ *                       last tile is paired with an idle CTA); 0 = single-CTA kernels only.
  * Unknown option or out-of-range value: DODE_EINVAL, nothing changes.  Asynchronous (orders later steps after earlier
  * ones where the option changes the stream they run on). */
-enum { DODE_OPT_TC_MIN_B = 0, DODE_OPT_LANES = 1, DODE_OPT_TC_KSPLIT = 2, DODE_OPT_PDL = 3, DODE_OPT_TC_BSTAGES = 4 };
+enum { DODE_OPT_TC_MIN_B = 0, DODE_OPT_LANES = 1, DODE_OPT_TC_KSPLIT = 2, DODE_OPT_PDL = 3, DODE_OPT_TC_BSTAGES = 4,
+       DODE_OPT_TC_PAIR = 5 };
 int dode_set_option(dode_ctx* ctx, int32_t option, int32_t value);
 
 /* NEXT-1 — Alg. 1 as the paper prints it, on the listed days of one cluster:

@@ -19,7 +19,7 @@ SO_PATH = os.path.join(_HERE, "libdode.so")
 DODE_OK, DODE_EINVAL, DODE_ENOMEM, DODE_ECUDA = 0, -1, -2, -3
 DODE_DENSE, DODE_CSR = 0, 1
 
-DODE_OPT_TC_MIN_B, DODE_OPT_LANES, DODE_OPT_TC_KSPLIT, DODE_OPT_PDL, DODE_OPT_TC_BSTAGES = 0, 1, 2, 3, 4
+DODE_OPT_TC_MIN_B, DODE_OPT_LANES, DODE_OPT_TC_KSPLIT, DODE_OPT_PDL, DODE_OPT_TC_BSTAGES, DODE_OPT_TC_PAIR = 0, 1, 2, 3, 4, 5
 
 EXPORTS = ["dode_create", "dode_set_option", "dode_reserve", "dode_spgd_step", "dode_spgd_step_host", "dode_adagrad_step", "dode_adagrad_reset", "dode_join", "dode_dar_build", "dode_assignment_build", "dode_assignment_build_csr", "dode_objective", "dode_r2", "dode_get_q", "dode_set_q",
            "dode_apply", "dode_apply_t", "dode_lipschitz", "dode_timing_enable", "dode_timing_read", "dode_probe_fp32_peak", "dode_visit_static", "dode_launch_count", "dode_last_path", "dode_sync",

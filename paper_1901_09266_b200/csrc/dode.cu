@@ -17,6 +17,7 @@
 #include <cub/device/device_reduce.cuh>
 #include <cuda/std/functional>
 #include "kernels_tc.cuh"
+#include "kernels_tc2.cuh"
 #include "kernels_dar.cuh"
 #include "kernels_probe.cuh"
 
@@ -29,7 +30,9 @@ struct TcBuf {
     int cap = 0, bn = 0;
     float* part = nullptr;                        // split-K partial sums [ksplit][T][tiles*128][bn]
     size_t part_cap = 0;                          // floats
-    CUtensorMap mapQ_f, mapQ_l, mapR_f, mapR_l;
+    CUtensorMap mapQ_f, mapQ_l, mapR_f, mapR_l;   // boxes of bn days
+    int bh = 0;                                   // CTA-pair kernel (kernels_tc2.cuh): boxes of bh = bn / 2 days
+    CUtensorMap mapQ_f2, mapQ_l2, mapR_f2, mapR_l2;
 };
 
 // Two internal streams that plain dode_spgd_step calls alternate on (tensor-core path): consecutive iterations touch
@@ -86,6 +89,7 @@ struct dode_ctx {
     long rpitch = 0;
     // kernel-selection options (dode_set_option)
     int tc_min_b = 8, opt_ksplit = 0, opt_bstages = 0;
+    int opt_pair = 1;                              // 0 = single-CTA kernels only, 1 = CTA pairs + single-CTA odd tile, 2 = pairs only
     bool opt_pdl = true;
     bool tc_ready = false, tc_attr = false;
     CUtensorMap mapA_fwd, mapA_fwd64, mapA_grad, mapA_grad64;
@@ -339,6 +343,27 @@ static int tc_setup(dode_ctx* ctx) {
     return DODE_OK;
 }
 
+// B tensor maps over the minibatch panels with boxes of `boxdays` days
+static int tc_make_bmaps(dode_ctx* ctx, TcBuf& tb, int boxdays, CUtensorMap* mQf, CUtensorMap* mQl, CUtensorMap* mRf, CUtensorMap* mRl) {
+    const size_t qlen = (size_t)ctx->dm.T * ctx->Np;
+    // B operands: K-major windows of the per-day vectors, SWIZZLE_128B tiles of {32 floats, boxdays days}
+    const uint64_t qd[2] = {(uint64_t)qlen, (uint64_t)tb.cap};
+    const uint64_t qs[1] = {(uint64_t)qlen * 4};
+    const uint32_t bb[2] = {(uint32_t)tc::kTileK, (uint32_t)boxdays};
+    int rc;
+    if ((rc = make_map(ctx, mQf, tb.Qg_full, 2, qd, qs, bb, true))) return rc;
+    // the correction operands: two bf16 planes (bf16(v) | bf16(v - tf32(v))) of tb.cap rows each in the same allocation
+    const uint64_t qd16[2] = {(uint64_t)qlen, (uint64_t)2 * tb.cap};
+    const uint64_t qs16[1] = {(uint64_t)qlen * 2};
+    if ((rc = make_map(ctx, mQl, tb.Qg_lo, 2, qd16, qs16, bb, false, true))) return rc;
+    const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)tb.cap};
+    const uint64_t rs[1] = {(uint64_t)ctx->rpitch * 4};
+    if ((rc = make_map(ctx, mRf, tb.rp_full, 2, rd, rs, bb, true))) return rc;
+    const uint64_t rd16[2] = {(uint64_t)ctx->rpitch, (uint64_t)2 * tb.cap};
+    const uint64_t rs16[1] = {(uint64_t)ctx->rpitch * 2};
+    return make_map(ctx, mRl, tb.rp_lo, 2, rd16, rs16, bb, false, true);
+}
+
 // panels for `rows` minibatch days (>= dsplit * bn) and B tensor maps with boxes of bn days
 static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows) {
     const dode_dims& d = ctx->dm;
@@ -348,7 +373,7 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows
         CU(cudaStreamSynchronize(st));
         cudaFree(tb.Qg_full); cudaFree(tb.Qg_lo); cudaFree(tb.rp_full); cudaFree(tb.rp_lo);
         tb.Qg_full = tb.Qg_lo = tb.rp_full = tb.rp_lo = nullptr;
-        tb.cap = 0; tb.bn = 0;
+        tb.cap = 0; tb.bn = 0; tb.bh = 0;
         CU(cudaMalloc(&tb.Qg_full, bn_alloc * qlen * 4)); CU(cudaMalloc(&tb.Qg_lo, bn_alloc * qlen * 4));
         CU(cudaMalloc(&tb.rp_full, (size_t)bn_alloc * ctx->rpitch * 4)); CU(cudaMalloc(&tb.rp_lo, (size_t)bn_alloc * ctx->rpitch * 4));
         CU(cudaMemsetAsync(tb.Qg_full, 0, bn_alloc * qlen * 4, st)); CU(cudaMemsetAsync(tb.Qg_lo, 0, bn_alloc * qlen * 4, st));
@@ -357,22 +382,8 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows
         tb.cap = bn_alloc;
     }
     if (tb.bn != bn) {
-        // B operands: K-major windows of the per-day vectors, SWIZZLE_128B tiles of {32 floats, bn days}
-        const uint64_t qd[2] = {(uint64_t)qlen, (uint64_t)tb.cap};
-        const uint64_t qs[1] = {(uint64_t)qlen * 4};
-        const uint32_t bb[2] = {(uint32_t)tc::kTileK, (uint32_t)bn};
         int rc;
-        if ((rc = make_map(ctx, &tb.mapQ_f, tb.Qg_full, 2, qd, qs, bb, true))) return rc;
-        // the correction operands: two bf16 planes (bf16(v) | bf16(v - tf32(v))) of tb.cap rows each in the same allocation
-        const uint64_t qd16[2] = {(uint64_t)qlen, (uint64_t)2 * tb.cap};
-        const uint64_t qs16[1] = {(uint64_t)qlen * 2};
-        if ((rc = make_map(ctx, &tb.mapQ_l, tb.Qg_lo, 2, qd16, qs16, bb, false, true))) return rc;
-        const uint64_t rd[2] = {(uint64_t)ctx->rpitch, (uint64_t)tb.cap};
-        const uint64_t rs[1] = {(uint64_t)ctx->rpitch * 4};
-        if ((rc = make_map(ctx, &tb.mapR_f, tb.rp_full, 2, rd, rs, bb, true))) return rc;
-        const uint64_t rd16[2] = {(uint64_t)ctx->rpitch, (uint64_t)2 * tb.cap};
-        const uint64_t rs16[1] = {(uint64_t)ctx->rpitch * 2};
-        if ((rc = make_map(ctx, &tb.mapR_l, tb.rp_lo, 2, rd16, rs16, bb, false, true))) return rc;
+        if ((rc = tc_make_bmaps(ctx, tb, bn, &tb.mapQ_f, &tb.mapQ_l, &tb.mapR_f, &tb.mapR_l))) return rc;
         tb.bn = bn;
     }
     if (!ctx->tc_attr) {
@@ -382,6 +393,8 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows
         CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32<true, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CU(cudaFuncSetAttribute(tc::banded_gemm_3xtf32_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->tc_attr = true;
     }
     return DODE_OK;
@@ -391,9 +404,27 @@ static int tc_ensure(dode_ctx* ctx, TcBuf& tb, cudaStream_t st, int bn, int rows
 struct TcGeom { int stages, bstages, nring; size_t smem; int ks_f, ks_g; size_t part_floats; };
 
 // minibatch of n days -> day groups per tile (1, or 2 above 128 days) and days per group (MMA N, multiple of 16)
-static void tc_day_groups(int n, int* dsplit, int* bn) {
+// (wider than 64 days: the CTA-pair kernel, whose two CTAs stage bn / 2 days each, so bn is a multiple of 32)
+static bool tc_pair_width(const dode_ctx* ctx, int n) { return ctx->opt_pair != 0 && n > 64; }
+static void tc_day_groups(const dode_ctx* ctx, int n, int* dsplit, int* bn) {
     *dsplit = n > 128 ? 2 : 1;
-    *bn = round_up(ceil_div(n, *dsplit), 16);
+    *bn = round_up(ceil_div(n, *dsplit), tc_pair_width(ctx, n) ? 32 : 16);
+}
+
+// shared-memory geometry of the CTA-pair kernel: B stages of bn / 2 days, one CTA per SM
+static TcGeom tc_pair_geometry(const dode_ctx* ctx, int bn) {
+    TcGeom g{};
+    const int bStage = bn * tc::kTileK * 4;        // (bn / 2 days) x (fp32 + two bf16 planes)
+    const int fixed = 512;
+    const int budget = 227 * 1024 - fixed;
+    int sb = ctx->opt_bstages > 0 ? ctx->opt_bstages : 4;      // measured on large_dense b = 256: 3 -> 55.7, 4 -> 55.1, 5 -> 56.0 ms per epoch
+    int sa = std::max(2, std::min((budget - sb * bStage) / tc::kABytes, 16));
+    sb = std::max(2, std::min(sb, sa));
+    g.stages = sa; g.bstages = sb;
+    g.nring = 2 * bn + 256 <= 512 ? 4 : 2;
+    g.smem = (size_t)sa * tc::kABytes + (size_t)sb * bStage + fixed;
+    g.ks_f = g.ks_g = 1;
+    return g;
 }
 
 static TcGeom tc_geometry(const dode_ctx* ctx, int bn, int dsplit) {
@@ -460,7 +491,7 @@ static cudaError_t launch_pdl(bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 
 static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const StepOpt& opt, TcBuf& tb, cudaStream_t st) {
     const dode_dims& d = ctx->dm;
     int dsplit, bn;
-    tc_day_groups(dl.n, &dsplit, &bn);
+    tc_day_groups(ctx, dl.n, &dsplit, &bn);
     int rc = tc_ensure(ctx, tb, st, bn, dsplit * bn);
     if (rc) return rc;
     const TcGeom geo0 = tc_geometry(ctx, bn, dsplit);
@@ -488,6 +519,17 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
     const int ks_f = geo.ks_f, ks_g = geo.ks_g;
     if ((rc = tc_ensure_part(ctx, tb, st, geo.part_floats))) return rc;
     p.part = tb.part;
+    // CTA pairs (kernels_tc2.cuh) for minibatches wider than 64 days, unless the pass is split along K
+    const bool pair = tc_pair_width(ctx, dl.n) && ks_f == 1 && ks_g == 1;
+    TcGeom pgeo{};
+    if (pair) {
+        pgeo = tc_pair_geometry(ctx, bn);
+        if (tb.bh != bn / 2) {
+            if ((rc = tc_make_bmaps(ctx, tb, bn / 2, &tb.mapQ_f2, &tb.mapQ_l2, &tb.mapR_f2, &tb.mapR_l2))) return rc;
+            tb.bh = bn / 2;
+        }
+    }
+    auto pkern = ada ? tc::banded_gemm_3xtf32_pair<true> : tc::banded_gemm_3xtf32_pair<false>;
     auto epilogue = [&](int Mt) -> int {           // second half of a split-K pass
         const dim3 g(ceil_div((long)Mt * (p.bnt / 4), 256), d.T);
         if (ada) tc::splitk_epilogue<true><<<g, 256, 0, st>>>(p, Mt, dl);
@@ -495,25 +537,45 @@ static int tc_step(dode_ctx* ctx, int c, const DayList& dl, float eta, const Ste
         ctx->launches++;
         return DODE_OK;
     };
+    // one pass over all output tiles: pairs of tiles on the pair kernel, an odd last tile (or everything, when pairs are
+    // not used) on the single-CTA kernel
+    auto run_pass = [&](int M, int ks, const CUtensorMap& mA, const CUtensorMap& mA64, const CUtensorMap& mBf, const CUtensorMap& mBl,
+                        const CUtensorMap& mBf2, const CUtensorMap& mBl2) -> int {
+        const int tiles = ceil_div(M, tc::kTileM);
+        int done = 0;
+        if (pair) {
+            const int npairs = ctx->opt_pair == 2 ? ceil_div(tiles, 2) : tiles / 2;
+            if (npairs > 0) {
+                p.mtile0 = 0; p.ksplit = 1; p.stages = pgeo.stages; p.bstages = pgeo.bstages; p.nring = pgeo.nring;
+                CU(launch_pdl(ctx->opt_pdl, pkern, dim3(2 * dsplit * npairs, d.T, 1), dim3(tc::kThreadsTC), pgeo.smem, st,
+                              mA, mA64, mBf2, mBl2, p, dl));
+                ctx->launches++;
+                done = 2 * npairs;
+            }
+        }
+        if (done < tiles) {
+            p.mtile0 = done; p.ksplit = ks; p.stages = geo.stages; p.bstages = geo.bstages; p.nring = geo.nring;
+            CU(launch_pdl(ctx->opt_pdl, kern, dim3((tiles - done) * dsplit, d.T, ks), dim3(tc::kThreadsTC), smem, st,
+                          mA, mA64, mBf, mBl, p, dl));
+            ctx->launches++;
+            if (ks > 1) epilogue(tiles * tc::kTileM);
+        }
+        return DODE_OK;
+    };
     {
         KernelTimer kt(ctx, KIND_FWD);
-        p.mode = 0; p.M = d.L; p.kunit = ctx->Np; p.ksplit = ks_f;
-        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.L, tc::kTileM) * dsplit, d.T, ks_f), dim3(tc::kThreadsTC), smem,
-                      st, ctx->mapA_fwd, ctx->mapA_fwd64, tb.mapQ_f, tb.mapQ_l, p, dl));
-        ctx->launches++;
-        if (ks_f > 1) epilogue(ceil_div(d.L, tc::kTileM) * tc::kTileM);
+        p.mode = 0; p.M = d.L; p.kunit = ctx->Np;
+        if ((rc = run_pass(d.L, ks_f, ctx->mapA_fwd, ctx->mapA_fwd64, tb.mapQ_f, tb.mapQ_l, tb.mapQ_f2, tb.mapQ_l2))) return rc;
     }
     {
         KernelTimer kt(ctx, KIND_GRAD);
-        p.mode = 1; p.M = d.N; p.kunit = ctx->Lp; p.ksplit = ks_g;
-        CU(launch_pdl(ctx->opt_pdl, kern, dim3(ceil_div(d.N, tc::kTileM) * dsplit, d.T, ks_g), dim3(tc::kThreadsTC), smem,
-                      st, ctx->mapA_grad, ctx->mapA_grad64, tb.mapR_f, tb.mapR_l, p, dl));
-        ctx->launches++;
-        if (ks_g > 1) epilogue(ceil_div(d.N, tc::kTileM) * tc::kTileM);
+        p.mode = 1; p.M = d.N; p.kunit = ctx->Lp;
+        if ((rc = run_pass(d.N, ks_g, ctx->mapA_grad, ctx->mapA_grad64, tb.mapR_f, tb.mapR_l, tb.mapR_f2, tb.mapR_l2))) return rc;
     }
     char buf[96];
-    snprintf(buf, sizeof buf, dsplit > 1 ? "tcgen05_3xtf32_fwd_bn%dx2+tcgen05_3xtf32_grad_bn%dx2"
-                                         : "tcgen05_3xtf32_fwd_bn%d+tcgen05_3xtf32_grad_bn%d", bn, bn);
+    snprintf(buf, sizeof buf, dsplit > 1 ? "tcgen05%s_3xtf32_fwd_bn%dx2+tcgen05%s_3xtf32_grad_bn%dx2"
+                                         : "tcgen05%s_3xtf32_fwd_bn%d+tcgen05%s_3xtf32_grad_bn%d",
+             pair ? "_pair" : "", bn, pair ? "_pair" : "", bn);
     ctx->path = buf;
     return DODE_OK;
 }
@@ -770,6 +832,10 @@ int dode_set_option(dode_ctx* ctx, int32_t option, int32_t value) {
             if (value != 0 && (value < 2 || value > 8)) return fail(ctx, DODE_EINVAL, "DODE_OPT_TC_BSTAGES must be 0 or in [2, 8]");
             ctx->opt_bstages = value;
             return DODE_OK;
+        case DODE_OPT_TC_PAIR:
+            if (value < 0 || value > 2) return fail(ctx, DODE_EINVAL, "DODE_OPT_TC_PAIR must be 0, 1 or 2");
+            ctx->opt_pair = value;
+            return DODE_OK;
         case DODE_OPT_PDL:
             if (value != 0 && value != 1) return fail(ctx, DODE_EINVAL, "DODE_OPT_PDL must be 0 or 1");
             ctx->opt_pdl = value != 0;
@@ -801,7 +867,7 @@ int dode_reserve(dode_ctx* ctx, int32_t max_days) {
             int rows = 0, bn_max = 16;
             for (int n = 1; n <= std::min<int>(max_days, kMaxDays); ++n) {
                 int ds, bn;
-                tc_day_groups(n, &ds, &bn);
+                tc_day_groups(ctx, n, &ds, &bn);
                 part = std::max(part, tc_geometry(ctx, bn, ds).part_floats);
                 rows = std::max(rows, ds * bn);
                 bn_max = std::max(bn_max, bn);

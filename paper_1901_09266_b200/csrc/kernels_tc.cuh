@@ -174,6 +174,7 @@ struct TcParams {
     int T, H;
     int kunit;           // K rows per lag (Np forward, Lp gradient)
     int slab0;           // c*T: first (cluster, time) slab of the A tensor map
+    int mtile0;          // first 128-output tile of this launch (a pass may be split between the pair and the single-CTA kernel)
     int Lp, Np;
     int bn;              // days per CTA (MMA N of the main product), a multiple of 16, <= 128
     int dsplit;          // day groups per output tile (1, or 2 for minibatches wider than 128 days): blockIdx.x % dsplit
@@ -287,7 +288,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     if ((smem_u32(smem) & 1023u) != 0u) __trap();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tt = blockIdx.y;                    // arrival interval t (forward) / departure interval s (gradient)
-    const int m0 = ((int)blockIdx.x / p.dsplit) * kTileM;
+    const int m0 = ((int)blockIdx.x / p.dsplit + p.mtile0) * kTileM;
     const int d0 = ((int)blockIdx.x % p.dsplit) * p.bn;       // first day (position in the list) of this CTA's group
     const int bBytes = p.bn * kTileK * 4;
     // Two rings, because the two operands have different latencies to hide: A streams from HBM (deep ring), the B
@@ -557,7 +558,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (!fused_epi) {                                   // split-K: raw partial sums, 16 consecutive days per thread
                 if (m < p.M) {
                     float4* dst = reinterpret_cast<float4*>(
-                        p.part + (((size_t)blockIdx.z * gridDim.y + tt) * ((size_t)(gridDim.x / p.dsplit) * kTileM) + m) * p.bnt + d0 + c0);
+                        p.part + (((size_t)blockIdx.z * gridDim.y + tt) * ((size_t)(gridDim.x / p.dsplit) * kTileM) + m) * p.bnt + d0 + c0);   // (split-K launches cover all tiles: mtile0 = 0)
 #pragma unroll
                     for (int j = 0; j < 16; j += 4) dst[j >> 2] = make_float4(sum[j], sum[j + 1], sum[j + 2], sum[j + 3]);
                 }

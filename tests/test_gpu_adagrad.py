@@ -74,6 +74,12 @@ def test_adagrad_row_chunks_tensor_core(b):
     assert "tcgen05" in _run(cfg)
 
 
+def test_adagrad_row_chunks_cta_pair_kernel():
+    """The Adagrad / row-mask epilogues of the CTA-pair kernel (minibatch wider than 64 days, an odd tile count)."""
+    cfg = synth.Config("ada_pair", N=300, L=150, T=60, H=3, C=1, D=192, b=96, K=6, kmin=3, kmax=12, label_mode="zero")
+    assert "tcgen05_pair" in _run(cfg)
+
+
 @pytest.mark.parametrize("b", [5, 40])
 def test_adagrad_row_chunks_csr(b):
     cfg = synth.Config("ada_csr", N=80, L=50, T=40, H=6, C=2, D=90, b=b, K=12, kmin=4, kmax=10)

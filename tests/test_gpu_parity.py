@@ -22,13 +22,15 @@ def _objective_cpu(p, q, days):
     return np.array([o.objective_day(p.R[p.labels[d]].numpy(), q[i], p.x[d].numpy()) for i, d in enumerate(days)])
 
 
-def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False, tc_min_b=None, ksplit=None):
+def _run_both(cfg, K=None, b=None, sample=None, csr=False, sparse_gen=False, tc_min_b=None, ksplit=None, pair=None):
     p = hz.make_problem_sparse(cfg) if sparse_gen else hz.make_problem(cfg)
     sched = synth.schedule(cfg, p.labels, K=K, b=b)
     etas = hz.oracle_etas(p)
     g = hz.GpuSolver(p, csr=csr, tc_min_b=tc_min_b)
     if ksplit is not None:
         g.P.dode_set_option(g.h, g.P.DODE_OPT_TC_KSPLIT, ksplit)
+    if pair is not None:
+        g.P.dode_set_option(g.h, g.P.DODE_OPT_TC_PAIR, pair)
     g.run(sched, etas)
     days = list(range(cfg.D)) if sample is None else list(sample)
     q_gpu = g.q(days)
@@ -354,6 +356,20 @@ def test_forced_split_k_on_ragged_shapes(ks):
     _run_both(cfg, sample=[0, 1, 40, 79], ksplit=ks)
 
 
+@pytest.mark.parametrize("pair", [0, 1, 2])
+@pytest.mark.parametrize("N,L,T,H,D,b", [(300, 200, 80, 3, 130, 130), (300, 200, 48, 3, 512, 256), (100, 384, 60, 5, 330, 165),
+                                         (520, 70, 90, 12, 128, 128), (130, 260, 100, 2, 192, 96)])
+def test_cta_pair_kernel(N, L, T, H, D, b, pair):
+    """Minibatches wider than 64 days on the CTA-pair kernel (tcgen05.mma.cta_group::2, kernels_tc2.cuh): even and odd
+    tile counts (the odd last tile on the single-CTA kernel, or paired with an idle CTA), a single tile (no pair at
+    all), half tiles, one and two day groups of 96 / 128 days, ragged day counts; DODE_OPT_TC_PAIR = 0 runs the same
+    shapes on the single-CTA kernels."""
+    cfg = synth.Config("pair", N=N, L=L, T=T, H=H, C=1, D=D, b=b, K=4, kmin=3, kmax=9, label_mode="zero")
+    sample = sorted({0, 1, b // 2 - 1, b // 2, b - 1, D // 2, D - 1})
+    path = _run_both(cfg, sample=sample, pair=pair)
+    assert ("_pair" in path) == (pair != 0), path
+
+
 def test_minibatch_larger_than_one_launch():
     """A minibatch of more than 256 days is split into several launches inside one dode_spgd_step (days are independent
     units); the sub-batches alternate on the internal streams."""
@@ -371,7 +387,7 @@ def test_options_and_reserve_keep_results():
     etas = hz.oracle_etas(p)
     want = hz.oracle_run(p, sched, etas)
     for opts in ({}, {"LANES": 0}, {"PDL": 0}, {"LANES": 0, "PDL": 0, "TC_KSPLIT": 3}, {"TC_MIN_B": 0}, {"TC_MIN_B": 100},
-                 {"TC_BSTAGES": 2}, {"TC_BSTAGES": 5, "TC_KSPLIT": 2}, {"TC_BSTAGES": 8}):
+                 {"TC_BSTAGES": 2}, {"TC_BSTAGES": 5, "TC_KSPLIT": 2}, {"TC_BSTAGES": 8}, {"TC_PAIR": 0}, {"TC_PAIR": 2}):
         g0 = hz.GpuSolver(p)                           # a throw-away pass first: the CUDA runtime loads kernel modules
         for k, v in opts.items():                      # lazily, which moves device memory at a kernel's first launch
             g0.P.dode_set_option(g0.h, getattr(g0.P, "DODE_OPT_" + k), v)
@@ -382,7 +398,7 @@ def test_options_and_reserve_keep_results():
         for k, v in opts.items():
             P.dode_set_option(g.h, getattr(P, "DODE_OPT_" + k), v)
         for bad in ((99, 1), (P.DODE_OPT_LANES, 2), (P.DODE_OPT_TC_KSPLIT, 33), (P.DODE_OPT_TC_MIN_B, -1), (P.DODE_OPT_PDL, -1),
-                    (P.DODE_OPT_TC_BSTAGES, 1), (P.DODE_OPT_TC_BSTAGES, 9)):
+                    (P.DODE_OPT_TC_BSTAGES, 1), (P.DODE_OPT_TC_BSTAGES, 9), (P.DODE_OPT_TC_PAIR, 3), (P.DODE_OPT_TC_PAIR, -1)):
             with pytest.raises(P.DodeError) as e:
                 P.dode_set_option(g.h, *bad)
             assert e.value.code == P.DODE_EINVAL
