@@ -417,11 +417,12 @@ static TcGeom tc_pair_geometry(const dode_ctx* ctx, int bn) {
     const int bStage = bn * tc::kTileK * 4;        // (bn / 2 days) x (fp32 + two bf16 planes)
     const int fixed = 512;
     const int budget = 227 * 1024 - fixed;
-    int sb = ctx->opt_bstages > 0 ? ctx->opt_bstages : 4;      // measured on large_dense b = 256: 3 -> 55.7, 4 -> 55.1, 5 -> 56.0 ms per epoch
-    int sa = std::max(2, std::min((budget - sb * bStage) / tc::kABytes, 16));
-    sb = std::max(2, std::min(sb, sa));
+    // 4 B stages and 4 TMEM A buffers, fixed: the issue loop of the kernel is unrolled for them (DODE_OPT_TC_BSTAGES steers
+    // the single-CTA kernels only).  Measured on large_dense b = 256: 3 -> 55.7, 4 -> 55.1, 5 -> 56.0 ms per epoch.
+    const int sb = 4;
+    const int sa = std::max(2, std::min((budget - sb * bStage) / tc::kABytes, 16));
     g.stages = sa; g.bstages = sb;
-    g.nring = 2 * bn + 256 <= 512 ? 4 : 2;
+    g.nring = 4;                                   // 2 * bn <= 256 accumulator columns + 4 x 64
     g.smem = (size_t)sa * tc::kABytes + (size_t)sb * bStage + fixed;
     g.ks_f = g.ks_g = 1;
     return g;

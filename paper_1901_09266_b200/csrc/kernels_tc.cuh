@@ -154,6 +154,20 @@ __device__ __forceinline__ uint64_t umma_desc_k_sw64(uint32_t saddr) {
     return d;
 }
 
+// The same two descriptors as compile-time constants of the layout (address 0), and a descriptor assembled from its
+// two 32-bit words: high word = layout constants, low word = address in 16-byte units | LBO bit.
+__host__ __device__ constexpr uint64_t umma_desc_k_sw128_c(uint32_t a16) {
+    return (uint64_t)a16 | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__host__ __device__ constexpr uint64_t umma_desc_k_sw64_c(uint32_t a16) {
+    return (uint64_t)a16 | ((uint64_t)1 << 16) | ((uint64_t)(512 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)4 << 61);
+}
+__device__ __forceinline__ uint64_t desc_pack(uint32_t lo, uint32_t hi) {
+    uint64_t d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "r"(lo), "r"(hi));
+    return d;
+}
+
 // kind::f16 instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = bn.
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int bn) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
@@ -434,11 +448,19 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp walks the loop, one elected lane issues =====
         const uint32_t idesc1 = umma_idesc_tf32(p.bn), idesc16 = umma_idesc_bf16(p.bn);
+        // Shared-memory descriptors: the high words are constants of the layout, the low word is the tile address in
+        // 16-byte units (+ the LBO bit), so a K slice or a ring stage is ONE 32-bit add away from the ring's base.
+        // (Building every descriptor from its byte address cost ~90 uniform-datapath instructions per chunk; with
+        // them the issuing warp — not the tensor pipe or the stream — set the pace of the wide-minibatch kernels.)
+        constexpr uint32_t hi128 = (uint32_t)(umma_desc_k_sw128_c(0) >> 32), hi64 = (uint32_t)(umma_desc_k_sw64_c(0) >> 32);
+        const uint32_t ring16 = ((smem_u32(ringB) & 0x3FFFFu) >> 4) | (1u << 16);
+        const uint32_t st16 = (uint32_t)bStage >> 4, bB16 = (uint32_t)bBytes >> 4;
+        const int pg_mask = per_group - 1, pg_shift = per_group >> 1;   // per_group is 1 or 2
         int s = 0, sb = 0;                                      // A stage (names the chunk's full barrier), B stage
         uint32_t fph[2] = {0u, 0u};                             // parity of the next phase of full[g][s], bit s
         for (int kc = 0; kc < nk; ++kc) {
             const int g = kc & 1, use = kc >> 1;
-            const int jr = g * per_group + use % per_group;
+            const int jr = g * per_group + (use & pg_mask);
             const bool restart = kc % kFlushChunks == 0;        // first chunk of a segment: the accumulators start over
             if (restart && kc > 0) {                            // drain: the splitter threads read the sums so far
                 if (elect_one()) umma_commit(accum);
@@ -448,19 +470,19 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             }
             mbar_wait(&full[g * SA + s], (fph[g] >> s) & 1u, 3, kc);
             fph[g] ^= 1u << s;
-            mbar_wait(&split[jr], (use / per_group) & 1, 4, kc);
+            mbar_wait(&split[jr], (use >> pg_shift) & 1, 4, kc);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t bf0 = smem_u32(ringB + (size_t)sb * bStage);
+            const uint32_t f16 = ring16 + (uint32_t)sb * st16;                  // fp32 B | bf16(B) | bf16(B_lo)
+            const uint32_t h16 = f16 + bB16, l16 = h16 + (bB16 >> 1);
             const uint32_t afull = tmem_ring + (uint32_t)jr * 64, a16 = afull + 32, alo16 = afull + 48;
-            const uint32_t bh0 = bf0 + bBytes, bl0 = bh0 + bBytes / 2;
             if (elect_one()) {
 #pragma unroll
                 for (int k = 0; k < kTileK / 8; ++k)             // main product, UMMA_K = 8 for tf32 (32 bytes of the 128-byte rows)
-                    umma_tf32_ts(tmem_d, afull + k * 8, umma_desc_k_sw128(bf0 + k * 32), idesc1, !(restart && k == 0));
+                    umma_tf32_ts(tmem_d, afull + k * 8, desc_pack(f16 + 2 * k, hi128), idesc1, !(restart && k == 0));
 #pragma unroll
                 for (int k = 0; k < kTileK / 16; ++k) {          // corrections in bf16, UMMA_K = 16 (32 bytes of the 64-byte rows)
-                    umma_bf16_ts(tmem_d + (uint32_t)p.bn, alo16 + k * 8, umma_desc_k_sw64(bh0 + k * 32), idesc16, !(restart && k == 0));  // a_lo * b
-                    umma_bf16_ts(tmem_d + (uint32_t)p.bn, a16 + k * 8, umma_desc_k_sw64(bl0 + k * 32), idesc16, 1);                       // a * b_lo
+                    umma_bf16_ts(tmem_d + (uint32_t)p.bn, alo16 + k * 8, desc_pack(h16 + 2 * k, hi64), idesc16, !(restart && k == 0));  // a_lo * b
+                    umma_bf16_ts(tmem_d + (uint32_t)p.bn, a16 + k * 8, desc_pack(l16 + 2 * k, hi64), idesc16, 1);                       // a * b_lo
                 }
                 umma_commit(&empty[sb]);
                 umma_commit(&a_empty[jr]);
@@ -505,10 +527,10 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
             if (++s == SA) s = 0;
             if ((kc & 1) != group) continue;
             const int use = kc >> 1;
-            const int jr = group * per_group + use % per_group;
+            const int jr = group * per_group + (use & (per_group - 1));       // per_group is 1 or 2
             mbar_wait(&full[group * SA + s], (fph >> s) & 1u, 6, kc);
             fph ^= 1u << s;
-            if (use >= per_group) mbar_wait(&a_empty[jr], (use / per_group - 1) & 1, 7, kc);
+            if (use >= per_group) mbar_wait(&a_empty[jr], ((use >> (per_group >> 1)) - 1) & 1, 7, kc);
             if (lane_base >= BM) { mbar_arrive(&split[jr]); continue; }    // rows never stored
             const float* A = reinterpret_cast<const float*>(smem + (size_t)s * kABytes) + row;
             const uint32_t t0 = tmem_ring + (uint32_t)jr * 64 + ((uint32_t)lane_base << 16);

@@ -191,6 +191,7 @@ banded_gemm_3xtf32_pair(const __grid_constant__ CUtensorMap mapA, const __grid_c
     const uint32_t tmem_d = *tmem_slot;
     const uint32_t tmem_ring = tmem_d + (uint32_t)acc_cols;
     const int per_group = nring >> 1;
+    if (SB != 4 || nring != 4) __trap();          // the MMA issue loop below is unrolled for this geometry
     // the leader's copies of the barriers the peer arrives on
     const uint32_t fullB_l = mapa_u32(smem_u32(fullB), 0), split_l = mapa_u32(smem_u32(split), 0);
     const uint32_t drained_l = mapa_u32(smem_u32(drained), 0);
@@ -264,39 +265,50 @@ banded_gemm_3xtf32_pair(const __grid_constant__ CUtensorMap mapA, const __grid_c
         if (leader) {
             // ===== MMA issuer (leader only) =====
             const uint32_t idesc1 = umma_idesc_tf32_pair(p.bn), idesc16 = umma_idesc_bf16_pair(p.bn);
-            int sb = 0;
-            uint32_t bph = 0u;                                      // parity of the next phase of fullB[sb], bit sb
-            for (int kc = 0; kc < nk; ++kc) {
-                const int g = kc & 1, use = kc >> 1;
-                const int jr = g * per_group + use % per_group;
-                const bool restart = kc % kFlushChunks == 0;
-                if (restart && kc > 0) {
+            // Shared-memory descriptors: the high words are constants of the layout, the low word is the tile address in
+            // 16-byte units (+ the LBO bit), so a K slice or a ring stage is ONE 32-bit add away from the ring's base.
+            // (Building every descriptor from its byte address cost ~90 uniform-datapath instructions per chunk, and
+            // the issuing warp — not the tensor pipe — set the pace: 930 cycles per chunk against 512 of tensor work.)
+            constexpr uint32_t hi128 = (uint32_t)(umma_desc_k_sw128_c(0) >> 32), hi64 = (uint32_t)(umma_desc_k_sw64_c(0) >> 32);
+            const uint32_t ring16 = (((smem_u32(ringB) & 0x3FFFFu) >> 4) | (1u << 16));
+            const uint32_t st16 = (uint32_t)bStage >> 4, bB16 = (uint32_t)bBytes >> 4;
+            // The ring geometry of the pair kernel is fixed (4 B stages, 4 TMEM A buffers), so chunk kc uses B stage kc % 4
+            // and TMEM buffer ((kc & 1) << 1) | ((kc >> 1) & 1), both static after unrolling by 4, and all barriers
+            // of a group of 4 chunks are in the same phase.
+            for (int kc0 = 0; kc0 < nk; kc0 += 4) {
+                const uint32_t par = ((uint32_t)kc0 >> 2) & 1u;
+                const bool restart = (kc0 & (kFlushChunks - 1)) == 0;   // first chunk of a segment: the accumulators start over
+                if (restart && kc0 > 0) {                               // drain: the splitter threads read the sums so far
                     if (elect_one()) umma_commit_pair(accum);
                     __syncwarp();
-                    mbar_wait_cluster(drained, (kc / kFlushChunks - 1) & 1, 2, kc);
+                    mbar_wait_cluster(drained, (kc0 / kFlushChunks - 1) & 1, 2, kc0);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 }
-                mbar_wait_cluster(&fullB[sb], (bph >> sb) & 1u, 3, kc);
-                bph ^= 1u << sb;
-                mbar_wait_cluster(&split[jr], (use / per_group) & 1, 4, kc);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t bf0 = smem_u32(ringB + (size_t)sb * bStage);
-                const uint32_t afull = tmem_ring + (uint32_t)jr * 64, a16 = afull + 32, alo16 = afull + 48;
-                const uint32_t bh0 = bf0 + bBytes, bl0 = bh0 + bBytes / 2;
-                if (elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < kTileK / 8; ++k)
-                        umma_tf32_ts_pair(tmem_d, afull + k * 8, umma_desc_k_sw128(bf0 + k * 32), idesc1, !(restart && k == 0));
+                for (int j = 0; j < 4; ++j) {
+                    const int kc = kc0 + j;
+                    if (kc >= nk) break;                                // warp-uniform
+                    const int jr = ((j & 1) << 1) | (j >> 1);
+                    mbar_wait_cluster(&fullB[j], par, 3, kc);
+                    mbar_wait_cluster(&split[jr], par, 4, kc);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t f16 = ring16 + (uint32_t)j * st16;   // fp32 B | bf16(B) | bf16(B_lo)
+                    const uint32_t h16 = f16 + bB16, l16 = h16 + (bB16 >> 1);
+                    const uint32_t afull = tmem_ring + (uint32_t)jr * 64, a16 = afull + 32, alo16 = afull + 48;
+                    if (elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < kTileK / 16; ++k) {
-                        umma_bf16_ts_pair(tmem_d + (uint32_t)p.bn, alo16 + k * 8, umma_desc_k_sw64(bh0 + k * 32), idesc16, !(restart && k == 0));
-                        umma_bf16_ts_pair(tmem_d + (uint32_t)p.bn, a16 + k * 8, umma_desc_k_sw64(bl0 + k * 32), idesc16, 1);
+                        for (int k = 0; k < kTileK / 8; ++k)
+                            umma_tf32_ts_pair(tmem_d, afull + k * 8, desc_pack(f16 + 2 * k, hi128), idesc1, !(restart && j == 0 && k == 0));
+#pragma unroll
+                        for (int k = 0; k < kTileK / 16; ++k) {
+                            umma_bf16_ts_pair(tmem_d + (uint32_t)p.bn, alo16 + k * 8, desc_pack(h16 + 2 * k, hi64), idesc16, !(restart && j == 0 && k == 0));
+                            umma_bf16_ts_pair(tmem_d + (uint32_t)p.bn, a16 + k * 8, desc_pack(l16 + 2 * k, hi64), idesc16, 1);
+                        }
+                        umma_commit_pair(&emptyB[j]);
+                        umma_commit_pair(&a_empty[jr]);
                     }
-                    umma_commit_pair(&emptyB[sb]);
-                    umma_commit_pair(&a_empty[jr]);
+                    __syncwarp();
                 }
-                __syncwarp();
-                if (++sb == SB) sb = 0;
             }
             if (elect_one()) {
                 if (nk == 0) { mbar_arrive(accum); mbar_arrive_cluster(mapa_u32(smem_u32(accum), 1)); }
@@ -337,13 +349,13 @@ banded_gemm_3xtf32_pair(const __grid_constant__ CUtensorMap mapA, const __grid_c
             if (++s == SA) s = 0;
             if ((kc & 1) != group) continue;
             const int use = kc >> 1;
-            const int jr = group * per_group + use % per_group;
+            const int jr = group * per_group + (use & (per_group - 1));     // per_group is 1 or 2
             const bool work = !dummy && lane_base < BM;              // rows that are stored at the end
             if (!dummy) {
                 mbar_wait(&fullA[group * SA + s], (fph >> s) & 1u, 6, kc);
                 fph ^= 1u << s;
             }
-            if (use >= per_group) mbar_wait_cluster(&a_empty[jr], (use / per_group - 1) & 1, 7, kc);
+            if (use >= per_group) mbar_wait_cluster(&a_empty[jr], ((use >> (per_group >> 1)) - 1) & 1, 7, kc);
             if (work) {
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const float* A = reinterpret_cast<const float*>(smem + (size_t)s * kABytes) + row;
