@@ -436,7 +436,7 @@ static TcGeom tc_geometry(const dode_ctx* ctx, int bn, int dsplit) {
     // bytes in flight per SM are what hides the HBM latency).  Two CTAs per SM when 256 TMEM columns suffice.
     // An SM has 228 KB of shared memory, 1 KB of it reserved per resident CTA; a CTA may use up to 227 KB.
     const int bStage = 2 * bn * tc::kTileK * 4;
-    const int fixed = 512;                         // barriers (2*SA + SB + 10 of them) + the TMEM slot
+    const int fixed = 512;                         // barriers (2*SA + 2*SB + 10 of them, SA <= 16, SB <= 8) + the TMEM slot
     const int acc_cols = 2 * bn;
     const bool two = acc_cols + 128 <= 256;
     const int budget = (two ? 228 * 1024 / 2 - 1024 : 227 * 1024) - fixed;

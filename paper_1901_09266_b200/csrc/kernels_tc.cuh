@@ -319,14 +319,15 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     const int aBytes = BM * kTileK * 4;
     const CUtensorMap* mA = half ? &mapA64 : &mapA;
     uint64_t* bars = reinterpret_cast<uint64_t*>(ringB + (size_t)SB * bStage);
-    // full: TMA landed (A and B of one chunk; armed when the A tile is requested, the B tiles join later).
-    // One barrier per (splitter group, A stage): chunk kc completes full[(kc & 1) * SA + kc % SA],
-    // so every waiter of a barrier (that group's splitters and the MMA warp) sees EVERY one of its phases in turn.  With
-    // one barrier per stage a group would have to watch the other group's chunks go by just to keep count, and a warp
-    // that is slow to start could fall two phases behind (a stage is refilled as soon as the OTHER group's MMAs retire)
-    // and wait for ever — seen once in ~300 steps on the multiyear shape.
+    // full: TMA landed an A tile.  One barrier per (splitter group, A stage): chunk kc completes
+    // full[(kc & 1) * SA + kc % SA], and only that group's splitters wait on it, so every waiter of a barrier sees EVERY
+    // one of its phases in turn.  (With one barrier per stage a group would have to watch the other group's chunks go by
+    // just to keep count, and a warp that is slow to start could fall two phases behind and wait for ever — seen once in
+    // ~300 steps on the multiyear shape.)  fullB: the B tiles of a chunk landed; only the MMA warp waits on it.  (One
+    // barrier for both made the splitters wait for the B tiles, which are requested three chunks later than the A tile.)
     uint64_t* full = bars;                        // [2][SA]
-    uint64_t* empty = bars + 2 * SA;              // [SB] MMAs of the chunk in this B stage retired
+    uint64_t* fullB = bars + 2 * SA;              // [SB]
+    uint64_t* empty = fullB + SB;                 // [SB] MMAs of the chunk in this B stage retired
     uint64_t* split = empty + SB;                 // [nring] A_hi/A_lo in TMEM
     uint64_t* a_empty = split + 4;                // [nring] MMAs that read this TMEM buffer retired
     uint64_t* accum = a_empty + 4;                // all MMAs issued so far retired (every drain and the end)
@@ -346,7 +347,7 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < SA; ++s) { mbar_init(&full[s], 1); mbar_init(&full[SA + s], 1); }
-        for (int s = 0; s < SB; ++s) mbar_init(&empty[s], 1);
+        for (int s = 0; s < SB; ++s) { mbar_init(&fullB[s], 1); mbar_init(&empty[s], 1); }
         for (int j = 0; j < nring; ++j) { mbar_init(&split[j], 128); mbar_init(&a_empty[j], 1); }
         mbar_init(accum, 1);
         mbar_init(drained, 256);
@@ -374,12 +375,11 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
     // under that kernel's tail.  The B tiles (panels written by the previous kernel) follow after the wait; the stage's
     // barrier expects the bytes of all three loads from the start.
     const int npre = min(SA, nk);
-    const int txBytes = aBytes + 2 * bBytes;
     if (warp == 0) {
         if (elect_one()) {
             for (int kc = 0; kc < npre; ++kc) {                  // (kc < SA: the stage index is kc)
                 uint64_t* fb = &full[(kc & 1) * SA + kc];
-                mbar_expect_tx(fb, txBytes);
+                mbar_expect_tx(fb, aBytes);
                 tma_load_3d(smem + (size_t)kc * kABytes, mA, fb, m0, (kbase + kc) * kTileK, p.slab0 + tt);
             }
         }
@@ -432,11 +432,12 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 if (kc >= SB && ka < nk) {                       // (ka >= SA >= npre: the first round was requested before the wait)
                     int sk = sa - SB; if (sk < 0) sk += SA;      // ka % SA == (kc - SB) % SA
                     uint64_t* fa = &full[(ka & 1) * SA + sk];
-                    mbar_expect_tx(fa, txBytes);
+                    mbar_expect_tx(fa, aBytes);
                     tma_load_3d(smem + (size_t)sk * kABytes, mA, fa, m0, (kbase + ka) * kTileK, p.slab0 + tt);
                 }
                 uint8_t* st = ringB + (size_t)sb * bStage;
-                uint64_t* fb = &full[(kc & 1) * SA + sa];
+                uint64_t* fb = &fullB[sb];
+                mbar_expect_tx(fb, 2 * bBytes);
                 tma_load_2d(st, &mapBf, fb, w0 + kc * kTileK, d0);
                 tma_load_2d(st + bBytes, &mapBl, fb, w0 + kc * kTileK, d0);                       // bf16(B)
                 tma_load_2d(st + bBytes + bBytes / 2, &mapBl, fb, w0 + kc * kTileK, p.pcap + d0);   // bf16(B_lo)
@@ -456,8 +457,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
         const uint32_t ring16 = ((smem_u32(ringB) & 0x3FFFFu) >> 4) | (1u << 16);
         const uint32_t st16 = (uint32_t)bStage >> 4, bB16 = (uint32_t)bBytes >> 4;
         const int pg_mask = per_group - 1, pg_shift = per_group >> 1;   // per_group is 1 or 2
-        int s = 0, sb = 0;                                      // A stage (names the chunk's full barrier), B stage
-        uint32_t fph[2] = {0u, 0u};                             // parity of the next phase of full[g][s], bit s
+        int sb = 0;                                             // B stage
+        uint32_t bph = 0u;                                      // parity of the next phase of fullB[sb], bit sb
         for (int kc = 0; kc < nk; ++kc) {
             const int g = kc & 1, use = kc >> 1;
             const int jr = g * per_group + (use & pg_mask);
@@ -468,8 +469,8 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 mbar_wait(drained, (kc / kFlushChunks - 1) & 1, 2, kc);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             }
-            mbar_wait(&full[g * SA + s], (fph[g] >> s) & 1u, 3, kc);
-            fph[g] ^= 1u << s;
+            mbar_wait(&fullB[sb], (bph >> sb) & 1u, 3, kc);
+            bph ^= 1u << sb;
             mbar_wait(&split[jr], (use >> pg_shift) & 1, 4, kc);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t f16 = ring16 + (uint32_t)sb * st16;                  // fp32 B | bf16(B) | bf16(B_lo)
@@ -488,7 +489,6 @@ banded_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_consta
                 umma_commit(&a_empty[jr]);
             }
             __syncwarp();
-            if (++s == SA) s = 0;
             if (++sb == SB) sb = 0;
         }
         if (elect_one()) { if (nk == 0) mbar_arrive(accum); else umma_commit(accum); }
