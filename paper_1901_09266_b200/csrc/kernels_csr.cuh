@@ -495,33 +495,40 @@ csr_grad(const int64_t* __restrict__ rowptr, const int32_t* __restrict__ kl, con
     const int64_t k0 = rowptr[rb], k1 = rowptr[rb + 1];
     const bool full = rbp == bp;
     const float* rrow = r + (size_t)sb * kRB * L * rbp;
+    // A chunk of 32 entries is fetched by the whole warp with coalesced loads and parked in shared memory; an entry's
+    // payload and its four values are then read back at a warp-uniform address (one LDS.32 + one LDS.128, one wavefront
+    // each) instead of five shuffles per gathered row: the pass is bound by the LSU/MIO pipe, which the 512-byte gathers
+    // already keep busy.
+    __shared__ float4 sval[8][32];
+    __shared__ int sidx[8][32];
+    const int wib = threadIdx.x >> 5;
     DayAcc<DV> accp[kRB];
     for (int64_t kb = k0; kb < k1; kb += 32) {
         const int64_t k = kb + lane;
-        const int o = k < k1 ? __ldg(kl + k) : 0;
-        const float4 v = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
         const int cnt = (int)min((int64_t)32, k1 - kb);
+        __syncwarp();                                // the previous chunk has been read
+        sidx[wib][lane] = k < k1 ? __ldg(kl + k) : 0;
+        sval[wib][lane] = k < k1 ? __ldg(val + k) : make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncwarp();
         int j = 0;
         if (full) {
             for (; j + kInFlightG <= cnt; j += kInFlightG) {
-                float rv[kInFlightG][DV]; float vv[kInFlightG][kRB];
+                float rv[kInFlightG][DV];
+#pragma unroll
+                for (int u = 0; u < kInFlightG; ++u) ld_days<DV>(rrow + (long)sidx[wib][j + u] * bp, lane, rv[u]);
 #pragma unroll
                 for (int u = 0; u < kInFlightG; ++u) {
-                    const int oo = __shfl_sync(0xffffffffu, o, j + u);
-                    vv[u][0] = __shfl_sync(0xffffffffu, v.x, j + u); vv[u][1] = __shfl_sync(0xffffffffu, v.y, j + u);
-                    vv[u][2] = __shfl_sync(0xffffffffu, v.z, j + u); vv[u][3] = __shfl_sync(0xffffffffu, v.w, j + u);
-                    ld_days<DV>(rrow + (long)oo * bp, lane, rv[u]);
+                    const float4 v = sval[wib][j + u];
+                    const float vv[kRB] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int i = 0; i < kRB; ++i) accp[i].fma(vv[i], rv[u]);
                 }
-#pragma unroll
-                for (int u = 0; u < kInFlightG; ++u)
-#pragma unroll
-                    for (int i = 0; i < kRB; ++i) accp[i].fma(vv[u][i], rv[u]);
             }
         }
         for (; j < cnt; ++j) {
-            const int oo = __shfl_sync(0xffffffffu, o, j);
-            const float v4[kRB] = {__shfl_sync(0xffffffffu, v.x, j), __shfl_sync(0xffffffffu, v.y, j),
-                                   __shfl_sync(0xffffffffu, v.z, j), __shfl_sync(0xffffffffu, v.w, j)};
+            const int oo = sidx[wib][j];
+            const float4 v = sval[wib][j];
+            const float v4[kRB] = {v.x, v.y, v.z, v.w};
             float rf[DV];
             if (full) {
                 ld_days<DV>(rrow + (long)oo * bp, lane, rf);
