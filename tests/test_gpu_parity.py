@@ -358,11 +358,12 @@ def test_forced_split_k_on_ragged_shapes(ks):
 
 @pytest.mark.parametrize("pair", [0, 1, 2])
 @pytest.mark.parametrize("N,L,T,H,D,b", [(300, 200, 80, 3, 130, 130), (300, 200, 48, 3, 512, 256), (100, 384, 60, 5, 330, 165),
-                                         (520, 70, 90, 12, 128, 128), (130, 260, 100, 2, 192, 96)])
+                                         (520, 70, 90, 12, 128, 128), (130, 260, 100, 2, 192, 96),
+                                         (40, 300, 200, 0, 100, 100), (33, 257, 160, 2, 129, 129)])
 def test_cta_pair_kernel(N, L, T, H, D, b, pair):
     """Minibatches wider than 64 days on the CTA-pair kernel (tcgen05.mma.cta_group::2, kernels_tc2.cuh): even and odd
     tile counts (the odd last tile on the single-CTA kernel, or paired with an idle CTA), a single tile (no pair at
-    all), half tiles, one and two day groups of 96 / 128 days, ragged day counts; DODE_OPT_TC_PAIR = 0 runs the same
+    all), half tiles, one and two day groups of 96 / 128 days, ragged day counts, K ranges shorter than the ring (H = 0); DODE_OPT_TC_PAIR = 0 runs the same
     shapes on the single-CTA kernels."""
     cfg = synth.Config("pair", N=N, L=L, T=T, H=H, C=1, D=D, b=b, K=4, kmin=3, kmax=9, label_mode="zero")
     sample = sorted({0, 1, b // 2 - 1, b // 2, b - 1, D // 2, D - 1})
