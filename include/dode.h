@@ -103,7 +103,8 @@ int dode_reserve(dode_ctx* ctx, int32_t max_days);
  *   DODE_OPT_PDL        1 = kernels of a step are chained by programmatic dependent launch (default), 0 = plain
  *                       stream order.
  *   DODE_OPT_TC_BSTAGES stages of the tcgen05 kernels' minibatch-panel (B) ring, 2..8; 0 = automatic (default).  The
- *                       operator (A) ring takes the rest of the shared memory.
+ *                       operator (A) ring takes the rest of the shared memory.  (Single-CTA kernels only: the CTA-pair
+ *                       kernel's ring geometry is fixed at 4 B stages.)
  *   DODE_OPT_TC_PAIR    tcgen05 kernels for minibatches wider than 64 days: 1 = pairs of CTAs on the two SMs of a TPC
  *                       (tcgen05.mma.cta_group::2 on 256-output tiles, each CTA staging half of the minibatch panel
  *                       tile), an odd last 128-output tile on the single-CTA kernel (default); 2 = pairs only (an odd
